@@ -1,0 +1,224 @@
+"""Seeded synthetic Hamiltonians (inputs only — none of the SP2 method's arithmetic lives here).
+
+These stand in for the paper's PROGRESS bio-benchmark (Table I) and the
+"soft matter synthetic Hamiltonians" of its Fig. 5, neither of which is available.
+The recipes are BASELINE.json's five `configs`, made concrete by SURVEY.md Appendix A:
+
+* RNG: ``numpy.random.default_rng(seed)`` (PCG64), seed 0; on-site noise drawn first, config-1's
+  dense Gaussian noise second.
+* Site index of an ``Lx x Ly x Lz`` lattice: ``i = (x*Ly + y)*Lz + z``; periodic in all directions.
+* On-site ``H_ii = delta*(+1 if (x+y+z) even else -1) + U[-a, a]``; hopping ``f(r)`` on the Euclidean
+  minimum-image distance ``r``.
+
+This module is used by the tests, bench.py and the smoke test to feed the SAME matrices to the CUDA path
+and to the CPU oracle.  It imports neither of them.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+
+import numpy as np
+
+
+# ----------------------------------------------------------------------------------------------
+# helpers
+# ----------------------------------------------------------------------------------------------
+def stencil_offsets(rmax: float):
+    """All integer displacements (dx,dy,dz) != 0 with Euclidean length <= rmax, with their length."""
+    R = int(math.floor(rmax))
+    out = []
+    for dx in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dz in range(-R, R + 1):
+                r2 = dx * dx + dy * dy + dz * dz
+                if 0 < r2 <= rmax * rmax + 1e-12:
+                    out.append((dx, dy, dz, math.sqrt(r2)))
+    return out
+
+
+def _site_coords(L):
+    Lx, Ly, Lz = L
+    x, y, z = np.meshgrid(np.arange(Lx), np.arange(Ly), np.arange(Lz), indexing="ij")
+    return x.ravel(), y.ravel(), z.ravel()
+
+
+def _onsite(L, delta, noise, rng):
+    x, y, z = _site_coords(L)
+    sign = np.where((x + y + z) % 2 == 0, 1.0, -1.0)
+    return delta * sign + rng.uniform(-noise, noise, size=sign.size)
+
+
+def lattice_dense(L, delta, noise, rmax, hop, seed=0):
+    """Dense symmetric H on a periodic Lx x Ly x Lz lattice; ``hop(r)`` is the hopping at distance r."""
+    Lx, Ly, Lz = L
+    N = Lx * Ly * Lz
+    rng = np.random.default_rng(seed)
+    H = np.zeros((N, N), dtype=np.float64)
+    idx = np.arange(N)
+    H[idx, idx] = _onsite(L, delta, noise, rng)
+    x, y, z = _site_coords(L)
+    for dx, dy, dz, r in stencil_offsets(rmax):
+        j = (((x + dx) % Lx) * Ly + (y + dy) % Ly) * Lz + (z + dz) % Lz
+        H[idx, j] += hop(r)  # j is a permutation of idx for one displacement: no duplicate targets per call
+    return H
+
+
+def _images_coincide(L, rmax):
+    """True when two different displacements can reach the same site (tiny boxes): use add.at then."""
+    return any(2 * math.floor(rmax) >= l for l in L)
+
+
+def lattice_ellpack(L, delta, noise, rmax, hop, M, seed=0):
+    """ELLPACK-R (Listing 1) H: value[N*M], index[N*M] (int32), nnz[N]; rows in ascending column order.
+
+    Unused slots hold value 0.0 / index 0.  Requires a box large enough that periodic images
+    of the stencil do not coincide (2*floor(rmax) < min(L)).
+    """
+    Lx, Ly, Lz = L
+    N = Lx * Ly * Lz
+    assert not _images_coincide(L, rmax), "box too small for a unique minimum image"
+    rng = np.random.default_rng(seed)
+    offs = stencil_offsets(rmax)
+    n_row = len(offs) + 1
+    assert n_row <= M
+    x, y, z = _site_coords(L)
+    cols = np.empty((N, n_row), dtype=np.int64)
+    vals = np.empty((N, n_row), dtype=np.float64)
+    cols[:, 0] = np.arange(N)
+    vals[:, 0] = _onsite(L, delta, noise, rng)
+    for q, (dx, dy, dz, r) in enumerate(offs, start=1):
+        cols[:, q] = (((x + dx) % Lx) * Ly + (y + dy) % Ly) * Lz + (z + dz) % Lz
+        vals[:, q] = hop(r)
+    order = np.argsort(cols, axis=1, kind="stable")
+    cols = np.take_along_axis(cols, order, axis=1)
+    vals = np.take_along_axis(vals, order, axis=1)
+    value = np.zeros((N, M), dtype=np.float64)
+    index = np.zeros((N, M), dtype=np.int32)
+    value[:, :n_row] = vals
+    index[:, :n_row] = cols.astype(np.int32)
+    nnz = np.full(N, n_row, dtype=np.int32)
+    return value, index, nnz
+
+
+def ring_dense(N, delta, noise, sigma, seed=0):
+    """Config 1: 1D ring, alternating on-site +/-delta + U[-noise,noise], NN hopping -1, plus symmetric
+    Gaussian noise of std sigma on every independent entry i<=j."""
+    rng = np.random.default_rng(seed)
+    i = np.arange(N)
+    H = np.zeros((N, N), dtype=np.float64)
+    H[i, i] = np.where(i % 2 == 0, delta, -delta) + rng.uniform(-noise, noise, size=N)
+    H[i, (i + 1) % N] += -1.0
+    H[(i + 1) % N, i] += -1.0
+    if sigma > 0:
+        G = rng.normal(0.0, sigma, size=(N, N))
+        H = H + (np.triu(G) + np.triu(G, 1).T)
+    return H
+
+
+def ellpack_from_dense(A, M, tol=0.0):
+    """Pack a dense matrix into ELLPACK-R keeping |a| > tol and the diagonal (ascending columns)."""
+    N = A.shape[0]
+    value = np.zeros((N, M), dtype=np.float64)
+    index = np.zeros((N, M), dtype=np.int32)
+    nnz = np.zeros(N, dtype=np.int32)
+    for i in range(N):
+        keep = np.abs(A[i]) > tol
+        keep[i] = True
+        c = np.nonzero(keep)[0]
+        assert c.size <= M, f"row {i} needs {c.size} > M={M}"
+        nnz[i] = c.size
+        index[i, : c.size] = c
+        value[i, : c.size] = A[i, c]
+    return value, index, nnz
+
+
+def ellpack_to_dense(value, index, nnz, N=None):
+    """Scatter an ELLPACK-R matrix into a dense array (test convenience)."""
+    n = value.shape[0] if N is None else N
+    M = value.shape[1]
+    D = np.zeros((n, n), dtype=np.float64)
+    mask = np.arange(M)[None, :] < np.asarray(nnz)[:, None]
+    rows = np.broadcast_to(np.arange(n)[:, None], (n, M))[mask]
+    D[rows, np.asarray(index)[mask]] = np.asarray(value)[mask]
+    return D
+
+
+# ----------------------------------------------------------------------------------------------
+# the BASELINE.json configs
+# ----------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class Workload:
+    name: str
+    kind: str  # "dense" | "ellpack"
+    N: int
+    n_occ: int
+    idem_tol: float
+    drop_tol: float = 0.0
+    precision: int = 0  # 0 = FP64, 1 = mixed
+    M: int = 0
+    lattice: tuple | None = None
+    note: str = ""
+
+
+WORKLOADS = {
+    # BASELINE.json configs[0]
+    "dense_n256": Workload("dense_n256", "dense", 256, 128, 1e-10, note="1D ring + dense Gaussian noise"),
+    # configs[1]
+    "dense_n2048": Workload("dense_n2048", "dense", 2048, 1024, 1e-10, lattice=(16, 16, 8), note="16x16x8, NN hopping"),
+    # configs[2]
+    "dense_n8192": Workload("dense_n8192", "dense", 8192, 4096, 1e-10, lattice=(32, 16, 16),
+                            note="32x16x16, -exp(-r/1.5), r<=6"),
+    # configs[3]
+    "mixed_n16384": Workload("mixed_n16384", "dense", 16384, 8192, 1e-6, precision=1, lattice=(32, 32, 16),
+                             note="32x32x16, -exp(-r/1.5), r<=6, mixed precision"),
+    # configs[4], literally as written (overflows M=512 at product 0 — SURVEY §8(d))
+    "ellpack_n65536_literal": Workload("ellpack_n65536_literal", "ellpack", 65536, 32768, 1e-8, 1e-6, M=512,
+                                       lattice=(64, 32, 32), note="64x32x32, -exp(-r/1.0), r<=3, delta=1.5"),
+    # configs[4] labelled fallback 5': delta=12, hopping -exp(-r/0.5); same N, stencil, M, tau
+    "ellpack_n65536": Workload("ellpack_n65536", "ellpack", 65536, 32768, 1e-8, 1e-6, M=512,
+                               lattice=(64, 32, 32), note="5' fallback: 64x32x32, -exp(-r/0.5), r<=3, delta=12"),
+}
+
+
+def make_dense(name: str, seed: int = 0) -> np.ndarray:
+    w = WORKLOADS[name]
+    if name == "dense_n256":
+        return ring_dense(256, 1.5, 0.1, 1e-3, seed)
+    if name == "dense_n2048":
+        return lattice_dense(w.lattice, 1.5, 0.2, 1.0, lambda r: -1.0, seed)
+    if name in ("dense_n8192", "mixed_n16384"):
+        return lattice_dense(w.lattice, 1.5, 0.2, 6.0, lambda r: -math.exp(-r / 1.5), seed)
+    raise KeyError(name)
+
+
+def make_ellpack(name: str, seed: int = 0):
+    w = WORKLOADS[name]
+    if name == "ellpack_n65536_literal":
+        return lattice_ellpack(w.lattice, 1.5, 0.2, 3.0, lambda r: -math.exp(-r / 1.0), w.M, seed)
+    if name == "ellpack_n65536":
+        return lattice_ellpack(w.lattice, 12.0, 0.2, 3.0, lambda r: -math.exp(-r / 0.5), w.M, seed)
+    raise KeyError(name)
+
+
+def small_long_range(L=(8, 8, 6), seed=0, rmax=3.0, decay=1.5, delta=1.5, noise=0.2):
+    """Reduced-size stand-in of the config-3/4 model for parity tests the oracle finishes in seconds."""
+    return lattice_dense(L, delta, noise, rmax, lambda r: -math.exp(-r / decay), seed)
+
+
+def small_sparse_model(L=(12, 10, 8), seed=0, M=512, delta=12.0, decay=0.5, rmax=3.0):
+    """Reduced-size stand-in of the 5' ELLPACK model."""
+    return lattice_ellpack(L, delta, 0.2, rmax, lambda r: -math.exp(-r / decay), M, seed)
+
+
+def planted_gap(N, n_occ, gap=1.0, width=1.0, seed=0):
+    """Random dense symmetric H = Q diag(eps) Q^T with n_occ levels in [-gap/2-width, -gap/2] and the rest in
+    [gap/2, gap/2+width]; Q from QR of a Gaussian matrix.  Returns (H, eps sorted ascending)."""
+    rng = np.random.default_rng(seed)
+    lo = -gap / 2 - width * rng.uniform(0, 1, size=n_occ)
+    hi = gap / 2 + width * rng.uniform(0, 1, size=N - n_occ)
+    eps = np.sort(np.concatenate([lo, hi]))
+    Q, _ = np.linalg.qr(rng.normal(size=(N, N)))
+    H = (Q * eps) @ Q.T
+    H = np.triu(H) + np.triu(H, 1).T  # bitwise symmetric
+    return H, eps
