@@ -1,0 +1,346 @@
+"""Thin ctypes binding of libbmlsp2.so (include/bml_sp2.h) — argument marshalling only.
+
+Every function has the name of the C entry point it calls and takes torch CUDA tensors for device memory; all
+arithmetic of the method runs in the library's sm_100a kernels.  There is no CPU fallback: if the library is missing
+or a tensor is not on a CUDA device this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass, field
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+LOG_LEN = 128
+ELL_MAX_M = 1024
+ELL_ACC_SLOTS = 4096
+BML_DENSE, BML_ELLPACK = 0, 1
+FLAG_CHECK_SYMMETRY = 1
+
+EXPORTS = [
+    "bml_version", "bml_status_string", "bml_gershgorin_workspace_bytes", "bml_gershgorin", "bml_trace",
+    "bml_sp2_workspace_bytes", "bml_sp2_dense", "bml_sp2_ellpack", "bml_x2_dense_workspace_bytes", "bml_x2_dense",
+    "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_probe_fp64_tensor_peak",
+]
+
+
+class bml_matrix_t(ctypes.Structure):
+    _fields_ = [
+        ("type", ctypes.c_int32),
+        ("M", ctypes.c_int32),
+        ("N", ctypes.c_int64),
+        ("ld", ctypes.c_int64),
+        ("value", ctypes.c_void_p),
+        ("index", ctypes.c_void_p),
+        ("nnz", ctypes.c_void_p),
+    ]
+
+
+class bml_sp2_params_t(ctypes.Structure):
+    _fields_ = [
+        ("n_occ", ctypes.c_int32),
+        ("max_products", ctypes.c_int32),
+        ("idem_tol", ctypes.c_double),
+        ("drop_tol", ctypes.c_double),
+        ("precision", ctypes.c_int32),
+        ("flags", ctypes.c_uint32),
+    ]
+
+
+class bml_sp2_stats_t(ctypes.Structure):
+    _fields_ = [
+        ("status", ctypes.c_int32),
+        ("n_products", ctypes.c_int32),
+        ("m_star", ctypes.c_int32),
+        ("overflow_row", ctypes.c_int32),
+        ("emin", ctypes.c_double),
+        ("emax", ctypes.c_double),
+        ("branch", ctypes.c_uint8 * LOG_LEN),
+        ("trace", ctypes.c_double * LOG_LEN),
+        ("idem", ctypes.c_double * LOG_LEN),
+        ("max_row_nnz", ctypes.c_int32 * LOG_LEN),
+    ]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB_PATH
+
+
+def load(build_if_missing: bool = True):
+    """dlopen libbmlsp2.so (building it with nvcc first if it is absent or stale) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build() if build_if_missing else _build.LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: run `python -m paper_2401_13772_b200.build` (there is no CPU fallback)")
+    L = ctypes.CDLL(path)
+    vp, sz, i32, i64, dbl = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+    MP, PP, SP = ctypes.POINTER(bml_matrix_t), ctypes.POINTER(bml_sp2_params_t), ctypes.POINTER(bml_sp2_stats_t)
+    L.bml_version.restype = ctypes.c_char_p
+    L.bml_status_string.restype = ctypes.c_char_p
+    L.bml_status_string.argtypes = [ctypes.c_int]
+    L.bml_gershgorin_workspace_bytes.restype = sz
+    L.bml_gershgorin_workspace_bytes.argtypes = [i64]
+    L.bml_gershgorin.restype = ctypes.c_int
+    L.bml_gershgorin.argtypes = [MP, vp, vp, sz, vp]
+    L.bml_trace.restype = ctypes.c_int
+    L.bml_trace.argtypes = [MP, vp, vp]
+    L.bml_sp2_workspace_bytes.restype = sz
+    L.bml_sp2_workspace_bytes.argtypes = [MP, PP]
+    for name in ("bml_sp2_dense", "bml_sp2_ellpack"):
+        f = getattr(L, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [MP, PP, MP, vp, sz, SP, vp]
+    L.bml_x2_dense_workspace_bytes.restype = sz
+    L.bml_x2_dense_workspace_bytes.argtypes = [i64, i32]
+    L.bml_x2_dense.restype = ctypes.c_int
+    L.bml_x2_dense.argtypes = [MP, MP, i32, i32, vp, vp, sz, vp]
+    L.bml_x2_ellpack_workspace_bytes.restype = sz
+    L.bml_x2_ellpack_workspace_bytes.argtypes = [i64]
+    L.bml_x2_ellpack.restype = ctypes.c_int
+    L.bml_x2_ellpack.argtypes = [MP, MP, i32, dbl, vp, vp, vp, sz, vp]
+    L.bml_probe_fp64_tensor_peak.restype = ctypes.c_int
+    L.bml_probe_fp64_tensor_peak.argtypes = [i32, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
+    _lib = L
+    return L
+
+
+def bml_version() -> str:
+    return load().bml_version().decode()
+
+
+def bml_status_string(status: int) -> str:
+    return load().bml_status_string(int(status)).decode()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# marshalling helpers
+# ------------------------------------------------------------------------------------------------------------
+def _require_cuda(t: torch.Tensor, dtype, what: str):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise RuntimeError(f"{what}: expected a CUDA tensor (libbmlsp2 has no CPU path)")
+    if t.dtype != dtype:
+        raise TypeError(f"{what}: expected {dtype}, got {t.dtype}")
+
+
+def _stream() -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def dense_desc(A: torch.Tensor) -> bml_matrix_t:
+    """Descriptor of a row-major 2-D float64 CUDA tensor (rows may be strided: ld = A.stride(0))."""
+    _require_cuda(A, torch.float64, "dense matrix")
+    if A.dim() != 2 or A.shape[0] != A.shape[1] or A.stride(1) != 1:
+        raise ValueError("dense matrix must be square, row-major with unit column stride")
+    return bml_matrix_t(BML_DENSE, 0, A.shape[0], A.stride(0), A.data_ptr(), None, None)
+
+
+def ellpack_desc(value: torch.Tensor, index: torch.Tensor, nnz: torch.Tensor) -> bml_matrix_t:
+    _require_cuda(value, torch.float64, "ellpack value")
+    _require_cuda(index, torch.int32, "ellpack index")
+    _require_cuda(nnz, torch.int32, "ellpack nnz")
+    if value.dim() != 2 or index.shape != value.shape or nnz.shape != (value.shape[0],):
+        raise ValueError("ellpack: value[N,M], index[N,M], nnz[N] expected")
+    if not (value.is_contiguous() and index.is_contiguous() and nnz.is_contiguous()):
+        raise ValueError("ellpack arrays must be contiguous")
+    N, M = value.shape
+    return bml_matrix_t(BML_ELLPACK, M, N, 0, value.data_ptr(), index.data_ptr(), nnz.data_ptr())
+
+
+def _workspace(nbytes: int, device) -> torch.Tensor:
+    # torch's caching allocator returns 512-byte aligned blocks; over-allocate and slice to a 1024-byte boundary
+    raw = torch.empty(int(nbytes) + 1024, dtype=torch.uint8, device=device)
+    off = (-raw.data_ptr()) % 1024
+    return raw[off:off + int(nbytes)]
+
+
+@dataclass
+class Sp2Result:
+    status: int
+    n_products: int
+    m_star: int
+    overflow_row: int
+    emin: float
+    emax: float
+    branch: str
+    trace: np.ndarray
+    idem: np.ndarray
+    max_row_nnz: np.ndarray
+    message: str = field(default="")
+
+
+def _result(st: bml_sp2_stats_t, rc: int) -> Sp2Result:
+    n = max(int(st.n_products), 0)
+    m = max(int(st.m_star), 0)
+    nb = m
+    return Sp2Result(
+        status=int(rc), n_products=n, m_star=int(st.m_star), overflow_row=int(st.overflow_row),
+        emin=float(st.emin), emax=float(st.emax),
+        branch="".join(str(int(b)) for b in st.branch[:nb]),
+        trace=np.array(st.trace[:n]), idem=np.array(st.idem[:n]), max_row_nnz=np.array(st.max_row_nnz[:n]),
+        message=bml_status_string(rc),
+    )
+
+
+# ------------------------------------------------------------------------------------------------------------
+# entry points (same names as the C ABI)
+# ------------------------------------------------------------------------------------------------------------
+def bml_gershgorin(H, out: torch.Tensor | None = None) -> torch.Tensor:
+    """H: dense tensor or (value, index, nnz).  Returns a CUDA float64 tensor [e_min, e_max] (asynchronous)."""
+    L = load()
+    desc = dense_desc(H) if isinstance(H, torch.Tensor) else ellpack_desc(*H)
+    dev = H.device if isinstance(H, torch.Tensor) else H[0].device
+    if out is None:
+        out = torch.empty(2, dtype=torch.float64, device=dev)
+    nbytes = L.bml_gershgorin_workspace_bytes(desc.N)
+    ws = torch.empty(max(nbytes, 8), dtype=torch.uint8, device=dev)
+    rc = L.bml_gershgorin(ctypes.byref(desc), out.data_ptr(), ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_gershgorin: {bml_status_string(rc)}")
+    return out
+
+
+def bml_trace(A, out: torch.Tensor | None = None) -> torch.Tensor:
+    L = load()
+    desc = dense_desc(A) if isinstance(A, torch.Tensor) else ellpack_desc(*A)
+    dev = A.device if isinstance(A, torch.Tensor) else A[0].device
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=dev)
+    rc = L.bml_trace(ctypes.byref(desc), out.data_ptr(), _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_trace: {bml_status_string(rc)}")
+    return out
+
+
+class DenseSolver:
+    """Pre-allocated buffers for repeated bml_sp2_dense calls on one problem size (bench.py's timed loop)."""
+
+    def __init__(self, N: int, device="cuda", precision: int = 0):
+        L = load()
+        self.N, self.precision = int(N), int(precision)
+        self.device = torch.device(device)
+        self.D = torch.empty((N, N), dtype=torch.float64, device=self.device)
+        d = bml_matrix_t(BML_DENSE, 0, N, N, None, None, None)
+        p = bml_sp2_params_t(1, 1, 1.0, 0.0, precision, 0)
+        self.ws_bytes = L.bml_sp2_workspace_bytes(ctypes.byref(d), ctypes.byref(p))
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, H: torch.Tensor, n_occ: int, idem_tol: float, max_products: int = 100, flags: int = 0):
+        L = load()
+        h, d = dense_desc(H), dense_desc(self.D)
+        p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), 0.0, self.precision, int(flags))
+        st = bml_sp2_stats_t()
+        rc = L.bml_sp2_dense(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
+                             ctypes.byref(st), _stream())
+        return self.D, _result(st, rc)
+
+
+def bml_sp2_dense(H: torch.Tensor, n_occ: int, idem_tol: float, max_products: int = 100, precision: int = 0,
+                  flags: int = 0):
+    """Dense SP2.  Returns (D CUDA tensor, Sp2Result)."""
+    _require_cuda(H, torch.float64, "H")
+    return DenseSolver(H.shape[0], H.device, precision).solve(H, n_occ, idem_tol, max_products, flags)
+
+
+class EllpackSolver:
+    def __init__(self, N: int, M: int, device="cuda"):
+        L = load()
+        self.N, self.M = int(N), int(M)
+        self.device = torch.device(device)
+        self.dv = torch.zeros((N, M), dtype=torch.float64, device=self.device)
+        self.di = torch.zeros((N, M), dtype=torch.int32, device=self.device)
+        self.dn = torch.zeros((N,), dtype=torch.int32, device=self.device)
+        d = bml_matrix_t(BML_ELLPACK, M, N, 0, None, None, None)
+        self.ws_bytes = L.bml_sp2_workspace_bytes(ctypes.byref(d), None)
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+        L = load()
+        h = ellpack_desc(value, index, nnz)
+        d = ellpack_desc(self.dv, self.di, self.dn)
+        p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), float(drop_tol), 0, 0)
+        st = bml_sp2_stats_t()
+        rc = L.bml_sp2_ellpack(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
+                               ctypes.byref(st), _stream())
+        return (self.dv, self.di, self.dn), _result(st, rc)
+
+
+def bml_sp2_ellpack(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+    """Sparse thresholded SP2 on ELLPACK-R.  Returns ((value, index, nnz) CUDA tensors of D, Sp2Result)."""
+    _require_cuda(value, torch.float64, "value")
+    return EllpackSolver(value.shape[0], value.shape[1], value.device).solve(value, index, nnz, n_occ, idem_tol,
+                                                                           drop_tol, max_products)
+
+
+def padded_ld(N: int) -> int:
+    return (int(N) + 15) // 16 * 16
+
+
+def bml_x2_dense(X: torch.Tensor, branch: int, precision: int = 0, Xnext: torch.Tensor | None = None, ws=None):
+    """One fused product on a padded iterate (ld multiple of 16).  Returns (Xnext, sums[4] CUDA tensor)."""
+    L = load()
+    x = dense_desc(X)
+    if Xnext is None:
+        Xnext = torch.empty_strided(X.shape, X.stride(), dtype=X.dtype, device=X.device)
+    xn = dense_desc(Xnext)
+    sums = torch.empty(4, dtype=torch.float64, device=X.device)
+    nbytes = L.bml_x2_dense_workspace_bytes(x.N, precision)
+    if ws is None:
+        ws = _workspace(nbytes, X.device)
+    rc = L.bml_x2_dense(ctypes.byref(x), ctypes.byref(xn), int(branch), int(precision), sums.data_ptr(),
+                        ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_x2_dense: {bml_status_string(rc)}")
+    return Xnext, sums
+
+
+def padded_dense(A: np.ndarray | torch.Tensor, device="cuda") -> torch.Tensor:
+    """Copy a square matrix into a zero-padded CUDA buffer with ld = padded_ld(N), 128-byte aligned; returns the
+    N x N view (stride ld)."""
+    A = torch.as_tensor(A, dtype=torch.float64)
+    N = A.shape[0]
+    ld = padded_ld(N)
+    raw = torch.zeros(N * ld + 16, dtype=torch.float64, device=device)
+    off = ((-raw.data_ptr()) % 128) // 8
+    buf = raw[off:off + N * ld].view(N, ld)
+    buf[:, :N].copy_(A)
+    return buf[:, :N]
+
+
+def bml_x2_ellpack(X, branch: int, drop_tol: float, out=None, ws=None):
+    """One fused thresholded product on ELLPACK-R rows in ascending column order.
+    Returns ((value, index, nnz), sums[4], info[4]) — all CUDA tensors."""
+    L = load()
+    value, index, nnz = X
+    x = ellpack_desc(value, index, nnz)
+    if out is None:
+        out = (torch.zeros_like(value), torch.zeros_like(index), torch.zeros_like(nnz))
+    o = ellpack_desc(*out)
+    sums = torch.empty(4, dtype=torch.float64, device=value.device)
+    info = torch.empty(4, dtype=torch.int32, device=value.device)
+    nbytes = L.bml_x2_ellpack_workspace_bytes(x.N)
+    if ws is None:
+        ws = _workspace(nbytes, value.device)
+    rc = L.bml_x2_ellpack(ctypes.byref(x), ctypes.byref(o), int(branch), float(drop_tol), sums.data_ptr(),
+                          info.data_ptr(), ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_x2_ellpack: {bml_status_string(rc)}")
+    return out, sums, info
+
+
+def bml_probe_fp64_tensor_peak(iters: int = 20000) -> float:
+    """FP64 tensor-pipe (DMMA) issue peak in TFLOP/s at the clocks of this run."""
+    L = load()
+    flops, ms = ctypes.c_double(), ctypes.c_double()
+    rc = L.bml_probe_fp64_tensor_peak(int(iters), ctypes.byref(flops), ctypes.byref(ms), _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_probe_fp64_tensor_peak: {bml_status_string(rc)}")
+    return flops.value / (ms.value * 1e-3) / 1e12

@@ -1,0 +1,357 @@
+// api.cu -- the C ABI of include/bml_sp2.h: argument checks, workspace carving, launch sequences.
+// No step of the method runs on the host; the host only enqueues kernels and reads the control block back once.
+#include <string.h>
+
+#include "common.cuh"
+
+namespace bmlsp2 {
+
+// dense_fp64.cu
+int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld);
+int dense_fp64_num_tiles(int64_t N);
+int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
+                         int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream);
+// dense_mixed.cu
+size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx);
+int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, double *X0, double *X1, int64_t ldx,
+                          Sp2Ctl *ctl, double *partials, const double *d_bounds, void *extra, cudaStream_t st);
+int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, Sp2Ctl *ctl, double *partials, void *extra,
+                        cudaStream_t st);
+// reductions.cu
+int launch_gershgorin(const bml_matrix_t *H, double *d_bounds, double *rowlh, cudaStream_t st);
+int launch_trace_dense(const double *A, int64_t ld, int N, double *d_out, cudaStream_t st);
+int launch_trace_ellpack(const bml_matrix_t *A, double *d_out, cudaStream_t st);
+int launch_rescale_dense(const bml_matrix_t *H, const double *d_bounds, double *X, int64_t ldx, cudaStream_t st);
+int launch_check_symmetry(const bml_matrix_t *H, int *d_flag, cudaStream_t st);
+int launch_init_ctl(Sp2Ctl *ctl, const double *d_bounds, const double *d_tr0, int n_occ, int max_products,
+                    double idem_tol, int loop_mode, int branch0, const int *fail_flag, cudaStream_t st);
+int launch_copy_out_dense(const double *buf0, const double *buf1, int64_t ldx, int N, const Sp2Ctl *ctl, double *D,
+                          int64_t ldd, cudaStream_t st);
+// ellpack.cu
+size_t ellpack_rowstats_bytes(int64_t N);
+int launch_rescale_ellpack(const bml_matrix_t *H, const double *d_bounds, double *xv, int32_t *xi, int32_t *xn,
+                           double *rowstats, double *d_tr0, int *fail_flag, cudaStream_t st);
+int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, double *v1, int32_t *i1, int32_t *n1,
+                      int64_t N, int M, double tau, Sp2Ctl *ctl, double *rowstats, cudaStream_t st);
+int launch_copy_out_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, const double *v1,
+                            const int32_t *i1, const int32_t *n1, int64_t N, int M, const Sp2Ctl *ctl, double *dv,
+                            int32_t *di, int32_t *dn, cudaStream_t st);
+int launch_x2_ellpack_info(const Sp2Ctl *ctl, int32_t *d_info, cudaStream_t st);
+// probe.cu
+int run_fp64_tensor_probe(int iters, double *flops, double *ms, cudaStream_t st);
+
+PFN_encodeTiled get_encode_tiled()
+{
+    static PFN_encodeTiled fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (PFN_encodeTiled)p;
+    }
+    return fn;
+}
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int64_t padded_ld(int64_t N) { return (N + 15) / 16 * 16; }
+
+constexpr size_t CTL_BYTES = 4096;      // Sp2Ctl
+constexpr size_t SCAL_BYTES = 256;      // bounds[2], tr0, flags
+static_assert(sizeof(Sp2Ctl) <= CTL_BYTES, "control block does not fit its slot");
+
+struct ScalarSlots {
+    double bounds[2];
+    double tr0;
+    double pad;
+    int32_t fail_flag[4];
+};
+static_assert(sizeof(ScalarSlots) <= SCAL_BYTES, "scalar slots");
+
+struct DenseWs {
+    Sp2Ctl *ctl;
+    ScalarSlots *scal;
+    double *rowlh, *partials, *X0, *X1;
+    void *extra;
+    int64_t ldx;
+    size_t total;
+};
+
+static DenseWs carve_dense(void *ws, int64_t N, int precision)
+{
+    DenseWs w;
+    uint8_t *p = (uint8_t *)ws;
+    size_t off = 0;
+    w.ctl = (Sp2Ctl *)(p + off); off += CTL_BYTES;
+    w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
+    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
+    w.partials = (double *)(p + off);
+    off = align_up(off + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
+    w.ldx = padded_ld(N);
+    w.X0 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
+    w.X1 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
+    w.extra = (void *)(p + off);
+    if (precision == 1) off = align_up(off + dense_mixed_extra_bytes(N, w.ldx), 1024);
+    w.total = off;
+    return w;
+}
+
+struct EllWs {
+    Sp2Ctl *ctl;
+    ScalarSlots *scal;
+    double *rowlh, *rowstats;
+    double *v0, *v1;
+    int32_t *i0, *i1, *n0, *n1;
+    size_t total;
+};
+
+static EllWs carve_ell(void *ws, int64_t N, int M, bool with_buffers)
+{
+    EllWs w;
+    uint8_t *p = (uint8_t *)ws;
+    size_t off = 0;
+    w.ctl = (Sp2Ctl *)(p + off); off += CTL_BYTES;
+    w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
+    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
+    w.rowstats = (double *)(p + off); off = align_up(off + ellpack_rowstats_bytes(N), 1024);
+    w.v0 = w.v1 = nullptr; w.i0 = w.i1 = w.n0 = w.n1 = nullptr;
+    if (with_buffers) {
+        const size_t nm = (size_t)N * (size_t)M;
+        w.v0 = (double *)(p + off); off = align_up(off + nm * 8, 1024);
+        w.v1 = (double *)(p + off); off = align_up(off + nm * 8, 1024);
+        w.i0 = (int32_t *)(p + off); off = align_up(off + nm * 4, 1024);
+        w.i1 = (int32_t *)(p + off); off = align_up(off + nm * 4, 1024);
+        w.n0 = (int32_t *)(p + off); off = align_up(off + (size_t)N * 4, 1024);
+        w.n1 = (int32_t *)(p + off); off = align_up(off + (size_t)N * 4, 1024);
+    }
+    w.total = off;
+    return w;
+}
+
+static bool dense_ok(const bml_matrix_t *A)
+{
+    return A && A->type == BML_DENSE && A->value && A->N > 0 && A->N <= 0x3fffffff && A->ld >= A->N;
+}
+static bool ell_ok(const bml_matrix_t *A)
+{
+    return A && A->type == BML_ELLPACK && A->value && A->index && A->nnz && A->N > 0 && A->N < (1 << 29) - 1 &&
+           A->M >= 1 && A->M <= BML_ELL_MAX_M;
+}
+static bool params_ok(const bml_sp2_params_t *p, int64_t N)
+{
+    return p && p->n_occ > 0 && (int64_t)p->n_occ < N && p->idem_tol > 0.0 && p->max_products >= 1 &&
+           p->max_products <= BML_SP2_LOG_LEN && p->drop_tol >= 0.0 && (p->precision == 0 || p->precision == 1);
+}
+
+static void fill_stats(bml_sp2_stats_t *stats, const Sp2Ctl &c)
+{
+    if (!stats) return;
+    memset(stats, 0, sizeof(*stats));
+    stats->status = c.status;
+    stats->m_star = c.m;
+    stats->n_products = c.n_done;
+    stats->overflow_row = c.fail_row;
+    stats->emin = c.emin;
+    stats->emax = c.emax;
+    memcpy(stats->branch, c.branch, sizeof(c.branch));
+    memcpy(stats->trace, c.trace, sizeof(c.trace));
+    memcpy(stats->idem, c.idem, sizeof(c.idem));
+    memcpy(stats->max_row_nnz, c.max_row_nnz, sizeof(c.max_row_nnz));
+}
+
+static int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
+{
+    Sp2Ctl h;
+    if (cudaMemcpyAsync(&h, d_ctl, sizeof(Sp2Ctl), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return BML_ERR_CUDA;
+    if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
+    fill_stats(stats, h);
+    return h.status;
+}
+
+}  // namespace bmlsp2
+
+using namespace bmlsp2;
+
+#define TRY(x) do { int _r = (x); if (_r != 0) { if (stats) { memset(stats, 0, sizeof(*stats)); stats->status = _r; stats->overflow_row = -1; } return _r; } } while (0)
+
+extern "C" {
+
+const char *bml_version(void) { return "0.1.0 (sm_100a)"; }
+
+const char *bml_status_string(int status)
+{
+    switch (status) {
+        case BML_OK: return "converged (S1: e_m < idem_tol)";
+        case BML_NOISE_FLOOR: return "stopped on the noise floor (S2); D valid, tolerance not reached";
+        case BML_MAX_PRODUCTS: return "max_products reached (S3); not converged";
+        case BML_ERR_INVALID: return "invalid argument";
+        case BML_ERR_DEGENERATE: return "degenerate spectral bounds (e_max - e_min <= 0)";
+        case BML_ERR_ELL_OVERFLOW: return "ELLPACK-R overflow: a row needs more than M slots";
+        case BML_ERR_CUDA: return "CUDA error";
+        case BML_ERR_NOT_SYMMETRIC: return "H is not symmetric";
+        case BML_ERR_ACC_CAPACITY: return "ELLPACK X^2 accumulator capacity exceeded";
+        default: return "unknown status";
+    }
+}
+
+size_t bml_gershgorin_workspace_bytes(int64_t N) { return N > 0 ? (size_t)2 * (size_t)N * sizeof(double) : 0; }
+
+int bml_gershgorin(const bml_matrix_t *H, double *d_bounds, void *d_workspace, size_t workspace_bytes,
+                   void *cuda_stream)
+{
+    if (!H || !d_bounds || !d_workspace) return BML_ERR_INVALID;
+    if (!(H->type == BML_DENSE ? dense_ok(H) : ell_ok(H))) return BML_ERR_INVALID;
+    if (workspace_bytes < bml_gershgorin_workspace_bytes(H->N)) return BML_ERR_INVALID;
+    return launch_gershgorin(H, d_bounds, (double *)d_workspace, (cudaStream_t)cuda_stream);
+}
+
+int bml_trace(const bml_matrix_t *A, double *d_trace, void *cuda_stream)
+{
+    if (!A || !d_trace) return BML_ERR_INVALID;
+    if (A->type == BML_DENSE) {
+        if (!dense_ok(A)) return BML_ERR_INVALID;
+        return launch_trace_dense(A->value, A->ld, (int)A->N, d_trace, (cudaStream_t)cuda_stream);
+    }
+    if (!ell_ok(A)) return BML_ERR_INVALID;
+    return launch_trace_ellpack(A, d_trace, (cudaStream_t)cuda_stream);
+}
+
+size_t bml_sp2_workspace_bytes(const bml_matrix_t *H, const bml_sp2_params_t *p)
+{
+    if (!H || H->N <= 0) return 0;
+    if (H->type == BML_DENSE) return carve_dense(nullptr, H->N, p ? p->precision : 0).total;
+    if (H->M < 1) return 0;
+    return carve_ell(nullptr, H->N, H->M, true).total;
+}
+
+int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,
+                  size_t workspace_bytes, bml_sp2_stats_t *stats, void *cuda_stream)
+{
+    if (!dense_ok(H) || !dense_ok(D) || D->N != H->N || !params_ok(p, H->N) || !d_workspace ||
+        D->value == H->value || ((uintptr_t)d_workspace & 1023) != 0)
+        TRY(BML_ERR_INVALID);
+    const int64_t N = H->N;
+    DenseWs w = carve_dense(d_workspace, N, p->precision);
+    if (workspace_bytes < w.total) TRY(BML_ERR_INVALID);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
+    TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // D0
+    if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) TRY(launch_check_symmetry(H, w.scal->fail_flag, st));
+    TRY(launch_rescale_dense(H, w.scal->bounds, w.X0, w.ldx, st));                            // D1
+    TRY(launch_trace_dense(w.X0, w.ldx, (int)N, &w.scal->tr0, st));
+    TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
+                        w.scal->fail_flag, st));
+    if (p->precision == 1) {
+        TRY(sp2_dense_mixed_solve(H, p, w.X0, w.X1, w.ldx, w.ctl, w.partials, w.scal->bounds, w.extra, st));
+    } else {
+        CUtensorMap map0, map1;
+        TRY(make_dense_map(&map0, w.X0, N, w.ldx));
+        TRY(make_dense_map(&map1, w.X1, N, w.ldx));
+        // D2-D5: every product is enqueued up front; launches after the stop rule fired exit at once
+        for (int l = 0; l < p->max_products; ++l)
+            TRY(launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, st));
+    }
+    TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
+    return finish_solve(w.ctl, stats, st);
+}
+
+size_t bml_x2_dense_workspace_bytes(int64_t N, int32_t precision)
+{
+    if (N <= 0) return 0;
+    size_t off = CTL_BYTES;
+    off = align_up(off + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
+    if (precision == 1) off = align_up(off + dense_mixed_extra_bytes(N, padded_ld(N)), 1024);
+    return off;
+}
+
+int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int32_t precision, double *d_sums,
+                 void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!dense_ok(X) || !dense_ok(Xnext) || X->N != Xnext->N || X->ld != Xnext->ld || (X->ld % 16) != 0 ||
+        ((uintptr_t)X->value & 127) != 0 || ((uintptr_t)Xnext->value & 127) != 0 || X->value == Xnext->value ||
+        !d_sums || !d_workspace || ((uintptr_t)d_workspace & 1023) != 0 || (precision != 0 && precision != 1) ||
+        workspace_bytes < bml_x2_dense_workspace_bytes(X->N, precision))
+        return BML_ERR_INVALID;
+    const int64_t N = X->N;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint8_t *p = (uint8_t *)d_workspace;
+    Sp2Ctl *ctl = (Sp2Ctl *)p;
+    double *partials = (double *)(p + CTL_BYTES);
+    void *extra = p + align_up(CTL_BYTES + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
+    int r = launch_init_ctl(ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
+    if (r) return r;
+    if (precision == 1) {
+        r = x2_dense_mixed_once(X, Xnext, ctl, partials, extra, st);
+    } else {
+        CUtensorMap map0, map1;
+        if ((r = make_dense_map(&map0, X->value, N, X->ld))) return r;
+        if ((r = make_dense_map(&map1, Xnext->value, N, X->ld))) return r;
+        r = launch_x2_dense_fp64(map0, map1, X->value, Xnext->value, X->ld, N, ctl, partials, st);
+    }
+    if (r) return r;
+    if (cudaMemcpyAsync(d_sums, ctl->sums, 4 * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    return 0;
+}
+
+int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,
+                    size_t workspace_bytes, bml_sp2_stats_t *stats, void *cuda_stream)
+{
+    if (!ell_ok(H) || !ell_ok(D) || D->N != H->N || D->M != H->M || !params_ok(p, H->N) || p->precision != 0 ||
+        !d_workspace || D->value == H->value || D->index == H->index || D->nnz == H->nnz ||
+        ((uintptr_t)d_workspace & 1023) != 0)
+        TRY(BML_ERR_INVALID);
+    const int64_t N = H->N;
+    const int M = H->M;
+    EllWs w = carve_ell(d_workspace, N, M, true);
+    if (workspace_bytes < w.total) TRY(BML_ERR_INVALID);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
+    TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // S0
+    TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowstats, &w.scal->tr0, w.scal->fail_flag, st));
+    TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
+                        w.scal->fail_flag, st));
+    for (int l = 0; l < p->max_products; ++l)                                                 // S2-S5
+        TRY(launch_x2_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, p->drop_tol, w.ctl, w.rowstats, st));
+    TRY(launch_copy_out_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, w.ctl, D->value, D->index, D->nnz, st));
+    return finish_solve(w.ctl, stats, st);
+}
+
+size_t bml_x2_ellpack_workspace_bytes(int64_t N)
+{
+    if (N <= 0) return 0;
+    return carve_ell(nullptr, N, 1, false).total;
+}
+
+int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, double drop_tol, double *d_sums,
+                   int32_t *d_info, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!ell_ok(X) || !ell_ok(Xnext) || X->N != Xnext->N || X->M != Xnext->M || X->value == Xnext->value ||
+        X->index == Xnext->index || X->nnz == Xnext->nnz || !d_sums || !d_info || !d_workspace ||
+        ((uintptr_t)d_workspace & 1023) != 0 || !(drop_tol >= 0.0) ||
+        workspace_bytes < bml_x2_ellpack_workspace_bytes(X->N))
+        return BML_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    EllWs w = carve_ell(d_workspace, X->N, X->M, false);
+    int r = launch_init_ctl(w.ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
+    if (r) return r;
+    r = launch_x2_ellpack(X->value, X->index, X->nnz, Xnext->value, Xnext->index, Xnext->nnz, X->N, X->M, drop_tol,
+                          w.ctl, w.rowstats, st);
+    if (r) return r;
+    if (cudaMemcpyAsync(d_sums, w.ctl->sums, 4 * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    return launch_x2_ellpack_info(w.ctl, d_info, st);
+}
+
+int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream)
+{
+    if (iters < 1 || !flops_out || !ms_out) return BML_ERR_INVALID;
+    return run_fp64_tensor_probe(iters, flops_out, ms_out, (cudaStream_t)cuda_stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,242 @@
+// dense_fp64.cu -- steps D3 + D4 + D5 of DESIGN.md: the fused FP64 symmetric-square kernel.
+//
+//   P_IJ = sum_K X_IK * X_JK^T      (X symmetric, so X^2 = X X^T: both operands are ROW panels of X, K-contiguous)
+//   only tiles I <= J are computed; the epilogue applies Eq. 6 / Eq. 7, accumulates tr P, ||P - X||_F^2,
+//   ||X||_F^2, tr X', and writes X'_IJ and its mirror X'_JI.  The last CTA reduces the per-tile partial sums in a
+//   fixed order and runs the stop rules / next branch bit on the device (no host round trip, P:201-208 done on-chip).
+//
+// Pipeline: one producer thread issues TMA (cp.async.bulk.tensor, 128B swizzle, FP64 tensor map) into a STAGES-deep
+// ring of { A panel 128 x 16, B panel 128 x 16 } tiles guarded by full/empty mbarriers; 8 consumer warps (2 x 4, warp
+// tile 64 x 32) read fragments with conflict-free LDS.64 and issue mma.sync m8n8k4 f64 (SASS DMMA.8x8x4).
+#include "common.cuh"
+
+namespace bmlsp2 {
+
+constexpr int D_BM = 128;          // tile rows (I panel)
+constexpr int D_BN = 128;          // tile cols (J panel)
+constexpr int D_BK = 16;           // k-slab: 16 doubles = 128 B = one SWIZZLE_128B row
+constexpr int D_STAGES = 6;        // 6 x 32 KB = 192 KB
+constexpr int D_CONSUMER_WARPS = 8;
+constexpr int D_PRODUCER_WARPS = 4;     // one warpgroup, so that setmaxnreg can hand its registers to the consumers
+constexpr int D_THREADS = (D_PRODUCER_WARPS + D_CONSUMER_WARPS) * 32;   // 384: ptxas caps at 168 regs/thread ...
+constexpr int D_REGS_PRODUCER = 40;     // ... re-split by setmaxnreg: 128 x 40 + 256 x 232 = 64512 = 384 x 168
+constexpr int D_REGS_CONSUMER = 232;
+constexpr int D_PANEL_BYTES = D_BM * D_BK * 8;   // 16 KB
+constexpr int D_STAGE_BYTES = 2 * D_PANEL_BYTES;
+constexpr size_t D_SMEM_BYTES = (size_t)D_STAGES * D_STAGE_BYTES + 1024 /*align*/ + 512 /*barriers + reduction scratch*/;
+
+// MMA row/col index g (0..7) -> physical row inside an 8-row group.  With the 128B TMA swizzle (16-byte chunk c of
+// row r stored at chunk c ^ (r & 7)) the four rows touched by one half-warp of an LDS.64 fragment load must have
+// distinct (r >> 1) & 3 to hit 32 distinct banks: g = 0..3 -> rows 0,2,4,6 and g = 4..7 -> rows 1,3,5,7.
+__device__ __forceinline__ int perm8(int g) { return ((g & 3) << 1) | (g >> 2); }
+
+// linear tile id -> (I, J), I <= J, enumerated column by column: t = J (J + 1) / 2 + I
+__device__ __forceinline__ void tile_decode(int t, int &I, int &J)
+{
+    int j = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while ((j + 1) * (j + 2) / 2 <= t) ++j;
+    while (j * (j + 1) / 2 > t) --j;
+    J = j;
+    I = t - j * (j + 1) / 2;
+}
+
+__global__ void __launch_bounds__(D_THREADS, 1)
+x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
+                     double *__restrict__ buf0, double *__restrict__ buf1, int64_t ld, int N,
+                     Sp2Ctl *__restrict__ ctl, double *__restrict__ partials)
+{
+    // every CTA sees the control block written by the previous product's finaliser (kernel boundary orders it)
+    if (ctl->done) return;
+    const int parity = ctl->parity;
+    const int branch = ctl->branch_cur;
+    const CUtensorMap *map = parity ? &map1 : &map0;
+    const double *__restrict__ X = parity ? buf1 : buf0;
+    double *__restrict__ Xn = parity ? buf0 : buf1;
+
+    extern __shared__ uint8_t smem_raw[];
+    // SWIZZLE_128B tiles need 1024-byte alignment; pointer arithmetic (no integer round trip) keeps the shared
+    // address space visible to the compiler so fragment loads stay LDS
+    uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t *full_bar = (uint64_t *)(smem + (size_t)D_STAGES * D_STAGE_BYTES);
+    uint64_t *empty_bar = full_bar + D_STAGES;
+    double (*s_red)[4] = (double (*)[4])(empty_bar + D_STAGES);          // [D_CONSUMER_WARPS][4]
+    int *s_last = (int *)(s_red + D_CONSUMER_WARPS);
+
+    const int warp_all = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = warp_all - D_PRODUCER_WARPS;      // consumer warp index 0..7 (negative: producer warpgroup)
+    int I, J;
+    tile_decode((int)blockIdx.x, I, J);
+    const bool diag = (I == J);
+    const int KT = (N + D_BK - 1) / D_BK;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < D_STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], D_CONSUMER_WARPS); }
+        mbar_fence_init();
+        fence_proxy_async();
+    }
+    __syncthreads();
+
+    if (warp < 0) {
+        // ===================== TMA producer warpgroup (one elected lane works) =====================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(D_REGS_PRODUCER));
+        if (warp_all == 0 && lane == 0) {
+            tma_prefetch_desc(map);
+            const uint32_t tx = diag ? D_PANEL_BYTES : D_STAGE_BYTES;
+            for (int kt = 0; kt < KT; ++kt) {
+                const int s = kt % D_STAGES;
+                const uint32_t ph = (uint32_t)(kt / D_STAGES) & 1u;
+                mbar_wait(&empty_bar[s], ph ^ 1u);   // first pass over the ring: passes immediately
+                mbar_expect_tx(&full_bar[s], tx);
+                uint8_t *dst = smem + (size_t)s * D_STAGE_BYTES;
+                tma_load_2d(dst, map, kt * D_BK, I * D_BM, &full_bar[s]);
+                if (!diag) tma_load_2d(dst + D_PANEL_BYTES, map, kt * D_BK, J * D_BN, &full_bar[s]);
+            }
+        }
+        // producer warp falls through to the final reduction barrier
+    } else {
+        // ===================== DMMA consumers =====================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(D_REGS_CONSUMER));
+        const int wm = warp >> 2, wn = warp & 3;     // 2 x 4 warps; warp tile 64 x 32
+        const int g = lane >> 2, t = lane & 3;
+        const int pg = perm8(g);
+        double acc[8][4][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+
+        // byte offset of this lane's element inside a panel for k-step kk: row pg (+ 8-row groups via immediates)
+        uint32_t koff[4];
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+            koff[kk] = (uint32_t)(pg * 128 + ((((kk * 2 + (t >> 1)) ^ pg) << 4) | ((t & 1) << 3)));
+        const uint8_t *a_base = smem + wm * 64 * 128;
+        const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * 32 * 128;
+
+        for (int kt = 0; kt < KT; ++kt) {
+            const int s = kt % D_STAGES;
+            const uint32_t ph = (uint32_t)(kt / D_STAGES) & 1u;
+            mbar_wait(&full_bar[s], ph);
+            const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                double a[8], b[4];
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    a[i] = *(const double *)(sa + koff[kk] + i * 8 * 128);
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    b[j] = *(const double *)(sb + koff[kk] + j * 8 * 128);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[s]);
+        }
+
+        // ===================== fused epilogue (D4) =====================
+        // lane holds C[g][2t], C[g][2t+1] of each 8x8 fragment -> physical (row perm8(g), cols perm8(2t), perm8(2t+1))
+        const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
+        double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
+        const int row0 = I * D_BM + wm * 64 + pg;
+        const int col0 = J * D_BN + wn * 32;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int r = row0 + i * 8;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int c = col0 + j * 8 + (h ? pc1 : pc0);
+                    // diagonal tiles: only the upper triangle (r <= c) is used and mirrored -> X' is bitwise symmetric
+                    if (r < N && c < N && (!diag || r <= c)) {
+                        const double p = acc[i][j][h];
+                        const double x = X[(int64_t)r * ld + c];
+                        const double d = p - x;
+                        const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
+                        Xn[(int64_t)r * ld + c] = xn;
+                        if (r == c) {
+                            s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
+                        } else {
+                            Xn[(int64_t)c * ld + r] = xn;                 // mirror
+                            s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
+                        }
+                    }
+                }
+            }
+        }
+        s_trp = warp_sum(s_trp); s_e = warp_sum(s_e); s_x = warp_sum(s_x); s_trn = warp_sum(s_trn);
+        if (lane == 0) { s_red[warp][0] = s_trp; s_red[warp][1] = s_e; s_red[warp][2] = s_x; s_red[warp][3] = s_trn; }
+    }
+    __syncthreads();
+
+    // ===================== per-tile partials, last-CTA finaliser (D5) =====================
+    if (threadIdx.x < 4) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < D_CONSUMER_WARPS; ++w) v += s_red[w][threadIdx.x];
+        partials[(size_t)blockIdx.x * 4 + threadIdx.x] = v;
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        *s_last = (prev + 1u == gridDim.x);
+    }
+    __syncthreads();
+    if (*s_last && warp_all == 0) {
+        __threadfence();
+        double s[4] = {0.0, 0.0, 0.0, 0.0};
+        const volatile double *vp = partials;
+        for (int tI = lane; tI < (int)gridDim.x; tI += 32) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s[q] += vp[(size_t)tI * 4 + q];
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) s[q] = warp_sum(s[q]);
+        if (lane == 0) sp2_finalise(ctl, s);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------
+int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
+{
+    PFN_encodeTiled enc = get_encode_tiled();
+    if (!enc) return BML_ERR_CUDA;
+    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)N};           // innermost first: columns (k), rows
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};     // bytes, dims 1..rank-1
+    const cuuint32_t box[2] = {(cuuint32_t)D_BK, (cuuint32_t)D_BM};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)base, dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
+}
+
+int dense_fp64_num_tiles(int64_t N)
+{
+    const int T = (int)((N + D_BM - 1) / D_BM);
+    return T * (T + 1) / 2;
+}
+
+// Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).
+int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
+                         int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(x2_dense_fp64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)D_SMEM_BYTES) !=
+            cudaSuccess)
+            return BML_ERR_CUDA;
+        attr_set = true;
+    }
+    x2_dense_fp64_kernel<<<dense_fp64_num_tiles(N), D_THREADS, D_SMEM_BYTES, stream>>>(map0, map1, buf0, buf1, ld,
+                                                                                       (int)N, ctl, partials);
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+}  // namespace bmlsp2
