@@ -1,0 +1,377 @@
+#!/usr/bin/env python
+"""bench.py -- SP2 time-to-D on one B200 (BASELINE.json metric), roofline of the dominant kernel, CPU-oracle baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload dense_n2048] [--impl ours|reference]
+
+A "step" is one whole pass of the hot path: one bml_sp2_dense (or bml_sp2_ellpack) solve = Gershgorin bounds +
+rescale + every fused X^2 product until the stop rule + output copy, on a seeded synthetic Hamiltonian.
+Prints ONE JSON line.  The path does not shard (north_star: one GPU, no collectives):
+with --gpus N > 1 (torchrun) every rank solves its own replica and the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "sp2_time_to_D_ms"
+PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 64 FMA/clk/SM
+
+
+# ----------------------------------------------------------------------------------------------------------
+# workload description (algorithmic work per product: DESIGN.md "Roofline")
+# ----------------------------------------------------------------------------------------------------------
+def dense_flops_per_product(N: int) -> float:
+    """Executed flops of one symmetric-square product: upper-triangle 128x128 tiles incl. the diagonal tiles,
+    2 * 128 * 128 * N flops each (2 N^3 (1 + 1/T) / 2 when 128 | N)."""
+    T = (N + 127) // 128
+    return 2.0 * (T * (T + 1) // 2) * 128.0 * 128.0 * N
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return json.load(open(path)), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+# ----------------------------------------------------------------------------------------------------------
+# clocks sampler (NVML), DURING the timed region
+# ----------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self._stop = index, [], set(), threading.Event()
+        self.max_mhz, self.ok = None, False
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def __enter__(self):
+        if self.ok:
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self.ok:
+            self.t.join(timeout=1.0)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the reference arm / cpu_baseline: the oracle, as it stands, on the host cores
+# ----------------------------------------------------------------------------------------------------------
+def oracle_time_to_D(wname: str, H, budget_s: float, n_products_full: int | None):
+    """Time the CPU oracle on `wname`.  Runs the full solve if it fits `budget_s`, else a bounded sample of the first
+    p products and extrapolates linearly in the product count (every product costs the same N^3 loop).
+    Returns (ms_time_to_D, sample description, cores)."""
+    import oracle
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[wname]
+    cores = oracle.omp_threads()
+    if w.kind == "dense":
+        t0 = time.perf_counter()
+        _, st = oracle.sp2_dense(H, w.n_occ, w.idem_tol, 2)          # 2 products: calibrates the per-product cost
+        per = (time.perf_counter() - t0) / 2
+        full = n_products_full or 32
+        if per * full <= budget_s:
+            t0 = time.perf_counter()
+            _, st = oracle.sp2_dense(H, w.n_occ, w.idem_tol, 100)
+            dt = time.perf_counter() - t0
+            return dt * 1e3, f"full oracle solve, {st['n_products']} products", cores
+        p = max(1, min(full, int(budget_s / per)))
+        t0 = time.perf_counter()
+        _, st = oracle.sp2_dense(H, w.n_occ, w.idem_tol, p)
+        dt = time.perf_counter() - t0
+        return dt / p * full * 1e3, f"first {p} of {full} products timed, scaled by {full}/{p}", cores
+    t0 = time.perf_counter()
+    _, st = oracle.sp2_ellpack(*H, w.n_occ, w.idem_tol, w.drop_tol, 1)
+    per = time.perf_counter() - t0
+    full = n_products_full or 12
+    p = max(1, min(full, int(budget_s / max(per, 1e-9))))
+    t0 = time.perf_counter()
+    _, st = oracle.sp2_ellpack(*H, w.n_occ, w.idem_tol, w.drop_tol, p)
+    dt = time.perf_counter() - t0
+    if p == full:
+        return dt * 1e3, f"full oracle solve, {st['n_products']} products", cores
+    return dt / p * full * 1e3, f"first {p} of {full} products timed, scaled by {full}/{p}", cores
+
+
+EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30, "ellpack_n65536": 12}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[args.workload]
+    H = hm.make_dense(args.workload) if w.kind == "dense" else hm.make_ellpack(args.workload)
+    total = args.steps + args.warmup
+    budget = max(1.0, 200.0 / total)       # whole run within a few minutes
+    times, sample, cores = [], "", 1
+    for it in range(total):
+        ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
+        if it >= args.warmup:
+            times.append(ms)
+    v = float(np.mean(times))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args.workload),
+        "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(name: str):
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[name]
+    cfg = {"workload": name, "kind": w.kind, "N": w.N, "n_occ": w.n_occ, "idem_tol": w.idem_tol, "note": w.note,
+           "seed": 0, "max_products": 100,
+           "l2": "flushed between steps (256 MiB write); H + both iterates (96 MiB at N=2048) then stay L2-resident "
+                 "within a step, which is part of the method"}
+    if w.kind == "ellpack":
+        cfg.update({"M": w.M, "drop_tol": w.drop_tol})
+    return cfg
+
+
+# ----------------------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+
+    from paper_2401_13772_b200 import api, hamiltonians as hm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl")
+    api.load()
+    dev = torch.device("cuda", local)
+    w = hm.WORKLOADS[args.workload]
+    dense = w.kind == "dense"
+
+    # ---- inputs: seeded synthetic Hamiltonian, resident in HBM; pinned host copies for the e2e leg
+    if dense:
+        H_np = hm.make_dense(args.workload)
+        H_host = torch.from_numpy(H_np).pin_memory()
+        H_dev = H_host.to(dev)
+        solver = api.DenseSolver(w.N, dev, precision=w.precision)
+        D_host = torch.empty((w.N, w.N), dtype=torch.float64).pin_memory()
+
+        def solve(Hd):
+            return solver.solve(Hd, w.n_occ, w.idem_tol, 100)
+    else:
+        H_np = hm.make_ellpack(args.workload)
+        H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
+        H_dev = tuple(a.to(dev) for a in H_host)
+        solver = api.EllpackSolver(w.N, w.M, dev)
+        D_host = tuple(torch.empty_like(a).pin_memory() for a in H_host)
+
+        def solve(Hd):
+            return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, 100)
+
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-ups, then exactly K timed steps
+    res = None
+    for _ in range(args.warmup):
+        _, res = solve(H_dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)                     # L2 flush, outside the per-step events
+            ev[k][0].record()
+            _, res = solve(H_dev)                     # synchronises the stream once, at its end (reads the stats)
+            ev[k][1].record()
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = float(np.mean(step_ms))
+    clocks = clk.summary()
+
+    # ---- e2e: host buffers through the public API; H2D of H and D2H of D inside the timed region
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
+    d2h = h2d
+    for _ in range(2):
+        Hd = H_host.to(dev, non_blocking=True) if dense else tuple(a.to(dev, non_blocking=True) for a in H_host)
+        D, _ = solve(Hd)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        if dense:
+            Hd = H_host.to(dev, non_blocking=True)
+            D, _ = solve(Hd)
+            D_host.copy_(D, non_blocking=True)
+        else:
+            Hd = tuple(a.to(dev, non_blocking=True) for a in H_host)
+            D, _ = solve(Hd)
+            for dst, src in zip(D_host, D):
+                dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    # ---- dominant kernel, timed alone with CUDA events on the launching stream
+    pk, pk_src = peaks()
+    roof = None
+    n_prod = int(res.n_products)
+    if dense and w.precision == 0:
+        lo_hi = api.bml_gershgorin(H_dev).cpu().numpy()
+        s = 1.0 / (lo_hi[1] - lo_hi[0])
+        X0 = api.padded_dense((lo_hi[1] * torch.eye(w.N, dtype=torch.float64) - H_host) * s, dev)
+        Xn = torch.empty_strided(X0.shape, X0.stride(), dtype=X0.dtype, device=dev)
+        ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(w.N, 0), dev)
+        reps = 20
+        for _ in range(3):
+            api.bml_x2_dense(X0, 1, 0, Xn, ws)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(reps):
+            api.bml_x2_dense(X0, 1, 0, Xn, ws)
+        b.record()
+        torch.cuda.synchronize()
+        k_ms = a.elapsed_time(b) / reps
+        peak_probe = api.bml_probe_fp64_tensor_peak(40000)
+        flops = dense_flops_per_product(w.N)
+        achieved = flops / (k_ms * 1e-3) / 1e12
+        nominal_ratio_peak = pk["bf16_tflops"] * (40.0 / 2250.0)
+        roof = {
+            "bound": "tensor", "kernel": "x2_dense_fp64_kernel", "achieved": achieved, "peak": peak_probe,
+            "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": None,
+            "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
+                           "(MEASURED_PEAKS.json has no FP64 entry)",
+            "peak_alt_bf16_ratio": nominal_ratio_peak,
+            "frac_alt": achieved / nominal_ratio_peak,
+            "peak_alt_source": f"{pk_src} bf16 burst x nominal FP64/bf16 ratio 40/2250",
+            "launch_ms": k_ms, "flops_per_launch": flops,
+            "in_step_tflops": flops * n_prod / (ms * 1e-3) / 1e12,
+        }
+    elif not dense:
+        nnz = H_dev[2]
+        roof = {"bound": "hbm", "kernel": "x2_ellpack_kernel", "achieved": None, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": None, "traffic": None}
+
+    # ---- aggregate over ranks: max time
+    if dist is not None:
+        t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = t[0].item(), t[1].item()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- CPU oracle baseline (rank 0, N = 1 only): bounded sample, ~10-30 s
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, sample, cores = oracle_time_to_D(args.workload, H_np, 25.0, n_prod)
+        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
+
+    launches_per_step = (2 + 1 + 1 + 1 + 100 + 1) if dense else (2 + 2 + 1 + 100 + 1)
+    line = {
+        "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": workload_config(args.workload),
+        "status": int(res.status), "n_products": n_prod, "branch": res.branch,
+        "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
+        "ms_per_product": ms / max(n_prod, 1),
+        "aggregate_solves_per_s": world / (ms * 1e-3),
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches_note": f"{launches_per_step} per step; {n_prod} of the 100 enqueued product launches do work, "
+                             "the rest exit on the device-side stop flag",
+        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="dense_n2048")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -313,7 +313,8 @@ int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix
 
     if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
     TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // S0
-    TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowstats, &w.scal->tr0, w.scal->fail_flag, st));
+    // the Gershgorin row buffer (2N doubles) is free again: reuse it for the N diagonal values of X_0
+    TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowlh, &w.scal->tr0, w.scal->fail_flag, st));
     TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                         w.scal->fail_flag, st));
     for (int l = 0; l < p->max_products; ++l)                                                 // S2-S5

@@ -23,7 +23,8 @@ constexpr int E_MAX_GRID = 1024;
 __device__ __forceinline__ int e_hash(int j) { return (int)(((uint32_t)j * 2654435761u) >> 20) & E_MASK; }
 
 static inline int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
-static inline size_t e_scratch_bytes(int M) { return (size_t)16 * (size_t)M; }   // sk[M] int, sn[M] int, sa[M] f64
+// row stage sa[M] f64, sk[M] int, sn[M] int; later aliased by the (column, slot) sort buffer of >= 32 entries
+static inline size_t e_scratch_bytes(int M) { return M >= 16 ? (size_t)16 * (size_t)M : 256; }
 static inline size_t e_warp_bytes(int M) { return (size_t)E_SLOTS * 12 + e_scratch_bytes(M); }
 
 size_t ellpack_rowstats_bytes(int64_t) { return (size_t)E_MAX_GRID * 4 * sizeof(double); }
@@ -65,7 +66,7 @@ x2_ellpack_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__
 
     extern __shared__ __align__(16) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    uint8_t *wbase = smem + (size_t)warp * ((size_t)E_SLOTS * 12 + (size_t)16 * M);
+    uint8_t *wbase = smem + (size_t)warp * ((size_t)E_SLOTS * 12 + (size_t)sort_cap * 8);
     double *vals = (double *)wbase;                                  // [E_SLOTS]
     int *keys = (int *)(wbase + (size_t)E_SLOTS * 8);                // [E_SLOTS]
     uint8_t *scratch = wbase + (size_t)E_SLOTS * 12;
@@ -414,10 +415,10 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
     int64_t grid = (N + nwarps - 1) / nwarps;
     if (grid > sms) grid = sms;
     if (grid > E_MAX_GRID) grid = E_MAX_GRID;
-    // the (j, slot) sort buffer aliases the 16*M-byte row stage: 2*M entries of 8 bytes
+    // the (j, slot) sort buffer aliases the row stage: e_scratch_bytes(M) / 8 entries
     // buffer 0 is only read while parity == 0 (the standalone entry point passes a const X there)
     x2_ellpack_kernel<<<(unsigned)grid, nwarps * 32, smem, st>>>((double *)v0, (int32_t *)i0, (int32_t *)n0, v1, i1, n1,
-                                                                 (int)N, M, tau, 2 * M, ctl, partials);
+                                                                 (int)N, M, tau, (int)(e_scratch_bytes(M) / 8), ctl, partials);
     BML_CHECK_LAUNCH();
     return 0;
 }
