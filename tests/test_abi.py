@@ -43,7 +43,9 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     #include "bml_sp2.h"
     int main(void){ printf("%zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t)); return 0; }
     """
-    exe = os.path.join(ROOT, "tests", "golden", ".sizeof_probe")
+    import tempfile
+
+    exe = os.path.join(tempfile.mkdtemp(), "sizeof_probe")
     subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=src.encode(), check=True)
     out = subprocess.run([exe], capture_output=True, check=True).stdout.split()
     os.remove(exe)
