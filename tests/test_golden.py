@@ -1,0 +1,107 @@
+"""Stored expected values (tests/golden/sp2_expected.json, written by tests/golden/make_golden.py from the CPU oracle only).
+
+CPU tier: the oracle as it stands must still reproduce the stored values (guards against silent oracle drift).
+GPU tier: the CUDA path must reproduce the stored branch strings / product counts bit-exactly and D within tolerance,
+including the full-size N=8192 config whose oracle run (~10-20 min) is too slow for the test suite itself.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_2401_13772_b200 import hamiltonians as hm
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "sp2_expected.json")
+TOL_D = 1e-10  # BASELINE.json north_star: relative Frobenius error of D in FP64
+
+
+@pytest.fixture(scope="module")
+def gold():
+    return json.load(open(GOLD))
+
+
+def _same_log(st, g):
+    assert st["status"] == g["status"] and st["m_star"] == g["m_star"] and st["n_products"] == g["n_products"]
+    assert st["branch"] == g["branch"]
+    assert (st["emin"], st["emax"]) == (g["emin"], g["emax"])
+    np.testing.assert_allclose(st["trace"], g["trace"], rtol=0, atol=1e-9)
+
+
+def test_oracle_reproduces_golden_dense_n256(oracle_mod, gold):
+    g = gold["dense_n256"]
+    D, st = oracle_mod.sp2_dense(hm.make_dense("dense_n256"), g["n_occ"], g["idem_tol"])
+    _same_log(st, g)
+    for i, j, v in g["D_samples"]:
+        assert D[i, j] == v
+    assert float(np.trace(D)) == g["D_trace"]
+
+
+def test_oracle_reproduces_golden_ellpack_small(oracle_mod, gold):
+    g = gold["ellpack_small_12x10x8"]
+    Hs = hm.small_sparse_model(tuple(g["lattice"]), M=g["M"])
+    (dv, di, dn), st = oracle_mod.sp2_ellpack(*Hs, g["n_occ"], g["idem_tol"], g["drop_tol"])
+    _same_log(st, g)
+    assert int(dn.sum()) == g["D_nnz_total"]
+    assert [int(x) for x in di[0, : dn[0]]] == g["D_row0_index"]
+    assert [float(x) for x in dv[0, : dn[0]]] == g["D_row0_value"]
+
+
+def test_golden_covers_the_dense_configs(gold):
+    for name in ("dense_n256", "dense_n2048"):
+        w = hm.WORKLOADS[name]
+        g = gold[name]
+        assert (g["N"], g["n_occ"], g["idem_tol"]) == (w.N, w.n_occ, w.idem_tol)
+        assert g["status"] == 0 and len(g["branch"]) == g["m_star"] == g["n_products"] - 1
+        assert abs(g["D_trace"] - w.n_occ) < 1e-9          # tr D = N_occ (projector invariant, Eq. 2)
+        assert abs(g["D_fro"] ** 2 - w.n_occ) < 1e-7       # ||D||_F^2 = tr D^2 = tr D
+
+
+# ------------------------------------------------------------------------------------------------------ GPU tier
+@pytest.fixture(scope="module")
+def api():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2401_13772_b200 import api as _api
+
+    _api.load()
+    return _api
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["dense_n256", "dense_n2048", "dense_n8192"])
+def test_gpu_matches_golden_dense(api, gold, name):
+    import torch
+
+    if name not in gold:
+        pytest.skip(f"{name} not in the golden file yet (run tests/golden/make_golden.py {name})")
+    g = gold[name]
+    H = torch.from_numpy(hm.make_dense(name)).cuda()
+    D, res = api.bml_sp2_dense(H, g["n_occ"], g["idem_tol"])
+    assert res.status == g["status"] and res.n_products == g["n_products"] and res.m_star == g["m_star"]
+    assert res.branch == g["branch"]
+    assert (res.emin, res.emax) == (g["emin"], g["emax"])
+    np.testing.assert_allclose(res.trace, g["trace"], rtol=0, atol=1e-8)
+    # sampled entries + norms of D: |D_ij - D_ij^oracle| <= TOL_D * ||D||_F is implied by relFro <= TOL_D
+    for i, j, v in g["D_samples"]:
+        assert abs(D[i, j].item() - v) <= TOL_D * g["D_fro"]
+    assert abs(torch.trace(D).item() - g["D_trace"]) <= 1e-8
+    assert abs(torch.linalg.norm(D).item() - g["D_fro"]) <= TOL_D * g["D_fro"]
+
+
+@pytest.mark.gpu
+def test_gpu_matches_golden_ellpack_small(api, gold):
+    import torch
+
+    g = gold["ellpack_small_12x10x8"]
+    Hs = hm.small_sparse_model(tuple(g["lattice"]), M=g["M"])
+    (dv, di, dn), res = api.bml_sp2_ellpack(*(torch.from_numpy(a).cuda() for a in Hs), g["n_occ"], g["idem_tol"],
+                                            g["drop_tol"])
+    assert res.status == g["status"] and res.n_products == g["n_products"] and res.branch == g["branch"]
+    assert [int(x) for x in res.max_row_nnz] == g["max_row_nnz"]
+    n0 = int(dn[0].item())
+    assert int(dn.sum().item()) == g["D_nnz_total"]
+    assert di[0, :n0].cpu().tolist() == g["D_row0_index"]
+    assert dv[0, :n0].cpu().tolist() == g["D_row0_value"]          # canonical accumulation order: bit-exact
