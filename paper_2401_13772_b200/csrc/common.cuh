@@ -185,6 +185,42 @@ __device__ __forceinline__ double comp_warp_sum(double s, double c)
     return s + c;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Tile order of the symmetric-square kernels.  Upper-triangle tiles (I <= J) of a T x T tile grid are visited in
+// super-blocks of G x G tiles (super-blocks column by column, tiles row by row inside one): the ~148 CTAs resident at
+// any time then share 2 G row panels of X instead of ~150, so panels are re-read from L2, not from HBM.  Every
+// super-block is launched with all G*G slots; slots below the diagonal or outside the grid exit at once (they still
+// take part in the last-CTA count).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int TILE_SB = 12;         // 12 x 12 = 144 tiles per super-block, about one wave of 148 SMs
+// small grids (the whole iterate sits in L2 anyway) keep the plain triangular order, which has no empty slots
+__host__ __device__ __forceinline__ bool tile_sb_plain(int T) { return T <= 2 * TILE_SB; }
+__host__ __device__ __forceinline__ int tile_sb_grid(int T)
+{
+    if (tile_sb_plain(T)) return T * (T + 1) / 2;
+    const int S = (T + TILE_SB - 1) / TILE_SB;
+    return S * (S + 1) / 2 * TILE_SB * TILE_SB;
+}
+// t -> (i, j), i <= j, column by column: t = j (j + 1) / 2 + i
+__device__ __forceinline__ void tri_decode(int t, int &i, int &j)
+{
+    j = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while ((j + 1) * (j + 2) / 2 <= t) ++j;
+    while (j * (j + 1) / 2 > t) --j;
+    i = t - j * (j + 1) / 2;
+}
+__device__ __forceinline__ bool tile_sb_decode(int bid, int T, int &I, int &J)
+{
+    if (tile_sb_plain(T)) { tri_decode(bid, I, J); return true; }
+    constexpr int GG = TILE_SB * TILE_SB;
+    const int sb = bid / GG, w = bid - sb * GG;
+    int bi, bj;
+    tri_decode(sb, bi, bj);
+    I = bi * TILE_SB + w / TILE_SB;
+    J = bj * TILE_SB + w % TILE_SB;
+    return I <= J && J < T;
+}
+
 // Host-side helpers (api.cu)
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,

@@ -30,16 +30,6 @@ constexpr size_t D_SMEM_BYTES = (size_t)D_STAGES * D_STAGE_BYTES + 1024 /*align*
 // distinct (r >> 1) & 3 to hit 32 distinct banks: g = 0..3 -> rows 0,2,4,6 and g = 4..7 -> rows 1,3,5,7.
 __device__ __forceinline__ int perm8(int g) { return ((g & 3) << 1) | (g >> 2); }
 
-// linear tile id -> (I, J), I <= J, enumerated column by column: t = J (J + 1) / 2 + I
-__device__ __forceinline__ void tile_decode(int t, int &I, int &J)
-{
-    int j = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((j + 1) * (j + 2) / 2 <= t) ++j;
-    while (j * (j + 1) / 2 > t) --j;
-    J = j;
-    I = t - j * (j + 1) / 2;
-}
-
 __global__ void __launch_bounds__(D_THREADS, 1)
 x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
                      double *__restrict__ buf0, double *__restrict__ buf1, int64_t ld, int N,
@@ -65,7 +55,7 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
     const int warp_all = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int warp = warp_all - D_PRODUCER_WARPS;      // consumer warp index 0..7 (negative: producer warpgroup)
     int I, J;
-    tile_decode((int)blockIdx.x, I, J);
+    const bool valid = tile_sb_decode((int)blockIdx.x, (N + D_BM - 1) / D_BM, I, J);    // CTA-uniform
     const bool diag = (I == J);
     const int KT = (N + D_BK - 1) / D_BK;
 
@@ -74,9 +64,12 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         mbar_fence_init();
         fence_proxy_async();
     }
+    if (threadIdx.x < D_CONSUMER_WARPS * 4) ((double *)s_red)[threadIdx.x] = 0.0;     // empty slots contribute zero
     __syncthreads();
 
-    if (warp < 0) {
+    if (!valid) {
+        // slot below the diagonal / outside the tile grid: nothing to compute
+    } else if (warp < 0) {
         // ===================== TMA producer warpgroup (one elected lane works) =====================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(D_REGS_PRODUCER));
         if (warp_all == 0 && lane == 0) {
@@ -217,10 +210,10 @@ int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
     return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
 }
 
+// number of CTAs (= per-CTA partial-sum slots) of one product: all slots of all super-blocks
 int dense_fp64_num_tiles(int64_t N)
 {
-    const int T = (int)((N + D_BM - 1) / D_BM);
-    return T * (T + 1) / 2;
+    return tile_sb_grid((int)((N + D_BM - 1) / D_BM));
 }
 
 // Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).

@@ -37,15 +37,6 @@ constexpr size_t M_SMEM_BYTES = (size_t)M_STAGES * M_STAGE_BYTES + 1024 /*align*
 // tcgen05 instruction descriptor (kind::f16): D = F32, A = B = BF16, both K-major, N = 128, M = 128
 constexpr uint32_t M_IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(M_BN >> 3) << 17) | ((uint32_t)(M_BM >> 4) << 24);
 
-__device__ __forceinline__ void tile_decode_m(int t, int &I, int &J)
-{
-    int j = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((j + 1) * (j + 2) / 2 <= t) ++j;
-    while (j * (j + 1) / 2 > t) --j;
-    J = j;
-    I = t - j * (j + 1) / 2;
-}
-
 // shared-memory matrix descriptor: K-major, SWIZZLE_64B, 8-row groups 512 bytes apart, sm_100 descriptor version 1
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr)
 {
@@ -137,7 +128,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
 
     const int warp_all = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int I, J;
-    tile_decode_m((int)blockIdx.x, I, J);
+    const bool valid = tile_sb_decode((int)blockIdx.x, (N + M_BM - 1) / M_BM, I, J);    // CTA-uniform
     const bool diag = (I == J);
     const int nslabs = (N + M_BK - 1) / M_BK;
     const int nchunks = (nslabs + M_KC_SLABS - 1) / M_KC_SLABS;
@@ -148,7 +139,8 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
         mbar_fence_init();
         fence_proxy_async();
     }
-    if (warp_all == 2) {
+    if (threadIdx.x < M_EPI_WARPS * 4) ((double *)s_red)[threadIdx.x] = 0.0;     // empty slots contribute zero
+    if (valid && warp_all == 2) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)),
                      "n"(M_TMEM_COLS)
                      : "memory");
@@ -159,7 +151,9 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     tc_fence_after();
     const uint32_t tmem_base = *(volatile uint32_t *)s_tmem;
 
-    if (warp_all < M_CTRL_WARPS) {
+    if (!valid) {
+        // slot below the diagonal / outside the tile grid: nothing to compute
+    } else if (warp_all < M_CTRL_WARPS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(M_REGS_CTRL));
         if (warp_all == 0 && lane == 0) {
             // ===================== TMA producer =====================
@@ -272,7 +266,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     }
     tc_fence_before();
     __syncthreads();
-    if (warp_all == 2) {
+    if (valid && warp_all == 2) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(M_TMEM_COLS) : "memory");
     }
