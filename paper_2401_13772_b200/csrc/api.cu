@@ -161,6 +161,12 @@ static void fill_stats(bml_sp2_stats_t *stats, const Sp2Ctl &c)
     memcpy(stats->max_row_nnz, c.max_row_nnz, sizeof(c.max_row_nnz));
 }
 
+EnqueueState &enqueue_state()
+{
+    static thread_local EnqueueState es;
+    return es;
+}
+
 static int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
 {
     Sp2Ctl h;
@@ -251,9 +257,9 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
         CUtensorMap map0, map1;
         TRY(make_dense_map(&map0, w.X0, N, w.ldx));
         TRY(make_dense_map(&map1, w.X1, N, w.ldx));
-        // D2-D5: every product is enqueued up front; launches after the stop rule fired exit at once
-        for (int l = 0; l < p->max_products; ++l)
-            TRY(launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, st));
+        // D2-D5: products are enqueued ahead of the device; launches after the stop rule fired exit at once
+        TRY(enqueue_products([&]() { return launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, st); },
+                             w.ctl, p->max_products, st));
     }
     TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
     return finish_solve(w.ctl, stats, st);
@@ -317,8 +323,9 @@ int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix
     TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowlh, &w.scal->tr0, w.scal->fail_flag, st));
     TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                         w.scal->fail_flag, st));
-    for (int l = 0; l < p->max_products; ++l)                                                 // S2-S5
-        TRY(launch_x2_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, p->drop_tol, w.ctl, w.rowstats, st));
+    TRY(enqueue_products([&]() { return launch_x2_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, p->drop_tol, w.ctl,
+                                                          w.rowstats, st); },
+                         w.ctl, p->max_products, st));                                            // S2-S5
     TRY(launch_copy_out_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, w.ctl, D->value, D->index, D->nnz, st));
     return finish_solve(w.ctl, stats, st);
 }

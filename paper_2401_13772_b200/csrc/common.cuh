@@ -227,4 +227,55 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 PFN_encodeTiled get_encode_tiled();
 
+// Enqueue the product launches of one solve without ever letting the GPU wait for the host: the first batch and one
+// batch AHEAD are always queued; after each batch the device-side stop flag is copied to pinned host memory and the
+// host waits on an event recorded behind the batch BEFORE the one in flight.  Launches behind the stop flag exit at
+// once on the device, so correctness never depends on the host seeing the flag; batching only bounds how many of
+// them are issued (at most two batches instead of max_products - n_products).
+constexpr int ENQ_FIRST = 16, ENQ_BATCH = 8, ENQ_RING = 4;
+struct EnqueueState {
+    int32_t *h_done = nullptr;          // pinned, ENQ_RING slots
+    cudaEvent_t ev[ENQ_RING] = {};
+    bool ok = false;
+    EnqueueState()
+    {
+        if (cudaHostAlloc((void **)&h_done, ENQ_RING * sizeof(int32_t), cudaHostAllocDefault) != cudaSuccess) return;
+        for (int i = 0; i < ENQ_RING; ++i)
+            if (cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) != cudaSuccess) return;
+        ok = true;
+    }
+};
+
+EnqueueState &enqueue_state();      // api.cu: one per host thread
+
+template <class LaunchFn>
+static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_products, cudaStream_t st)
+{
+    EnqueueState &es = enqueue_state();
+    if (!es.ok) {                       // no pinned memory / events: plain enqueue of everything
+        for (int l = 0; l < max_products; ++l) { int r = launch_one(); if (r) return r; }
+        return 0;
+    }
+    int enq = 0, batch = 0;
+    auto enqueue_batch = [&](int n) -> int {
+        for (int l = 0; l < n && enq < max_products; ++l, ++enq) { int r = launch_one(); if (r) return r; }
+        const int slot = batch % ENQ_RING;
+        if (cudaMemcpyAsync(&es.h_done[slot], &d_ctl->done, sizeof(int32_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaEventRecord(es.ev[slot], st) != cudaSuccess)
+            return BML_ERR_CUDA;
+        ++batch;
+        return 0;
+    };
+    int r = enqueue_batch(ENQ_FIRST);
+    if (r) return r;
+    while (enq < max_products) {
+        if ((r = enqueue_batch(ENQ_BATCH))) return r;          // one batch ahead ...
+        const int prev = (batch - 2) % ENQ_RING;               // ... then look at the batch before it
+        if (cudaEventSynchronize(es.ev[prev]) != cudaSuccess) return BML_ERR_CUDA;
+        if (es.h_done[prev]) break;
+    }
+    return 0;
+}
+
+
 }  // namespace bmlsp2

@@ -361,9 +361,8 @@ int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, doub
     if ((r = make_plane_map(&m0, p0, N, ldx))) return r;
     if ((r = make_plane_map(&m1, p1, N, ldx))) return r;
     if ((r = launch_split(X0, ldx, N, p0, st))) return r;
-    for (int l = 0; l < p->max_products; ++l)
-        if ((r = launch_x2_mixed(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st))) return r;
-    return 0;
+    return enqueue_products([&]() { return launch_x2_mixed(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st); }, ctl,
+                            p->max_products, st);
 }
 
 int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, Sp2Ctl *ctl, double *partials, void *extra,
