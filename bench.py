@@ -32,10 +32,11 @@ PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 
 # workload description (algorithmic work per product: DESIGN.md "Roofline")
 # ----------------------------------------------------------------------------------------------------------
 def dense_flops_per_product(N: int) -> float:
-    """Executed flops of one symmetric-square product: upper-triangle 128x128 tiles incl. the diagonal tiles,
-    2 * 128 * 128 * N flops each (2 N^3 (1 + 1/T) / 2 when 128 | N)."""
-    T = (N + 127) // 128
-    return 2.0 * (T * (T + 1) // 2) * 128.0 * 128.0 * N
+    """Executed flops of one symmetric-square product: upper-triangle BT x BT tiles incl. the diagonal tiles,
+    2 * BT * BT * N flops each (2 N^3 (1 + 1/T) / 2 when BT | N); BT = 128 above N = 1024."""
+    bt = 32 if N <= 512 else (64 if N <= 1024 else 128)      # dense_fp64_tile() of the library
+    T = (N + bt - 1) // bt
+    return 2.0 * (T * (T + 1) // 2) * float(bt) * float(bt) * N
 
 
 def peaks():

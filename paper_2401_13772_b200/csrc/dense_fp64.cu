@@ -12,29 +12,36 @@
 
 namespace bmlsp2 {
 
-constexpr int D_BM = 128;          // tile rows (I panel)
-constexpr int D_BN = 128;          // tile cols (J panel)
+// Tile edge BT (tile = BT x BT): 128 for the roofline regime; 64 / 32 for small matrices, where 128 x 128 tiles would
+// leave most SMs idle (N = 256 has 3 tiles of 128 but 36 of 32) and a product is pure latency.  The 8 consumer warps
+// always form a 2 x 4 grid: warp tile (BT/2) x (BT/4).
 constexpr int D_BK = 16;           // k-slab: 16 doubles = 128 B = one SWIZZLE_128B row
-constexpr int D_STAGES = 6;        // 6 x 32 KB = 192 KB
+constexpr int D_STAGES = 6;        // 6 x 32 KB = 192 KB at BT = 128
 constexpr int D_CONSUMER_WARPS = 8;
 constexpr int D_PRODUCER_WARPS = 4;     // one warpgroup, so that setmaxnreg can hand its registers to the consumers
 constexpr int D_THREADS = (D_PRODUCER_WARPS + D_CONSUMER_WARPS) * 32;   // 384: ptxas caps at 168 regs/thread ...
 constexpr int D_REGS_PRODUCER = 40;     // ... re-split by setmaxnreg: 128 x 40 + 256 x 232 = 64512 = 384 x 168
 constexpr int D_REGS_CONSUMER = 232;
-constexpr int D_PANEL_BYTES = D_BM * D_BK * 8;   // 16 KB
-constexpr int D_STAGE_BYTES = 2 * D_PANEL_BYTES;
-constexpr size_t D_SMEM_BYTES = (size_t)D_STAGES * D_STAGE_BYTES + 1024 /*align*/ + 512 /*barriers + reduction scratch*/;
+constexpr int d_panel_bytes(int BT) { return BT * D_BK * 8; }       // 16 KB at BT = 128
+constexpr int d_stage_bytes(int BT) { return 2 * d_panel_bytes(BT); }
+constexpr size_t d_smem_bytes(int BT)
+{
+    return (size_t)D_STAGES * d_stage_bytes(BT) + 1024 /*align*/ + 512 /*barriers + reduction scratch*/;
+}
 
 // MMA row/col index g (0..7) -> physical row inside an 8-row group.  With the 128B TMA swizzle (16-byte chunk c of
 // row r stored at chunk c ^ (r & 7)) the four rows touched by one half-warp of an LDS.64 fragment load must have
 // distinct (r >> 1) & 3 to hit 32 distinct banks: g = 0..3 -> rows 0,2,4,6 and g = 4..7 -> rows 1,3,5,7.
 __device__ __forceinline__ int perm8(int g) { return ((g & 3) << 1) | (g >> 2); }
 
+template <int BT>
 __global__ void __launch_bounds__(D_THREADS, 1)
 x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
                      double *__restrict__ buf0, double *__restrict__ buf1, int64_t ld, int N,
                      Sp2Ctl *__restrict__ ctl, double *__restrict__ partials)
 {
+    constexpr int D_BM = BT, D_BN = BT, D_PANEL_BYTES = d_panel_bytes(BT), D_STAGE_BYTES = d_stage_bytes(BT);
+    constexpr int MI = BT / 16, NI = BT / 32;        // 8 x 8 fragments per warp tile (BT/2) x (BT/4)
     // every CTA sees the control block written by the previous product's finaliser (kernel boundary orders it)
     if (ctl->done) return;
     const int parity = ctl->parity;
@@ -92,19 +99,19 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         const int wm = warp >> 2, wn = warp & 3;     // 2 x 4 warps; warp tile 64 x 32
         const int g = lane >> 2, t = lane & 3;
         const int pg = perm8(g);
-        double acc[8][4][2];
+        double acc[MI][NI][2];
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < MI; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+            for (int j = 0; j < NI; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
 
         // byte offset of this lane's element inside a panel for k-step kk: row pg (+ 8-row groups via immediates)
         uint32_t koff[4];
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
             koff[kk] = (uint32_t)(pg * 128 + ((((kk * 2 + (t >> 1)) ^ pg) << 4) | ((t & 1) << 3)));
-        const uint8_t *a_base = smem + wm * 64 * 128;
-        const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * 32 * 128;
+        const uint8_t *a_base = smem + wm * (D_BM / 2) * 128;
+        const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * (D_BN / 4) * 128;
 
         for (int kt = 0; kt < KT; ++kt) {
             const int s = kt % D_STAGES;
@@ -113,17 +120,17 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
             const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
-                double a[8], b[4];
+                double a[MI], b[NI];
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
+                for (int i = 0; i < MI; ++i)
                     a[i] = *(const double *)(sa + koff[kk] + i * 8 * 128);
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NI; ++j)
                     b[j] = *(const double *)(sb + koff[kk] + j * 8 * 128);
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
+                for (int i = 0; i < MI; ++i)
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
@@ -133,13 +140,13 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         // lane holds C[g][2t], C[g][2t+1] of each 8x8 fragment -> physical (row perm8(g), cols perm8(2t), perm8(2t+1))
         const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
-        const int row0 = I * D_BM + wm * 64 + pg;
-        const int col0 = J * D_BN + wn * 32;
+        const int row0 = I * D_BM + wm * (D_BM / 2) + pg;
+        const int col0 = J * D_BN + wn * (D_BN / 4);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < MI; ++i) {
             const int r = row0 + i * 8;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < NI; ++j) {
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int c = col0 + j * 8 + (h ? pc1 : pc0);
@@ -196,13 +203,16 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
 // ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
+// tile edge for an N x N product: the roofline tile unless that leaves most of the chip idle
+int dense_fp64_tile(int64_t N) { return N <= 512 ? 32 : (N <= 1024 ? 64 : 128); }
+
 int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
 {
     PFN_encodeTiled enc = get_encode_tiled();
     if (!enc) return BML_ERR_CUDA;
     const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)N};           // innermost first: columns (k), rows
     const cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};     // bytes, dims 1..rank-1
-    const cuuint32_t box[2] = {(cuuint32_t)D_BK, (cuuint32_t)D_BM};
+    const cuuint32_t box[2] = {(cuuint32_t)D_BK, (cuuint32_t)dense_fp64_tile(N)};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)base, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -213,23 +223,35 @@ int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
 // number of CTAs (= per-CTA partial-sum slots) of one product: all slots of all super-blocks
 int dense_fp64_num_tiles(int64_t N)
 {
-    return tile_sb_grid((int)((N + D_BM - 1) / D_BM));
+    const int bt = dense_fp64_tile(N);
+    return tile_sb_grid((int)((N + bt - 1) / bt));
+}
+
+template <int BT>
+static int launch_x2_dense_fp64_t(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1,
+                                  int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(x2_dense_fp64_kernel<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)d_smem_bytes(BT)) != cudaSuccess)
+            return BML_ERR_CUDA;
+        attr_set = true;
+    }
+    x2_dense_fp64_kernel<BT><<<dense_fp64_num_tiles(N), D_THREADS, d_smem_bytes(BT), stream>>>(map0, map1, buf0, buf1, ld,
+                                                                                              (int)N, ctl, partials);
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
 // Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
                          int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(x2_dense_fp64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)D_SMEM_BYTES) !=
-            cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
+    switch (dense_fp64_tile(N)) {
+        case 32: return launch_x2_dense_fp64_t<32>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
+        case 64: return launch_x2_dense_fp64_t<64>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
+        default: return launch_x2_dense_fp64_t<128>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
     }
-    x2_dense_fp64_kernel<<<dense_fp64_num_tiles(N), D_THREADS, D_SMEM_BYTES, stream>>>(map0, map1, buf0, buf1, ld,
-                                                                                       (int)N, ctl, partials);
-    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
 }  // namespace bmlsp2
