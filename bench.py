@@ -142,7 +142,8 @@ def oracle_time_to_D(wname: str, H, budget_s: float, n_products_full: int | None
     return dt / p * full * 1e3, f"first {p} of {full} products timed, scaled by {full}/{p}", cores
 
 
-EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30, "ellpack_n65536": 12}
+EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30,
+                     "mixed_bf16x3_n16384": 30, "ellpack_n65536": 12}
 
 
 def run_reference(args):
@@ -315,32 +316,34 @@ def run_ours(args):
             "launch_ms": k_ms, "flops_per_launch": flops,
             "in_step_tflops": flops * n_prod / (ms * 1e-3) / 1e12,
         }
-    elif dense and w.precision == 1:
-        # mixed mode: the fused split-BF16 tcgen05 product, timed alone through bml_x2_dense(precision=1); that entry
-        # point also runs the (HBM-bound, ~2% of the time) FP64 -> 3 x BF16 split of its input
+    elif dense and w.precision != 0:
+        # mixed mode: the fused split-plane tcgen05 product, timed alone through bml_x2_dense(precision); that entry
+        # point also runs the (HBM-bound, ~2% of the time) FP64 -> 16-bit planes split of its input
+        terms = 3.0 if w.precision == 1 else 6.0          # FP16 x 2: hh, hl, lh; BF16 x 3: six cross terms
         lo_hi = api.bml_gershgorin(H_dev).cpu().numpy()
         s = 1.0 / (lo_hi[1] - lo_hi[0])
         X0 = api.padded_dense((lo_hi[1] * torch.eye(w.N, dtype=torch.float64) - H_host) * s, dev)
         Xn = torch.empty_strided(X0.shape, X0.stride(), dtype=X0.dtype, device=dev)
-        ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(w.N, 1), dev)
+        ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(w.N, w.precision), dev)
         reps = 10
         for _ in range(3):
-            api.bml_x2_dense(X0, 1, 1, Xn, ws)
+            api.bml_x2_dense(X0, 1, w.precision, Xn, ws)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         a.record()
         for _ in range(reps):
-            api.bml_x2_dense(X0, 1, 1, Xn, ws)
+            api.bml_x2_dense(X0, 1, w.precision, Xn, ws)
         b.record()
         torch.cuda.synchronize()
         k_ms = a.elapsed_time(b) / reps
-        flops = 6.0 * dense_flops_per_product(w.N)        # six BF16 cross terms per product
+        flops = terms * dense_flops_per_product(w.N)      # executed 16-bit tensor flops per product
         achieved = flops / (k_ms * 1e-3) / 1e12
         roof = {
             "bound": "tensor", "kernel": "x2_dense_mixed_kernel", "achieved": achieved, "peak": pk["bf16_tflops"],
             "unit": "TFLOP/s", "frac": achieved / pk["bf16_tflops"], "traffic": None,
-            "peak_source": f"{pk_src} bf16 burst (cuBLAS) from MEASURED_PEAKS.json; kernel timed alone "
-                           "(launch includes the FP64->BF16x3 split of its input)",
+            "peak_source": f"{pk_src} bf16 burst (cuBLAS) from MEASURED_PEAKS.json (fp16 and bf16 share the tcgen05 "
+                           "kind::f16 rate); kernel timed alone (launch includes the FP64 -> 16-bit planes split)",
+            "cross_terms": terms,
             "launch_ms": k_ms, "flops_per_launch": flops,
             "in_step_tflops": flops * n_prod / (ms * 1e-3) / 1e12,
             "in_step_frac_of_sustained": flops * n_prod / (ms * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
@@ -405,12 +408,13 @@ def run_ours(args):
         if n_enq - 8 >= max(n_prod, 16):
             break
     n_enq = min(n_enq, 100)
-    pre = (2 + 1 + 1 + 1 + (1 if w.precision == 1 else 0)) if dense else (2 + 2 + 1)
+    pre = (2 + 1 + 1 + 1 + (1 if w.precision != 0 else 0)) if dense else (2 + 2 + 1)
     launches_per_step = pre + n_enq + 1
     line = {
         "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16x3 products + f64 accumulate/update" if (dense and w.precision == 1) else "f64",
+        "dtype": {0: "f64", 1: "fp16x2 split products (fp32 TMEM chunks) + f64 accumulate/update",
+                  2: "bf16x3 split products (fp32 TMEM chunks) + f64 accumulate/update"}[w.precision if dense else 0],
         "data": "synthetic", "config": workload_config(args.workload),
         "status": int(res.status), "n_products": n_prod, "branch": res.branch,
         "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,

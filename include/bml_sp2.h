@@ -83,8 +83,10 @@ typedef struct {
     int32_t  max_products;  /* cap on X^2 products (Listing 2 `maxiter`), 1..BML_SP2_LOG_LEN             */
     double   idem_tol;      /* tolerance on e_m = ||X_m^2 - X_m||_F / ||X_m||_F                                 */
     double   drop_tol;      /* tau: keep |v| >= tau or the diagonal (ellpack only; 0 keeps everything)          */
-    int32_t  precision;     /* dense only: 0 = FP64 DMMA products; 1 = mixed (split-BF16 tcgen05 products with
-                               FP32 TMEM accumulation promoted to FP64 every K-chunk; FP64 traces and updates)  */
+    int32_t  precision;     /* dense only: 0 = FP64 DMMA products; 1, 2 = mixed precision: tcgen05 products of 16-bit
+                               planes of X with FP32 TMEM accumulation promoted to FP64 every 128 columns of K, FP64
+                               traces, norms and updates.  1 = two FP16 planes, X = Xh + 2^-11 Xl (3 cross terms);
+                               2 = three BF16 planes, X = Xh + Xm + Xl (6 cross terms)                            */
     uint32_t flags;         /* BML_SP2_FLAG_* */
 } bml_sp2_params_t;
 
@@ -143,7 +145,7 @@ BML_API int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bm
  * bml_x2_dense: the fused symmetric-square kernel (steps D3 + D4 of DESIGN.md) on a caller-supplied iterate.
  *   X: dense N x N, bitwise symmetric, ld a multiple of 16 elements, value 128-byte aligned.  Xnext: same shape/ld
  *   <- branch ? 2X - X*X : X*X  (Eq. 7 / Eq. 6), both triangles written.  d_sums: DEVICE double[4] <-
- *   { tr(X*X), ||X*X - X||_F^2, ||X||_F^2, tr(Xnext) }.  precision as in bml_sp2_params_t.
+ *   { tr(X*X), ||X*X - X||_F^2, ||X||_F^2, tr(Xnext) }.  precision (0, 1, 2) as in bml_sp2_params_t.
  *   d_workspace >= bml_x2_dense_workspace_bytes(N, precision).
  * bml_x2_ellpack: the thresholded row-wise product + update (steps S3 + S4) on a caller-supplied iterate whose rows
  *   are in ascending column order.  Xnext <- branch ? thr(2X - thr(X*X)) : thr(X*X).  d_sums: DEVICE double[4] <-

@@ -12,11 +12,12 @@ int dense_fp64_num_tiles(int64_t N);
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
                          int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream);
 // dense_mixed.cu
+int dense_mixed_num_tiles(int64_t N);
 size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx);
 int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, double *X0, double *X1, int64_t ldx,
                           Sp2Ctl *ctl, double *partials, const double *d_bounds, void *extra, cudaStream_t st);
-int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, Sp2Ctl *ctl, double *partials, void *extra,
-                        cudaStream_t st);
+int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, int precision, Sp2Ctl *ctl, double *partials,
+                        void *extra, cudaStream_t st);
 // reductions.cu
 int launch_gershgorin(const bml_matrix_t *H, double *d_bounds, double *rowlh, cudaStream_t st);
 int launch_trace_dense(const double *A, int64_t ld, int N, double *d_out, cudaStream_t st);
@@ -70,6 +71,13 @@ struct ScalarSlots {
 };
 static_assert(sizeof(ScalarSlots) <= SCAL_BYTES, "scalar slots");
 
+// per-CTA partial-sum slots: enough for the grid of either dense product kernel
+static inline size_t partial_slots(int64_t N)
+{
+    const int a = dense_fp64_num_tiles(N), b = dense_mixed_num_tiles(N);
+    return (size_t)(a > b ? a : b);
+}
+
 struct DenseWs {
     Sp2Ctl *ctl;
     ScalarSlots *scal;
@@ -88,12 +96,12 @@ static DenseWs carve_dense(void *ws, int64_t N, int precision)
     w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
     w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
     w.partials = (double *)(p + off);
-    off = align_up(off + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
+    off = align_up(off + partial_slots(N) * 4 * sizeof(double), 1024);
     w.ldx = padded_ld(N);
     w.X0 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
     w.X1 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
     w.extra = (void *)(p + off);
-    if (precision == 1) off = align_up(off + dense_mixed_extra_bytes(N, w.ldx), 1024);
+    if (precision != 0) off = align_up(off + dense_mixed_extra_bytes(N, w.ldx), 1024);
     w.total = off;
     return w;
 }
@@ -142,7 +150,7 @@ static bool ell_ok(const bml_matrix_t *A)
 static bool params_ok(const bml_sp2_params_t *p, int64_t N)
 {
     return p && p->n_occ > 0 && (int64_t)p->n_occ < N && p->idem_tol > 0.0 && p->max_products >= 1 &&
-           p->max_products <= BML_SP2_LOG_LEN && p->drop_tol >= 0.0 && (p->precision == 0 || p->precision == 1);
+           p->max_products <= BML_SP2_LOG_LEN && p->drop_tol >= 0.0 && p->precision >= 0 && p->precision <= 2;
 }
 
 static void fill_stats(bml_sp2_stats_t *stats, const Sp2Ctl &c)
@@ -251,7 +259,7 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
     TRY(launch_trace_dense(w.X0, w.ldx, (int)N, &w.scal->tr0, st));
     TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                         w.scal->fail_flag, st));
-    if (p->precision == 1) {
+    if (p->precision != 0) {
         TRY(sp2_dense_mixed_solve(H, p, w.X0, w.X1, w.ldx, w.ctl, w.partials, w.scal->bounds, w.extra, st));
     } else {
         CUtensorMap map0, map1;
@@ -269,8 +277,8 @@ size_t bml_x2_dense_workspace_bytes(int64_t N, int32_t precision)
 {
     if (N <= 0) return 0;
     size_t off = CTL_BYTES;
-    off = align_up(off + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
-    if (precision == 1) off = align_up(off + dense_mixed_extra_bytes(N, padded_ld(N)), 1024);
+    off = align_up(off + partial_slots(N) * 4 * sizeof(double), 1024);
+    if (precision != 0) off = align_up(off + dense_mixed_extra_bytes(N, padded_ld(N)), 1024);
     return off;
 }
 
@@ -279,7 +287,7 @@ int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int
 {
     if (!dense_ok(X) || !dense_ok(Xnext) || X->N != Xnext->N || X->ld != Xnext->ld || (X->ld % 16) != 0 ||
         ((uintptr_t)X->value & 127) != 0 || ((uintptr_t)Xnext->value & 127) != 0 || X->value == Xnext->value ||
-        !d_sums || !d_workspace || ((uintptr_t)d_workspace & 1023) != 0 || (precision != 0 && precision != 1) ||
+        !d_sums || !d_workspace || ((uintptr_t)d_workspace & 1023) != 0 || precision < 0 || precision > 2 ||
         workspace_bytes < bml_x2_dense_workspace_bytes(X->N, precision))
         return BML_ERR_INVALID;
     const int64_t N = X->N;
@@ -287,11 +295,11 @@ int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int
     uint8_t *p = (uint8_t *)d_workspace;
     Sp2Ctl *ctl = (Sp2Ctl *)p;
     double *partials = (double *)(p + CTL_BYTES);
-    void *extra = p + align_up(CTL_BYTES + (size_t)dense_fp64_num_tiles(N) * 4 * sizeof(double), 1024);
+    void *extra = p + align_up(CTL_BYTES + partial_slots(N) * 4 * sizeof(double), 1024);
     int r = launch_init_ctl(ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
     if (r) return r;
-    if (precision == 1) {
-        r = x2_dense_mixed_once(X, Xnext, ctl, partials, extra, st);
+    if (precision != 0) {
+        r = x2_dense_mixed_once(X, Xnext, precision, ctl, partials, extra, st);
     } else {
         CUtensorMap map0, map1;
         if ((r = make_dense_map(&map0, X->value, N, X->ld))) return r;

@@ -1,19 +1,26 @@
 // dense_mixed.cu -- mixed-precision dense X^2 (BASELINE.json configs[3]; not in the paper, readings item 17).
 //
-// X (FP64 master) is kept next to its three-way BF16 split  X = Xh + Xm + Xl  (Xh = bf16(X), Xm = bf16(X - Xh),
-// Xl = bf16(X - Xh - Xm): 3 x 8 mantissa bits).  One product tile P_IJ = sum_K X_IK X_JK^T is evaluated on the 5th-gen
-// tensor cores as the six cross terms of weight <= 2
-//        Xh Xl^T + Xl Xh^T + Xm Xm^T + Xh Xm^T + Xm Xh^T + Xh Xh^T
-// with tcgen05.mma.kind::f16 (BF16 x BF16 products are exact in FP32), FP32 accumulation in TMEM over a K-chunk of
-// M_KC columns only; every chunk is read back with tcgen05.ld and added to FP64 accumulators held in registers by the
-// eight epilogue warps (two TMEM accumulator buffers: the next chunk's MMAs run while the previous chunk is promoted).
-// The FP64 epilogue is the one of the FP64 kernel (Eq. 6 / Eq. 7, tr P, ||P - X||^2, ||X||^2, tr X', mirrored write,
-// last-CTA finaliser) and additionally writes the BF16 planes of X' for the next product.
+// X (FP64 master) is kept next to a split into 16-bit planes; one product tile P_IJ = sum_K X_IK X_JK^T is evaluated on
+// the 5th-gen tensor cores (tcgen05.mma.kind::f16, operands staged by TMA, FP32 accumulators in TMEM) as a sum of
+// plane cross terms.  The FP32 accumulator only ever holds a K-chunk of M_KC columns; every chunk is read back with
+// tcgen05.ld and added to FP64 accumulators held in registers by the eight epilogue warps (two TMEM accumulator
+// buffers: the next chunk's MMAs run while the previous chunk is promoted).  The FP64 epilogue is the one of the FP64
+// kernel (Eq. 6 / Eq. 7, tr P, ||P - X||^2, ||X||^2, tr X', mirrored write, last-CTA finaliser) and additionally writes
+// the planes of X' for the next product.  Two splits are built (bml_sp2_params_t::precision):
+//
+//   precision 1, FP16 x 2 (default):  X = Xh + 2^-11 Xl,  Xh = fp16(X), Xl = fp16(2^11 (X - Xh))   (2 x 11 bits; the
+//       scaling keeps the residual plane out of the FP16 subnormal range).  Three cross terms per 16 columns of K, two
+//       MMAs:  Xh [Xh ; Xl]^T  (N = 256: hh into accumulator columns 0..127, hl into 128..255)  and  Xl Xh^T
+//       (N = 128, into 128..255).  Promotion:  acc += double(big + 2^-11 small).  The dropped Xl Xl^T term is <= 2^-22.
+//       The large term hh has the accumulator to itself: 8 FP32 updates per chunk instead of 48.
+//   precision 2, BF16 x 3:  X = Xh + Xm + Xl (bf16 each, 3 x 8 bits); the six cross terms of weight <= 2,
+//       Xh Xl^T + Xl Xh^T + Xm Xm^T + Xh Xm^T + Xm Xh^T + Xh Xh^T, 12 MMAs (N = 128) per 32 columns, one accumulator.
 //
 // Roles (384 threads): warp 0 = TMA producer (one lane), warp 1 = MMA issuer (one lane), warp 2 = TMEM allocator,
-// warps 4..11 = epilogue (thread <-> one accumulator row, 64 columns).  Shared memory: M_STAGES x { A planes h,m,l ;
-// B planes h,m,l } of 128 rows x 32 bf16 (64-byte rows, SWIZZLE_64B, K-major UMMA canonical layout).
+// warps 4..11 = epilogue (thread <-> one accumulator row, 64 columns).  Shared memory: STAGES x { A planes ; B planes }
+// of 128 rows x 32 elements (64-byte rows, SWIZZLE_64B, K-major UMMA canonical layout).
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "common.cuh"
 
@@ -21,21 +28,33 @@ namespace bmlsp2 {
 
 constexpr int M_BM = 128;
 constexpr int M_BN = 128;
-constexpr int M_BK = 32;                       // bf16 elements per k-slab = 64 bytes = one SWIZZLE_64B row
-constexpr int M_STAGES = 4;
+constexpr int M_BK = 32;                       // 16-bit elements per k-slab = 64 bytes = one SWIZZLE_64B row
 constexpr int M_KC_SLABS = 4;                  // K-chunk promoted to FP64 = 4 slabs = 128 columns
 constexpr int M_PLANE_TILE = M_BM * M_BK * 2;  // 8 KB
-constexpr int M_STAGE_BYTES = 6 * M_PLANE_TILE;
 constexpr int M_EPI_WARPS = 8;
 constexpr int M_CTRL_WARPS = 4;
 constexpr int M_THREADS = (M_CTRL_WARPS + M_EPI_WARPS) * 32;
 constexpr int M_REGS_CTRL = 56;
 constexpr int M_REGS_EPI = 224;                // 128 x 56 + 256 x 224 = 64512
-constexpr int M_TMEM_COLS = 256;               // two 128-column FP32 accumulator buffers
-constexpr size_t M_SMEM_BYTES = (size_t)M_STAGES * M_STAGE_BYTES + 1024 /*align*/ + 1024 /*barriers, scratch*/;
+constexpr int M_MAX_PLANES = 3;
 
-// tcgen05 instruction descriptor (kind::f16): D = F32, A = B = BF16, both K-major, N = 128, M = 128
-constexpr uint32_t M_IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(M_BN >> 3) << 17) | ((uint32_t)(M_BM >> 4) << 24);
+enum { MV_F16X2 = 1, MV_BF16X3 = 2 };          // = bml_sp2_params_t::precision
+
+template <int V> struct MixedCfg;
+template <> struct MixedCfg<MV_F16X2> {
+    static constexpr int PLANES = 2, STAGES = 6, ACC_COLS = 256;    // hh | hl + lh
+    static constexpr uint32_t FMT = 0;                              // F16
+};
+template <> struct MixedCfg<MV_BF16X3> {
+    static constexpr int PLANES = 3, STAGES = 4, ACC_COLS = 128;
+    static constexpr uint32_t FMT = 1;                              // BF16
+};
+
+// tcgen05 instruction descriptor (kind::f16): D = F32, A/B format, both K-major, N, M = 128
+__host__ __device__ constexpr uint32_t m_idesc(uint32_t fmt, int n)
+{
+    return (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(M_BM >> 4) << 24);
+}
 
 // shared-memory matrix descriptor: K-major, SWIZZLE_64B, 8-row groups 512 bytes apart, sm_100 descriptor version 1
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr)
@@ -43,13 +62,14 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr)
     return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)(512u >> 4) << 32) | (1ull << 46) | (4ull << 61);
 }
 
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate)
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                         uint32_t accumulate)
 {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(M_IDESC), "r"(accumulate)
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint64_t *bar)
@@ -60,67 +80,79 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar)
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-// 32 lanes x 32 consecutive FP32 columns of TMEM -> 32 registers per thread (thread = its own lane)
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+// 32 lanes x 16 consecutive FP32 columns of TMEM -> 16 registers per thread (thread = its own lane)
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
 {
     asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr)
         : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// X = h + m + l in BF16 (round to nearest at every level)
-__device__ __forceinline__ void split3(double x, __nv_bfloat16 &h, __nv_bfloat16 &m, __nv_bfloat16 &l)
+// split of one FP64 value into the raw 16-bit patterns of the planes (round to nearest at every level)
+template <int V>
+__device__ __forceinline__ void split_planes(double x, uint16_t (&pl)[M_MAX_PLANES])
 {
-    h = __double2bfloat16(x);
-    const double r1 = x - (double)__bfloat162float(h);
-    m = __double2bfloat16(r1);
-    const double r2 = r1 - (double)__bfloat162float(m);
-    l = __double2bfloat16(r2);
+    if (V == MV_F16X2) {
+        const __half h = __double2half(x);
+        const double r1 = x - (double)__half2float(h);
+        pl[0] = __half_as_ushort(h);
+        pl[1] = __half_as_ushort(__double2half(r1 * 2048.0));
+        pl[2] = 0;
+    } else {
+        const __nv_bfloat16 h = __double2bfloat16(x);
+        const double r1 = x - (double)__bfloat162float(h);
+        const __nv_bfloat16 m = __double2bfloat16(r1);
+        const double r2 = r1 - (double)__bfloat162float(m);
+        pl[0] = __bfloat16_as_ushort(h);
+        pl[1] = __bfloat16_as_ushort(m);
+        pl[2] = __bfloat16_as_ushort(__double2bfloat16(r2));
+    }
 }
 
-// planes[p][r][c], p = 0 (h), 1 (m), 2 (l); leading dimension ldp elements
+// planes[p][r][c], p = 0 .. PLANES-1; leading dimension ldp elements
+template <int V>
 __global__ void __launch_bounds__(256)
-split_planes_kernel(const double *__restrict__ X, int64_t ld, int N, __nv_bfloat16 *__restrict__ planes, int64_t ldp)
+split_planes_kernel(const double *__restrict__ X, int64_t ld, int N, uint16_t *__restrict__ planes, int64_t ldp)
 {
     const int64_t plane = (int64_t)N * ldp;
     const int64_t total = (int64_t)N * N;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         const int64_t r = e / N, c = e - r * N;
-        __nv_bfloat16 h, m, l;
-        split3(X[r * ld + c], h, m, l);
-        planes[r * ldp + c] = h;
-        planes[plane + r * ldp + c] = m;
-        planes[2 * plane + r * ldp + c] = l;
+        uint16_t pl[M_MAX_PLANES];
+        split_planes<V>(X[r * ld + c], pl);
+#pragma unroll
+        for (int p = 0; p < MixedCfg<V>::PLANES; ++p) planes[p * plane + r * ldp + c] = pl[p];
     }
 }
 
+template <int V>
 __global__ void __launch_bounds__(M_THREADS, 1)
 x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
-                      double *__restrict__ buf0, double *__restrict__ buf1, __nv_bfloat16 *__restrict__ pl0,
-                      __nv_bfloat16 *__restrict__ pl1, int64_t ld, int N, Sp2Ctl *__restrict__ ctl,
+                      double *__restrict__ buf0, double *__restrict__ buf1, uint16_t *__restrict__ pl0,
+                      uint16_t *__restrict__ pl1, int64_t ld, int N, Sp2Ctl *__restrict__ ctl,
                       double *__restrict__ partials)
 {
+    using Cfg = MixedCfg<V>;
+    constexpr int PLANES = Cfg::PLANES, STAGES = Cfg::STAGES, ACC_COLS = Cfg::ACC_COLS;
+    constexpr int STAGE_BYTES = 2 * PLANES * M_PLANE_TILE;
     if (ctl->done) return;
     const int parity = ctl->parity;
     const int branch = ctl->branch_cur;
     const CUtensorMap *map = parity ? &map1 : &map0;
     const double *__restrict__ X = parity ? buf1 : buf0;
     double *__restrict__ Xn = parity ? buf0 : buf1;
-    __nv_bfloat16 *__restrict__ Pn = parity ? pl0 : pl1;
+    uint16_t *__restrict__ Pn = parity ? pl0 : pl1;
 
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    uint64_t *full_bar = (uint64_t *)(smem + (size_t)M_STAGES * M_STAGE_BYTES);
-    uint64_t *empty_bar = full_bar + M_STAGES;
-    uint64_t *tfull_bar = empty_bar + M_STAGES;       // [2] accumulator buffer ready for the epilogue
+    uint64_t *full_bar = (uint64_t *)(smem + (size_t)STAGES * STAGE_BYTES);
+    uint64_t *empty_bar = full_bar + STAGES;
+    uint64_t *tfull_bar = empty_bar + STAGES;         // [2] accumulator buffer ready for the epilogue
     uint64_t *tempty_bar = tfull_bar + 2;             // [2] accumulator buffer drained
     double (*s_red)[4] = (double (*)[4])(tempty_bar + 2);   // [M_EPI_WARPS][4]
     uint32_t *s_tmem = (uint32_t *)(s_red + M_EPI_WARPS);
@@ -134,7 +166,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     const int nchunks = (nslabs + M_KC_SLABS - 1) / M_KC_SLABS;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < M_STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(&tfull_bar[b], 1); mbar_init(&tempty_bar[b], M_EPI_WARPS); }
         mbar_fence_init();
         fence_proxy_async();
@@ -142,7 +174,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     if (threadIdx.x < M_EPI_WARPS * 4) ((double *)s_red)[threadIdx.x] = 0.0;     // empty slots contribute zero
     if (valid && warp_all == 2) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)),
-                     "n"(M_TMEM_COLS)
+                     "n"(2 * ACC_COLS)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -158,30 +190,27 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
         if (warp_all == 0 && lane == 0) {
             // ===================== TMA producer =====================
             tma_prefetch_desc(map);
-            const uint32_t tx = (diag ? 3u : 6u) * M_PLANE_TILE;
+            const uint32_t tx = (diag ? 1u : 2u) * PLANES * M_PLANE_TILE;
             for (int slab = 0; slab < nslabs; ++slab) {
-                const int s = slab % M_STAGES;
-                const uint32_t ph = (uint32_t)(slab / M_STAGES) & 1u;
+                const int s = slab % STAGES;
+                const uint32_t ph = (uint32_t)(slab / STAGES) & 1u;
                 mbar_wait(&empty_bar[s], ph ^ 1u);
                 mbar_expect_tx(&full_bar[s], tx);
-                uint8_t *dst = smem + (size_t)s * M_STAGE_BYTES;
+                uint8_t *dst = smem + (size_t)s * STAGE_BYTES;
 #pragma unroll
-                for (int p = 0; p < 3; ++p)
+                for (int p = 0; p < PLANES; ++p)
                     tma_load_2d(dst + p * M_PLANE_TILE, map, slab * M_BK, p * N + I * M_BM, &full_bar[s]);
                 if (!diag) {
 #pragma unroll
-                    for (int p = 0; p < 3; ++p)
-                        tma_load_2d(dst + (3 + p) * M_PLANE_TILE, map, slab * M_BK, p * N + J * M_BN, &full_bar[s]);
+                    for (int p = 0; p < PLANES; ++p)
+                        tma_load_2d(dst + (PLANES + p) * M_PLANE_TILE, map, slab * M_BK, p * N + J * M_BN, &full_bar[s]);
                 }
             }
         } else if (warp_all == 1 && lane == 0) {
             // ===================== MMA issuer =====================
-            // cross terms, smallest first: (A plane, B plane)
-            const int ta[6] = {0, 2, 1, 0, 1, 0};
-            const int tb[6] = {2, 0, 1, 1, 0, 0};
             for (int slab = 0; slab < nslabs; ++slab) {
-                const int s = slab % M_STAGES;
-                const uint32_t ph = (uint32_t)(slab / M_STAGES) & 1u;
+                const int s = slab % STAGES;
+                const uint32_t ph = (uint32_t)(slab / STAGES) & 1u;
                 const int chunk = slab / M_KC_SLABS, within = slab % M_KC_SLABS;
                 const int buf = chunk & 1;
                 if (within == 0) {
@@ -190,16 +219,30 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
                 }
                 mbar_wait(&full_bar[s], ph);
                 tc_fence_after();
-                const uint32_t a_base = smem_u32(smem + (size_t)s * M_STAGE_BYTES);
-                const uint32_t b_base = diag ? a_base : a_base + 3 * M_PLANE_TILE;
-                const uint32_t d_tmem = tmem_base + (uint32_t)buf * M_BN;
+                const uint32_t a_base = smem_u32(smem + (size_t)s * STAGE_BYTES);
+                const uint32_t b_base = diag ? a_base : a_base + PLANES * M_PLANE_TILE;
+                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * ACC_COLS);
+                if (V == MV_F16X2) {
+                    // planes of one operand are adjacent in shared memory: [Bh ; Bl] is one 256-row K-major operand
+                    const uint64_t ah = umma_desc(a_base), al = umma_desc(a_base + M_PLANE_TILE);
+                    const uint64_t bh = umma_desc(b_base);
 #pragma unroll
-                for (int t = 0; t < 6; ++t) {
-                    const uint64_t ad = umma_desc(a_base + ta[t] * M_PLANE_TILE);
-                    const uint64_t bd = umma_desc(b_base + tb[t] * M_PLANE_TILE);
+                    for (int ks = 0; ks < M_BK / 16; ++ks) {   // UMMA_K = 16 elements = 32 bytes = 2 descriptor units
+                        umma_f16(d_tmem, ah + 2 * ks, bh + 2 * ks, m_idesc(Cfg::FMT, 256), (within | ks) != 0 ? 1u : 0u);
+                        umma_f16(d_tmem + M_BN, al + 2 * ks, bh + 2 * ks, m_idesc(Cfg::FMT, 128), 1u);
+                    }
+                } else {
+                    // cross terms, smallest first: (A plane, B plane)
+                    const int ta[6] = {0, 2, 1, 0, 1, 0};
+                    const int tb[6] = {2, 0, 1, 1, 0, 0};
 #pragma unroll
-                    for (int ks = 0; ks < M_BK / 16; ++ks)     // UMMA_K = 16 bf16 = 32 bytes = 2 descriptor units
-                        umma_bf16(d_tmem, ad + 2 * ks, bd + 2 * ks, (within | t | ks) != 0 ? 1u : 0u);
+                    for (int t = 0; t < 6; ++t) {
+                        const uint64_t ad = umma_desc(a_base + ta[t] * M_PLANE_TILE);
+                        const uint64_t bd = umma_desc(b_base + tb[t] * M_PLANE_TILE);
+#pragma unroll
+                        for (int ks = 0; ks < M_BK / 16; ++ks)
+                            umma_f16(d_tmem, ad + 2 * ks, bd + 2 * ks, m_idesc(Cfg::FMT, 128), (within | t | ks) != 0 ? 1u : 0u);
+                    }
                 }
                 umma_commit(&empty_bar[s]);                   // frees the smem stage when these MMAs have read it
                 if (within == M_KC_SLABS - 1 || slab == nslabs - 1) umma_commit(&tfull_bar[buf]);
@@ -219,12 +262,21 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
             mbar_wait(&tfull_bar[buf], ((uint32_t)chunk >> 1) & 1u);
             tc_fence_after();
 #pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-                uint32_t v[32];
-                tmem_ld32(t_lane + (uint32_t)(buf * M_BN + hh * 32), v);
-                tmem_ld_wait();
+            for (int g = 0; g < 4; ++g) {
+                uint32_t v[16];
+                tmem_ld16(t_lane + (uint32_t)(buf * ACC_COLS + g * 16), v);
+                if (V == MV_F16X2) {
+                    uint32_t w[16];
+                    tmem_ld16(t_lane + (uint32_t)(buf * ACC_COLS + M_BN + g * 16), w);
+                    tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) acc[hh * 32 + i] += (double)__uint_as_float(v[i]);
+                    for (int i = 0; i < 16; ++i)
+                        acc[g * 16 + i] += (double)fmaf(__uint_as_float(w[i]), 0x1p-11f, __uint_as_float(v[i]));
+                } else {
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) acc[g * 16 + i] += (double)__uint_as_float(v[i]);
+                }
             }
             tc_fence_before();
             __syncwarp();
@@ -245,17 +297,19 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
                     const double x = X[(int64_t)r * ld + c];
                     const double d = p - x;
                     const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
-                    __nv_bfloat16 h, m, l;
-                    split3(xn, h, m, l);
+                    uint16_t pl[M_MAX_PLANES];
+                    split_planes<V>(xn, pl);
                     const int64_t o = (int64_t)r * ld + c;
                     Xn[o] = xn;
-                    Pn[o] = h; Pn[plane + o] = m; Pn[2 * plane + o] = l;
+#pragma unroll
+                    for (int k = 0; k < PLANES; ++k) Pn[k * plane + o] = pl[k];
                     if (r == c) {
                         s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
                     } else {
                         const int64_t ot = (int64_t)c * ld + r;       // mirror
                         Xn[ot] = xn;
-                        Pn[ot] = h; Pn[plane + ot] = m; Pn[2 * plane + ot] = l;
+#pragma unroll
+                        for (int k = 0; k < PLANES; ++k) Pn[k * plane + ot] = pl[k];
                         s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
                     }
                 }
@@ -268,7 +322,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     __syncthreads();
     if (valid && warp_all == 2) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(M_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(2 * ACC_COLS) : "memory");
     }
 
     // ===================== per-tile partials, last-CTA finaliser (D5) =====================
@@ -302,81 +356,90 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
 // ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
-int dense_fp64_num_tiles(int64_t N);
+// number of CTAs (= per-CTA partial-sum slots) of one mixed product (128 x 128 tiles)
+int dense_mixed_num_tiles(int64_t N) { return tile_sb_grid((int)((N + M_BM - 1) / M_BM)); }
 
-// the three BF16 planes of one iterate, stacked: rows p * N + r, leading dimension ldp (= the FP64 iterate's ld)
-static int make_plane_map(CUtensorMap *map, const __nv_bfloat16 *base, int64_t N, int64_t ldp)
+// the planes of one iterate, stacked: rows p * N + r, leading dimension ldp (= the FP64 iterate's ld)
+template <int V>
+static int make_plane_map(CUtensorMap *map, const uint16_t *base, int64_t N, int64_t ldp)
 {
     PFN_encodeTiled enc = get_encode_tiled();
     if (!enc) return BML_ERR_CUDA;
-    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)(3 * N)};
-    const cuuint64_t strides[1] = {(cuuint64_t)ldp * sizeof(__nv_bfloat16)};
+    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)(MixedCfg<V>::PLANES * N)};
+    const cuuint64_t strides[1] = {(cuuint64_t)ldp * sizeof(uint16_t)};
     const cuuint32_t box[2] = {(cuuint32_t)M_BK, (cuuint32_t)M_BM};
     const cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (void *)base, dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = enc(map, V == MV_F16X2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                     (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
 }
 
+// room for the larger split (3 planes) so that the workspace size does not depend on the variant
 static inline size_t plane_set_bytes(int64_t N, int64_t ldx)
 {
-    return ((size_t)3 * (size_t)N * (size_t)ldx * sizeof(__nv_bfloat16) + 1023) / 1024 * 1024;
+    return ((size_t)M_MAX_PLANES * (size_t)N * (size_t)ldx * sizeof(uint16_t) + 1023) / 1024 * 1024;
 }
 
 size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx) { return 2 * plane_set_bytes(N, ldx); }
 
-static int launch_split(const double *X, int64_t ld, int64_t N, __nv_bfloat16 *planes, cudaStream_t st)
+template <int V>
+static int launch_split(const double *X, int64_t ld, int64_t N, uint16_t *planes, cudaStream_t st)
 {
     int64_t blocks = (N * N + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    split_planes_kernel<<<(unsigned)blocks, 256, 0, st>>>(X, ld, (int)N, planes, ld);
+    split_planes_kernel<V><<<(unsigned)blocks, 256, 0, st>>>(X, ld, (int)N, planes, ld);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
-static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double *b0, double *b1, __nv_bfloat16 *p0,
-                           __nv_bfloat16 *p1, int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t st)
+template <int V>
+static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double *b0, double *b1, uint16_t *p0,
+                           uint16_t *p1, int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t st)
 {
+    constexpr size_t smem = (size_t)MixedCfg<V>::STAGES * 2 * MixedCfg<V>::PLANES * M_PLANE_TILE + 1024 /*align*/ +
+                            1024 /*barriers, scratch*/;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(x2_dense_mixed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)M_SMEM_BYTES) !=
+        if (cudaFuncSetAttribute(x2_dense_mixed_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
             cudaSuccess)
             return BML_ERR_CUDA;
         attr_set = true;
     }
-    x2_dense_mixed_kernel<<<dense_fp64_num_tiles(N), M_THREADS, M_SMEM_BYTES, st>>>(m0, m1, b0, b1, p0, p1, ld, (int)N,
-                                                                                    ctl, partials);
+    x2_dense_mixed_kernel<V><<<dense_mixed_num_tiles(N), M_THREADS, smem, st>>>(m0, m1, b0, b1, p0, p1, ld, (int)N, ctl,
+                                                                                partials);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
-// X0 (already rescaled, in buffer 0) -> planes of buffer 0, then max_products fused products
+template <int V>
+static int solve_v(int64_t N, int max_products, double *X0, double *X1, int64_t ldx, Sp2Ctl *ctl, double *partials,
+                   void *extra, cudaStream_t st)
+{
+    uint16_t *p0 = (uint16_t *)extra;
+    uint16_t *p1 = (uint16_t *)((uint8_t *)extra + plane_set_bytes(N, ldx));
+    CUtensorMap m0, m1;
+    int r;
+    if ((r = make_plane_map<V>(&m0, p0, N, ldx))) return r;
+    if ((r = make_plane_map<V>(&m1, p1, N, ldx))) return r;
+    if ((r = launch_split<V>(X0, ldx, N, p0, st))) return r;
+    if (max_products == 1) return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st);
+    return enqueue_products([&]() { return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st); }, ctl,
+                            max_products, st);
+}
+
+// X0 (already rescaled, in buffer 0) -> planes of buffer 0, then the fused products
 int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, double *X0, double *X1, int64_t ldx,
                           Sp2Ctl *ctl, double *partials, const double *, void *extra, cudaStream_t st)
 {
-    const int64_t N = H->N;
-    __nv_bfloat16 *p0 = (__nv_bfloat16 *)extra;
-    __nv_bfloat16 *p1 = (__nv_bfloat16 *)((uint8_t *)extra + plane_set_bytes(N, ldx));
-    CUtensorMap m0, m1;
-    int r;
-    if ((r = make_plane_map(&m0, p0, N, ldx))) return r;
-    if ((r = make_plane_map(&m1, p1, N, ldx))) return r;
-    if ((r = launch_split(X0, ldx, N, p0, st))) return r;
-    return enqueue_products([&]() { return launch_x2_mixed(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st); }, ctl,
-                            p->max_products, st);
+    if (p->precision == MV_BF16X3) return solve_v<MV_BF16X3>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st);
+    return solve_v<MV_F16X2>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st);
 }
 
-int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, Sp2Ctl *ctl, double *partials, void *extra,
-                        cudaStream_t st)
+// one product on a caller-supplied iterate (the control block was initialised in standalone mode)
+int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, int precision, Sp2Ctl *ctl, double *partials,
+                        void *extra, cudaStream_t st)
 {
-    const int64_t N = X->N, ld = X->ld;
-    __nv_bfloat16 *p0 = (__nv_bfloat16 *)extra;
-    __nv_bfloat16 *p1 = (__nv_bfloat16 *)((uint8_t *)extra + plane_set_bytes(N, ld));
-    CUtensorMap m0, m1;
-    int r;
-    if ((r = make_plane_map(&m0, p0, N, ld))) return r;
-    if ((r = make_plane_map(&m1, p1, N, ld))) return r;
-    if ((r = launch_split(X->value, ld, N, p0, st))) return r;
-    return launch_x2_mixed(m0, m1, X->value, Xn->value, p0, p1, ld, N, ctl, partials, st);
+    if (precision == MV_BF16X3) return solve_v<MV_BF16X3>(X->N, 1, X->value, Xn->value, X->ld, ctl, partials, extra, st);
+    return solve_v<MV_F16X2>(X->N, 1, X->value, Xn->value, X->ld, ctl, partials, extra, st);
 }
 
 }  // namespace bmlsp2

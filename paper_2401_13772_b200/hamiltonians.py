@@ -155,7 +155,7 @@ class Workload:
     n_occ: int
     idem_tol: float
     drop_tol: float = 0.0
-    precision: int = 0  # 0 = FP64, 1 = mixed
+    precision: int = 0  # 0 = FP64, 1 = mixed (FP16 x 2 split), 2 = mixed (BF16 x 3 split)
     M: int = 0
     lattice: tuple | None = None
     note: str = ""
@@ -172,6 +172,9 @@ WORKLOADS = {
     # configs[3]
     "mixed_n16384": Workload("mixed_n16384", "dense", 16384, 8192, 1e-6, precision=1, lattice=(32, 32, 16),
                              note="32x32x16, -exp(-r/1.5), r<=6, mixed precision"),
+    # configs[3] with the three-plane BF16 split instead of the default two-plane FP16 split
+    "mixed_bf16x3_n16384": Workload("mixed_bf16x3_n16384", "dense", 16384, 8192, 1e-6, precision=2, lattice=(32, 32, 16),
+                                    note="32x32x16, -exp(-r/1.5), r<=6, mixed precision (BF16 x 3 planes)"),
     # configs[4], literally as written (overflows M=512 at product 0 — SURVEY §8(d))
     "ellpack_n65536_literal": Workload("ellpack_n65536_literal", "ellpack", 65536, 32768, 1e-8, 1e-6, M=512,
                                        lattice=(64, 32, 32), note="64x32x32, -exp(-r/1.0), r<=3, delta=1.5"),
@@ -187,7 +190,7 @@ def make_dense(name: str, seed: int = 0) -> np.ndarray:
         return ring_dense(256, 1.5, 0.1, 1e-3, seed)
     if name == "dense_n2048":
         return lattice_dense(w.lattice, 1.5, 0.2, 1.0, lambda r: -1.0, seed)
-    if name in ("dense_n8192", "mixed_n16384"):
+    if name in ("dense_n8192", "mixed_n16384", "mixed_bf16x3_n16384"):
         return lattice_dense(w.lattice, 1.5, 0.2, 6.0, lambda r: -math.exp(-r / 1.5), seed)
     raise KeyError(name)
 

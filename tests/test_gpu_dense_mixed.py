@@ -1,5 +1,6 @@
-"""GPU parity, dense mixed-precision mode (BASELINE.json configs[3]; readings item 17): split-BF16 tcgen05
-products with FP32 TMEM accumulation promoted to FP64 every 128 columns, FP64 traces / norms / updates.
+"""GPU parity, dense mixed-precision mode (BASELINE.json configs[3]; readings item 17): tcgen05 products of
+16-bit planes of X (precision 1: two scaled FP16 planes, the default; precision 2: three BF16 planes) with FP32 TMEM
+accumulation promoted to FP64 every 128 columns, FP64 traces / norms / updates.
 
 The oracle of this mode is the FP64 CPU oracle run with the mixed config's tolerance (1e-6).  Required (north_star):
 identical branch string and product count, relative Frobenius error of D <= 1e-5.  One product is held to
@@ -39,9 +40,13 @@ def to_gpu(A):
     return torch.from_numpy(np.ascontiguousarray(A)).cuda()
 
 
+PRECISIONS = [1, 2]
+
+
 @pytest.mark.parametrize("N", [1, 2, 7, 128, 129, 200, 384, 515])
 @pytest.mark.parametrize("branch", [0, 1])
-def test_x2_mixed_one_product(api, oracle_mod, N, branch):
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_x2_mixed_one_product(api, oracle_mod, N, branch, precision):
     """One fused mixed-precision product on sizes spanning several 128x128 tiles, ragged tails and a K tail that is
     not a multiple of the 32-column slab or of the 128-column promotion chunk."""
     import torch
@@ -51,7 +56,7 @@ def test_x2_mixed_one_product(api, oracle_mod, N, branch):
     X = (A + A.T) / 2 + np.diag(rng.uniform(0.0, 1.0, N))
     P = oracle_mod.x2_dense(X)
     ref = 2.0 * X - P if branch else P
-    Xn, sums = api.bml_x2_dense(api.padded_dense(X), branch, 1)
+    Xn, sums = api.bml_x2_dense(api.padded_dense(X), branch, precision)
     got = Xn.cpu().numpy()
     scale = np.linalg.norm(P)
     assert np.linalg.norm(got - ref) <= TOL_P_MIXED * scale
@@ -64,9 +69,9 @@ def test_x2_mixed_one_product(api, oracle_mod, N, branch):
     assert abs(s[3] - np.trace(got)) <= 1e-12 * max(1.0, np.abs(np.diag(got)).sum())
 
 
-def _check_mixed_solve(api, oracle_mod, H, n_occ, tol=TOL_MIXED_IDEM):
+def _check_mixed_solve(api, oracle_mod, H, n_occ, precision, tol=TOL_MIXED_IDEM):
     D_ref, st = oracle_mod.sp2_dense(H, n_occ, tol)
-    D, res = api.bml_sp2_dense(to_gpu(H), n_occ, tol, 100, 1)
+    D, res = api.bml_sp2_dense(to_gpu(H), n_occ, tol, 100, precision)
     assert st["status"] == 0 and res.status == 0
     assert res.n_products == st["n_products"] and res.m_star == st["m_star"]
     assert res.branch == st["branch"]
@@ -78,25 +83,29 @@ def _check_mixed_solve(api, oracle_mod, H, n_occ, tol=TOL_MIXED_IDEM):
     return res, st
 
 
-def test_sp2_mixed_config1_model_n256(api, oracle_mod):
-    _check_mixed_solve(api, oracle_mod, hm.make_dense("dense_n256"), 128)
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_sp2_mixed_config1_model_n256(api, oracle_mod, precision):
+    _check_mixed_solve(api, oracle_mod, hm.make_dense("dense_n256"), 128, precision)
 
 
 @pytest.mark.parametrize("N,n_occ,seed", [(64, 20, 1), (200, 77, 2), (333, 100, 3)])
-def test_sp2_mixed_planted_gap(api, oracle_mod, N, n_occ, seed):
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_sp2_mixed_planted_gap(api, oracle_mod, N, n_occ, seed, precision):
     H, _ = hm.planted_gap(N, n_occ, gap=1.0, width=1.0, seed=seed)
-    _check_mixed_solve(api, oracle_mod, H, n_occ)
+    _check_mixed_solve(api, oracle_mod, H, n_occ, precision)
 
 
-def test_sp2_mixed_small_long_range(api, oracle_mod):
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_sp2_mixed_small_long_range(api, oracle_mod, precision):
     """Reduced-size stand-in of the configs[3] Hamiltonian model (same hopping law, 8x8x6 box)."""
     H = hm.small_long_range((8, 8, 6))
-    _check_mixed_solve(api, oracle_mod, H, H.shape[0] // 2)
+    _check_mixed_solve(api, oracle_mod, H, H.shape[0] // 2, precision)
 
 
-def test_sp2_mixed_config2_model_n2048(api, oracle_mod):
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_sp2_mixed_config2_model_n2048(api, oracle_mod, precision):
     w = hm.WORKLOADS["dense_n2048"]
-    _check_mixed_solve(api, oracle_mod, hm.make_dense("dense_n2048"), w.n_occ)
+    _check_mixed_solve(api, oracle_mod, hm.make_dense("dense_n2048"), w.n_occ, precision)
 
 
 def test_mixed_rejects_sparse_and_bad_precision(api):
@@ -104,10 +113,11 @@ def test_mixed_rejects_sparse_and_bad_precision(api):
 
     X = api.padded_dense(np.eye(4))
     with pytest.raises(RuntimeError):
-        api.bml_x2_dense(X, 0, 2)
+        api.bml_x2_dense(X, 0, 3)
 
 
-def test_config4_n16384_sampled_product_and_solve(api, oracle_mod):
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config4_n16384_sampled_product_and_solve(api, oracle_mod, precision):
     """BASELINE.json configs[3] at full size (N=16384, mixed precision, tol 1e-6), in the launch configuration
     bench.py times.  The CPU oracle cannot finish an N=16384 solve in test time, so: (a) one fused mixed product on
     the oracle's X_0 is compared with the oracle on sampled entries (each an N-term compensated dot product), incl.
@@ -129,7 +139,7 @@ def test_config4_n16384_sampled_product_and_solve(api, oracle_mod):
     # |x_ik x_kj| summed over k bounds what the truncating FP32 accumulation and the dropped cross terms can lose
     mag = np.einsum("ik,ik->i", np.abs(X0[rows]), np.abs(X0[:, cols].T))
     for branch in (0, 1):
-        Xn, sums = api.bml_x2_dense(Xg, branch, 1)
+        Xn, sums = api.bml_x2_dense(Xg, branch, precision)
         got = Xn[torch.from_numpy(rows).cuda(), torch.from_numpy(cols).cuda()].cpu().numpy()
         expect = 2.0 * X0[rows, cols] - ref if branch else ref
         assert (np.abs(got - expect) <= 4e-6 * mag + 1e-12).all()
@@ -138,7 +148,7 @@ def test_config4_n16384_sampled_product_and_solve(api, oracle_mod):
         del Xn
     del Xg
     Hg = to_gpu(H)
-    D, res = api.bml_sp2_dense(Hg, w.n_occ, w.idem_tol, 100, 1)
+    D, res = api.bml_sp2_dense(Hg, w.n_occ, w.idem_tol, 100, precision)
     assert res.status == 0
     assert (res.emin, res.emax) == (lo, hi)
     assert res.branch == "10010110011001100101100101010" and res.n_products == 30
