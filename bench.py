@@ -39,6 +39,16 @@ def dense_flops_per_product(N: int) -> float:
     return 2.0 * (T * (T + 1) // 2) * float(bt) * float(bt) * N
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r01_ncu_kernels.md names the commands); None = no capture of this workload.
+NCU_TRAFFIC_BYTES = {
+    "dense_n2048": 34.8e6,          # 33.6 MB read (= N^2 x 8 B: X read once) + 1.2 MB written (X' stays in L2)
+    "mixed_n16384": None,
+    "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (super-block tile order)
+    "ellpack_n65536": 0.631e9,      # 0.251 GB read + 0.380 GB written
+}
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -189,6 +199,26 @@ def workload_config(name: str):
 
 
 # ----------------------------------------------------------------------------------------------------------
+# multi-rank aggregation (replicas only: DESIGN.md 7)
+# ----------------------------------------------------------------------------------------------------------
+def aggregate_over_ranks(values, dist=None, device=None):
+    """MAX over ranks of each timing in `values` (the slowest replica sets the job time).  `dist` is an initialised
+    torch.distributed module or None for a single process.  No data-path collective exists: this is the only one."""
+    import torch
+
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def replicas_per_second(world: int, ms: float) -> float:
+    """Whole-job throughput of `world` independent replicas that each finish one solve in <= ms."""
+    return world / (ms * 1e-3)
+
+
+# ----------------------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -307,7 +337,7 @@ def run_ours(args):
         nominal_ratio_peak = pk["bf16_tflops"] * (40.0 / 2250.0)
         roof = {
             "bound": "tensor", "kernel": "x2_dense_fp64_kernel", "achieved": achieved, "peak": peak_probe,
-            "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": None,
+            "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
             "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
                            "(MEASURED_PEAKS.json has no FP64 entry)",
             "peak_alt_bf16_ratio": nominal_ratio_peak,
@@ -340,7 +370,7 @@ def run_ours(args):
         achieved = flops / (k_ms * 1e-3) / 1e12
         roof = {
             "bound": "tensor", "kernel": "x2_dense_mixed_kernel", "achieved": achieved, "peak": pk["bf16_tflops"],
-            "unit": "TFLOP/s", "frac": achieved / pk["bf16_tflops"], "traffic": None,
+            "unit": "TFLOP/s", "frac": achieved / pk["bf16_tflops"], "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
             "peak_source": f"{pk_src} bf16 burst (cuBLAS) from MEASURED_PEAKS.json (fp16 and bf16 share the tcgen05 "
                            "kind::f16 rate); kernel timed alone (launch includes the FP64 -> 16-bit planes split)",
             "cross_terms": terms,
@@ -374,7 +404,7 @@ def run_ours(args):
         achieved = comp_bytes / (k_ms * 1e-3) / 1e9
         roof = {
             "bound": "hbm", "kernel": "x2_ellpack_kernel", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-            "frac": achieved / pk["hbm_gbs"], "traffic": None,
+            "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
             "peak_source": f"{pk_src} copy bandwidth from MEASURED_PEAKS.json",
             "note": "achieved = COMPULSORY bytes (read X_5 + write X_6, 12 B per stored entry + 4 B per row) / time; "
                     "the kernel is bound by shared-memory hash updates and issue slots, not HBM (DESIGN.md 5.4)",
@@ -384,10 +414,7 @@ def run_ours(args):
         }
 
     # ---- aggregate over ranks: max time
-    if dist is not None:
-        t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms = t[0].item(), t[1].item()
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
 
     if rank != 0:
         if dist is not None:
@@ -419,7 +446,7 @@ def run_ours(args):
         "status": int(res.status), "n_products": n_prod, "branch": res.branch,
         "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
         "ms_per_product": ms / max(n_prod, 1),
-        "aggregate_solves_per_s": world / (ms * 1e-3),
+        "aggregate_solves_per_s": replicas_per_second(world, ms),
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps},
         "gpu_launches": launches_per_step * args.steps,

@@ -60,6 +60,9 @@ def test_sass_contains_the_blackwell_instructions():
     sass = subprocess.run(["cuobjdump", "-sass", build.build()], capture_output=True, text=True).stdout
     assert "DMMA.8x8x4" in sass
     assert "UTMALDG" in sass
+    # the mixed-precision path must be tcgen05 MMAs with TMEM accumulators read back by tcgen05.ld
+    assert "UTCHMMA" in sass
+    assert "LDTM" in sass
 
 
 def test_product_and_oracle_do_not_import_each_other():
