@@ -9,8 +9,10 @@ namespace bmlsp2 {
 // dense_fp64.cu
 int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld);
 int dense_fp64_num_tiles(int64_t N);
+size_t dense_fp64_sk_bytes(int64_t N);
+int dense_fp64_sk_reset(void *sk, int64_t N, cudaStream_t st);
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
-                         int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream);
+                         int64_t N, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream);
 // dense_mixed.cu
 int dense_mixed_num_tiles(int64_t N);
 size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx);
@@ -82,6 +84,7 @@ struct DenseWs {
     Sp2Ctl *ctl;
     ScalarSlots *scal;
     double *rowlh, *partials, *X0, *X1;
+    void *sk;          // split-tile scratch of the persistent FP64 kernel
     void *extra;
     int64_t ldx;
     size_t total;
@@ -97,6 +100,7 @@ static DenseWs carve_dense(void *ws, int64_t N, int precision)
     w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
     w.partials = (double *)(p + off);
     off = align_up(off + partial_slots(N) * 4 * sizeof(double), 1024);
+    w.sk = (void *)(p + off); off = align_up(off + dense_fp64_sk_bytes(N), 1024);
     w.ldx = padded_ld(N);
     w.X0 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
     w.X1 = (double *)(p + off); off = align_up(off + (size_t)N * w.ldx * sizeof(double), 1024);
@@ -266,7 +270,8 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
         TRY(make_dense_map(&map0, w.X0, N, w.ldx));
         TRY(make_dense_map(&map1, w.X1, N, w.ldx));
         // D2-D5: products are enqueued ahead of the device; launches after the stop rule fired exit at once
-        TRY(enqueue_products([&]() { return launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, st); },
+        TRY(dense_fp64_sk_reset(w.sk, N, st));
+        TRY(enqueue_products([&]() { return launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, w.sk, st); },
                              w.ctl, p->max_products, st));
     }
     TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
@@ -278,6 +283,7 @@ size_t bml_x2_dense_workspace_bytes(int64_t N, int32_t precision)
     if (N <= 0) return 0;
     size_t off = CTL_BYTES;
     off = align_up(off + partial_slots(N) * 4 * sizeof(double), 1024);
+    off = align_up(off + dense_fp64_sk_bytes(N), 1024);
     if (precision != 0) off = align_up(off + dense_mixed_extra_bytes(N, padded_ld(N)), 1024);
     return off;
 }
@@ -295,7 +301,8 @@ int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int
     uint8_t *p = (uint8_t *)d_workspace;
     Sp2Ctl *ctl = (Sp2Ctl *)p;
     double *partials = (double *)(p + CTL_BYTES);
-    void *extra = p + align_up(CTL_BYTES + partial_slots(N) * 4 * sizeof(double), 1024);
+    void *sk = p + align_up(CTL_BYTES + partial_slots(N) * 4 * sizeof(double), 1024);
+    void *extra = (uint8_t *)sk + align_up(dense_fp64_sk_bytes(N), 1024);
     int r = launch_init_ctl(ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
     if (r) return r;
     if (precision != 0) {
@@ -304,7 +311,8 @@ int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int
         CUtensorMap map0, map1;
         if ((r = make_dense_map(&map0, X->value, N, X->ld))) return r;
         if ((r = make_dense_map(&map1, Xnext->value, N, X->ld))) return r;
-        r = launch_x2_dense_fp64(map0, map1, X->value, Xnext->value, X->ld, N, ctl, partials, st);
+        if ((r = dense_fp64_sk_reset(sk, N, st))) return r;
+        r = launch_x2_dense_fp64(map0, map1, X->value, Xnext->value, X->ld, N, ctl, partials, sk, st);
     }
     if (r) return r;
     if (cudaMemcpyAsync(d_sums, ctl->sums, 4 * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)

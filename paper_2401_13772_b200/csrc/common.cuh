@@ -31,6 +31,7 @@ struct Sp2Ctl {
     int32_t max_products;
     int32_t loop_mode;     // 1 = inside bml_sp2_* (apply stop rules), 0 = standalone bml_x2_* call
     int32_t n_done;        // number of X^2 products evaluated so far
+    uint32_t epoch;        // launch counter of this solve (>= 1): tags the split-tile hand-off flags of the FP64 kernel
     double idem_tol;
     double tr_cur;         // tr X_m
     double emin, emax;
@@ -47,6 +48,7 @@ __device__ __forceinline__ void sp2_finalise(Sp2Ctl *ctl, const double s[4])
 {
     ctl->sums[0] = s[0]; ctl->sums[1] = s[1]; ctl->sums[2] = s[2]; ctl->sums[3] = s[3];
     ctl->arrivals = 0;
+    ctl->epoch += 1u;
     if (!ctl->loop_mode) return;
     const int m = ctl->m;
     ctl->n_done = m + 1;

@@ -201,6 +201,254 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Persistent variant for the roofline regime (128 x 128 tiles): one CTA per SM walks a fixed work list.
+//   * tiles (upper triangle, t = J (J + 1) / 2 + I) are dealt out in full waves of G = gridDim.x: CTA c takes tile
+//     w G + c of wave w and runs the whole K loop of it;
+//   * the R = tiles mod G tiles of the last, partial wave are split along K ("stream-K"): their R KT k-slabs are cut
+//     into G equal contiguous ranges, one per CTA, so that every SM works until the end instead of R of them doing a
+//     whole tile while G - R idle (N = 2048: 136 tiles on 148 SMs; N = 8192: 2080 = 14 x 148 + 8).
+//     The CTA whose range holds k-slab 0 of a tile owns the tile: the others store their FP64 partial accumulators to
+//     global scratch (one 128 KB slot per CTA, thread-major so the stores coalesce) and raise a flag tagged with the
+//     launch epoch; the owner adds the partials in ascending CTA order (fixed order: bit-reproducible) and runs the
+//     fused epilogue.  Launched cooperatively, so all CTAs are resident and the flag waits cannot starve.
+// The TMA ring and the mbarrier phases run on across work items; the fused epilogue (D4) and the finaliser (D5) are
+// those of the kernel above.
+// ------------------------------------------------------------------------------------------------------------
+struct SkItem {
+    int tile, kt0, kt1;
+};
+// it-th work item of CTA c (identical arithmetic in every role); false when the list is exhausted
+__device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, SkItem &w)
+{
+    const int W = tiles / G, R = tiles - W * G;
+    if (it < W) { w.tile = it * G + c; w.kt0 = 0; w.kt1 = KT; return true; }
+    if (R == 0) return false;
+    const int64_t UT = (int64_t)R * KT;
+    const int64_t u0 = (int64_t)c * UT / G, u1 = (int64_t)(c + 1) * UT / G;
+    const int64_t tl = u0 / KT + (it - W);
+    const int64_t b = tl * KT;
+    const int64_t s = u0 > b ? u0 : b, f = u1 < b + KT ? u1 : b + KT;
+    if (s >= f) return false;
+    w.tile = W * G + (int)tl; w.kt0 = (int)(s - b); w.kt1 = (int)(f - b);
+    return true;
+}
+__device__ __forceinline__ void consumers_bar()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(D_CONSUMER_WARPS * 32) : "memory");
+}
+
+constexpr int SK_ACC = 64;                                             // FP64 accumulators per consumer thread
+constexpr size_t SK_SLOT_DOUBLES = (size_t)SK_ACC * D_CONSUMER_WARPS * 32;   // 128 x 128
+
+__global__ void __launch_bounds__(D_THREADS, 1)
+x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
+                        double *__restrict__ buf0, double *__restrict__ buf1, int64_t ld, int N,
+                        Sp2Ctl *__restrict__ ctl, double *__restrict__ partials, double *__restrict__ sk_scratch,
+                        unsigned int *__restrict__ sk_flags)
+{
+    constexpr int BT = 128, D_BM = BT, D_BN = BT, D_PANEL_BYTES = d_panel_bytes(BT), D_STAGE_BYTES = d_stage_bytes(BT);
+    constexpr int MI = BT / 16, NI = BT / 32;
+    if (ctl->done) return;
+    const int parity = ctl->parity;
+    const int branch = ctl->branch_cur;
+    const unsigned int epoch = ctl->epoch;
+    const CUtensorMap *map = parity ? &map1 : &map0;
+    const double *__restrict__ X = parity ? buf1 : buf0;
+    double *__restrict__ Xn = parity ? buf0 : buf1;
+
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t *full_bar = (uint64_t *)(smem + (size_t)D_STAGES * D_STAGE_BYTES);
+    uint64_t *empty_bar = full_bar + D_STAGES;
+    double (*s_red)[4] = (double (*)[4])(empty_bar + D_STAGES);          // [D_CONSUMER_WARPS][4]
+    int *s_last = (int *)(s_red + D_CONSUMER_WARPS);
+
+    const int warp_all = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = warp_all - D_PRODUCER_WARPS;
+    const int T = (N + D_BM - 1) / D_BM, tiles = T * (T + 1) / 2;
+    const int KT = (N + D_BK - 1) / D_BK;
+    const int G = (int)gridDim.x, c = (int)blockIdx.x;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < D_STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], D_CONSUMER_WARPS); }
+        mbar_fence_init();
+        fence_proxy_async();
+    }
+    if (threadIdx.x < D_CONSUMER_WARPS * 4) ((double *)s_red)[threadIdx.x] = 0.0;
+    __syncthreads();
+
+    if (warp < 0) {
+        // ===================== TMA producer warpgroup (one elected lane works) =====================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(D_REGS_PRODUCER));
+        if (warp_all == 0 && lane == 0) {
+            tma_prefetch_desc(map);
+            int slab = 0;
+            SkItem w;
+            for (int it = 0; sk_item(it, c, G, tiles, KT, w); ++it) {
+                int I, J;
+                tri_decode(w.tile, I, J);
+                const bool diag = (I == J);
+                const uint32_t tx = diag ? D_PANEL_BYTES : D_STAGE_BYTES;
+                for (int kt = w.kt0; kt < w.kt1; ++kt, ++slab) {
+                    const int s = slab % D_STAGES;
+                    const uint32_t ph = (uint32_t)(slab / D_STAGES) & 1u;
+                    mbar_wait(&empty_bar[s], ph ^ 1u);
+                    mbar_expect_tx(&full_bar[s], tx);
+                    uint8_t *dst = smem + (size_t)s * D_STAGE_BYTES;
+                    tma_load_2d(dst, map, kt * D_BK, I * D_BM, &full_bar[s]);
+                    if (!diag) tma_load_2d(dst + D_PANEL_BYTES, map, kt * D_BK, J * D_BN, &full_bar[s]);
+                }
+            }
+        }
+    } else {
+        // ===================== DMMA consumers =====================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(D_REGS_CONSUMER));
+        const int wm = warp >> 2, wn = warp & 3;     // 2 x 4 warps; warp tile 64 x 32
+        const int g = lane >> 2, t = lane & 3;
+        const int pg = perm8(g);
+        const int ctid = warp * 32 + lane;           // consumer thread id 0..255
+        uint32_t koff[4];
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+            koff[kk] = (uint32_t)(pg * 128 + ((((kk * 2 + (t >> 1)) ^ pg) << 4) | ((t & 1) << 3)));
+        const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
+        double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
+        int slab = 0;
+        SkItem w;
+        for (int it = 0; sk_item(it, c, G, tiles, KT, w); ++it) {
+            int I, J;
+            tri_decode(w.tile, I, J);
+            const bool diag = (I == J);
+            double acc[MI][NI][2];
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+                for (int j = 0; j < NI; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+            const uint8_t *a_base = smem + wm * (D_BM / 2) * 128;
+            const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * (D_BN / 4) * 128;
+            for (int kt = w.kt0; kt < w.kt1; ++kt, ++slab) {
+                const int s = slab % D_STAGES;
+                const uint32_t ph = (uint32_t)(slab / D_STAGES) & 1u;
+                mbar_wait(&full_bar[s], ph);
+                const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk) {
+                    double a[MI], b[NI];
+#pragma unroll
+                    for (int i = 0; i < MI; ++i) a[i] = *(const double *)(sa + koff[kk] + i * 8 * 128);
+#pragma unroll
+                    for (int j = 0; j < NI; ++j) b[j] = *(const double *)(sb + koff[kk] + j * 8 * 128);
+#pragma unroll
+                    for (int i = 0; i < MI; ++i)
+#pragma unroll
+                        for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty_bar[s]);
+            }
+
+            if (w.kt0 > 0) {
+                // ---------- contributor: hand the partial accumulators to the tile's owner ----------
+                double *slot = sk_scratch + (size_t)c * SK_SLOT_DOUBLES + ctid;
+#pragma unroll
+                for (int i = 0; i < MI; ++i)
+#pragma unroll
+                    for (int j = 0; j < NI; ++j) {
+                        __stcg(slot + (size_t)((i * NI + j) * 2 + 0) * 256, acc[i][j][0]);
+                        __stcg(slot + (size_t)((i * NI + j) * 2 + 1) * 256, acc[i][j][1]);
+                    }
+                __threadfence();
+                consumers_bar();
+                if (ctid == 0) atomicExch(&sk_flags[c], epoch);
+                continue;
+            }
+            if (w.kt1 < KT) {
+                // ---------- owner of a split tile: add the other CTAs' partials in ascending CTA order ----------
+                const int W = tiles / G, R = tiles - W * G;
+                const int64_t UT = (int64_t)R * KT;
+                const int64_t tile_end = (int64_t)(w.tile - W * G + 1) * KT;
+                for (int c2 = c + 1; c2 < G; ++c2) {
+                    const int64_t v0 = (int64_t)c2 * UT / G, v1 = (int64_t)(c2 + 1) * UT / G;
+                    if (v0 >= tile_end) break;
+                    if (v1 <= v0) continue;
+                    if (ctid == 0) {
+                        while (atomicAdd(&sk_flags[c2], 0u) != epoch) __nanosleep(64);
+                        __threadfence();
+                    }
+                    consumers_bar();
+                    const double *slot = sk_scratch + (size_t)c2 * SK_SLOT_DOUBLES + ctid;
+#pragma unroll
+                    for (int i = 0; i < MI; ++i)
+#pragma unroll
+                        for (int j = 0; j < NI; ++j) {
+                            acc[i][j][0] += __ldcg(slot + (size_t)((i * NI + j) * 2 + 0) * 256);
+                            acc[i][j][1] += __ldcg(slot + (size_t)((i * NI + j) * 2 + 1) * 256);
+                        }
+                }
+            }
+
+            // ===================== fused epilogue (D4) =====================
+            const int row0 = I * D_BM + wm * (D_BM / 2) + pg;
+            const int col0 = J * D_BN + wn * (D_BN / 4);
+#pragma unroll
+            for (int i = 0; i < MI; ++i) {
+                const int r = row0 + i * 8;
+#pragma unroll
+                for (int j = 0; j < NI; ++j) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int cc = col0 + j * 8 + (h ? pc1 : pc0);
+                        if (r < N && cc < N && (!diag || r <= cc)) {
+                            const double p = acc[i][j][h];
+                            const double x = X[(int64_t)r * ld + cc];
+                            const double d = p - x;
+                            const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
+                            Xn[(int64_t)r * ld + cc] = xn;
+                            if (r == cc) {
+                                s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
+                            } else {
+                                Xn[(int64_t)cc * ld + r] = xn;                // mirror
+                                s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        s_trp = warp_sum(s_trp); s_e = warp_sum(s_e); s_x = warp_sum(s_x); s_trn = warp_sum(s_trn);
+        if (lane == 0) { s_red[warp][0] = s_trp; s_red[warp][1] = s_e; s_red[warp][2] = s_x; s_red[warp][3] = s_trn; }
+    }
+    __syncthreads();
+
+    // ===================== per-CTA partial sums, last-CTA finaliser (D5) =====================
+    if (threadIdx.x < 4) {
+        double v = 0.0;
+#pragma unroll
+        for (int w2 = 0; w2 < D_CONSUMER_WARPS; ++w2) v += s_red[w2][threadIdx.x];
+        partials[(size_t)blockIdx.x * 4 + threadIdx.x] = v;
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        *s_last = (prev + 1u == gridDim.x);
+    }
+    __syncthreads();
+    if (*s_last && warp_all == 0) {
+        __threadfence();
+        double s[4] = {0.0, 0.0, 0.0, 0.0};
+        const volatile double *vp = partials;
+        for (int tI = lane; tI < (int)gridDim.x; tI += 32) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s[q] += vp[(size_t)tI * 4 + q];
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) s[q] = warp_sum(s[q]);
+        if (lane == 0) sp2_finalise(ctl, s);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
 // tile edge for an N x N product: the roofline tile unless that leaves most of the chip idle
@@ -220,11 +468,66 @@ int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
     return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
 }
 
-// number of CTAs (= per-CTA partial-sum slots) of one product: all slots of all super-blocks
+constexpr int SK_MAX_GRID = 256;      // scratch slots / flags provisioned for the persistent kernel
+
+static int sk_grid()
+{
+    static int g = 0;
+    if (!g) {
+        int dev = 0, sms = 0, coop = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop)
+            return 0;
+        g = sms < SK_MAX_GRID ? sms : SK_MAX_GRID;      // one CTA per SM (198 KB of shared memory each)
+    }
+    return g;
+}
+
+// number of CTAs (= per-CTA partial-sum slots) of one product
 int dense_fp64_num_tiles(int64_t N)
 {
     const int bt = dense_fp64_tile(N);
+    if (bt == 128) return SK_MAX_GRID;
     return tile_sb_grid((int)((N + bt - 1) / bt));
+}
+
+// global scratch of the persistent kernel: one partial-tile slot per CTA + the hand-off flags
+size_t dense_fp64_sk_bytes(int64_t N)
+{
+    if (dense_fp64_tile(N) != 128) return 0;
+    return (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double) + 1024;
+}
+
+// flags must not hold a tag from an earlier solve in the same workspace: zero them when a solve starts
+int dense_fp64_sk_reset(void *sk, int64_t N, cudaStream_t st)
+{
+    if (dense_fp64_tile(N) != 128) return 0;
+    unsigned int *flags = (unsigned int *)((uint8_t *)sk + (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double));
+    return cudaMemsetAsync(flags, 0, 1024, st) == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+static int launch_x2_dense_fp64_sk(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1,
+                                   int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream)
+{
+    const int G = sk_grid();
+    if (G <= 0 || !sk) return BML_ERR_CUDA;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(x2_dense_fp64_sk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)d_smem_bytes(128)) != cudaSuccess)
+            return BML_ERR_CUDA;
+        attr_set = true;
+    }
+    double *scratch = (double *)sk;
+    unsigned int *flags = (unsigned int *)((uint8_t *)sk + (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double));
+    int n = (int)N;
+    CUtensorMap m0 = map0, m1 = map1;
+    void *args[] = {&m0, &m1, &buf0, &buf1, &ld, &n, &ctl, &partials, &scratch, &flags};
+    if (cudaLaunchCooperativeKernel((const void *)x2_dense_fp64_sk_kernel, dim3((unsigned)G), dim3(D_THREADS), args,
+                                    d_smem_bytes(128), stream) != cudaSuccess)
+        return BML_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
 template <int BT>
@@ -244,13 +547,14 @@ static int launch_x2_dense_fp64_t(const CUtensorMap &map0, const CUtensorMap &ma
 }
 
 // Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).
+// sk: the scratch of dense_fp64_sk_bytes(N) bytes (used by the persistent 128 x 128 kernel only)
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
-                         int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream)
+                         int64_t N, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream)
 {
     switch (dense_fp64_tile(N)) {
         case 32: return launch_x2_dense_fp64_t<32>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
         case 64: return launch_x2_dense_fp64_t<64>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
-        default: return launch_x2_dense_fp64_t<128>(map0, map1, buf0, buf1, ld, N, ctl, partials, stream);
+        default: return launch_x2_dense_fp64_sk(map0, map1, buf0, buf1, ld, N, ctl, partials, sk, stream);
     }
 }
 

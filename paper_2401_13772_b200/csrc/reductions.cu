@@ -141,7 +141,7 @@ __global__ void sp2_init_ctl_kernel(Sp2Ctl *ctl, const double *__restrict__ boun
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     ctl->m = 0; ctl->done = 0; ctl->status = BML_MAX_PRODUCTS; ctl->parity = 0;
     ctl->overflow_row = INT32_MAX; ctl->overflow_upd = INT32_MAX; ctl->acc_row = INT32_MAX;
-    ctl->nnz_max_p = 0; ctl->nnz_max_upd = 0; ctl->fail_row = -1; ctl->arrivals = 0; ctl->n_done = 0;
+    ctl->nnz_max_p = 0; ctl->nnz_max_upd = 0; ctl->fail_row = -1; ctl->arrivals = 0; ctl->n_done = 0; ctl->epoch = 1u;
     ctl->n_occ = n_occ; ctl->max_products = max_products; ctl->loop_mode = loop_mode; ctl->idem_tol = idem_tol;
     for (int q = 0; q < 4; ++q) ctl->sums[q] = 0.0;
     if (loop_mode) {

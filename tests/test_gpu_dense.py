@@ -54,10 +54,12 @@ def test_gershgorin_and_trace_dense(api, oracle_mod, N, ld):
 
 
 # ------------------------------------------------------------------------------------------------ D3 + D4
-@pytest.mark.parametrize("N", [1, 2, 7, 128, 129, 200, 384, 515])
+@pytest.mark.parametrize("N", [1, 2, 7, 128, 129, 200, 384, 515, 640, 1000, 1100, 1283])
 @pytest.mark.parametrize("branch", [0, 1])
 def test_x2_dense_one_product_elementwise(api, oracle_mod, N, branch):
-    """One fused product on sizes that span several 128x128 tiles with ragged tails (and the degenerate N=1,2)."""
+    """One fused product on sizes that span several tiles with ragged tails (and the degenerate N=1,2): 32 x 32 tiles
+    up to N = 512, 64 x 64 up to 1024, and above that the persistent 128 x 128 kernel, whose 45 / 66 tiles at
+    N = 1100 / 1283 are all split along K across the 148 CTAs (stream-K hand-off of partial accumulators)."""
     rng = np.random.default_rng(1000 + N)
     X = rng.uniform(-1, 1, size=(N, N)) / np.sqrt(N)
     X = np.triu(X) + np.triu(X, 1).T
