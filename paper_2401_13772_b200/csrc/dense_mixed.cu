@@ -18,7 +18,8 @@
 //
 // Roles (384 threads): warp 0 = TMA producer (one lane), warp 1 = MMA issuer (one lane), warp 2 = TMEM allocator,
 // warps 4..11 = epilogue (thread <-> one accumulator row, 64 columns).  Shared memory: STAGES x { A planes ; B planes }
-// of 128 rows x 32 elements (64-byte rows, SWIZZLE_64B, K-major UMMA canonical layout).
+// of 128 rows x BK elements (K-major UMMA canonical layout; 128-byte rows / SWIZZLE_128B for the two-plane split,
+// 64-byte rows / SWIZZLE_64B for the three-plane split).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -28,9 +29,7 @@ namespace bmlsp2 {
 
 constexpr int M_BM = 128;
 constexpr int M_BN = 128;
-constexpr int M_BK = 32;                       // 16-bit elements per k-slab = 64 bytes = one SWIZZLE_64B row
-constexpr int M_KC_SLABS = 4;                  // K-chunk promoted to FP64 = 4 slabs = 128 columns
-constexpr int M_PLANE_TILE = M_BM * M_BK * 2;  // 8 KB
+constexpr int M_KC = 128;                      // K-chunk promoted to FP64 (columns)
 constexpr int M_EPI_WARPS = 8;
 constexpr int M_CTRL_WARPS = 4;
 constexpr int M_THREADS = (M_CTRL_WARPS + M_EPI_WARPS) * 32;
@@ -41,13 +40,15 @@ constexpr int M_MAX_PLANES = 3;
 enum { MV_F16X2 = 1, MV_BF16X3 = 2 };          // = bml_sp2_params_t::precision
 
 template <int V> struct MixedCfg;
+// BK = 16-bit elements per k-slab: one shared-memory row of the K-major operand tile.  128-byte rows (SWIZZLE_128B)
+// make every TMA request a full L2 line; the three-plane variant only has room for 64-byte rows (SWIZZLE_64B).
 template <> struct MixedCfg<MV_F16X2> {
-    static constexpr int PLANES = 2, STAGES = 6, ACC_COLS = 256;    // hh | hl + lh
-    static constexpr uint32_t FMT = 0;                              // F16
+    static constexpr int PLANES = 2, BK = 64, STAGES = 3, ACC_COLS = 256;    // accumulator: hh | hl + lh
+    static constexpr uint32_t FMT = 0;                                       // F16
 };
 template <> struct MixedCfg<MV_BF16X3> {
-    static constexpr int PLANES = 3, STAGES = 4, ACC_COLS = 128;
-    static constexpr uint32_t FMT = 1;                              // BF16
+    static constexpr int PLANES = 3, BK = 32, STAGES = 4, ACC_COLS = 128;
+    static constexpr uint32_t FMT = 1;                                       // BF16
 };
 
 // tcgen05 instruction descriptor (kind::f16): D = F32, A/B format, both K-major, N, M = 128
@@ -56,10 +57,13 @@ __host__ __device__ constexpr uint32_t m_idesc(uint32_t fmt, int n)
     return (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(M_BM >> 4) << 24);
 }
 
-// shared-memory matrix descriptor: K-major, SWIZZLE_64B, 8-row groups 512 bytes apart, sm_100 descriptor version 1
+// shared-memory matrix descriptor: K-major, rows of ROW_BYTES (64: SWIZZLE_64B, 128: SWIZZLE_128B), 8-row groups
+// 8 * ROW_BYTES apart, sm_100 descriptor version 1
+template <int ROW_BYTES>
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr)
 {
-    return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)(512u >> 4) << 32) | (1ull << 46) | (4ull << 61);
+    constexpr uint64_t layout = ROW_BYTES == 128 ? 2ull : 4ull;
+    return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((8u * ROW_BYTES) >> 4) << 32) | (1ull << 46) | (layout << 61);
 }
 
 __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
@@ -138,7 +142,8 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
                       double *__restrict__ partials)
 {
     using Cfg = MixedCfg<V>;
-    constexpr int PLANES = Cfg::PLANES, STAGES = Cfg::STAGES, ACC_COLS = Cfg::ACC_COLS;
+    constexpr int PLANES = Cfg::PLANES, STAGES = Cfg::STAGES, ACC_COLS = Cfg::ACC_COLS, M_BK = Cfg::BK;
+    constexpr int M_PLANE_TILE = M_BM * M_BK * 2, M_KC_SLABS = M_KC / M_BK, ROWB = M_BK * 2;
     constexpr int STAGE_BYTES = 2 * PLANES * M_PLANE_TILE;
     if (ctl->done) return;
     const int parity = ctl->parity;
@@ -224,8 +229,8 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
                 const uint32_t d_tmem = tmem_base + (uint32_t)(buf * ACC_COLS);
                 if (V == MV_F16X2) {
                     // planes of one operand are adjacent in shared memory: [Bh ; Bl] is one 256-row K-major operand
-                    const uint64_t ah = umma_desc(a_base), al = umma_desc(a_base + M_PLANE_TILE);
-                    const uint64_t bh = umma_desc(b_base);
+                    const uint64_t ah = umma_desc<ROWB>(a_base), al = umma_desc<ROWB>(a_base + M_PLANE_TILE);
+                    const uint64_t bh = umma_desc<ROWB>(b_base);
 #pragma unroll
                     for (int ks = 0; ks < M_BK / 16; ++ks) {   // UMMA_K = 16 elements = 32 bytes = 2 descriptor units
                         umma_f16(d_tmem, ah + 2 * ks, bh + 2 * ks, m_idesc(Cfg::FMT, 256), (within | ks) != 0 ? 1u : 0u);
@@ -237,8 +242,8 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
                     const int tb[6] = {2, 0, 1, 1, 0, 0};
 #pragma unroll
                     for (int t = 0; t < 6; ++t) {
-                        const uint64_t ad = umma_desc(a_base + ta[t] * M_PLANE_TILE);
-                        const uint64_t bd = umma_desc(b_base + tb[t] * M_PLANE_TILE);
+                        const uint64_t ad = umma_desc<ROWB>(a_base + ta[t] * M_PLANE_TILE);
+                        const uint64_t bd = umma_desc<ROWB>(b_base + tb[t] * M_PLANE_TILE);
 #pragma unroll
                         for (int ks = 0; ks < M_BK / 16; ++ks)
                             umma_f16(d_tmem, ad + 2 * ks, bd + 2 * ks, m_idesc(Cfg::FMT, 128), (within | t | ks) != 0 ? 1u : 0u);
@@ -367,10 +372,11 @@ static int make_plane_map(CUtensorMap *map, const uint16_t *base, int64_t N, int
     if (!enc) return BML_ERR_CUDA;
     const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)(MixedCfg<V>::PLANES * N)};
     const cuuint64_t strides[1] = {(cuuint64_t)ldp * sizeof(uint16_t)};
-    const cuuint32_t box[2] = {(cuuint32_t)M_BK, (cuuint32_t)M_BM};
+    const cuuint32_t box[2] = {(cuuint32_t)MixedCfg<V>::BK, (cuuint32_t)M_BM};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(map, V == MV_F16X2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
-                     (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                     (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     MixedCfg<V>::BK == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
 }
@@ -396,8 +402,8 @@ template <int V>
 static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double *b0, double *b1, uint16_t *p0,
                            uint16_t *p1, int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t st)
 {
-    constexpr size_t smem = (size_t)MixedCfg<V>::STAGES * 2 * MixedCfg<V>::PLANES * M_PLANE_TILE + 1024 /*align*/ +
-                            1024 /*barriers, scratch*/;
+    constexpr size_t smem = (size_t)MixedCfg<V>::STAGES * 2 * MixedCfg<V>::PLANES * (M_BM * MixedCfg<V>::BK * 2) +
+                            1024 /*align*/ + 1024 /*barriers, scratch*/;
     static bool attr_set = false;
     if (!attr_set) {
         if (cudaFuncSetAttribute(x2_dense_mixed_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
