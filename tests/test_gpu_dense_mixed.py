@@ -4,8 +4,9 @@ accumulation promoted to FP64 every 128 columns, FP64 traces / norms / updates.
 
 The oracle of this mode is the FP64 CPU oracle run with the mixed config's tolerance (1e-6).  Required (north_star):
 identical branch string and product count, relative Frobenius error of D <= 1e-5.  One product is held to
-relFro <= 3e-6 (three BF16 planes keep 24 mantissa bits, the six cross
-terms drop relative 2^-23, and the truncating FP32 accumulation over a 128-column chunk adds <= 48 x 2^-24)."""
+relFro <= 3e-6 (DESIGN.md 5.3 "Error budget": the planes keep 22-24 mantissa bits, the dropped cross terms are
+<= 2^-22, and the truncating FP32 accumulation over a 128-column chunk adds a bias of up to 48 x 2^-24; measured
+3.7e-7 for the FP16 split and 9e-7 for the BF16 split)."""
 import numpy as np
 import pytest
 
