@@ -337,7 +337,9 @@ def run_ours(args):
         achieved = flops / (k_ms * 1e-3) / 1e12
         nominal_ratio_peak = pk["bf16_tflops"] * (40.0 / 2250.0)
         roof = {
-            "bound": "tensor", "kernel": "x2_dense_fp64_kernel", "achieved": achieved, "peak": peak_probe,
+            "bound": "tensor",
+            "kernel": "x2_dense_fp64_sk_kernel" if w.N > 1024 else "x2_dense_fp64_kernel<%d>" % (32 if w.N <= 512 else 64),
+            "achieved": achieved, "peak": peak_probe,
             "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
             "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
                            "(MEASURED_PEAKS.json has no FP64 entry)",
