@@ -359,7 +359,7 @@ x2_ellpack_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__
         // ---------------- phase C: select X' entries, compact (j, slot) into the sort buffer ----------------
         for (int s0 = 0; s0 < E_SLOTS; s0 += E_GT) {
             const int s = s0 + tg;
-            const int key = keys[s];
+            const int key = s < E_SLOTS ? keys[s] : E_EMPTY;
             bool keep = false;
             int j = 0;
             if (key != E_EMPTY) {
