@@ -227,3 +227,48 @@ def test_config3_n8192_one_product_sampled_and_solve_invariants(api, oracle_mod)
     assert (torch.linalg.norm(D2 - D) / torch.linalg.norm(D)).item() < 10 * w.idem_tol
     Hg = to_gpu(H)
     assert (torch.linalg.norm(Hg @ D - D @ Hg) / torch.linalg.norm(Hg)).item() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ properties (T3)
+def test_sp2_persistent_kernel_full_parity_n1152(api, oracle_mod):
+    """N = 1152 (> 1024) runs the persistent 128 x 128 kernel: 45 tiles on 148 CTAs, every tile split along K and
+    reassembled from FP64 partials.  Full solve against the oracle, element by element."""
+    H = hm.small_long_range((12, 12, 8))
+    D, res, _ = _check_solve(api, oracle_mod, H, H.shape[0] // 2, 1e-10)
+    assert res.status == 0
+    assert np.linalg.norm(H @ D - D @ H) / np.linalg.norm(H) < 1e-12
+
+
+@pytest.mark.parametrize("a,b", [(3.0, 0.0), (0.25, -7.5), (1.0, 100.0)])
+def test_sp2_shift_scale_invariance_on_gpu(api, a, b):
+    """H -> a H + b I (a > 0) leaves X_0, hence the branch string, m* and D unchanged (SURVEY 8(c) pins)."""
+    H, _ = hm.planted_gap(150, 60, gap=1.0, width=2.0, seed=11)
+    D0, r0 = api.bml_sp2_dense(to_gpu(H), 60, 1e-10)
+    D1, r1 = api.bml_sp2_dense(to_gpu(a * H + b * np.eye(150)), 60, 1e-10)
+    assert r0.status == r1.status == 0
+    assert r1.branch == r0.branch and r1.n_products == r0.n_products
+    assert relfro(D1.cpu().numpy(), D0.cpu().numpy()) < 1e-11
+
+
+def test_sp2_permutation_similarity_on_gpu(api):
+    """H -> P H P^T gives P D P^T with the same branch string (tile assignment must not matter)."""
+    N, n_occ = 700, 300          # 64 x 64 tiles, ragged
+    H, _ = hm.planted_gap(N, n_occ, gap=1.0, width=2.0, seed=12)
+    perm = np.random.default_rng(1).permutation(N)
+    Hp = H[np.ix_(perm, perm)]
+    D0, r0 = api.bml_sp2_dense(to_gpu(H), n_occ, 1e-10)
+    D1, r1 = api.bml_sp2_dense(to_gpu(Hp), n_occ, 1e-10)
+    assert r0.status == r1.status == 0 and r1.branch == r0.branch
+    assert relfro(D1.cpu().numpy(), D0.cpu().numpy()[np.ix_(perm, perm)]) < 1e-11
+
+
+def test_sp2_dense_is_bit_reproducible(api):
+    """Fixed-order reductions and the fixed stream-K summation order: two solves of the same H give the same bits."""
+    H = hm.small_long_range((12, 12, 8))
+    D0, r0 = api.bml_sp2_dense(to_gpu(H), 576, 1e-10)
+    D0 = D0.clone()
+    D1, r1 = api.bml_sp2_dense(to_gpu(H), 576, 1e-10)
+    import torch
+
+    assert torch.equal(D0, D1)
+    assert np.array_equal(r0.trace, r1.trace) and np.array_equal(r0.idem, r1.idem)
