@@ -151,13 +151,14 @@ BML_API int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bm
  *   are in ascending column order.  Xnext <- branch ? thr(2X - thr(X*X)) : thr(X*X).  d_sums: DEVICE double[4] <-
  *   { tr thr(X*X), ||thr(X*X) - X||_F^2 over the union pattern, ||X||_F^2, tr(Xnext) };
  *   d_info: DEVICE int32[4] <- { lowest row with > M kept entries or INT32_MAX, lowest row exceeding the accumulator
- *   or INT32_MAX, max kept row length, 0 }.  d_workspace >= bml_x2_ellpack_workspace_bytes(N).
+ *   or INT32_MAX, max kept row length, 0 }.  d_workspace >= bml_x2_ellpack_workspace_bytes(N, M).
+ *   X must be bitwise symmetric (X_ij == X_ji): row i is accumulated for the columns j >= i only and mirrored.
  * Asynchronous.  Return 0, -1 or -4.
  */
 BML_API size_t bml_x2_dense_workspace_bytes(int64_t N, int32_t precision);
 BML_API int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int32_t precision, double *d_sums,
                  void *d_workspace, size_t workspace_bytes, void *cuda_stream);
-BML_API size_t bml_x2_ellpack_workspace_bytes(int64_t N);
+BML_API size_t bml_x2_ellpack_workspace_bytes(int64_t N, int32_t M);
 BML_API int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, double drop_tol, double *d_sums,
                    int32_t *d_info, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 

@@ -104,7 +104,7 @@ def load(build_if_missing: bool = True):
     L.bml_x2_dense.restype = ctypes.c_int
     L.bml_x2_dense.argtypes = [MP, MP, i32, i32, vp, vp, sz, vp]
     L.bml_x2_ellpack_workspace_bytes.restype = sz
-    L.bml_x2_ellpack_workspace_bytes.argtypes = [i64]
+    L.bml_x2_ellpack_workspace_bytes.argtypes = [i64, ctypes.c_int32]
     L.bml_x2_ellpack.restype = ctypes.c_int
     L.bml_x2_ellpack.argtypes = [MP, MP, i32, dbl, vp, vp, vp, sz, vp]
     L.bml_probe_fp64_tensor_peak.restype = ctypes.c_int
@@ -326,7 +326,7 @@ def bml_x2_ellpack(X, branch: int, drop_tol: float, out=None, ws=None):
     o = ellpack_desc(*out)
     sums = torch.empty(4, dtype=torch.float64, device=value.device)
     info = torch.empty(4, dtype=torch.int32, device=value.device)
-    nbytes = L.bml_x2_ellpack_workspace_bytes(x.N)
+    nbytes = L.bml_x2_ellpack_workspace_bytes(x.N, x.M)
     if ws is None:
         ws = _workspace(nbytes, value.device)
     rc = L.bml_x2_ellpack(ctypes.byref(x), ctypes.byref(o), int(branch), float(drop_tol), sums.data_ptr(),

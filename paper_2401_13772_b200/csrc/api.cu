@@ -34,8 +34,10 @@ int launch_copy_out_dense(const double *buf0, const double *buf1, int64_t ldx, i
 size_t ellpack_rowstats_bytes(int64_t N);
 int launch_rescale_ellpack(const bml_matrix_t *H, const double *d_bounds, double *xv, int32_t *xi, int32_t *xn,
                            double *rowstats, double *d_tr0, int *fail_flag, cudaStream_t st);
+size_t ellpack_sym_bytes(int64_t N, int M);
+int ellpack_sym_reset(void *sym, int64_t N, int M, cudaStream_t st);
 int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, double *v1, int32_t *i1, int32_t *n1,
-                      int64_t N, int M, double tau, Sp2Ctl *ctl, double *rowstats, cudaStream_t st);
+                      int64_t N, int M, double tau, Sp2Ctl *ctl, double *rowstats, void *sym, cudaStream_t st);
 int launch_copy_out_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, const double *v1,
                             const int32_t *i1, const int32_t *n1, int64_t N, int M, const Sp2Ctl *ctl, double *dv,
                             int32_t *di, int32_t *dn, cudaStream_t st);
@@ -114,6 +116,7 @@ struct EllWs {
     Sp2Ctl *ctl;
     ScalarSlots *scal;
     double *rowlh, *rowstats;
+    void *sym;          // scratch of the symmetric product (upper parts + lower lists)
     double *v0, *v1;
     int32_t *i0, *i1, *n0, *n1;
     size_t total;
@@ -128,6 +131,7 @@ static EllWs carve_ell(void *ws, int64_t N, int M, bool with_buffers)
     w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
     w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
     w.rowstats = (double *)(p + off); off = align_up(off + ellpack_rowstats_bytes(N), 1024);
+    w.sym = (void *)(p + off); off = align_up(off + ellpack_sym_bytes(N, M), 1024);
     w.v0 = w.v1 = nullptr; w.i0 = w.i1 = w.n0 = w.n1 = nullptr;
     if (with_buffers) {
         const size_t nm = (size_t)N * (size_t)M;
@@ -339,17 +343,18 @@ int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix
     TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowlh, &w.scal->tr0, w.scal->fail_flag, st));
     TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                         w.scal->fail_flag, st));
+    TRY(ellpack_sym_reset(w.sym, N, M, st));
     TRY(enqueue_products([&]() { return launch_x2_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, p->drop_tol, w.ctl,
-                                                          w.rowstats, st); },
+                                                          w.rowstats, w.sym, st); },
                          w.ctl, p->max_products, st));                                            // S2-S5
     TRY(launch_copy_out_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, w.ctl, D->value, D->index, D->nnz, st));
     return finish_solve(w.ctl, stats, st);
 }
 
-size_t bml_x2_ellpack_workspace_bytes(int64_t N)
+size_t bml_x2_ellpack_workspace_bytes(int64_t N, int32_t M)
 {
-    if (N <= 0) return 0;
-    return carve_ell(nullptr, N, 1, false).total;
+    if (N <= 0 || M < 1) return 0;
+    return carve_ell(nullptr, N, M, false).total;
 }
 
 int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, double drop_tol, double *d_sums,
@@ -358,14 +363,15 @@ int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, d
     if (!ell_ok(X) || !ell_ok(Xnext) || X->N != Xnext->N || X->M != Xnext->M || X->value == Xnext->value ||
         X->index == Xnext->index || X->nnz == Xnext->nnz || !d_sums || !d_info || !d_workspace ||
         ((uintptr_t)d_workspace & 1023) != 0 || !(drop_tol >= 0.0) ||
-        workspace_bytes < bml_x2_ellpack_workspace_bytes(X->N))
+        workspace_bytes < bml_x2_ellpack_workspace_bytes(X->N, X->M))
         return BML_ERR_INVALID;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     EllWs w = carve_ell(d_workspace, X->N, X->M, false);
     int r = launch_init_ctl(w.ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
     if (r) return r;
+    if ((r = ellpack_sym_reset(w.sym, X->N, X->M, st))) return r;
     r = launch_x2_ellpack(X->value, X->index, X->nnz, Xnext->value, Xnext->index, Xnext->nnz, X->N, X->M, drop_tol,
-                          w.ctl, w.rowstats, st);
+                          w.ctl, w.rowstats, w.sym, st);
     if (r) return r;
     if (cudaMemcpyAsync(d_sums, w.ctl->sums, 4 * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
         return BML_ERR_CUDA;

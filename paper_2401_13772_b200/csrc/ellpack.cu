@@ -1,13 +1,17 @@
 // ellpack.cu -- the sparse path of DESIGN.md on ELLPACK-R (Listing 1): S1 rescale, S3 thresholded row-wise
 // SpGEMM X*X, S4 fused update / norms / canonical (ascending-column) write-back, S5 finaliser.
 //
-// Gustavson row merge ("sparse-sparse matrix multiply").  A GROUP of E_GW warps owns one output row at a time;
-// E_MAX_GROUPS groups share a CTA (one CTA per SM), each with its own open-addressing hash accumulator in shared
-// memory (BML_ELL_ACC_SLOTS keys + FP64 values).  For every stored entry p of row i (ascending p) the group's 128
-// threads take the entries of row k = index[i][p] (unique columns, one or more per thread) and do
-// acc[j] = fma(x_ik, x_kj, acc[j]); a group barrier separates step p from step p+1.  Contributions to one output
-// entry are therefore added in order of increasing p, each as one fma: the canonical order of the oracle (DESIGN.md
-// readings item 11) -- values are bit-identical to it, not merely close.
+// Gustavson row merge ("sparse-sparse matrix multiply") in two kernels per product:
+//   x2_ellpack_upper_kernel    row i of thr(X X) for the columns j >= i only (X is bitwise symmetric, so P_ij and P_ji
+//                              are the same chain of fma's); every kept entry is also appended to the list of row j
+//   x2_ellpack_assemble_kernel full row = sorted(appended entries) ++ upper part; update, threshold, norms, write-back
+// Kernel 1: a GROUP of E_GW warps owns one output row at a time; E_MAX_GROUPS groups share a CTA (one CTA per SM),
+// each with its own open-addressing hash accumulator in shared memory (BML_ELL_ACC_SLOTS keys + FP64 values).  For
+// every stored entry p of row i (ascending p) the group's 128 threads take the entries of row k = index[i][p] with
+// column >= i (a suffix found by binary search while row i is staged) and do acc[j] = fma(x_ik, x_kj, acc[j]); a
+// group barrier separates step p from step p+1.  Contributions to one output entry are therefore added in order of
+// increasing p, each as one fma: the canonical order of the oracle (readings item 11) -- values are
+// bit-identical to it, not merely close.
 //
 // The gathers of rows k are issued two p-steps ahead into registers (coalesced: a warp reads 32 consecutive slots of
 // row k), so their L2 latency is hidden behind the hash updates of the current step.  The hash keeps 32 consecutive
@@ -23,9 +27,6 @@ constexpr int E_BUCKETS = E_SLOTS / 32;
 constexpr int E_BUCKET_SHIFT = 32 - 7;  // log2(E_BUCKETS) = 7
 static_assert(E_BUCKETS == 128, "bucket hash is written for 4096 slots");
 constexpr int E_EMPTY = -1;
-constexpr int E_DROPPED = 1 << 30;    // P entry fell below tau (value zeroed)
-constexpr int E_INX = 1 << 29;        // column also present in row i of X
-constexpr int E_KEY = (1 << 29) - 1;
 constexpr int E_GW = 4;               // warps per row group
 constexpr int E_GT = E_GW * 32;       // threads per row group
 constexpr int E_MAX_GROUPS = 4;       // row groups (= rows in flight) per CTA
@@ -148,84 +149,265 @@ __device__ __forceinline__ int e_probe_insert(int *keys, double *vals, int j, in
     }
 }
 
+// ============================================================================================================
+// Symmetric evaluation (the default path).  X is bitwise symmetric, so P_ij and P_ji are the same chain of fma's
+// (same products x_ik x_kj = x_jk x_ki, same ascending k): bit-identical.  Kernel 1 therefore accumulates, for row i,
+// only the columns j >= i: of every gathered row k it takes the SUFFIX starting at the first column >= i (found by
+// binary search while row i is staged), which halves the multiply-adds.  It thresholds and sorts that upper part,
+// stores it, and appends a copy (i, P_ij) to the "lower list" of every row j > i.  Kernel 2 assembles each full row of
+// P = sorted(lower list) ++ upper part and runs the fused update / threshold / norms / write-back against row i of X.
+// ============================================================================================================
+
+// gather of the suffix of row k = sk[p]: sn[p] = (first slot << 16) | count
 template <int CC>
-__device__ __forceinline__ void e_gather(Gather<CC> &g, int p, int n_i, const double *__restrict__ xv,
+__device__ __forceinline__ void s_gather(Gather<CC> &g, int &cnt, int p, int n_i, const double *__restrict__ xv,
                                          const int32_t *__restrict__ xi, int M, const int *sk, const int *sn, int tg)
 {
 #pragma unroll
     for (int c = 0; c < CC; ++c) { g.j[c] = -1; g.v[c] = 0.0; }
+    cnt = 0;
     if (p < n_i) {
-        const int n_k = sn[p];
-        const int32_t *pi = xi + (int64_t)sk[p] * M + tg;
-        const double *pv = xv + (int64_t)sk[p] * M + tg;
+        const int pk = sn[p];
+        const int n_k = pk & 0xffff;
+        cnt = n_k;
+        const int64_t base = (int64_t)sk[p] * M + (pk >> 16) + tg;
+        const int32_t *pi = xi + base;
+        const double *pv = xv + base;
 #pragma unroll
         for (int c = 0; c < CC; ++c) {
-            if (c * E_GT + tg < n_k) { g.j[c] = __ldg(pi + c * E_GT); g.v[c] = __ldg(pv + c * E_GT); }
+            if (c * E_GT < n_k) {             // group-uniform: chunks beyond the suffix issue nothing
+                if (c * E_GT + tg < n_k) { g.j[c] = __ldg(pi + c * E_GT); g.v[c] = __ldg(pv + c * E_GT); }
+            }
         }
     }
 }
 
-template <int CC>
-__device__ __forceinline__ bool e_accumulate(const Gather<CC> &g, double a, int *keys, double *vals)
+// hash update of the first NC chunks of a gathered suffix (straight-line: the NC lookups are independent)
+template <int NC, int CC>
+__device__ __forceinline__ bool s_accumulate(const Gather<CC> &g, double a, int *keys, double *vals)
 {
-    int slot[CC], key[CC];
+    static_assert(NC <= CC, "chunk count");
+    int slot[NC], key[NC];
     bool full = false;
 #pragma unroll
-    for (int c = 0; c < CC; ++c) slot[c] = e_hash(g.j[c]);
+    for (int c = 0; c < NC; ++c) slot[c] = e_hash(g.j[c]);
 #pragma unroll
-    for (int c = 0; c < CC; ++c) key[c] = keys[slot[c]];
+    for (int c = 0; c < NC; ++c) key[c] = keys[slot[c]];
 #pragma unroll
-    for (int c = 0; c < CC; ++c) {
+    for (int c = 0; c < NC; ++c) {
         if (g.j[c] >= 0 && key[c] != g.j[c]) {
             slot[c] = e_probe_insert(keys, vals, g.j[c], slot[c], key[c]);
             if (slot[c] < 0) { full = true; slot[c] = 0; }
         }
     }
-    double acc[CC];
+    double acc[NC];
 #pragma unroll
-    for (int c = 0; c < CC; ++c) acc[c] = vals[slot[c]];
+    for (int c = 0; c < NC; ++c) acc[c] = vals[slot[c]];
 #pragma unroll
-    for (int c = 0; c < CC; ++c)
+    for (int c = 0; c < NC; ++c)
         if (g.j[c] >= 0 && !full) vals[slot[c]] = fma(a, g.v[c], acc[c]);
     return full;
 }
 
-// gathers run two p-steps ahead of the accumulation (three register buffers, rotated by unrolling)
+// one p-step: dispatch on the number of E_GT-entry chunks the suffix really has (group-uniform), then the group
+// barrier that orders step p before step p + 1; an empty suffix costs nothing
 template <int CC>
-__device__ __forceinline__ bool accumulate_row(const double *__restrict__ xv, const int32_t *__restrict__ xi, int M,
-                                               int n_i, const double *sa, const int *sk, const int *sn, int *keys,
-                                               double *vals, int tg, int grp)
+__device__ __forceinline__ bool s_step(const Gather<CC> &g, int cnt, double a, int *keys, double *vals, int grp, bool full)
 {
-    bool full = false;      // this thread ran out of accumulator slots
+    if (cnt <= 0) return full;
+    const int nc = (cnt + E_GT - 1) / E_GT;
+    if (nc == 1) full |= s_accumulate<1, CC>(g, a, keys, vals);
+    else if (CC >= 2 && nc == 2) full |= s_accumulate<(CC >= 2 ? 2 : CC), CC>(g, a, keys, vals);
+    else if (CC >= 3 && nc == 3) full |= s_accumulate<(CC >= 3 ? 3 : CC), CC>(g, a, keys, vals);
+    else if (CC >= 4 && nc == 4) full |= s_accumulate<(CC >= 4 ? 4 : CC), CC>(g, a, keys, vals);
+    else full |= s_accumulate<CC, CC>(g, a, keys, vals);
+    return group_bar_or(grp, full);
+}
+
+template <int CC>
+__device__ __forceinline__ bool s_accumulate_row(const double *__restrict__ xv, const int32_t *__restrict__ xi, int M,
+                                                 int n_i, const double *sa, const int *sk, const int *sn, int *keys,
+                                                 double *vals, int tg, int grp)
+{
+    bool full = false;
     Gather<CC> gA, gB, gC;
-    e_gather<CC>(gA, 0, n_i, xv, xi, M, sk, sn, tg);
-    e_gather<CC>(gB, 1, n_i, xv, xi, M, sk, sn, tg);
+    int nA, nB, nC;
+    s_gather<CC>(gA, nA, 0, n_i, xv, xi, M, sk, sn, tg);
+    s_gather<CC>(gB, nB, 1, n_i, xv, xi, M, sk, sn, tg);
     for (int p = 0; p < n_i; p += 3) {
-        e_gather<CC>(gC, p + 2, n_i, xv, xi, M, sk, sn, tg);
-        full |= e_accumulate<CC>(gA, sa[p], keys, vals);
-        full = group_bar_or(grp, full);
+        s_gather<CC>(gC, nC, p + 2, n_i, xv, xi, M, sk, sn, tg);
+        full = s_step<CC>(gA, nA, sa[p], keys, vals, grp, full);
         if (p + 1 < n_i) {
-            e_gather<CC>(gA, p + 3, n_i, xv, xi, M, sk, sn, tg);
-            full |= e_accumulate<CC>(gB, sa[p + 1], keys, vals);
-            full = group_bar_or(grp, full);
+            s_gather<CC>(gA, nA, p + 3, n_i, xv, xi, M, sk, sn, tg);
+            full = s_step<CC>(gB, nB, sa[p + 1], keys, vals, grp, full);
         }
         if (p + 2 < n_i) {
-            e_gather<CC>(gB, p + 4, n_i, xv, xi, M, sk, sn, tg);
-            full |= e_accumulate<CC>(gC, sa[p + 2], keys, vals);
-            full = group_bar_or(grp, full);
+            s_gather<CC>(gB, nB, p + 4, n_i, xv, xi, M, sk, sn, tg);
+            full = s_step<CC>(gC, nC, sa[p + 2], keys, vals, grp, full);
         }
-        if (full) break;     // group-uniform: every thread got the same OR at the same barrier
+        if (full) break;
     }
     return full;
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// S3 + S4: thresholded row product, fused update, norms, sorted write-back.
+// Kernel 1 (S3, upper half): P_ij for j >= i, thresholded, sorted; lower copies appended to the rows j > i.
+//   tv/ti/tn : upper part of thr(X X), row-major ELLPACK-R (ascending columns)
+//   lv/li/lcnt : per row j, the entries (i, P_ji = P_ij) with i < j, in arrival order; lcnt[j] counts ALL arrivals
+//                (slots beyond M are not written: the row has overflowed then anyway)
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(E_MAX_GROUPS * E_GT, 1)
-x2_ellpack_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__restrict__ n0,
-                  double *__restrict__ v1, int32_t *__restrict__ i1, int32_t *__restrict__ n1, int N, int M,
-                  double tau, int sort_cap, Sp2Ctl *__restrict__ ctl, double *__restrict__ partials)
+x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
+                        const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
+                        int N, int M, double tau, int sort_cap, Sp2Ctl *__restrict__ ctl, double *__restrict__ tv,
+                        int32_t *__restrict__ ti, int32_t *__restrict__ tn, double *__restrict__ lv,
+                        int32_t *__restrict__ li, int32_t *__restrict__ lcnt)
+{
+    if (ctl->done) return;
+    const int parity = ctl->parity;
+    const double *__restrict__ xv = parity ? v1 : v0;
+    const int32_t *__restrict__ xi = parity ? i1 : i0;
+    const int32_t *__restrict__ xn = parity ? n1 : n0;
+
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int ngroups = blockDim.x / E_GT;
+    const int grp = threadIdx.x / E_GT, tg = threadIdx.x % E_GT, lane = threadIdx.x & 31;
+    uint8_t *gbase = smem + (size_t)grp * ((size_t)E_SLOTS * 12 + (size_t)sort_cap * 8);
+    double *vals = (double *)gbase;
+    int *keys = (int *)(gbase + (size_t)E_SLOTS * 8);
+    uint8_t *scratch = gbase + (size_t)E_SLOTS * 12;
+    double *sa = (double *)scratch;
+    int *sk = (int *)(scratch + (size_t)8 * M);
+    int *sn = sk + M;
+    unsigned long long *sortbuf = (unsigned long long *)scratch;     // aliases sa/sk/sn after the accumulation
+    __shared__ int s_kept[E_MAX_GROUPS], s_nkmax[E_MAX_GROUPS][2];
+
+    int w_acc = INT32_MAX;
+    if (tg == 0) { s_nkmax[grp][0] = 0; s_nkmax[grp][1] = 0; }
+    group_bar(grp);
+    int it = 0;
+    for (int64_t row64 = (int64_t)blockIdx.x * ngroups + grp; row64 < N; row64 += (int64_t)gridDim.x * ngroups) {
+        const int row = (int)row64;
+        const int64_t rbase = (int64_t)row * M;
+        const int n_i = min(xn[row], M);
+        {
+            int4 *k4 = (int4 *)keys;
+            const int4 e4 = make_int4(E_EMPTY, E_EMPTY, E_EMPTY, E_EMPTY);
+            for (int s = tg; s < E_SLOTS / 4; s += E_GT) k4[s] = e4;
+        }
+        int nk_max = 0;
+        for (int p = tg; p < n_i; p += E_GT) {
+            const int k = xi[rbase + p];
+            const int n_k = min(xn[k], M);
+            // first slot of row k whose column is >= row (rows are in ascending column order)
+            const int32_t *rk = xi + (int64_t)k * M;
+            int lo = 0, hi = n_k;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (__ldg(rk + mid) < row) lo = mid + 1; else hi = mid;
+            }
+            sk[p] = k;
+            sa[p] = xv[rbase + p];
+            sn[p] = (lo << 16) | (n_k - lo);
+            nk_max = max(nk_max, n_k - lo);
+        }
+        nk_max = __reduce_max_sync(0xffffffffu, nk_max);
+        if (lane == 0) atomicMax(&s_nkmax[grp][it & 1], nk_max);
+        if (tg == 0) { s_kept[grp] = 0; s_nkmax[grp][(it + 1) & 1] = 0; }
+        group_bar(grp);
+        const int chunks = (s_nkmax[grp][it & 1] + E_GT - 1) / E_GT;
+        ++it;
+
+        bool full;
+#define S_ACC(CC) full = s_accumulate_row<CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, tg, grp)
+        if (chunks <= 1) S_ACC(1);
+        else if (chunks == 2) S_ACC(2);
+        else if (chunks == 3) S_ACC(3);
+        else if (chunks == 4) S_ACC(4);
+        else if (chunks <= 6) S_ACC(6);
+        else S_ACC(8);
+#undef S_ACC
+        if (full) {                       // accumulator capacity exceeded: status -6
+            w_acc = min(w_acc, row);
+            if (tg == 0) tn[row] = 0;
+            group_bar(grp);
+            continue;
+        }
+
+        // threshold (keep |p| >= tau or the diagonal) and compact (column, slot) into the sort buffer
+        for (int s0 = 0; s0 < E_SLOTS; s0 += E_GT) {
+            const int s = s0 + tg;
+            const int key = s < E_SLOTS ? keys[s] : E_EMPTY;
+            const bool keep = key != E_EMPTY && (fabs(vals[s]) >= tau || key == row);
+            if (keep && key != row) {         // mirror: P_ji = P_ij, appended to row j = key (j > row); counts are exact
+                const int pos = atomicAdd(&lcnt[key], 1);
+                if (pos < M) { li[(int64_t)key * M + pos] = row; lv[(int64_t)key * M + pos] = vals[s]; }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            if (bal) {
+                int base = 0;
+                if (lane == 0) base = atomicAdd(&s_kept[grp], __popc(bal));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (keep) {
+                    const int pos = base + __popc(bal & ((1u << lane) - 1u));
+                    if (pos < sort_cap) sortbuf[pos] = ((unsigned long long)(unsigned)key << 32) | (unsigned)s;
+                }
+            }
+        }
+        group_bar(grp);
+        const int kept = s_kept[grp];
+        if (tg == 0) tn[row] = kept;          // may exceed M: kernel 2 turns that into the overflow status
+        const int nw = min(kept, min(M, sort_cap));
+        int n2 = 32;
+        while (n2 < nw) n2 <<= 1;
+        for (int q = nw + tg; q < n2; q += E_GT) sortbuf[q] = ~0ull;
+        // (entries beyond nw only exist when the row has overflowed; they are not needed then)
+        group_bitonic_sort(sortbuf, n2, tg, grp);
+        for (int q = tg; q < nw; q += E_GT) {
+            const unsigned long long e = sortbuf[q];
+            const int j = (int)(e >> 32);
+            const double v = vals[(int)(e & 0xffffffffu)];
+            ti[rbase + q] = j;
+            tv[rbase + q] = v;
+        }
+        group_bar(grp);
+    }
+    if (w_acc != INT32_MAX && tg == 0) atomicMin(&ctl->acc_row, w_acc);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Kernel 2 (S4 + S5): one warp per row.  P_i = sorted(lower list) ++ upper part; then, against row i of X:
+// ||P - X||^2 over the union pattern, ||X||^2, X' = b ? thr(2X - P) : P, tr P, tr X', sorted write-back, and the
+// last-CTA finaliser.  All sums run over sorted lists in a fixed lane-strided order: bit-reproducible.
+// Per-warp shared memory: pc[M] int, pf[M] uint8, pv[M] double, ec[M] int, ev[M] double, sortbuf[pow2(M)] u64 (a row
+// of P longer than M is an overflow and is not assembled).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int A_MAX_WARPS = 6;
+static inline size_t a_warp_bytes(int M)
+{
+    const size_t m = M < 16 ? 16 : M;
+    const size_t b = m * 4 + m + m * 8 + m * 4 + m * 8 + (size_t)next_pow2((int)m) * 8;
+    return (b + 63) / 64 * 64;
+}
+
+// first index q in [0, n) with c[q] >= key (c ascending)
+__device__ __forceinline__ int a_lower_bound(const int *c, int n, int key)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (c[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(A_MAX_WARPS * 32)
+x2_ellpack_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__restrict__ n0,
+                           double *__restrict__ v1, int32_t *__restrict__ i1, int32_t *__restrict__ n1, int N, int M,
+                           double tau, Sp2Ctl *__restrict__ ctl, double *__restrict__ partials,
+                           const double *__restrict__ tv, const int32_t *__restrict__ ti,
+                           const int32_t *__restrict__ tn, const double *__restrict__ lv,
+                           const int32_t *__restrict__ li, int32_t *__restrict__ lcnt, int warp_bytes)
 {
     if (ctl->done) return;
     const int parity = ctl->parity;
@@ -238,208 +420,163 @@ x2_ellpack_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__
     int32_t *__restrict__ on = parity ? n0 : n1;
 
     extern __shared__ __align__(16) uint8_t smem[];
-    const int ngroups = blockDim.x / E_GT;
-    const int grp = threadIdx.x / E_GT, tg = threadIdx.x % E_GT, wg = tg >> 5, lane = threadIdx.x & 31;
-    uint8_t *gbase = smem + (size_t)grp * ((size_t)E_SLOTS * 12 + (size_t)sort_cap * 8);
-    double *vals = (double *)gbase;                                  // [E_SLOTS]
-    int *keys = (int *)(gbase + (size_t)E_SLOTS * 8);                // [E_SLOTS]
-    uint8_t *scratch = gbase + (size_t)E_SLOTS * 12;
-    double *sa = (double *)scratch;                                  // [M] values of row i
-    int *sk = (int *)(scratch + (size_t)8 * M);                      // [M] columns of row i (= rows k to merge)
-    int *sn = sk + M;                                                // [M] nnz of those rows
-    unsigned long long *sortbuf = (unsigned long long *)scratch;     // aliases sa/sk/sn after phase B
-    __shared__ double s_part[E_MAX_GROUPS * E_GW][4];
-    __shared__ int s_cntp[E_MAX_GROUPS], s_kept[E_MAX_GROUPS], s_nkmax[E_MAX_GROUPS][2];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int m = M < 16 ? 16 : M;
+    int cap2 = 1;
+    while (cap2 < m) cap2 <<= 1;
+    uint8_t *wb = smem + (size_t)warp * warp_bytes;
+    double *pv = (double *)wb;                                           // [m] values of P_i, later of X'_i
+    double *ev = pv + m;                                                 // [m] kept X-only entries
+    unsigned long long *sortbuf = (unsigned long long *)(ev + m);        // [cap2]
+    int *pc = (int *)(sortbuf + cap2);                                   // [m] columns of P_i
+    int *ec = pc + m;                                                    // [m]
+    uint8_t *pf = (uint8_t *)(ec + m);                                   // [m] 0 = P only, 1 = in X and kept, 2 = in X, dropped
+    __shared__ double s_part[A_MAX_WARPS][4];
     __shared__ int s_last;
 
-    double w_trp = 0.0, w_e = 0.0, w_x = 0.0, w_trn = 0.0;          // this thread's running sums over its rows
-    int w_ovf_p = INT32_MAX, w_ovf_u = INT32_MAX, w_acc = INT32_MAX, w_max_p = 0, w_max_u = 0;   // group-uniform
+    double w_trp = 0.0, w_e = 0.0, w_x = 0.0, w_trn = 0.0;
+    int w_ovf_p = INT32_MAX, w_ovf_u = INT32_MAX, w_max_p = 0, w_max_u = 0;
 
-    if (tg == 0) { s_nkmax[grp][0] = 0; s_nkmax[grp][1] = 0; }
-    group_bar(grp);
-    int it = 0;
-    for (int64_t row64 = (int64_t)blockIdx.x * ngroups + grp; row64 < N; row64 += (int64_t)gridDim.x * ngroups) {
+    for (int64_t row64 = (int64_t)blockIdx.x * nwarps + warp; row64 < N; row64 += (int64_t)gridDim.x * nwarps) {
         const int row = (int)row64;
         const int64_t rbase = (int64_t)row * M;
         const int n_i = min(xn[row], M);
-        // clear the key table; stage row i
-        {
-            int4 *k4 = (int4 *)keys;
-            const int4 e4 = make_int4(E_EMPTY, E_EMPTY, E_EMPTY, E_EMPTY);
-            for (int s = tg; s < E_SLOTS / 4; s += E_GT) k4[s] = e4;
-        }
-        int nk_max = 0;
-        for (int p = tg; p < n_i; p += E_GT) {
-            const int k = xi[rbase + p];
-            const int n_k = min(xn[k], M);
-            sk[p] = k;
-            sa[p] = xv[rbase + p];
-            sn[p] = n_k;
-            nk_max = max(nk_max, n_k);
-        }
-        nk_max = __reduce_max_sync(0xffffffffu, nk_max);
-        if (lane == 0) atomicMax(&s_nkmax[grp][it & 1], nk_max);
-        // per-row counters: the previous row's readers are behind its closing barrier
-        if (tg == 0) { s_cntp[grp] = 0; s_kept[grp] = 0; s_nkmax[grp][(it + 1) & 1] = 0; }
-        group_bar(grp);
-        const int chunks = (s_nkmax[grp][it & 1] + E_GT - 1) / E_GT;     // group-uniform
-        ++it;
-
-        // ---------------- accumulate: acc[j] = fma(x_ik, x_kj, acc[j]), p ascending ----------------
-        bool full;
-#define E_ACC(CC) full = accumulate_row<CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, tg, grp)
-        if (chunks <= 1) E_ACC(1);
-        else if (chunks == 2) E_ACC(2);
-        else if (chunks == 3) E_ACC(3);
-        else if (chunks == 4) E_ACC(4);
-        else if (chunks <= 6) E_ACC(6);
-        else E_ACC(8);
-#undef E_ACC
-        if (full) {                       // accumulator capacity exceeded: status -6
-            w_acc = min(w_acc, row);
-            if (tg == 0) on[row] = 0;
-            group_bar(grp);
+        const int u_all = tn[row], l_all = lcnt[row];
+        __syncwarp();
+        if (lane == 0) lcnt[row] = 0;                 // ready for the next product
+        const int cnt_p = u_all + l_all;              // stored length of row i of P = thr(X X)
+        w_max_p = max(w_max_p, cnt_p);
+        if (cnt_p > M) {                              // ELLPACK-R overflow of P: status -3 in the finaliser
+            w_ovf_p = min(w_ovf_p, row);
+            if (lane == 0) on[row] = 0;
             continue;
         }
-
-        // ---------------- phase A: threshold P = thr_tau(X X) (keep |p| >= tau or the diagonal) ----------------
-        double r_trp = 0.0, r_e = 0.0, r_x = 0.0, r_trn = 0.0;
-        int cnt_p = 0;
-        for (int s = tg; s < E_SLOTS; s += E_GT) {
-            const int key = keys[s];
-            if (key != E_EMPTY) {
-                const double pv = vals[s];
-                if (fabs(pv) >= tau || key == row) {
-                    ++cnt_p;
-                    if (key == row) r_trp += pv;
-                } else {
-                    keys[s] = key | E_DROPPED;
-                    vals[s] = 0.0;
-                }
-            }
+        const int n_l = l_all, u = u_all, np = n_l + u;
+        // ---- lower part: sort the appended (row j, value) pairs by column
+        int n2 = 32;
+        while (n2 < n_l) n2 <<= 1;
+        for (int q = lane; q < n2; q += 32)
+            sortbuf[q] = q < n_l ? (((unsigned long long)(unsigned)li[rbase + q] << 32) | (unsigned)q) : ~0ull;
+        __syncwarp();
+        if (n_l > 1) warp_bitonic_sort(sortbuf, n2, lane);
+        for (int q = lane; q < n_l; q += 32) {
+            const unsigned long long e = sortbuf[q];
+            pc[q] = (int)(e >> 32);
+            pv[q] = lv[rbase + (int)(e & 0xffffffffu)];
+            pf[q] = 0;
         }
-        cnt_p = __reduce_add_sync(0xffffffffu, cnt_p);
-        if (lane == 0 && cnt_p) atomicAdd(&s_cntp[grp], cnt_p);
-        group_bar(grp);
-        // ---------------- phase B: entries of row i of X: norms, update value, mark ----------------
-        for (int p = tg; p < n_i; p += E_GT) {
-            const int j = sk[p];
-            const double x = sa[p];
-            // normally present (x_ii * x_ij touched it); a row stored without its diagonal may miss it: then P_ij is
-            // absent and the column enters the union pattern as an X-only entry (value 0, dropped)
-            int slot = e_hash(j), tries = 0;
-            const int stride = e_stride(j);
-            while (true) {
-                const int key = keys[slot];
-                if (key != E_EMPTY && (key & E_KEY) == j) break;
-                if (key == E_EMPTY) {
-                    const int old = atomicCAS(&keys[slot], E_EMPTY, j | E_DROPPED);
-                    if (old == E_EMPTY) { vals[slot] = 0.0; break; }
-                    if ((old & E_KEY) == j) break;
-                }
-                if (++tries > E_SLOTS) { full = true; slot = -1; break; }
-                slot = e_next(slot, tries, stride);
-            }
-            if (slot >= 0) {
-                const double pk = vals[slot];                                   // 0 if dropped
+        for (int q = lane; q < u; q += 32) {
+            pc[n_l + q] = ti[rbase + q];
+            pv[n_l + q] = tv[rbase + q];
+            pf[n_l + q] = 0;
+        }
+        __syncwarp();
+        // ---- entries of row i of X: match against P_i (binary search in the sorted columns), norms, update
+        double r_trp = 0.0, r_e = 0.0, r_x = 0.0, r_trn = 0.0;
+        int ne = 0;                                   // kept X-only entries (warp-uniform)
+        for (int p0 = 0; p0 < n_i; p0 += 32) {
+            const int p = p0 + lane;
+            bool keepx = false;
+            int j = 0;
+            double xnew = 0.0;
+            if (p < n_i) {
+                j = xi[rbase + p];
+                const double x = xv[rbase + p];
+                const int q = a_lower_bound(pc, np, j);
+                const bool found = q < np && pc[q] == j;
+                const double pk = found ? pv[q] : 0.0;            // absent from thr(X X): 0
                 const double d = pk - x;
                 r_e += d * d;
                 r_x += x * x;
-                keys[slot] |= E_INX;
-                if (branch) vals[slot] = 2.0 * x - pk;                          // Eq. 7 on the union pattern
-            }
-        }
-        if (group_bar_or(grp, full)) {
-            w_acc = min(w_acc, row);
-            if (tg == 0) on[row] = 0;
-            group_bar(grp);
-            continue;
-        }
-        cnt_p = s_cntp[grp];
-        // ---------------- phase C: select X' entries, compact (j, slot) into the sort buffer ----------------
-        for (int s0 = 0; s0 < E_SLOTS; s0 += E_GT) {
-            const int s = s0 + tg;
-            const int key = s < E_SLOTS ? keys[s] : E_EMPTY;
-            bool keep = false;
-            int j = 0;
-            if (key != E_EMPTY) {
-                j = key & E_KEY;
-                const double v = vals[s];
-                const bool inx = (key & E_INX) != 0, dropped = (key & E_DROPPED) != 0;
-                if (!inx) {
-                    // column only in P: X' = -p (branch) or p, kept iff P kept it; its (P - X)^2 = p^2 is added in
-                    // the sorted write-back pass so that the sum does not depend on which slot the key landed in
-                    if (!dropped) {
-                        keep = true;
-                        if (branch) vals[s] = -v;
-                    }
-                } else if (branch) {
-                    keep = (fabs(v) >= tau) || (j == row);
+                xnew = branch ? (2.0 * x - pk) : pk;              // Eq. 7 on the union pattern : Eq. 6
+                if (found) {
+                    if (j == row) r_trp += pk;
+                    const bool keep = branch ? (fabs(xnew) >= tau || j == row) : true;
+                    pv[q] = xnew;
+                    pf[q] = keep ? 1 : 2;
+                    if (keep && j == row) r_trn += xnew;
                 } else {
-                    keep = !dropped;
+                    keepx = branch && (fabs(xnew) >= tau || j == row);
+                    if (keepx && j == row) r_trn += xnew;
                 }
-                if (keep && j == row) r_trn += vals[s];
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, keepx);
+            if (keepx) {
+                const int pos = ne + __popc(bal & ((1u << lane) - 1u));
+                ec[pos] = j;
+                ev[pos] = xnew;
+            }
+            ne += __popc(bal);
+        }
+        __syncwarp();
+        // ---- columns only in P: (P - X)^2 = p^2, X' = -p (Eq. 7) or p, always kept; then compact the kept entries
+        int kept = 0;
+        for (int q0 = 0; q0 < np; q0 += 32) {
+            const int q = q0 + lane;
+            bool keep = false;
+            if (q < np) {
+                if (pf[q] == 0) {
+                    const double pk = pv[q];
+                    r_e += pk * pk;
+                    const double xnew = branch ? -pk : pk;
+                    pv[q] = xnew;
+                    if (pc[q] == row) { r_trp += pk; r_trn += xnew; }
+                    keep = true;
+                } else {
+                    keep = pf[q] == 1;
+                }
             }
             const unsigned bal = __ballot_sync(0xffffffffu, keep);
-            if (bal) {
-                int base = 0;
-                if (lane == 0) base = atomicAdd(&s_kept[grp], __popc(bal));
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (keep) {
-                    const int pos = base + __popc(bal & ((1u << lane) - 1u));
-                    if (pos < sort_cap) sortbuf[pos] = ((unsigned long long)(unsigned)j << 32) | (unsigned)s;
-                }
+            if (keep) {
+                const int pos = kept + __popc(bal & ((1u << lane) - 1u));
+                if (pos < cap2) sortbuf[pos] = ((unsigned long long)(unsigned)pc[q] << 32) | (unsigned)q;
             }
+            kept += __popc(bal);
         }
-        group_bar(grp);
-        const int kept = s_kept[grp];
-        w_max_p = max(w_max_p, cnt_p);
+        for (int q = lane; q < ne; q += 32) {
+            const int pos = kept + q;
+            if (pos < cap2) sortbuf[pos] = ((unsigned long long)(unsigned)ec[q] << 32) | (0x80000000u | (unsigned)q);
+        }
+        kept += ne;
+        __syncwarp();
         w_max_u = max(w_max_u, kept);
-        if (cnt_p > M) w_ovf_p = min(w_ovf_p, row);
         if (kept > M) {
             w_ovf_u = min(w_ovf_u, row);
-            if (tg == 0) on[row] = 0;
+            if (lane == 0) on[row] = 0;
         } else {
-            // ---------------- sort ascending by column, write the row, zero-fill unused slots ----------------
-            int n2 = 32;
-            while (n2 < kept) n2 <<= 1;
-            for (int q = kept + tg; q < n2; q += E_GT) sortbuf[q] = ~0ull;
-            group_bitonic_sort(sortbuf, n2, tg, grp);
-            for (int q = tg; q < M; q += E_GT) {
+            int k2 = 32;
+            while (k2 < kept) k2 <<= 1;
+            for (int q = kept + lane; q < k2; q += 32) sortbuf[q] = ~0ull;
+            __syncwarp();
+            warp_bitonic_sort(sortbuf, k2, lane);
+            for (int q = lane; q < M; q += 32) {
                 int j = 0; double v = 0.0;
                 if (q < kept) {
                     const unsigned long long e = sortbuf[q];
+                    const unsigned src = (unsigned)(e & 0xffffffffu);
                     j = (int)(e >> 32);
-                    const int s = (int)(e & 0xffffffffu);
-                    v = vals[s];
-                    if (!(keys[s] & E_INX)) r_e += v * v;            // P-only column: (P - X)^2 = p^2
+                    v = (src & 0x80000000u) ? ev[src & 0x7fffffffu] : pv[src];
                 }
                 oi[rbase + q] = j;
                 ov[rbase + q] = v;
             }
-            if (tg == 0) on[row] = kept;
+            if (lane == 0) on[row] = kept;
         }
-        w_trp += r_trp; w_e += r_e; w_x += r_x; w_trn += r_trn;
-        group_bar(grp);     // the scratch / table are reused by the next row
+        w_trp += warp_sum(r_trp); w_e += warp_sum(r_e); w_x += warp_sum(r_x); w_trn += warp_sum(r_trn);
+        __syncwarp();
     }
-
     // ---------------- per-CTA partials (fixed order), flags, last-CTA finaliser (S5) ----------------
-    w_trp = warp_sum(w_trp); w_e = warp_sum(w_e); w_x = warp_sum(w_x); w_trn = warp_sum(w_trn);
     if (lane == 0) {
-        double *sp = s_part[grp * E_GW + wg];
-        sp[0] = w_trp; sp[1] = w_e; sp[2] = w_x; sp[3] = w_trn;
-    }
-    if (tg == 0) {
+        s_part[warp][0] = w_trp; s_part[warp][1] = w_e; s_part[warp][2] = w_x; s_part[warp][3] = w_trn;
         if (w_ovf_p != INT32_MAX) atomicMin(&ctl->overflow_row, w_ovf_p);
         if (w_ovf_u != INT32_MAX) atomicMin(&ctl->overflow_upd, w_ovf_u);
-        if (w_acc != INT32_MAX) atomicMin(&ctl->acc_row, w_acc);
         atomicMax(&ctl->nnz_max_p, w_max_p);
         atomicMax(&ctl->nnz_max_upd, w_max_u);
     }
     __syncthreads();
     if (threadIdx.x < 4) {
         double v = 0.0;
-        for (int w = 0; w < ngroups * E_GW; ++w) v += s_part[w][threadIdx.x];
+        for (int w = 0; w < nwarps; ++w) v += s_part[w][threadIdx.x];
         partials[(size_t)blockIdx.x * 4 + threadIdx.x] = v;
     }
     __threadfence();
@@ -449,7 +586,7 @@ x2_ellpack_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__
         s_last = (prev + 1u == gridDim.x);
     }
     __syncthreads();
-    if (s_last && threadIdx.x < 32) {
+    if (s_last && warp == 0) {
         __threadfence();
         double s[4] = {0.0, 0.0, 0.0, 0.0};
         const volatile double *vp = partials;
@@ -579,30 +716,79 @@ static int sm_count()
     return sms;
 }
 
+// bytes of the scratch the symmetric product needs: upper parts (tv, ti, tn) and lower lists (lv, li, lcnt)
+size_t ellpack_sym_bytes(int64_t N, int M)
+{
+    const size_t nm = (size_t)N * (size_t)M;
+    auto up = [](size_t x) { return (x + 1023) / 1024 * 1024; };
+    return 2 * up(nm * 8) + 2 * up(nm * 4) + 2 * up((size_t)N * 4);
+}
+
+// the lower-list counters must be zero when a solve starts (kernel 2 re-zeroes them after every product)
+int ellpack_sym_reset(void *sym, int64_t N, int M, cudaStream_t st)
+{
+    const size_t nm = (size_t)N * (size_t)M;
+    auto up = [](size_t x) { return (x + 1023) / 1024 * 1024; };
+    uint8_t *p = (uint8_t *)sym + 2 * up(nm * 8) + 2 * up(nm * 4) + up((size_t)N * 4);
+    return cudaMemsetAsync(p, 0, (size_t)N * 4, st) == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+// One product = kernel 1 (upper half of thr(X X) + mirror append) followed by kernel 2 (assemble, update, finalise).
 int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, double *v1, int32_t *i1, int32_t *n1,
-                      int64_t N, int M, double tau, Sp2Ctl *ctl, double *partials, cudaStream_t st)
+                      int64_t N, int M, double tau, Sp2Ctl *ctl, double *partials, void *sym, cudaStream_t st)
 {
     const int sms = sm_count();
-    if (sms <= 0) return BML_ERR_CUDA;
-    const size_t smem_cap = 227 * 1024 - 1024;      // static shared memory of the kernel stays below 1 KB
+    if (sms <= 0 || !sym) return BML_ERR_CUDA;
+    const size_t nm = (size_t)N * (size_t)M;
+    auto up = [](size_t x) { return (x + 1023) / 1024 * 1024; };
+    uint8_t *p = (uint8_t *)sym;
+    double *tv = (double *)p; p += up(nm * 8);
+    double *lv = (double *)p; p += up(nm * 8);
+    int32_t *ti = (int32_t *)p; p += up(nm * 4);
+    int32_t *li = (int32_t *)p; p += up(nm * 4);
+    int32_t *tn = (int32_t *)p; p += up((size_t)N * 4);
+    int32_t *lcnt = (int32_t *)p;
+
+    // ---- kernel 1
+    const size_t smem_cap = 227 * 1024 - 1024;
     int ngroups = (int)(smem_cap / e_group_bytes(M));
     if (ngroups > E_MAX_GROUPS) ngroups = E_MAX_GROUPS;
     if (ngroups < 1 || M > 8 * E_GT) return BML_ERR_INVALID;
-    const size_t smem = (size_t)ngroups * e_group_bytes(M);
-    static size_t attr_smem = 0;
-    if (smem > attr_smem) {
-        if (cudaFuncSetAttribute(x2_ellpack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    const size_t smem1 = (size_t)ngroups * e_group_bytes(M);
+    static size_t attr1 = 0;
+    if (smem1 > attr1) {
+        if (cudaFuncSetAttribute(x2_ellpack_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1) !=
+            cudaSuccess)
             return BML_ERR_CUDA;
-        attr_smem = smem;
+        attr1 = smem1;
     }
-    int64_t grid = (N + ngroups - 1) / ngroups;
-    if (grid > sms) grid = sms;
-    if (grid > E_MAX_GRID) grid = E_MAX_GRID;
-    // the (j, slot) sort buffer aliases the row stage: e_scratch_bytes(M) / 8 entries
+    int64_t grid1 = (N + ngroups - 1) / ngroups;
+    if (grid1 > sms) grid1 = sms;
+    x2_ellpack_upper_kernel<<<(unsigned)grid1, ngroups * E_GT, smem1, st>>>(
+        v0, i0, n0, v1, i1, n1, (int)N, M, tau, (int)(e_scratch_bytes(M) / 8), ctl, tv, ti, tn, lv, li, lcnt);
+    BML_CHECK_LAUNCH();
+
+    // ---- kernel 2
+    const size_t wbytes = a_warp_bytes(M);
+    int nwarps = (int)(smem_cap / wbytes);
+    if (nwarps > A_MAX_WARPS) nwarps = A_MAX_WARPS;
+    if (nwarps < 1) return BML_ERR_INVALID;
+    const size_t smem2 = (size_t)nwarps * wbytes;
+    static size_t attr2 = 48 * 1024;
+    if (smem2 > attr2) {
+        if (cudaFuncSetAttribute(x2_ellpack_assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) !=
+            cudaSuccess)
+            return BML_ERR_CUDA;
+        attr2 = smem2;
+    }
+    int64_t grid2 = (N + nwarps - 1) / nwarps;
+    const int64_t per_sm = (int64_t)(smem_cap / smem2) > 0 ? (int64_t)(smem_cap / smem2) : 1;
+    if (grid2 > sms * per_sm) grid2 = sms * per_sm;
+    if (grid2 > E_MAX_GRID) grid2 = E_MAX_GRID;
     // buffer 0 is only read while parity == 0 (the standalone entry point passes a const X there)
-    x2_ellpack_kernel<<<(unsigned)grid, ngroups * E_GT, smem, st>>>((double *)v0, (int32_t *)i0, (int32_t *)n0, v1, i1,
-                                                                     n1, (int)N, M, tau, (int)(e_scratch_bytes(M) / 8),
-                                                                     ctl, partials);
+    x2_ellpack_assemble_kernel<<<(unsigned)grid2, nwarps * 32, smem2, st>>>(
+        (double *)v0, (int32_t *)i0, (int32_t *)n0, v1, i1, n1, (int)N, M, tau, ctl, partials, tv, ti, tn, lv, li, lcnt,
+        (int)wbytes);
     BML_CHECK_LAUNCH();
     return 0;
 }
