@@ -171,6 +171,19 @@ BML_API int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t b
  */
 BML_API int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream);
 
+/*
+ * Introspection of the host-computable work distribution of the dense kernels (pure host functions, no GPU needed;
+ * they run the same arithmetic as the kernels and exist so that the partition can be tested exhaustively on a CPU).
+ * bml_dense_work_item: the it-th work item of CTA `cta` (of n_ctas) of the persistent FP64 kernel for an N x N product
+ *   (N > 1024).  out5 <- { tile, I, J, kt_begin, kt_end }: tile (I, J), I <= J, of 128 x 128, k-slabs [kt_begin, kt_end)
+ *   of ceil(N / 16).  Returns 0, 1 when the CTA's list has fewer than it + 1 items, or -1.
+ * bml_dense_mixed_tile_count / bml_dense_mixed_tile_of_cta: grid size of the mixed kernel and the tile of a CTA
+ *   (out2 <- { I, J }); returns 1 for the empty slots of the super-block order.
+ */
+BML_API int bml_dense_work_item(int64_t N, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out5);
+BML_API int bml_dense_mixed_tile_count(int64_t N);
+BML_API int bml_dense_mixed_tile_of_cta(int64_t N, int32_t cta, int32_t *out2);
+
 BML_API const char *bml_status_string(int status);
 /* "major.minor.patch (sm_100a)" */
 BML_API const char *bml_version(void);

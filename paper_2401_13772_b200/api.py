@@ -25,6 +25,7 @@ EXPORTS = [
     "bml_version", "bml_status_string", "bml_gershgorin_workspace_bytes", "bml_gershgorin", "bml_trace",
     "bml_sp2_workspace_bytes", "bml_sp2_dense", "bml_sp2_ellpack", "bml_x2_dense_workspace_bytes", "bml_x2_dense",
     "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_probe_fp64_tensor_peak",
+    "bml_dense_work_item", "bml_dense_mixed_tile_count", "bml_dense_mixed_tile_of_cta",
 ]
 
 
@@ -109,6 +110,12 @@ def load(build_if_missing: bool = True):
     L.bml_x2_ellpack.argtypes = [MP, MP, i32, dbl, vp, vp, vp, sz, vp]
     L.bml_probe_fp64_tensor_peak.restype = ctypes.c_int
     L.bml_probe_fp64_tensor_peak.argtypes = [i32, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
+    L.bml_dense_work_item.restype = ctypes.c_int
+    L.bml_dense_work_item.argtypes = [i64, i32, i32, i32, ctypes.POINTER(ctypes.c_int32)]
+    L.bml_dense_mixed_tile_count.restype = ctypes.c_int
+    L.bml_dense_mixed_tile_count.argtypes = [i64]
+    L.bml_dense_mixed_tile_of_cta.restype = ctypes.c_int
+    L.bml_dense_mixed_tile_of_cta.argtypes = [i64, i32, ctypes.POINTER(ctypes.c_int32)]
     _lib = L
     return L
 
@@ -334,6 +341,34 @@ def bml_x2_ellpack(X, branch: int, drop_tol: float, out=None, ws=None):
     if rc != 0:
         raise RuntimeError(f"bml_x2_ellpack: {bml_status_string(rc)}")
     return out, sums, info
+
+
+def bml_dense_work_items(N: int, n_ctas: int, cta: int):
+    """Work list of one CTA of the persistent FP64 kernel: [(tile, I, J, kt_begin, kt_end), ...] (host arithmetic)."""
+    L = load()
+    out = (ctypes.c_int32 * 5)()
+    items, it = [], 0
+    while True:
+        rc = L.bml_dense_work_item(int(N), int(n_ctas), int(cta), it, out)
+        if rc == 1:
+            return items
+        if rc != 0:
+            raise RuntimeError(f"bml_dense_work_item: {bml_status_string(rc)}")
+        items.append(tuple(out))
+        it += 1
+
+
+def bml_dense_mixed_tiles(N: int):
+    """CTA -> tile map of the mixed kernel: list of (I, J) or None for the empty slots (host arithmetic)."""
+    L = load()
+    out = (ctypes.c_int32 * 2)()
+    res = []
+    for cta in range(L.bml_dense_mixed_tile_count(int(N))):
+        rc = L.bml_dense_mixed_tile_of_cta(int(N), cta, out)
+        if rc < 0:
+            raise RuntimeError(f"bml_dense_mixed_tile_of_cta: {bml_status_string(rc)}")
+        res.append(None if rc == 1 else (out[0], out[1]))
+    return res
 
 
 def bml_probe_fp64_tensor_peak(iters: int = 20000) -> float:

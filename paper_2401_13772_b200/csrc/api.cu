@@ -9,6 +9,8 @@ namespace bmlsp2 {
 // dense_fp64.cu
 int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld);
 int dense_fp64_num_tiles(int64_t N);
+int dense_fp64_work_item(int64_t N, int n_ctas, int cta, int it, int32_t out[5]);
+int dense_mixed_tile_of_cta(int64_t N, int cta, int32_t out[2]);
 size_t dense_fp64_sk_bytes(int64_t N);
 int dense_fp64_sk_reset(void *sk, int64_t N, cudaStream_t st);
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
@@ -376,6 +378,20 @@ int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, d
     if (cudaMemcpyAsync(d_sums, w.ctl->sums, 4 * sizeof(double), cudaMemcpyDeviceToDevice, st) != cudaSuccess)
         return BML_ERR_CUDA;
     return launch_x2_ellpack_info(w.ctl, d_info, st);
+}
+
+int bml_dense_work_item(int64_t N, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out5)
+{
+    if (!out5) return BML_ERR_INVALID;
+    return dense_fp64_work_item(N, n_ctas, cta, it, out5);
+}
+
+int bml_dense_mixed_tile_count(int64_t N) { return N < 1 ? 0 : dense_mixed_num_tiles(N); }
+
+int bml_dense_mixed_tile_of_cta(int64_t N, int32_t cta, int32_t *out2)
+{
+    if (!out2) return BML_ERR_INVALID;
+    return dense_mixed_tile_of_cta(N, cta, out2);
 }
 
 int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream)

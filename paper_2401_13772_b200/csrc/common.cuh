@@ -204,14 +204,14 @@ __host__ __device__ __forceinline__ int tile_sb_grid(int T)
     return S * (S + 1) / 2 * TILE_SB * TILE_SB;
 }
 // t -> (i, j), i <= j, column by column: t = j (j + 1) / 2 + i
-__device__ __forceinline__ void tri_decode(int t, int &i, int &j)
+__host__ __device__ __forceinline__ void tri_decode(int t, int &i, int &j)
 {
     j = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
     while ((j + 1) * (j + 2) / 2 <= t) ++j;
     while (j * (j + 1) / 2 > t) --j;
     i = t - j * (j + 1) / 2;
 }
-__device__ __forceinline__ bool tile_sb_decode(int bid, int T, int &I, int &J)
+__host__ __device__ __forceinline__ bool tile_sb_decode(int bid, int T, int &I, int &J)
 {
     if (tile_sb_plain(T)) { tri_decode(bid, I, J); return true; }
     constexpr int GG = TILE_SB * TILE_SB;

@@ -218,7 +218,7 @@ struct SkItem {
     int tile, kt0, kt1;
 };
 // it-th work item of CTA c (identical arithmetic in every role); false when the list is exhausted
-__device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, SkItem &w)
+__host__ __device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, SkItem &w)
 {
     const int W = tiles / G, R = tiles - W * G;
     if (it < W) { w.tile = it * G + c; w.kt0 = 0; w.kt1 = KT; return true; }
@@ -547,6 +547,19 @@ static int launch_x2_dense_fp64_t(const CUtensorMap &map0, const CUtensorMap &ma
 }
 
 // Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).
+// host-side view of the persistent kernel's work list (the same sk_item() the device runs): bml_dense_work_item
+int dense_fp64_work_item(int64_t N, int n_ctas, int cta, int it, int32_t out[5])
+{
+    if (N <= 1024 || n_ctas < 1 || cta < 0 || cta >= n_ctas || it < 0) return BML_ERR_INVALID;
+    const int T = (int)((N + 127) / 128), tiles = T * (T + 1) / 2, KT = (int)((N + D_BK - 1) / D_BK);
+    SkItem w;
+    if (!sk_item(it, cta, n_ctas, tiles, KT, w)) return 1;
+    int I, J;
+    tri_decode(w.tile, I, J);
+    out[0] = w.tile; out[1] = I; out[2] = J; out[3] = w.kt0; out[4] = w.kt1;
+    return 0;
+}
+
 // sk: the scratch of dense_fp64_sk_bytes(N) bytes (used by the persistent 128 x 128 kernel only)
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
                          int64_t N, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream)

@@ -364,6 +364,17 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
 // number of CTAs (= per-CTA partial-sum slots) of one mixed product (128 x 128 tiles)
 int dense_mixed_num_tiles(int64_t N) { return tile_sb_grid((int)((N + M_BM - 1) / M_BM)); }
 
+// host-side view of the CTA -> tile map of the mixed kernel (the same tile_sb_decode() the device runs)
+int dense_mixed_tile_of_cta(int64_t N, int cta, int32_t out[2])
+{
+    const int T = (int)((N + M_BM - 1) / M_BM);
+    if (N < 1 || cta < 0 || cta >= tile_sb_grid(T)) return BML_ERR_INVALID;
+    int I, J;
+    if (!tile_sb_decode(cta, T, I, J)) return 1;
+    out[0] = I; out[1] = J;
+    return 0;
+}
+
 // the planes of one iterate, stacked: rows p * N + r, leading dimension ldp (= the FP64 iterate's ld)
 template <int V>
 static int make_plane_map(CUtensorMap *map, const uint16_t *base, int64_t N, int64_t ldp)
