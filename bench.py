@@ -441,7 +441,8 @@ def run_ours(args):
             break
     n_enq = min(n_enq, 100)
     pre = (2 + 1 + 1 + 1 + (1 if w.precision != 0 else 0)) if dense else (2 + 2 + 1)
-    launches_per_step = pre + n_enq * (1 if dense else 2) + 1      # a sparse product is two kernels
+    # a sparse product is two kernels; a mixed product is the FP64-diagonal kernel + the tcgen05 kernel
+    launches_per_step = pre + n_enq * (2 if (not dense or w.precision != 0) else 1) + 1
     line = {
         "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,

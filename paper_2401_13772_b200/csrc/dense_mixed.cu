@@ -134,12 +134,38 @@ split_planes_kernel(const double *__restrict__ X, int64_t ld, int N, uint16_t *_
     }
 }
 
+// "FP64 traces" (BASELINE.json configs[3]): the diagonal of X^2 in full FP64 from the master iterate,
+// dsq[i] = sum_k X_ik^2 (X symmetric), one warp per row, fixed summation order.  The product kernel writes these values on
+// the diagonal instead of its mixed-precision ones, so tr(X^2) -- and with it tr X_{m+1}, which decides the next branch
+// -- carries FP64 round-off only (the mixed products' one-sided truncation bias would otherwise sit in the trace:
+// 4.5e-3 at N = 16384).  One extra read of X per product (HBM-bound, ~2% of the product time).
+__global__ void __launch_bounds__(256)
+diag_x2_fp64_kernel(const double *__restrict__ buf0, const double *__restrict__ buf1, int64_t ld, int N,
+                    const Sp2Ctl *__restrict__ ctl, double *__restrict__ dsq)
+{
+    if (ctl->done) return;
+    const double *__restrict__ X = ctl->parity ? buf1 : buf0;
+    const int lane = threadIdx.x & 31;
+    const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= N) return;
+    const double *__restrict__ xr = X + (int64_t)row * ld;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int k = lane;
+    for (; k + 96 < N; k += 128) {
+        const double a = xr[k], b = xr[k + 32], c = xr[k + 64], d = xr[k + 96];
+        s0 = fma(a, a, s0); s1 = fma(b, b, s1); s2 = fma(c, c, s2); s3 = fma(d, d, s3);
+    }
+    for (; k < N; k += 32) { const double a = xr[k]; s0 = fma(a, a, s0); }
+    const double s = warp_sum((s0 + s1) + (s2 + s3));
+    if (lane == 0) dsq[row] = s;
+}
+
 template <int V>
 __global__ void __launch_bounds__(M_THREADS, 1)
 x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
                       double *__restrict__ buf0, double *__restrict__ buf1, uint16_t *__restrict__ pl0,
                       uint16_t *__restrict__ pl1, int64_t ld, int N, Sp2Ctl *__restrict__ ctl,
-                      double *__restrict__ partials)
+                      double *__restrict__ partials, const double *__restrict__ dsq)
 {
     using Cfg = MixedCfg<V>;
     constexpr int PLANES = Cfg::PLANES, STAGES = Cfg::STAGES, ACC_COLS = Cfg::ACC_COLS, M_BK = Cfg::BK;
@@ -298,7 +324,7 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
             for (int i = 0; i < 64; ++i) {
                 const int c = c0 + i;
                 if (c < N && (!diag || r <= c)) {
-                    const double p = acc[i];
+                    const double p = (r == c) ? dsq[r] : acc[i];       // FP64 diagonal (diag_x2_fp64_kernel)
                     const double x = X[(int64_t)r * ld + c];
                     const double d = p - x;
                     const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
@@ -398,7 +424,10 @@ static inline size_t plane_set_bytes(int64_t N, int64_t ldx)
     return ((size_t)M_MAX_PLANES * (size_t)N * (size_t)ldx * sizeof(uint16_t) + 1023) / 1024 * 1024;
 }
 
-size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx) { return 2 * plane_set_bytes(N, ldx); }
+size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx)
+{
+    return 2 * plane_set_bytes(N, ldx) + ((size_t)N * sizeof(double) + 1023) / 1024 * 1024;     // + dsq[N]
+}
 
 template <int V>
 static int launch_split(const double *X, int64_t ld, int64_t N, uint16_t *planes, cudaStream_t st)
@@ -411,7 +440,8 @@ static int launch_split(const double *X, int64_t ld, int64_t N, uint16_t *planes
 
 template <int V>
 static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double *b0, double *b1, uint16_t *p0,
-                           uint16_t *p1, int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t st)
+                           uint16_t *p1, int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, double *dsq,
+                           cudaStream_t st)
 {
     constexpr size_t smem = (size_t)MixedCfg<V>::STAGES * 2 * MixedCfg<V>::PLANES * (M_BM * MixedCfg<V>::BK * 2) +
                             1024 /*align*/ + 1024 /*barriers, scratch*/;
@@ -422,8 +452,9 @@ static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double 
             return BML_ERR_CUDA;
         attr_set = true;
     }
+    diag_x2_fp64_kernel<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(b0, b1, ld, (int)N, ctl, dsq);
     x2_dense_mixed_kernel<V><<<dense_mixed_num_tiles(N), M_THREADS, smem, st>>>(m0, m1, b0, b1, p0, p1, ld, (int)N, ctl,
-                                                                                partials);
+                                                                                partials, dsq);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
@@ -433,14 +464,15 @@ static int solve_v(int64_t N, int max_products, double *X0, double *X1, int64_t 
 {
     uint16_t *p0 = (uint16_t *)extra;
     uint16_t *p1 = (uint16_t *)((uint8_t *)extra + plane_set_bytes(N, ldx));
+    double *dsq = (double *)((uint8_t *)extra + 2 * plane_set_bytes(N, ldx));
     CUtensorMap m0, m1;
     int r;
     if ((r = make_plane_map<V>(&m0, p0, N, ldx))) return r;
     if ((r = make_plane_map<V>(&m1, p1, N, ldx))) return r;
     if ((r = launch_split<V>(X0, ldx, N, p0, st))) return r;
-    if (max_products == 1) return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st);
-    return enqueue_products([&]() { return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, st); }, ctl,
-                            max_products, st);
+    if (max_products == 1) return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, dsq, st);
+    return enqueue_products([&]() { return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, dsq, st); },
+                            ctl, max_products, st);
 }
 
 // X0 (already rescaled, in buffer 0) -> planes of buffer 0, then the fused products
