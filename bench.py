@@ -44,7 +44,7 @@ def dense_flops_per_product(N: int) -> float:
 NCU_TRAFFIC_BYTES = {
     "dense_n2048": 41.8e6,          # 33.9 MB read (= N^2 x 8 B: X read once) + 7.9 MB written (X' mostly stays in L2)
     "dense_n8192": 6.08e9,          # 5.55 GB read (row panels re-read) + 0.53 GB written
-    "mixed_n16384": 20.8e9,         # 17.3 GB read + 3.5 GB written (FP16 x 2 planes, super-block tile order)
+    "mixed_n16384": 20.4e9,         # 17.2 GB read + 3.2 GB written (FP16 x 2 planes, super-block tile order)
     "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (capture quoted in DESIGN.md 5.3)
     "ellpack_n65536": 1.25e9,       # kernel 1: 0.246 + 0.190 GB; kernel 2: 0.451 + 0.363 GB (read + written)
 }
