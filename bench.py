@@ -125,6 +125,19 @@ def oracle_time_to_D(wname: str, H, budget_s: float, n_products_full: int | None
 
     w = hm.WORKLOADS[wname]
     cores = oracle.omp_threads()
+    if w.kind == "dense" and w.N > 6000:
+        # a full oracle product is N^3 multiply-adds (minutes to hours here): time one product of the oracle on the
+        # leading 4096 x 4096 principal block of the same Hamiltonian and scale by (N / 4096)^3 x products
+        nb = 4096
+        Hb = np.ascontiguousarray(H[:nb, :nb])
+        lo, hi = oracle.gershgorin_dense(Hb)
+        Xb = oracle.rescale_dense(Hb, lo, hi)
+        t0 = time.perf_counter()
+        oracle.x2_dense(Xb)
+        per = (time.perf_counter() - t0) * (w.N / nb) ** 3
+        full = n_products_full or 32
+        return per * full * 1e3, (f"one oracle product on the leading {nb}x{nb} principal block, "
+                                  f"scaled by ({w.N}/{nb})^3 x {full} products"), cores
     if w.kind == "dense":
         t0 = time.perf_counter()
         _, st = oracle.sp2_dense(H, w.n_occ, w.idem_tol, 2)          # 2 products: calibrates the per-product cost
