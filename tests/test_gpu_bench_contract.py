@@ -1,0 +1,39 @@
+"""bench.py's output contract on a GPU: one JSON line with the keys the driver reads, for the smallest dense workload
+(the default line is the same code path on configs[1])."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_bench_prints_one_json_line_with_the_contract_keys():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", "--workload",
+                          "dense_n256"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "e2e", "gpu_launches", "roofline", "cpu_baseline", "clocks"):
+        assert key in d, key
+    assert d["metric"] == "sp2_time_to_D_ms" and d["unit"] == "ms" and d["higher_is_better"] is False
+    assert d["n_gpus"] == 1 and d["steps"] == 3 and d["vs_baseline"] is None and d["data"] == "synthetic"
+    assert d["config"]["workload"] == "dense_n256" and "model" not in d["config"]
+    assert d["status"] == 0 and d["n_products"] == 15 and d["branch"] == "10010110010110"
+    assert d["e2e"]["h2d_bytes_per_step"] == 256 * 256 * 8 and d["e2e"]["value"] >= d["value"] * 0.5
+    assert d["gpu_launches"] > 0
+    r = d["roofline"]
+    assert r["bound"] == "tensor" and r["unit"] == "TFLOP/s" and 0 < r["frac"] <= 1.1 and r["peak"] > 20
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert d["clocks"]["sm_max_mhz"] and "reasons" in d["clocks"]
