@@ -159,6 +159,11 @@ class Workload:
     M: int = 0
     lattice: tuple | None = None
     note: str = ""
+    # Chebyshev workloads (kind "cheby"): chemical potential, inverse temperature, Eq. 10 factors L + 1 = k m
+    mu: float = 0.0
+    beta: float = 0.0
+    k: int = 0
+    m: int = 0
 
 
 WORKLOADS = {
@@ -184,8 +189,21 @@ WORKLOADS = {
 }
 
 
+# Chebyshev expansion workloads (PAPER.md IV.B, Fig. 3 P:247 sizes N = 500, 1000, 2000, 4000).
+# The paper's inputs for Fig. 3 are not given; stand-in: a gapless ("metallic") periodic lattice -- uniform on-site
+# level + U[-0.2, 0.2], nearest-neighbour hopping -1 -- at k_B T = 1/6 hopping units, mu = 0 (about half filling),
+# expansion order L = 255 = 16 x 16 - 1 (truncation error 1.2e-10 relative at N = 500), i.e. the vanishing-gap / finite-temperature case SP2 cannot treat.
+for _name, _L3 in (("cheby_n500", (10, 10, 5)), ("cheby_n1000", (10, 10, 10)), ("cheby_n2000", (20, 10, 10)),
+                   ("cheby_n4000", (20, 20, 10)), ("cheby_n8000", (20, 20, 20))):
+    _N = _L3[0] * _L3[1] * _L3[2]
+    WORKLOADS[_name] = Workload(_name, "cheby", _N, _N // 2, 0.0, lattice=_L3, mu=0.0, beta=6.0, k=16, m=16,
+                                note="%dx%dx%d gapless lattice, NN hopping -1, kT=1/6, L=255" % _L3)
+
+
 def make_dense(name: str, seed: int = 0) -> np.ndarray:
     w = WORKLOADS[name]
+    if w.kind == "cheby":
+        return lattice_dense(w.lattice, 0.0, 0.2, 1.0, lambda r: -1.0, seed)
     if name == "dense_n256":
         return ring_dense(256, 1.5, 0.1, 1e-3, seed)
     if name == "dense_n2048":
