@@ -1,4 +1,4 @@
-"""Thin ctypes binding of libbmlsp2.so (include/bml_sp2.h) — argument marshalling only.
+"""Thin ctypes binding of libbmlsp2.so (include/bml_sp2.h, include/bml_chebyshev.h) — argument marshalling only.
 
 Every function has the name of the C entry point it calls and takes torch CUDA tensors for device memory; all
 arithmetic of the method runs in the library's sm_100a kernels.  There is no CPU fallback: if the library is missing
@@ -26,7 +26,11 @@ EXPORTS = [
     "bml_sp2_workspace_bytes", "bml_sp2_dense", "bml_sp2_ellpack", "bml_x2_dense_workspace_bytes", "bml_x2_dense",
     "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_probe_fp64_tensor_peak",
     "bml_dense_work_item", "bml_dense_mixed_tile_count", "bml_dense_mixed_tile_of_cta",
+    # include/bml_chebyshev.h
+    "bml_chebyshev_workspace_bytes", "bml_chebyshev_dense", "bml_symm_ab_workspace_bytes", "bml_symm_ab_dense",
+    "bml_cheb_schedule", "bml_symm_work_item",
 ]
+CHEB_MAX_K, CHEB_MAX_M, CHEB_MAX_TERMS, SYMM_MAX_JOBS = 32, 32, 1024, 16
 
 
 class bml_matrix_t(ctypes.Structure):
@@ -64,6 +68,31 @@ class bml_sp2_stats_t(ctypes.Structure):
         ("trace", ctypes.c_double * LOG_LEN),
         ("idem", ctypes.c_double * LOG_LEN),
         ("max_row_nnz", ctypes.c_int32 * LOG_LEN),
+    ]
+
+
+class bml_cheb_params_t(ctypes.Structure):
+    _fields_ = [
+        ("mu", ctypes.c_double),
+        ("beta", ctypes.c_double),
+        ("k", ctypes.c_int32),
+        ("m", ctypes.c_int32),
+        ("flags", ctypes.c_uint32),
+        ("pad", ctypes.c_uint32),
+    ]
+
+
+class bml_cheb_stats_t(ctypes.Structure):
+    _fields_ = [
+        ("status", ctypes.c_int32),
+        ("n_products", ctypes.c_int32),
+        ("n_launches", ctypes.c_int32),
+        ("L", ctypes.c_int32),
+        ("emin", ctypes.c_double),
+        ("emax", ctypes.c_double),
+        ("trace", ctypes.c_double),
+        ("c", ctypes.c_double * CHEB_MAX_TERMS),
+        ("d", ctypes.c_double * CHEB_MAX_TERMS),
     ]
 
 
@@ -116,6 +145,20 @@ def load(build_if_missing: bool = True):
     L.bml_dense_mixed_tile_count.argtypes = [i64]
     L.bml_dense_mixed_tile_of_cta.restype = ctypes.c_int
     L.bml_dense_mixed_tile_of_cta.argtypes = [i64, i32, ctypes.POINTER(ctypes.c_int32)]
+    i32p, dblp = ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(dbl)
+    L.bml_chebyshev_workspace_bytes.restype = sz
+    L.bml_chebyshev_workspace_bytes.argtypes = [i64, i32, i32]
+    L.bml_chebyshev_dense.restype = ctypes.c_int
+    L.bml_chebyshev_dense.argtypes = [MP, ctypes.POINTER(bml_cheb_params_t), MP, vp, sz,
+                                      ctypes.POINTER(bml_cheb_stats_t), vp]
+    L.bml_symm_ab_workspace_bytes.restype = sz
+    L.bml_symm_ab_workspace_bytes.argtypes = []
+    L.bml_symm_ab_dense.restype = ctypes.c_int
+    L.bml_symm_ab_dense.argtypes = [vp, i64, i64, i64, i32, i32, i32p, i32p, i32p, i32p, dblp, dblp, dblp, vp, sz, vp]
+    L.bml_cheb_schedule.restype = ctypes.c_int
+    L.bml_cheb_schedule.argtypes = [i32, i32p, i32p, i32p]
+    L.bml_symm_work_item.restype = ctypes.c_int
+    L.bml_symm_work_item.argtypes = [i64, i32, i32, i32, i32, i32p]
     _lib = L
     return L
 
@@ -379,3 +422,126 @@ def bml_probe_fp64_tensor_peak(iters: int = 20000) -> float:
     if rc != 0:
         raise RuntimeError(f"bml_probe_fp64_tensor_peak: {bml_status_string(rc)}")
     return flops.value / (ms.value * 1e-3) / 1e12
+
+
+# ------------------------------------------------------------------------------------------------------------
+# include/bml_chebyshev.h
+# ------------------------------------------------------------------------------------------------------------
+@dataclass
+class ChebResult:
+    status: int
+    n_products: int
+    n_launches: int
+    L: int
+    emin: float
+    emax: float
+    trace: float
+    c: np.ndarray          # c_0 .. c_L
+    d: np.ndarray          # d[i, j], shape (k, m)
+    message: str = field(default="")
+
+
+class ChebyshevSolver:
+    """Pre-allocated workspace for repeated bml_chebyshev_dense calls on one (N, k, m)."""
+
+    def __init__(self, N: int, k: int, m: int, device="cuda"):
+        L = load()
+        self.N, self.k, self.m = int(N), int(k), int(m)
+        self.device = torch.device(device)
+        self.D = torch.empty((N, N), dtype=torch.float64, device=self.device)
+        self.ws_bytes = L.bml_chebyshev_workspace_bytes(self.N, self.k, self.m)
+        if self.ws_bytes == 0:
+            raise RuntimeError("bml_chebyshev_workspace_bytes: " + bml_status_string(-1))
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, H: torch.Tensor, mu: float, beta: float, flags: int = 0):
+        L = load()
+        h, d = dense_desc(H), dense_desc(self.D)
+        p = bml_cheb_params_t(float(mu), float(beta), self.k, self.m, int(flags), 0)
+        st = bml_cheb_stats_t()
+        rc = L.bml_chebyshev_dense(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(),
+                                   self.ws_bytes, ctypes.byref(st), _stream())
+        n = self.k * self.m
+        res = ChebResult(status=int(rc), n_products=int(st.n_products), n_launches=int(st.n_launches), L=int(st.L),
+                         emin=float(st.emin), emax=float(st.emax), trace=float(st.trace), c=np.array(st.c[:n]),
+                         d=np.array(st.d[:n]).reshape(self.m, self.k).T.copy(), message=bml_status_string(rc))
+        return self.D, res
+
+
+def bml_chebyshev_dense(H: torch.Tensor, mu: float, beta: float, k: int, m: int, flags: int = 0):
+    """D ~ f_mu(H) by the resummed Chebyshev expansion (Eq. 10-14).  Returns (D CUDA tensor, ChebResult)."""
+    _require_cuda(H, torch.float64, "H")
+    if not (2 <= int(k) <= CHEB_MAX_K and 1 <= int(m) <= CHEB_MAX_M and int(k) * int(m) <= CHEB_MAX_TERMS):
+        D = torch.empty_like(H)
+        h, d = dense_desc(H), dense_desc(D)
+        p = bml_cheb_params_t(float(mu), float(beta), int(k), int(m), int(flags), 0)
+        st = bml_cheb_stats_t()
+        rc = load().bml_chebyshev_dense(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), None, 0, ctypes.byref(st),
+                                        _stream())
+        return D, ChebResult(int(rc), 0, 0, 0, 0.0, 0.0, 0.0, np.zeros(0), np.zeros((0, 0)), bml_status_string(rc))
+    return ChebyshevSolver(H.shape[0], k, m, H.device).solve(H, mu, beta, flags)
+
+
+def matrix_slab(mats, device="cuda"):
+    """Copy square matrices into one zero-padded CUDA slab (slot s at s * slot_elems, ld = padded_ld(N), 128-byte
+    aligned).  Returns (slab tensor [n, slot_elems], N, ld, slot_elems)."""
+    mats = [torch.as_tensor(np.asarray(a), dtype=torch.float64) for a in mats]
+    N = mats[0].shape[0]
+    ld = padded_ld(N)
+    slot_elems = (N * ld + 127) // 128 * 128
+    raw = torch.zeros(len(mats) * slot_elems + 16, dtype=torch.float64, device=device)
+    off = ((-raw.data_ptr()) % 128) // 8
+    slab = raw[off:off + len(mats) * slot_elems].view(len(mats), slot_elems)
+    for s, a in enumerate(mats):
+        slab[s, :N * ld].view(N, ld)[:, :N].copy_(a)
+    return slab, N, ld, slot_elems
+
+
+def slab_matrix(slab: torch.Tensor, s: int, N: int, ld: int) -> torch.Tensor:
+    return slab[s, :N * ld].view(N, ld)[:, :N]
+
+
+def bml_symm_ab_dense(slab: torch.Tensor, N: int, ld: int, jobs, ws=None):
+    """One grouped launch on a slab from matrix_slab().  jobs: [(a, b, c or -1, out, alpha, beta, gamma), ...]:
+    slot[out] <- alpha slot[a] slot[b] + beta slot[c] + gamma I.  Asynchronous; results are written into the slab."""
+    L = load()
+    _require_cuda(slab, torch.float64, "slab")
+    n = len(jobs)
+    i32a, dbla = ctypes.c_int32 * max(n, 1), ctypes.c_double * max(n, 1)
+    cols = list(zip(*jobs)) if n else [[]] * 7
+    a, b, c, o = (i32a(*[int(v) for v in col]) for col in cols[:4])
+    al, be, ga = (dbla(*[float(v) for v in col]) for col in cols[4:])
+    nbytes = L.bml_symm_ab_workspace_bytes()
+    if ws is None:
+        ws = _workspace(nbytes, slab.device)
+    rc = L.bml_symm_ab_dense(slab.data_ptr(), int(N), int(ld), int(slab.stride(0)), int(slab.shape[0]), n, a, b, c, o,
+                             al, be, ga, ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_symm_ab_dense: {bml_status_string(rc)}")
+    return slab
+
+
+def bml_cheb_schedule(k: int):
+    """[(i, level, a, b)] for i = 2..k with T_i = 2 T_a T_b - T_{a-b} (host arithmetic)."""
+    L = load()
+    n = max(int(k) - 1, 1)
+    lv, a, b = (ctypes.c_int32 * n)(), (ctypes.c_int32 * n)(), (ctypes.c_int32 * n)()
+    rc = L.bml_cheb_schedule(int(k), lv, a, b)
+    if rc < 0:
+        raise RuntimeError(f"bml_cheb_schedule: {bml_status_string(rc)}")
+    return [(i, lv[i - 2], a[i - 2], b[i - 2]) for i in range(2, int(k) + 1)]
+
+
+def bml_symm_work_items(N: int, n_jobs: int, n_ctas: int, cta: int):
+    """Work list of one CTA of a grouped launch: [(job, I, J, kt_begin, kt_end, tile_edge), ...] (host arithmetic)."""
+    L = load()
+    out = (ctypes.c_int32 * 6)()
+    items, it = [], 0
+    while True:
+        rc = L.bml_symm_work_item(int(N), int(n_jobs), int(n_ctas), int(cta), it, out)
+        if rc == 1:
+            return items
+        if rc != 0:
+            raise RuntimeError(f"bml_symm_work_item: {bml_status_string(rc)}")
+        items.append(tuple(out))
+        it += 1

@@ -1,4 +1,4 @@
-"""Build libbmlsp2.so (hand-written sm_100a CUDA + the C ABI of include/bml_sp2.h) in-tree with nvcc.
+"""Build libbmlsp2.so (hand-written sm_100a CUDA + the C ABI of include/*.h) in-tree with nvcc.
 
     python -m paper_2401_13772_b200.build [--force] [--verbose]
 
@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 LIB_PATH = os.path.join(_HERE, "libbmlsp2.so")
-SOURCES = ["api.cu", "dense_fp64.cu", "dense_mixed.cu", "ellpack.cu", "reductions.cu", "probe.cu"]
+SOURCES = ["api.cu", "dense_fp64.cu", "dense_mixed.cu", "ellpack.cu", "reductions.cu", "probe.cu", "symm_ab.cu",
+           "chebyshev.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
     "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr", "-fmad=true",
@@ -33,7 +34,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB_PATH):
         return True
     t = os.path.getmtime(LIB_PATH)
-    deps = [os.path.join(_CSRC, f) for f in os.listdir(_CSRC)] + [os.path.join(_INC, "bml_sp2.h"), __file__]
+    deps = [os.path.join(_CSRC, f) for f in os.listdir(_CSRC)] + [os.path.join(_INC, f) for f in os.listdir(_INC)] + [__file__]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -3,6 +3,7 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "symm_ab.cuh"
 
 namespace bmlsp2 {
 
@@ -44,6 +45,11 @@ int launch_copy_out_ellpack(const double *v0, const int32_t *i0, const int32_t *
                             const int32_t *i1, const int32_t *n1, int64_t N, int M, const Sp2Ctl *ctl, double *dv,
                             int32_t *di, int32_t *dn, cudaStream_t st);
 int launch_x2_ellpack_info(const Sp2Ctl *ctl, int32_t *d_info, cudaStream_t st);
+// chebyshev.cu
+size_t cheb_workspace_bytes(int64_t N, int k, int m);
+int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b);
+int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws,
+                     bml_cheb_stats_t *stats, cudaStream_t st);
 // probe.cu
 int run_fp64_tensor_probe(int iters, double *flops, double *ms, cudaStream_t st);
 
@@ -392,6 +398,79 @@ int bml_dense_mixed_tile_of_cta(int64_t N, int32_t cta, int32_t *out2)
 {
     if (!out2) return BML_ERR_INVALID;
     return dense_mixed_tile_of_cta(N, cta, out2);
+}
+
+// ---------------------------------------------- bml_chebyshev.h ----------------------------------------------
+static bool cheb_params_ok(const bml_cheb_params_t *p)
+{
+    return p && p->k >= 2 && p->k <= BML_CHEB_MAX_K && p->m >= 1 && p->m <= BML_CHEB_MAX_M &&
+           p->k * p->m <= BML_CHEB_MAX_TERMS && p->beta > 0.0 && p->mu == p->mu;
+}
+
+size_t bml_chebyshev_workspace_bytes(int64_t N, int32_t k, int32_t m)
+{
+    if (N <= 0 || k < 2 || k > BML_CHEB_MAX_K || m < 1 || m > BML_CHEB_MAX_M) return 0;
+    return cheb_workspace_bytes(N, k, m);
+}
+
+int bml_chebyshev_dense(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *d_workspace,
+                        size_t workspace_bytes, bml_cheb_stats_t *stats, void *cuda_stream)
+{
+    int r = BML_OK;
+    if (!dense_ok(H) || !dense_ok(D) || D->N != H->N || !cheb_params_ok(p) || !d_workspace ||
+        D->value == H->value || ((uintptr_t)d_workspace & 1023) != 0 ||
+        workspace_bytes < bml_chebyshev_workspace_bytes(H->N, p->k, p->m))
+        r = BML_ERR_INVALID;
+    else
+        r = cheb_dense_solve(H, p, D, d_workspace, stats, (cudaStream_t)cuda_stream);
+    if (r < 0 && stats) { memset(stats, 0, sizeof(*stats)); stats->status = r; }
+    return r;
+}
+
+size_t bml_symm_ab_workspace_bytes(void) { return symm_ab_sk_bytes(); }
+
+int bml_symm_ab_dense(double *base, int64_t N, int64_t ld, int64_t slot_elems, int32_t n_slots, int32_t n_jobs,
+                      const int32_t *a_slot, const int32_t *b_slot, const int32_t *c_slot, const int32_t *out_slot,
+                      const double *alpha, const double *beta, const double *gamma, void *d_workspace,
+                      size_t workspace_bytes, void *cuda_stream)
+{
+    if (!base || N < 1 || N > 0x3fffffff || ld < N || (ld % 16) != 0 || ((uintptr_t)base & 127) != 0 ||
+        slot_elems < N * ld || (slot_elems % 16) != 0 || n_slots < 1 || n_jobs < 1 || n_jobs > BML_SYMM_MAX_JOBS ||
+        !a_slot || !b_slot || !c_slot || !out_slot || !alpha || !beta || !gamma || !d_workspace ||
+        ((uintptr_t)d_workspace & 1023) != 0 || workspace_bytes < symm_ab_sk_bytes())
+        return BML_ERR_INVALID;
+    SymmBatch batch;
+    memset(&batch, 0, sizeof(batch));
+    batch.n_jobs = n_jobs;
+    for (int q = 0; q < n_jobs; ++q) {
+        if (a_slot[q] < 0 || a_slot[q] >= n_slots || b_slot[q] < 0 || b_slot[q] >= n_slots || c_slot[q] < -1 ||
+            c_slot[q] >= n_slots || out_slot[q] < 0 || out_slot[q] >= n_slots)
+            return BML_ERR_INVALID;
+        for (int q2 = 0; q2 < n_jobs; ++q2)      // an output must not be an operand of the same launch
+            if (out_slot[q] == a_slot[q2] || out_slot[q] == b_slot[q2] || (q2 != q && out_slot[q] == out_slot[q2]) ||
+                (q2 != q && out_slot[q] == c_slot[q2]))
+                return BML_ERR_INVALID;
+        SymmJob &jb = batch.job[q];
+        jb.a = a_slot[q]; jb.b = b_slot[q];
+        jb.C = c_slot[q] < 0 ? nullptr : base + (int64_t)c_slot[q] * slot_elems;
+        jb.Out = base + (int64_t)out_slot[q] * slot_elems;
+        jb.ldc = ld; jb.ldo = ld;
+        jb.alpha = alpha[q]; jb.beta = beta[q]; jb.gamma = gamma[q];
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUtensorMap map;
+    int r = make_slab_map(&map, base, N, ld, slot_elems, n_slots);
+    if (r) return r;
+    if ((r = symm_ab_sk_reset(d_workspace, st))) return r;
+    return launch_symm_ab(map, batch, N, d_workspace, 1u, st);
+}
+
+int bml_cheb_schedule(int32_t k, int32_t *level, int32_t *a, int32_t *b) { return cheb_schedule(k, level, a, b); }
+
+int bml_symm_work_item(int64_t N, int32_t n_jobs, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out6)
+{
+    if (!out6) return BML_ERR_INVALID;
+    return symm_ab_work_item(N, n_jobs, n_ctas, cta, it, out6);
 }
 
 int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream)

@@ -1,0 +1,287 @@
+// chebyshev.cu -- the Chebyshev / Paterson-Stockmeyer Fermi-operator path (PAPER.md IV.B):
+// device-side coefficients (c_n of Eq. 8, d_{i,j} of Eq. 10), the map H -> H~ = T_1, the partial sums S_j (Eq. 12) and
+// the launch sequence.  The matrix products themselves are the grouped kernel of symm_ab.cu.
+#include <string.h>
+
+#include "symm_ab.cuh"
+
+namespace bmlsp2 {
+
+// reductions.cu
+int launch_gershgorin(const bml_matrix_t *H, double *d_bounds, double *rowlh, cudaStream_t st);
+int launch_trace_dense(const double *A, int64_t ld, int N, double *d_out, cudaStream_t st);
+int launch_check_symmetry(const bml_matrix_t *H, int *d_flag, cudaStream_t st);
+
+// Device-resident record of one expansion; copied to the host once, at the end of the call.
+struct ChebCtl {
+    double bounds[2];      // Gershgorin e_min, e_max
+    double trace;          // tr D
+    int32_t fail;          // 0, or BML_ERR_DEGENERATE
+    int32_t not_symmetric; // set by the symmetry check
+    int32_t pad[2];
+    double c[BML_CHEB_MAX_TERMS];
+    double d[BML_CHEB_MAX_TERMS];      // d_{i,j} at d[j * k + i]
+};
+constexpr size_t CHEB_TAB_DOUBLES = 8 * BML_CHEB_MAX_TERMS;   // cos(pi j / (2 N_q)), j < 4 N_q, N_q = 2 (L + 1)
+
+// f_mu(eps) = 1 / (1 + exp(beta (eps - mu))), written so that exp never overflows (reading C2)
+__device__ __forceinline__ double fermi_fn(double eps, double mu, double beta)
+{
+    const double z = beta * (eps - mu);
+    if (z >= 0.0) { const double e = exp(-z); return e / (1.0 + e); }
+    return 1.0 / (1.0 + exp(z));
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// c_n (Eq. 8) by Chebyshev-Gauss quadrature on N_q = 2 (L + 1) nodes (reading C3), then d_{i,j} (Eq. 10) by dividing
+// the series by T_k with Eq. 11 (reading C4).  One CTA; scalar work, O(L N_q) table look-ups + O(L m) for the division.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int CC_THREADS = 1024;
+__global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl, double *__restrict__ tab,
+                                                                   double mu, double beta, int k, int m)
+{
+    __shared__ double s_f[2 * BML_CHEB_MAX_TERMS];     // f at the nodes
+    __shared__ double s_p[BML_CHEB_MAX_TERMS];         // dividend of the current division step
+    __shared__ double s_q[BML_CHEB_MAX_TERMS];         // its quotient
+    const int terms = k * m, Nq = 2 * terms;
+    const double emin = ctl->bounds[0], emax = ctl->bounds[1];
+    if (threadIdx.x == 0) ctl->fail = (emax - emin > 0.0) ? 0 : BML_ERR_DEGENERATE;
+    // exact angles: every cosine needed is cos(pi j / (2 N_q)) with an integer j reduced mod 4 N_q
+    for (int j = threadIdx.x; j < 4 * Nq; j += CC_THREADS) tab[j] = cospi((double)j / (double)(2 * Nq));
+    __syncthreads();
+    for (int q = threadIdx.x; q < Nq; q += CC_THREADS) {
+        const double x = tab[2 * q + 1];                                // cos(pi (q + 1/2) / N_q)
+        s_f[q] = fermi_fn(0.5 * (emax - emin) * x + 0.5 * (emax + emin), mu, beta);
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < terms; n += CC_THREADS) {
+        double s = 0.0;
+        unsigned j = (unsigned)n % (unsigned)(4 * Nq);                  // n (2 q + 1) mod 4 N_q, incrementally
+        const unsigned step = (2u * (unsigned)n) % (unsigned)(4 * Nq);
+        for (int q = 0; q < Nq; ++q) {
+            s = fma(s_f[q], tab[j], s);
+            j += step;
+            if (j >= (unsigned)(4 * Nq)) j -= (unsigned)(4 * Nq);
+        }
+        const double cn = (n == 0 ? 1.0 : 2.0) / (double)Nq * s;
+        ctl->c[n] = cn;
+        s_p[n] = cn;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    // p = T_k q + r, deg r < k: for n > k, T_n = 2 T_k T_{n-k} - T_{|n-2k|}; T_k = T_k T_0 (Eq. 11), highest n first
+    int len = terms;
+    for (int j = 0; j < m; ++j) {
+        const int qlen = len - k;
+        for (int i = 0; i < qlen; ++i) s_q[i] = 0.0;
+        for (int n = len - 1; n > k; --n) {
+            const double pn = s_p[n];
+            s_q[n - k] += 2.0 * pn;
+            const int r = n - 2 * k;
+            s_p[r < 0 ? -r : r] -= pn;
+        }
+        if (len > k) s_q[0] += s_p[k];
+        for (int i = 0; i < k; ++i) ctl->d[j * k + i] = s_p[i];
+        for (int i = 0; i < qlen; ++i) s_p[i] = s_q[i];
+        len = qlen;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// T_1 = H~ = (2 H - (e_max + e_min) I) / (e_max - e_min)   (reading C1).  One pass: N^2 x 8 B read + written.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void cheb_map_kernel(const double *__restrict__ H, int64_t ldh, double *__restrict__ T1, int64_t ld, int N,
+                                const ChebCtl *__restrict__ ctl)
+{
+    const double emin = ctl->bounds[0], emax = ctl->bounds[1];
+    const double shift = emax + emin, width = emax - emin;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N) return;
+    for (int r = blockIdx.y; r < N; r += gridDim.y) {
+        const double h = H[(int64_t)r * ldh + c];
+        T1[(int64_t)r * ld + c] = (2.0 * h - (r == c ? shift : 0.0)) / width;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// S_j = sum_{i<k} d_{i,j} T_i, j = 0 .. m-1 (Eq. 12), all m sums in ONE pass over T_1 .. T_{k-1} (T_0 = I adds
+// d_{0,j} on the diagonal): every T_i element is read once and feeds m accumulators held in registers, where the paper
+// computes the S_j as m separate sums on concurrent streams.  HBM-bound: (k - 1 + m) N^2 x 8 B.
+// slab: slot s holds the matrix at slab + s * slot_elems; T_i in slot i - 1, S_j in slot k + j.
+// ------------------------------------------------------------------------------------------------------------
+template <int MJ>
+__global__ void __launch_bounds__(256) cheb_sums_kernel(double *__restrict__ slab, int64_t slot_elems, int64_t ld, int N,
+                                                        int k, int m, const ChebCtl *__restrict__ ctl)
+{
+    __shared__ double s_d[BML_CHEB_MAX_TERMS];
+    for (int i = threadIdx.x; i < k * m; i += blockDim.x) s_d[i] = ctl->d[i];
+    __syncthreads();
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N) return;
+    for (int r = blockIdx.y; r < N; r += gridDim.y) {
+        const int64_t off = (int64_t)r * ld + c;
+        double acc[MJ];
+#pragma unroll
+        for (int j = 0; j < MJ; ++j) acc[j] = (r == c && j < m) ? s_d[j * k] : 0.0;
+        for (int i = 1; i < k; ++i) {
+            const double t = __ldg(slab + (int64_t)(i - 1) * slot_elems + off);
+#pragma unroll
+            for (int j = 0; j < MJ; ++j)
+                if (j < m) acc[j] = fma(s_d[j * k + i], t, acc[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < MJ; ++j)
+            if (j < m) slab[(int64_t)(k + j) * slot_elems + off] = acc[j];
+    }
+}
+
+template <int MJ>
+static int launch_sums_t(double *slab, int64_t slot_elems, int64_t ld, int N, int k, int m, const ChebCtl *ctl,
+                         cudaStream_t st)
+{
+    const dim3 grid((unsigned)((N + 255) / 256), (unsigned)(N < 2048 ? N : 2048));
+    cheb_sums_kernel<MJ><<<grid, 256, 0, st>>>(slab, slot_elems, ld, N, k, m, ctl);
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------
+// doubling schedule of reading C5: T_i = 2 T_a T_b - T_{a-b}, a = ceil(i / 2), b = floor(i / 2); level = ceil(log2 i)
+int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b)
+{
+    if (k < 2 || k > BML_CHEB_MAX_K) return BML_ERR_INVALID;
+    int levels = 0;
+    for (int i = 2; i <= k; ++i) {
+        int lv = 0;
+        while ((1 << lv) < i) ++lv;
+        if (level) level[i - 2] = lv;
+        if (a) a[i - 2] = (i + 1) / 2;
+        if (b) b[i - 2] = i / 2;
+        if (lv > levels) levels = lv;
+    }
+    return levels;
+}
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct ChebWs {
+    ChebCtl *ctl;
+    double *tab;
+    double *rowlh;
+    void *sk;
+    double *slab;
+    int64_t ld, slot_elems;
+    size_t total;
+};
+
+static ChebWs carve_cheb(void *ws, int64_t N, int k, int m)
+{
+    ChebWs w;
+    uint8_t *p = (uint8_t *)ws;
+    size_t off = 0;
+    w.ctl = (ChebCtl *)(p + off); off = align_up(off + sizeof(ChebCtl), 1024);
+    w.tab = (double *)(p + off); off = align_up(off + CHEB_TAB_DOUBLES * sizeof(double), 1024);
+    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
+    w.sk = (void *)(p + off); off = align_up(off + symm_ab_sk_bytes(), 1024);
+    w.ld = (N + 15) / 16 * 16;
+    w.slot_elems = (int64_t)align_up((size_t)N * w.ld, 128);
+    w.slab = (double *)(p + off); off = align_up(off + (size_t)(k + m) * w.slot_elems * sizeof(double), 1024);
+    w.total = off;
+    return w;
+}
+
+size_t cheb_workspace_bytes(int64_t N, int k, int m) { return carve_cheb(nullptr, N, k, m).total; }
+
+int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, bml_cheb_stats_t *stats,
+                     cudaStream_t st)
+{
+    const int64_t N = H->N;
+    const int k = p->k, m = p->m;
+    ChebWs w = carve_cheb(ws, N, k, m);
+    auto slot = [&](int s) { return w.slab + (int64_t)s * w.slot_elems; };      // T_i: slot i - 1; S_j: slot k + j
+#define CK(x) do { int _r = (x); if (_r != 0) return _r; } while (0)
+    if (cudaMemsetAsync(w.ctl, 0, 64, st) != cudaSuccess) return BML_ERR_CUDA;
+    CK(launch_gershgorin(H, w.ctl->bounds, w.rowlh, st));
+    if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) CK(launch_check_symmetry(H, &w.ctl->not_symmetric, st));
+    cheb_coeff_kernel<<<1, CC_THREADS, 0, st>>>(w.ctl, w.tab, p->mu, p->beta, k, m);
+    {
+        const dim3 grid((unsigned)((N + 255) / 256), (unsigned)(N < 2048 ? N : 2048));
+        cheb_map_kernel<<<grid, 256, 0, st>>>(H->value, H->ld, slot(0), w.ld, (int)N, w.ctl);
+    }
+    if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
+
+    CUtensorMap map;
+    CK(make_slab_map(&map, w.slab, N, w.ld, w.slot_elems, k + m));
+    CK(symm_ab_sk_reset(w.sk, st));
+    unsigned int epoch = 0;
+    int n_launches = 0;
+
+    // T_2 .. T_k, one grouped launch per doubling level (Eq. 13-14)
+    int32_t level[BML_CHEB_MAX_K], ta[BML_CHEB_MAX_K], tb[BML_CHEB_MAX_K];
+    const int levels = cheb_schedule(k, level, ta, tb);
+    for (int lv = 1; lv <= levels; ++lv) {
+        SymmBatch batch;
+        memset(&batch, 0, sizeof(batch));
+        for (int i = 2; i <= k; ++i) {
+            if (level[i - 2] != lv) continue;
+            SymmJob &jb = batch.job[batch.n_jobs++];
+            jb.a = ta[i - 2] - 1; jb.b = tb[i - 2] - 1;
+            jb.Out = slot(i - 1); jb.ldo = w.ld; jb.ldc = w.ld;
+            jb.alpha = 2.0;
+            if (ta[i - 2] == tb[i - 2]) { jb.C = nullptr; jb.beta = 0.0; jb.gamma = -1.0; }     // - T_0
+            else { jb.C = slot(0); jb.beta = -1.0; jb.gamma = 0.0; }                            // - T_1
+        }
+        CK(launch_symm_ab(map, batch, N, w.sk, ++epoch, st));
+        ++n_launches;
+    }
+
+    // S_0 .. S_{m-1} (Eq. 12)
+    if (m <= 4) CK(launch_sums_t<4>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
+    else if (m <= 8) CK(launch_sums_t<8>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
+    else if (m <= 16) CK(launch_sums_t<16>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
+    else CK(launch_sums_t<32>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
+
+    // Eq. 10, innermost bracket first: R_{m-1} = S_{m-1}; R_j = T_k R_{j+1} + S_j, written over S_j; R_0 -> D
+    for (int j = m - 2; j >= 0; --j) {
+        SymmBatch batch;
+        memset(&batch, 0, sizeof(batch));
+        batch.n_jobs = 1;
+        SymmJob &jb = batch.job[0];
+        jb.a = k - 1; jb.b = k + j + 1;
+        jb.C = slot(k + j); jb.ldc = w.ld;
+        jb.Out = (j == 0) ? D->value : slot(k + j);
+        jb.ldo = (j == 0) ? D->ld : w.ld;
+        jb.alpha = 1.0; jb.beta = 1.0; jb.gamma = 0.0;
+        CK(launch_symm_ab(map, batch, N, w.sk, ++epoch, st));
+        ++n_launches;
+    }
+    if (m == 1 && cudaMemcpy2DAsync(D->value, (size_t)D->ld * 8, slot(k), (size_t)w.ld * 8, (size_t)N * 8, (size_t)N,
+                                    cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    CK(launch_trace_dense(D->value, D->ld, (int)N, &w.ctl->trace, st));
+#undef CK
+
+    // the one host round trip of the call
+    ChebCtl h;
+    if (cudaMemcpyAsync(&h, w.ctl, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return BML_ERR_CUDA;
+    if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
+    int status = BML_OK;
+    if (h.fail) status = h.fail;
+    else if (h.not_symmetric) status = BML_ERR_NOT_SYMMETRIC;
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->status = status;
+        stats->n_products = (k - 1) + (m - 1);
+        stats->n_launches = n_launches;
+        stats->L = k * m - 1;
+        stats->emin = h.bounds[0]; stats->emax = h.bounds[1];
+        stats->trace = h.trace;
+        memcpy(stats->c, h.c, sizeof(double) * (size_t)(k * m));
+        memcpy(stats->d, h.d, sizeof(double) * (size_t)(k * m));
+    }
+    return status;
+}
+
+}  // namespace bmlsp2

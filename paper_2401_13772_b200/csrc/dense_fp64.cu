@@ -8,31 +8,10 @@
 // Pipeline: one producer thread issues TMA (cp.async.bulk.tensor, 128B swizzle, FP64 tensor map) into a STAGES-deep
 // ring of { A panel 128 x 16, B panel 128 x 16 } tiles guarded by full/empty mbarriers; 8 consumer warps (2 x 4, warp
 // tile 64 x 32) read fragments with conflict-free LDS.64 and issue mma.sync m8n8k4 f64 (SASS DMMA.8x8x4).
-#include "common.cuh"
+#include "dense_fp64_core.cuh"
 
 namespace bmlsp2 {
 
-// Tile edge BT (tile = BT x BT): 128 for the roofline regime; 64 / 32 for small matrices, where 128 x 128 tiles would
-// leave most SMs idle (N = 256 has 3 tiles of 128 but 36 of 32) and a product is pure latency.  The 8 consumer warps
-// always form a 2 x 4 grid: warp tile (BT/2) x (BT/4).
-constexpr int D_BK = 16;           // k-slab: 16 doubles = 128 B = one SWIZZLE_128B row
-constexpr int D_STAGES = 6;        // 6 x 32 KB = 192 KB at BT = 128
-constexpr int D_CONSUMER_WARPS = 8;
-constexpr int D_PRODUCER_WARPS = 4;     // one warpgroup, so that setmaxnreg can hand its registers to the consumers
-constexpr int D_THREADS = (D_PRODUCER_WARPS + D_CONSUMER_WARPS) * 32;   // 384: ptxas caps at 168 regs/thread ...
-constexpr int D_REGS_PRODUCER = 40;     // ... re-split by setmaxnreg: 128 x 40 + 256 x 232 = 64512 = 384 x 168
-constexpr int D_REGS_CONSUMER = 232;
-constexpr int d_panel_bytes(int BT) { return BT * D_BK * 8; }       // 16 KB at BT = 128
-constexpr int d_stage_bytes(int BT) { return 2 * d_panel_bytes(BT); }
-constexpr size_t d_smem_bytes(int BT)
-{
-    return (size_t)D_STAGES * d_stage_bytes(BT) + 1024 /*align*/ + 512 /*barriers + reduction scratch*/;
-}
-
-// MMA row/col index g (0..7) -> physical row inside an 8-row group.  With the 128B TMA swizzle (16-byte chunk c of
-// row r stored at chunk c ^ (r & 7)) the four rows touched by one half-warp of an LDS.64 fragment load must have
-// distinct (r >> 1) & 3 to hit 32 distinct banks: g = 0..3 -> rows 0,2,4,6 and g = 4..7 -> rows 1,3,5,7.
-__device__ __forceinline__ int perm8(int g) { return ((g & 3) << 1) | (g >> 2); }
 
 template <int BT>
 __global__ void __launch_bounds__(D_THREADS, 1)
@@ -105,11 +84,8 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
 #pragma unroll
             for (int j = 0; j < NI; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
 
-        // byte offset of this lane's element inside a panel for k-step kk: row pg (+ 8-row groups via immediates)
         uint32_t koff[4];
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk)
-            koff[kk] = (uint32_t)(pg * 128 + ((((kk * 2 + (t >> 1)) ^ pg) << 4) | ((t & 1) << 3)));
+        dmma_koff(lane, koff);
         const uint8_t *a_base = smem + wm * (D_BM / 2) * 128;
         const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * (D_BN / 4) * 128;
 
@@ -118,20 +94,7 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
             const uint32_t ph = (uint32_t)(kt / D_STAGES) & 1u;
             mbar_wait(&full_bar[s], ph);
             const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
-#pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-                double a[MI], b[NI];
-#pragma unroll
-                for (int i = 0; i < MI; ++i)
-                    a[i] = *(const double *)(sa + koff[kk] + i * 8 * 128);
-#pragma unroll
-                for (int j = 0; j < NI; ++j)
-                    b[j] = *(const double *)(sb + koff[kk] + j * 8 * 128);
-#pragma unroll
-                for (int i = 0; i < MI; ++i)
-#pragma unroll
-                    for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-            }
+            dmma_slab<MI, NI>(acc, sa, sb, koff);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
         }
@@ -214,31 +177,6 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
 // The TMA ring and the mbarrier phases run on across work items; the fused epilogue (D4) and the finaliser (D5) are
 // those of the kernel above.
 // ------------------------------------------------------------------------------------------------------------
-struct SkItem {
-    int tile, kt0, kt1;
-};
-// it-th work item of CTA c (identical arithmetic in every role); false when the list is exhausted
-__host__ __device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, SkItem &w)
-{
-    const int W = tiles / G, R = tiles - W * G;
-    if (it < W) { w.tile = it * G + c; w.kt0 = 0; w.kt1 = KT; return true; }
-    if (R == 0) return false;
-    const int64_t UT = (int64_t)R * KT;
-    const int64_t u0 = (int64_t)c * UT / G, u1 = (int64_t)(c + 1) * UT / G;
-    const int64_t tl = u0 / KT + (it - W);
-    const int64_t b = tl * KT;
-    const int64_t s = u0 > b ? u0 : b, f = u1 < b + KT ? u1 : b + KT;
-    if (s >= f) return false;
-    w.tile = W * G + (int)tl; w.kt0 = (int)(s - b); w.kt1 = (int)(f - b);
-    return true;
-}
-__device__ __forceinline__ void consumers_bar()
-{
-    asm volatile("bar.sync 1, %0;" ::"n"(D_CONSUMER_WARPS * 32) : "memory");
-}
-
-constexpr int SK_ACC = 64;                                             // FP64 accumulators per consumer thread
-constexpr size_t SK_SLOT_DOUBLES = (size_t)SK_ACC * D_CONSUMER_WARPS * 32;   // 128 x 128
 
 __global__ void __launch_bounds__(D_THREADS, 1)
 x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
@@ -308,9 +246,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
         const int pg = perm8(g);
         const int ctid = warp * 32 + lane;           // consumer thread id 0..255
         uint32_t koff[4];
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk)
-            koff[kk] = (uint32_t)(pg * 128 + ((((kk * 2 + (t >> 1)) ^ pg) << 4) | ((t & 1) << 3)));
+        dmma_koff(lane, koff);
         const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
         int slab = 0;
@@ -331,18 +267,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
                 const uint32_t ph = (uint32_t)(slab / D_STAGES) & 1u;
                 mbar_wait(&full_bar[s], ph);
                 const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
-#pragma unroll
-                for (int kk = 0; kk < 4; ++kk) {
-                    double a[MI], b[NI];
-#pragma unroll
-                    for (int i = 0; i < MI; ++i) a[i] = *(const double *)(sa + koff[kk] + i * 8 * 128);
-#pragma unroll
-                    for (int j = 0; j < NI; ++j) b[j] = *(const double *)(sb + koff[kk] + j * 8 * 128);
-#pragma unroll
-                    for (int i = 0; i < MI; ++i)
-#pragma unroll
-                        for (int j = 0; j < NI; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-                }
+                dmma_slab<MI, NI>(acc, sa, sb, koff);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty_bar[s]);
             }
@@ -468,9 +393,7 @@ int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
     return r == CUDA_SUCCESS ? 0 : BML_ERR_CUDA;
 }
 
-constexpr int SK_MAX_GRID = 256;      // scratch slots / flags provisioned for the persistent kernel
-
-static int sk_grid()
+int sk_grid()
 {
     static int g = 0;
     if (!g) {

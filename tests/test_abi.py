@@ -10,13 +10,18 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared():
-    text = open(os.path.join(ROOT, "include", "bml_sp2.h")).read()
-    return sorted(set(re.findall(r"BML_API\s+[\w\s\*]+?\b(bml_\w+)\s*\(", text)))
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for f in sorted(os.listdir(inc)):
+        if f.endswith(".h"):
+            names |= set(re.findall(r"BML_API\s+[\w\s\*]+?\b(bml_\w+)\s*\(", open(os.path.join(inc, f)).read()))
+    return sorted(names)
 
 
 def test_header_declares_the_north_star_entry_points():
     names = _declared()
-    for required in ("bml_sp2_dense", "bml_sp2_ellpack", "bml_gershgorin", "bml_trace"):
+    for required in ("bml_sp2_dense", "bml_sp2_ellpack", "bml_gershgorin", "bml_trace", "bml_chebyshev_dense",
+                     "bml_symm_ab_dense"):
         assert required in names
 
 
@@ -26,7 +31,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     path = build.build()
     lib = ctypes.CDLL(path)
     for name in _declared():
-        assert hasattr(lib, name), f"{name} declared in include/bml_sp2.h but not exported"
+        assert hasattr(lib, name), f"{name} declared in include/*.h but not exported"
     lib.bml_version.restype = ctypes.c_char_p
     assert b"sm_100a" in lib.bml_version()
     lib.bml_status_string.restype = ctypes.c_char_p
@@ -40,8 +45,9 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     # the ctypes mirrors must have the C layout of the header (checked against gcc's sizeof)
     src = r"""
     #include <stdio.h>
-    #include "bml_sp2.h"
-    int main(void){ printf("%zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t)); return 0; }
+    #include "bml_chebyshev.h"
+    int main(void){ printf("%zu %zu %zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t),
+                           sizeof(bml_cheb_params_t), sizeof(bml_cheb_stats_t)); return 0; }
     """
     import tempfile
 
@@ -50,7 +56,8 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     out = subprocess.run([exe], capture_output=True, check=True).stdout.split()
     os.remove(exe)
     assert [int(x) for x in out] == [ctypes.sizeof(api.bml_matrix_t), ctypes.sizeof(api.bml_sp2_params_t),
-                                    ctypes.sizeof(api.bml_sp2_stats_t)]
+                                    ctypes.sizeof(api.bml_sp2_stats_t), ctypes.sizeof(api.bml_cheb_params_t),
+                                    ctypes.sizeof(api.bml_cheb_stats_t)]
 
 
 def test_sass_contains_the_blackwell_instructions():

@@ -56,3 +56,65 @@ def test_work_item_rejects_bad_arguments():
     assert L.bml_dense_work_item(512, 148, 0, 0, out) == -1       # small matrices do not use the persistent kernel
     assert L.bml_dense_work_item(2048, 148, 148, 0, out) == -1
     assert L.bml_dense_work_item(2048, 148, 0, 0, None) == -1
+
+
+# ------------------------------------------------ grouped Chebyshev products ----------------------------------------
+@pytest.mark.parametrize("N,n_jobs,G", [(1, 1, 148), (40, 1, 148), (256, 1, 148), (256, 8, 148), (500, 2, 148),
+                                        (1000, 4, 148), (2000, 1, 148), (2000, 8, 148), (4000, 3, 132), (1283, 16, 7)])
+def test_grouped_work_list_covers_every_unit_of_every_job_once(N, n_jobs, G):
+    """bml_symm_work_item: every (job, tile, k-slab) is covered exactly once; a split tile has one owner (the part that
+    starts at k-slab 0) followed by its contributors on the next CTAs; at most one contributed partial per CTA."""
+    bt = 32 if N <= 512 else (64 if N <= 1024 else 128)
+    T = (N + bt - 1) // bt
+    KT = (N + 15) // 16
+    cover = {}
+    units = []
+    for c in range(G):
+        items = api.bml_symm_work_items(N, n_jobs, G, c)
+        n_contrib = 0
+        for job, I, J, k0, k1, edge in items:
+            assert edge == bt and 0 <= job < n_jobs and 0 <= I <= J < T and 0 <= k0 < k1 <= KT
+            cover.setdefault((job, I, J), []).append((k0, k1, c))
+            n_contrib += k0 > 0
+        assert n_contrib <= 1
+        units.append(sum(k1 - k0 for *_, k0, k1, _ in items))
+    assert len(cover) == n_jobs * T * (T + 1) // 2
+    W = (n_jobs * T * (T + 1) // 2) // G
+    for parts in cover.values():
+        parts.sort()
+        assert parts[0][0] == 0 and parts[-1][1] == KT
+        for (a0, a1, ca), (b0, b1, cb) in zip(parts, parts[1:]):
+            assert a1 == b0 and cb > ca
+        # the CTAs between the owner and its last contributor that hold no part of this tile have no part of the split
+        # wave at all (fewer k-slabs than CTAs): the owner's scan skips them
+        holders = [p[2] for p in parts]
+        for cc in range(holders[0], holders[-1] + 1):
+            assert cc in holders or units[cc] == W * KT
+    assert sum(units) == n_jobs * T * (T + 1) // 2 * KT
+    tail = [u - W * KT for u in units]
+    assert max(tail) - min(tail) <= 1
+
+
+@pytest.mark.parametrize("k", list(range(2, 33)))
+def test_doubling_schedule(k):
+    """bml_cheb_schedule (reading C5): T_i = 2 T_a T_b - T_{a-b} with a + b = i, a - b in {0, 1}, and both operands
+    come from strictly earlier levels (so one level is one grouped launch)."""
+    sched = api.bml_cheb_schedule(k)
+    assert [s[0] for s in sched] == list(range(2, k + 1))
+    level_of = {0: 0, 1: 0}
+    for i, lv, a, b in sched:
+        assert a + b == i and a - b in (0, 1)
+        assert level_of[a] < lv and level_of[b] < lv
+        assert 2 ** (lv - 1) < i <= 2 ** lv
+        level_of[i] = lv
+    per_level = {}
+    for i, lv, a, b in sched:
+        per_level[lv] = per_level.get(lv, 0) + 1
+    assert max(per_level.values()) <= api.SYMM_MAX_JOBS
+
+
+def test_schedule_rejects_bad_k():
+    L = api.load()
+    assert L.bml_cheb_schedule(1, None, None, None) == -1
+    assert L.bml_cheb_schedule(33, None, None, None) == -1
+    assert L.bml_cheb_schedule(16, None, None, None) == 4
