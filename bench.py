@@ -3,6 +3,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload dense_n2048] [--impl ours|reference]
 
+Workloads: the BASELINE.json configs (dense_n256, dense_n2048 [default], dense_n8192, mixed_n16384, mixed_bf16x3_n16384,
+ellpack_n65536) and, for the Chebyshev expansion of PAPER.md IV.B, cheby_n500 / n1000 / n2000 / n4000 / n8000 (one step =
+one bml_chebyshev_dense call; metric chebyshev_time_to_D_ms).
+
 A "step" is one whole pass of the hot path: one bml_sp2_dense (or bml_sp2_ellpack) solve = Gershgorin bounds +
 rescale + every fused X^2 product until the stop rule + output copy, on a seeded synthetic Hamiltonian.
 Prints ONE JSON line.  The path does not shard (north_star: one GPU, no collectives):
@@ -25,6 +29,7 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 METRIC = "sp2_time_to_D_ms"
+METRIC_CHEBY = "chebyshev_time_to_D_ms"     # SURVEY 8(f) item f-1 workloads (--workload cheby_n*)
 PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 64 FMA/clk/SM
 
 
@@ -166,6 +171,49 @@ def oracle_time_to_D(wname: str, H, budget_s: float, n_products_full: int | None
     return dt / p * full * 1e3, f"first {p} of {full} products timed, scaled by {full}/{p}", cores
 
 
+def oracle_cheby_time_to_D(wname: str, H, budget_s: float):
+    """Time the Chebyshev oracle (oracle/chebyshev.py, chebyshev_ps: the same k + m - 2 products as the GPU path, numpy
+    FP64) on `wname`; above N = 2500 a bounded sample: two products 2 A B - C and two scaled additions at full size,
+    scaled to the k + m - 2 products and k m additions of the expansion.  Also times the LAPACK diagonalisation route
+    (what Fig. 3 of the paper divides by) when it fits the budget.  Returns (ms, sample, cores, extra dict)."""
+    from oracle import chebyshev as och
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[wname]
+    try:
+        from threadpoolctl import threadpool_info
+
+        cores = max([int(t.get("num_threads", 1)) for t in threadpool_info()] or [1])      # the BLAS pool numpy uses
+    except Exception:
+        cores = os.cpu_count() or 1
+    extra = {}
+    if w.N <= 2500:
+        t0 = time.perf_counter()
+        och.chebyshev_ps(H, w.mu, w.beta, w.k, w.m)
+        ms = (time.perf_counter() - t0) * 1e3
+        sample = f"full oracle expansion (chebyshev_ps), {w.k + w.m - 2} products, numpy/BLAS threads"
+    else:
+        emin, emax = och.gershgorin(H)
+        Ht = och.map_to_unit(H, emin, emax)
+        t0 = time.perf_counter()
+        T2 = och.symm_ab(Ht, Ht, None, 2.0, 0.0, -1.0)
+        och.symm_ab(T2, Ht, Ht, 2.0, -1.0, 0.0)
+        per = (time.perf_counter() - t0) / 2
+        t0 = time.perf_counter()
+        S = 0.3 * Ht
+        S = S + 0.2 * T2
+        axpy = (time.perf_counter() - t0) / 2
+        ms = (per * (w.k + w.m - 2) + axpy * w.k * w.m) * 1e3
+        sample = (f"2 of {w.k + w.m - 2} oracle products and 2 of {w.k * w.m} scaled additions timed at full size, "
+                  "scaled")
+    if w.N <= 4000 and budget_s >= 20.0:
+        t0 = time.perf_counter()
+        och.fermi_exact(H, w.mu, w.beta)
+        extra["diagonalisation_ms"] = (time.perf_counter() - t0) * 1e3
+        extra["diagonalisation_note"] = "numpy.linalg.eigh + U f(Lambda) U^T on the host: the route Fig. 3 compares with"
+    return ms, sample, cores, extra
+
+
 EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30,
                      "mixed_bf16x3_n16384": 30, "ellpack_n65536": 12}
 
@@ -177,17 +225,20 @@ def run_reference(args):
     from paper_2401_13772_b200 import hamiltonians as hm
 
     w = hm.WORKLOADS[args.workload]
-    H = hm.make_dense(args.workload) if w.kind == "dense" else hm.make_ellpack(args.workload)
+    H = hm.make_dense(args.workload) if w.kind != "ellpack" else hm.make_ellpack(args.workload)
     total = args.steps + args.warmup
     budget = max(1.0, 200.0 / total)       # whole run within a few minutes
     times, sample, cores = [], "", 1
     for it in range(total):
-        ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
+        if w.kind == "cheby":
+            ms, sample, cores, _ = oracle_cheby_time_to_D(args.workload, H, 0.0)
+        else:
+            ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
         if it >= args.warmup:
             times.append(ms)
     v = float(np.mean(times))
     line = {
-        "impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": METRIC_CHEBY if w.kind == "cheby" else METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": workload_config(args.workload),
@@ -209,6 +260,12 @@ def workload_config(name: str):
                  "within a step, which is part of the method"}
     if w.kind == "ellpack":
         cfg.update({"M": w.M, "drop_tol": w.drop_tol})
+    if w.kind == "cheby":
+        for key in ("n_occ", "idem_tol", "max_products"):
+            cfg.pop(key)
+        cfg["l2"] = "flushed between steps (256 MiB write)"
+        cfg.update({"mu": w.mu, "beta": w.beta, "k": w.k, "m": w.m, "L": w.k * w.m - 1,
+                    "products": w.k + w.m - 2})
     return cfg
 
 
@@ -480,6 +537,136 @@ def run_ours(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------------------------
+# our arm, Chebyshev workloads: same contract, one bml_chebyshev_dense call per step
+# ----------------------------------------------------------------------------------------------------------
+def run_cheby(args):
+    import torch
+
+    from paper_2401_13772_b200 import api, hamiltonians as hm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl")
+    api.load()
+    dev = torch.device("cuda", local)
+    w = hm.WORKLOADS[args.workload]
+    H_np = hm.make_dense(args.workload)
+    H_host = torch.from_numpy(H_np).pin_memory()
+    H_dev = H_host.to(dev)
+    solver = api.ChebyshevSolver(w.N, w.k, w.m, dev)
+    D_host = torch.empty((w.N, w.N), dtype=torch.float64).pin_memory()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    res = None
+    for _ in range(args.warmup):
+        _, res = solver.solve(H_dev, w.mu, w.beta)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)
+            ev[k][0].record()
+            _, res = solver.solve(H_dev, w.mu, w.beta)
+            ev[k][1].record()
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = float(np.mean(step_ms))
+    clocks = clk.summary()
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = d2h = H_host.numel() * 8
+    for _ in range(2):
+        solver.solve(H_host.to(dev, non_blocking=True), w.mu, w.beta)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        D, _ = solver.solve(H_host.to(dev, non_blocking=True), w.mu, w.beta)
+        D_host.copy_(D, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    # dominant kernel: one product alpha A B + beta C + gamma I of this size, timed alone
+    T1 = (2.0 * H_host - (res.emax + res.emin) * torch.eye(w.N, dtype=torch.float64)) / (res.emax - res.emin)
+    slab, n, ld, _ = api.matrix_slab([T1, T1 @ T1, torch.zeros_like(T1)], dev)
+    ws = api._workspace(api.load().bml_symm_ab_workspace_bytes(), dev)
+    job = [(0, 1, 0, 2, 2.0, -1.0, 0.0)]
+    reps = 20
+    for _ in range(3):
+        api.bml_symm_ab_dense(slab, n, ld, job, ws)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(reps):
+        api.bml_symm_ab_dense(slab, n, ld, job, ws)
+    b.record()
+    torch.cuda.synchronize()
+    k_ms = a.elapsed_time(b) / reps
+    peak_probe = api.bml_probe_fp64_tensor_peak(40000)
+    flops = dense_flops_per_product(w.N)
+    achieved = flops / (k_ms * 1e-3) / 1e12
+    n_prod = int(res.n_products)
+    bt = 32 if w.N <= 512 else (64 if w.N <= 1024 else 128)
+    pk, pk_src = peaks()
+    sums_bytes = float(w.k - 1 + w.m) * w.N * w.N * 8
+    roof = {
+        "bound": "tensor", "kernel": "symm_ab_fp64_kernel<%d>" % bt, "achieved": achieved, "peak": peak_probe,
+        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+        "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
+                       "(MEASURED_PEAKS.json has no FP64 entry)",
+        "launch_ms": k_ms, "flops_per_launch": flops,
+        "in_step_tflops": flops * n_prod / (ms * 1e-3) / 1e12,
+        "sums_kernel": {"bound": "hbm", "kernel": "cheb_sums_kernel", "bytes_per_launch": sums_bytes,
+                        "ms_at_peak": sums_bytes / (pk["hbm_gbs"] * 1e9) * 1e3, "peak": pk["hbm_gbs"],
+                        "peak_source": f"{pk_src} copy bandwidth from MEASURED_PEAKS.json"},
+    }
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, sample, cores, extra = oracle_cheby_time_to_D(args.workload, H_np, 25.0)
+        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample, **extra}
+    # gershgorin (2) + coefficients + map + product launches + partial sums + trace
+    launches_per_step = 2 + 1 + 1 + int(res.n_launches) + 1 + 1
+    line = {
+        "metric": METRIC_CHEBY, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(args.workload),
+        "status": int(res.status), "n_products": n_prod, "n_product_launches": int(res.n_launches),
+        "trace_D": res.trace, "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)),
+        "wall_s_timed_region": t_wall, "ms_per_product": ms / max(n_prod, 1),
+        "aggregate_solves_per_s": replicas_per_second(world, ms),
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches_note": f"{launches_per_step} per step: 2 Gershgorin + coefficients + map + "
+                             f"{int(res.n_launches)} grouped product launches ({n_prod} products) + partial sums + trace",
+        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -492,6 +679,10 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    if hm.WORKLOADS[args.workload].kind == "cheby":
+        return run_cheby(args)
     return run_ours(args)
 
 

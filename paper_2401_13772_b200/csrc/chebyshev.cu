@@ -34,7 +34,8 @@ __device__ __forceinline__ double fermi_fn(double eps, double mu, double beta)
 
 // ------------------------------------------------------------------------------------------------------------
 // c_n (Eq. 8) by Chebyshev-Gauss quadrature on N_q = 2 (L + 1) nodes (reading C3), then d_{i,j} (Eq. 10) by dividing
-// the series by T_k with Eq. 11 (reading C4).  One CTA; scalar work, O(L N_q) table look-ups + O(L m) for the division.
+// the series by T_k with Eq. 11 (reading C4).  One CTA; scalar work: O(L N_q) table look-ups, then m division steps of
+// 2k parallel chains of <= m / 2 subtractions.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int CC_THREADS = 1024;
 __global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl, double *__restrict__ tab,
@@ -42,7 +43,6 @@ __global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl,
 {
     __shared__ double s_f[2 * BML_CHEB_MAX_TERMS];     // f at the nodes
     __shared__ double s_p[BML_CHEB_MAX_TERMS];         // dividend of the current division step
-    __shared__ double s_q[BML_CHEB_MAX_TERMS];         // its quotient
     const int terms = k * m, Nq = 2 * terms;
     const double emin = ctl->bounds[0], emax = ctl->bounds[1];
     if (threadIdx.x == 0) ctl->fail = (emax - emin > 0.0) ? 0 : BML_ERR_DEGENERATE;
@@ -54,35 +54,48 @@ __global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl,
         s_f[q] = fermi_fn(0.5 * (emax - emin) * x + 0.5 * (emax + emin), mu, beta);
     }
     __syncthreads();
-    for (int n = threadIdx.x; n < terms; n += CC_THREADS) {
+    // one warp per coefficient, the N_q nodes dealt out to its lanes: j = n (2 q + 1) mod 4 N_q, advanced by 64 n
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int n = warp; n < terms; n += CC_THREADS / 32) {
+        const unsigned period = (unsigned)(4 * Nq);
+        unsigned j = ((unsigned)n * (2u * (unsigned)lane + 1u)) % period;
+        const unsigned step = (64u * (unsigned)n) % period;
         double s = 0.0;
-        unsigned j = (unsigned)n % (unsigned)(4 * Nq);                  // n (2 q + 1) mod 4 N_q, incrementally
-        const unsigned step = (2u * (unsigned)n) % (unsigned)(4 * Nq);
-        for (int q = 0; q < Nq; ++q) {
+        for (int q = lane; q < Nq; q += 32) {
             s = fma(s_f[q], tab[j], s);
             j += step;
-            if (j >= (unsigned)(4 * Nq)) j -= (unsigned)(4 * Nq);
+            if (j >= period) j -= period;
         }
+        s = warp_sum(s);
         const double cn = (n == 0 ? 1.0 : 2.0) / (double)Nq * s;
-        ctl->c[n] = cn;
-        s_p[n] = cn;
+        if (lane == 0) { ctl->c[n] = cn; s_p[n] = cn; }
     }
     __syncthreads();
-    if (threadIdx.x != 0) return;
-    // p = T_k q + r, deg r < k: for n > k, T_n = 2 T_k T_{n-k} - T_{|n-2k|}; T_k = T_k T_0 (Eq. 11), highest n first
+    // p = T_k q + r, deg r < k: for n > k, T_n = 2 T_k T_{n-k} - T_{|n-2k|}; T_k = T_k T_0 (Eq. 11), highest n first.
+    // Going down from the highest n, p_n is final once p_{n+2k} has been subtracted from it, so the 2k residue classes
+    // of n mod 2k are independent chains (one thread each); the reflected targets |n - 2k| = 2k - n, k < n < 2k, come
+    // after the chains.  Every p_i sees the same subtractions in the same order as in the one-thread loop.
+    const int tid = threadIdx.x;
     int len = terms;
     for (int j = 0; j < m; ++j) {
         const int qlen = len - k;
-        for (int i = 0; i < qlen; ++i) s_q[i] = 0.0;
-        for (int n = len - 1; n > k; --n) {
-            const double pn = s_p[n];
-            s_q[n - k] += 2.0 * pn;
-            const int r = n - 2 * k;
-            s_p[r < 0 ? -r : r] -= pn;
+        if (tid < 2 * k && tid < len) {
+            int n = tid + (len - 1 - tid) / (2 * k) * (2 * k);           // largest index of this class below len
+            double above = s_p[n];
+            for (n -= 2 * k; n >= 0; n -= 2 * k) {
+                above = s_p[n] - above;
+                s_p[n] = above;
+            }
         }
-        if (len > k) s_q[0] += s_p[k];
-        for (int i = 0; i < k; ++i) ctl->d[j * k + i] = s_p[i];
-        for (int i = 0; i < qlen; ++i) s_p[i] = s_q[i];
+        __syncthreads();
+        if (tid > 0 && tid < k && 2 * k - tid < len) s_p[tid] -= s_p[2 * k - tid];
+        __syncthreads();
+        if (tid < k) ctl->d[j * k + tid] = s_p[tid];
+        double qv = 0.0;
+        if (tid < qlen) qv = (tid == 0) ? s_p[k] : 2.0 * s_p[tid + k];
+        __syncthreads();
+        if (tid < qlen) s_p[tid] = qv;
+        __syncthreads();
         len = qlen;
     }
 }
@@ -113,25 +126,44 @@ template <int MJ>
 __global__ void __launch_bounds__(256) cheb_sums_kernel(double *__restrict__ slab, int64_t slot_elems, int64_t ld, int N,
                                                         int k, int m, const ChebCtl *__restrict__ ctl)
 {
-    __shared__ double s_d[BML_CHEB_MAX_TERMS];
-    for (int i = threadIdx.x; i < k * m; i += blockDim.x) s_d[i] = ctl->d[i];
+    // s_d[i * MJ + j] = d_{i,j} (0 for j >= m): the MJ coefficients of one T_i are contiguous -> 128-bit broadcast loads
+    __shared__ __align__(16) double s_d[BML_CHEB_MAX_K * MJ];
+    for (int idx = threadIdx.x; idx < k * MJ; idx += blockDim.x) {
+        const int i = idx / MJ, j = idx - i * MJ;
+        s_d[idx] = j < m ? ctl->d[j * k + i] : 0.0;
+    }
     __syncthreads();
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    // two adjacent columns per thread (ld is even and rows are 128-byte aligned, so the pair is one 16-byte access;
+    // a pair that straddles N reads a pad column and stores only its first element)
+    const int c = (blockIdx.x * blockDim.x + threadIdx.x) * 2;
     if (c >= N) return;
+    const bool two = c + 1 < N;
     for (int r = blockIdx.y; r < N; r += gridDim.y) {
         const int64_t off = (int64_t)r * ld + c;
-        double acc[MJ];
+        double acc0[MJ], acc1[MJ];
 #pragma unroll
-        for (int j = 0; j < MJ; ++j) acc[j] = (r == c && j < m) ? s_d[j * k] : 0.0;
+        for (int j = 0; j < MJ; ++j) {
+            acc0[j] = (r == c) ? s_d[j] : 0.0;
+            acc1[j] = (r == c + 1) ? s_d[j] : 0.0;
+        }
+#pragma unroll 8
         for (int i = 1; i < k; ++i) {
-            const double t = __ldg(slab + (int64_t)(i - 1) * slot_elems + off);
+            const double2 t = __ldg((const double2 *)(slab + (int64_t)(i - 1) * slot_elems + off));
 #pragma unroll
-            for (int j = 0; j < MJ; ++j)
-                if (j < m) acc[j] = fma(s_d[j * k + i], t, acc[j]);
+            for (int j = 0; j < MJ; ++j) {
+                const double dij = s_d[i * MJ + j];
+                acc0[j] = fma(dij, t.x, acc0[j]);
+                acc1[j] = fma(dij, t.y, acc1[j]);
+            }
         }
 #pragma unroll
-        for (int j = 0; j < MJ; ++j)
-            if (j < m) slab[(int64_t)(k + j) * slot_elems + off] = acc[j];
+        for (int j = 0; j < MJ; ++j) {
+            if (j < m) {
+                double *dst = slab + (int64_t)(k + j) * slot_elems + off;
+                if (two) *(double2 *)dst = make_double2(acc0[j], acc1[j]);
+                else *dst = acc0[j];
+            }
+        }
     }
 }
 
@@ -139,7 +171,11 @@ template <int MJ>
 static int launch_sums_t(double *slab, int64_t slot_elems, int64_t ld, int N, int k, int m, const ChebCtl *ctl,
                          cudaStream_t st)
 {
-    const dim3 grid((unsigned)((N + 255) / 256), (unsigned)(N < 2048 ? N : 2048));
+    // about 8 CTAs per SM in total, each walking several rows: the staging of d_{i,j} is paid once per CTA
+    const unsigned gx = (unsigned)((N + 511) / 512);
+    unsigned gy = (8u * 148u + gx - 1) / gx;
+    if (gy > (unsigned)N) gy = (unsigned)N;
+    const dim3 grid(gx, gy);
     cheb_sums_kernel<MJ><<<grid, 256, 0, st>>>(slab, slot_elems, ld, N, k, m, ctl);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }

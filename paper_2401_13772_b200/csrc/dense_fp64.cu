@@ -89,14 +89,14 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         const uint8_t *a_base = smem + wm * (D_BM / 2) * 128;
         const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * (D_BN / 4) * 128;
 
+        StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
         for (int kt = 0; kt < KT; ++kt) {
             const int s = kt % D_STAGES;
             const uint32_t ph = (uint32_t)(kt / D_STAGES) & 1u;
             mbar_wait(&full_bar[s], ph);
             const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
             dmma_slab<MI, NI>(acc, sa, sb, koff);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[s]);
+            release.after_slab(empty_bar, s, lane);
         }
 
         // ===================== fused epilogue (D4) =====================
@@ -145,7 +145,9 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
     }
     __syncthreads();
     if (threadIdx.x == 0) {
+        __threadfence();      // release: cumulative over the partial sums the barrier above ordered before this thread
         const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        __threadfence();      // acquire, before the barrier below hands the verdict to the finalising warp
         *s_last = (prev + 1u == gridDim.x);
     }
     __syncthreads();
@@ -250,6 +252,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
         const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
         int slab = 0;
+        StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
         SkItem w;
         for (int it = 0; sk_item(it, c, G, tiles, KT, w); ++it) {
             int I, J;
@@ -268,8 +271,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
                 mbar_wait(&full_bar[s], ph);
                 const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
                 dmma_slab<MI, NI>(acc, sa, sb, koff);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty_bar[s]);
+                release.after_slab(empty_bar, s, lane);
             }
 
             if (w.kt0 > 0) {
@@ -284,7 +286,12 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
                     }
                 __threadfence();
                 consumers_bar();
-                if (ctid == 0) atomicExch(&sk_flags[c], epoch);
+                if (ctid == 0) {
+                    // release by the thread that raises the flag, AFTER the barrier: cumulative over every consumer
+                    // thread's stores (a fence before the barrier alone does not order them before this write)
+                    __threadfence();
+                    atomicExch(&sk_flags[c], epoch);
+                }
                 continue;
             }
             if (w.kt1 < KT) {
@@ -355,7 +362,9 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
     }
     __syncthreads();
     if (threadIdx.x == 0) {
+        __threadfence();      // release: cumulative over the partial sums the barrier above ordered before this thread
         const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        __threadfence();      // acquire, before the barrier below hands the verdict to the finalising warp
         *s_last = (prev + 1u == gridDim.x);
     }
     __syncthreads();

@@ -57,6 +57,24 @@ __device__ __forceinline__ void dmma_slab(double (&acc)[MI][NI][2], const uint8_
     }
 }
 
+// Release of a ring stage back to the TMA producer, ONE SLAB LATE.  ptxas schedules a stage's mbarrier.arrive right
+// behind the ISSUE of the slab's last fragment loads (the MMAs that consume them follow it), and the arrive does not
+// wait for those loads to have read shared memory: when the consumers run close behind the producer (short, store-only
+// epilogues; measured on the grouped Chebyshev launches, ~1 wrong 32-byte fragment chunk per 40000 tiles) the refill of
+// the stage could land under the last k-step's loads.  Releasing stage n only after the loads of slab n + 1 were issued
+// closes that: shared-memory loads of one warp complete in order, and slab n + 1's first MMAs -- issued before that
+// point -- already needed its own first loads, hence every load of slab n, to have completed.  Costs one of the
+// D_STAGES stages of look-ahead.
+struct StageRelease {
+    int owed = -1;          // stage read by the previous slab, not yet released
+    __device__ __forceinline__ void after_slab(uint64_t *empty_bar, int s, int lane)
+    {
+        __syncwarp();
+        if (lane == 0 && owed >= 0) mbar_arrive(&empty_bar[owed]);
+        owed = s;
+    }
+};
+
 // ------------------------------------------------------------------------------------------------------------
 // Work list of the persistent kernels (see dense_fp64.cu): full waves of tiles, then a K-split last wave.
 // ------------------------------------------------------------------------------------------------------------

@@ -413,7 +413,9 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
     }
     __syncthreads();
     if (threadIdx.x == 0) {
+        __threadfence();      // release: cumulative over the partial sums the barrier above ordered before this thread
         const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        __threadfence();      // acquire, before the barrier below hands the verdict to the finalising warp
         *s_last = (prev + 1u == gridDim.x);
     }
     __syncthreads();

@@ -582,7 +582,9 @@ x2_ellpack_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, in
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
+        __threadfence();      // release: cumulative over the partial sums the barrier above ordered before this thread
         const uint32_t prev = atomicAdd(&ctl->arrivals, 1u);
+        __threadfence();      // acquire, before the barrier below hands the verdict to the finalising warp
         s_last = (prev + 1u == gridDim.x);
     }
     __syncthreads();

@@ -89,6 +89,7 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
     dmma_koff(lane, koff);
     const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
     int slab = 0;
+    StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
     SkItem w;
     for (int it = 0; sk_item(it, c, G, total, KT, w); ++it) {
         const int q = w.tile / tiles;
@@ -108,8 +109,7 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
             const uint32_t ph = (uint32_t)(slab / D_STAGES) & 1u;
             mbar_wait(&full_bar[s], ph);
             dmma_slab<MI, NI>(acc, a_base + (size_t)s * STAGE_BYTES, b_base + (size_t)s * STAGE_BYTES, koff);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[s]);
+            release.after_slab(empty_bar, s, lane);
         }
 
         if (w.kt0 > 0) {
@@ -124,7 +124,12 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
                 }
             __threadfence();
             consumers_bar();
-            if (ctid == 0) atomicExch(&sk_flags[c], epoch);
+            if (ctid == 0) {
+                // release by the thread that raises the flag, AFTER the barrier: cumulative over every consumer
+                // thread's stores (a fence before the barrier alone does not order them before this write)
+                __threadfence();
+                atomicExch(&sk_flags[c], epoch);
+            }
             continue;
         }
         if (w.kt1 < KT) {

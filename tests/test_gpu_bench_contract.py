@@ -37,3 +37,24 @@ def test_bench_prints_one_json_line_with_the_contract_keys():
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
     assert d["clocks"]["sm_max_mhz"] and "reasons" in d["clocks"]
+
+
+def test_bench_contract_chebyshev_workload():
+    """Same contract on a Chebyshev workload (--workload cheby_n500): its own metric name, the grouped product kernel
+    as the roofline kernel, and the oracle + diagonalisation timings in cpu_baseline."""
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--workload", "cheby_n500", "--steps", "3",
+                          "--warmup", "3"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["metric"] == "chebyshev_time_to_D_ms" and d["unit"] == "ms" and d["higher_is_better"] is False
+    assert d["status"] == 0 and d["n_products"] == 30 and d["config"]["L"] == 255
+    assert d["roofline"]["kernel"].startswith("symm_ab_fp64_kernel") and 0 < d["roofline"]["frac"] <= 1.0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
+    assert d["e2e"]["h2d_bytes_per_step"] == 500 * 500 * 8 and d["e2e"]["value"] >= d["value"] * 0.5
+    assert d["gpu_launches"] == 3 * (6 + 19)

@@ -111,6 +111,31 @@ def test_symm_ab_is_bit_reproducible(api):
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
+def test_grouped_store_only_launches_are_bit_reproducible(api):
+    """Regression test of the ring-stage release (dense_fp64_core.cuh StageRelease): grouped launches of products with
+    no C term have a store-only epilogue, the consumers then run close behind the TMA producer, and a stage released
+    before its last fragment loads had completed used to be refilled under them -- about 1 launch in 20 at N = 4000
+    came back with a few wrong 32-byte fragment chunks.  150 launches x 8 jobs must be bitwise identical."""
+    import torch
+
+    N = 2048
+    rng = np.random.default_rng(11)
+    G = rng.normal(size=(N, N)) / np.sqrt(N)
+    X = (G + G.T) / 4
+    X2 = X @ X
+    mats = [X, np.triu(X2) + np.triu(X2, 1).T, np.eye(N) - X] + [np.zeros((N, N))] * 8
+    slab, n, ld, se = api.matrix_slab(mats)
+    ws = api._workspace(api.load().bml_symm_ab_workspace_bytes(), "cuda")
+    ops = [(0, 0), (1, 0), (1, 1), (2, 1), (2, 2), (0, 2), (1, 2), (0, 1)]
+    jobs = [(a, b, -1, 3 + q, 2.0, 0.0, -1.0) for q, (a, b) in enumerate(ops)]
+    api.bml_symm_ab_dense(slab, n, ld, jobs, ws)
+    ref = slab[3:].clone()
+    check_product(api.slab_matrix(slab, 4, n, ld).cpu().numpy(), mats[1], mats[0], None, 2.0, 0.0, -1.0)
+    for it in range(150):
+        api.bml_symm_ab_dense(slab, n, ld, jobs, ws)
+        assert torch.equal(slab[3:], ref), f"launch {it} differs"
+
+
 def test_symm_ab_rejects_bad_arguments(api):
     A, B, C = commuting_pair(40, 1)
     slab, n, ld, se = api.matrix_slab([A, B, C])
