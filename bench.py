@@ -51,6 +51,7 @@ NCU_TRAFFIC_BYTES = {
     "dense_n8192": 6.08e9,          # 5.55 GB read (row panels re-read) + 0.53 GB written
     "mixed_n16384": 20.4e9,         # 17.2 GB read + 3.2 GB written (FP16 x 2 planes, super-block tile order)
     "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (capture quoted in DESIGN.md 5.3)
+    "cheby_n2000": 98.1e6,          # grouped product kernel, one Eq. 10 step: 85.3 MB read + 12.8 MB written
     "ellpack_n65536": 1.25e9,       # kernel 1: 0.246 + 0.190 GB; kernel 2: 0.451 + 0.363 GB (read + written)
 }
 
