@@ -272,3 +272,22 @@ def test_sp2_dense_is_bit_reproducible(api):
 
     assert torch.equal(D0, D1)
     assert np.array_equal(r0.trace, r1.trace) and np.array_equal(r0.idem, r1.idem)
+
+
+def test_sp2_square_kernel_many_launches_bit_reproducible(api):
+    """The persistent FP64 kernel repeated 300 times on one iterate (N = 2048, every tile K-split; and N = 3000, full
+    waves + a split wave): any race in the TMA ring (dense_fp64_core.cuh StageRelease) or in the split-tile hand-off
+    would show as a launch whose output differs in a few elements."""
+    import torch
+
+    for N in (2048, 3000):
+        rng = np.random.default_rng(N)
+        G = rng.normal(size=(N, N)) / np.sqrt(N)
+        X = api.padded_dense((G + G.T) / 4 + 0.5 * np.eye(N))
+        Xn = torch.empty_strided(X.shape, X.stride(), dtype=X.dtype, device="cuda")
+        ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(N, 0), "cuda")
+        api.bml_x2_dense(X, 0, 0, Xn, ws)
+        ref = Xn.clone()
+        for it in range(300):
+            _, sums = api.bml_x2_dense(X, 0, 0, Xn, ws)
+            assert torch.equal(Xn, ref), f"N={N}: launch {it} differs"
