@@ -1,4 +1,4 @@
-"""Thin ctypes binding of libbmlsp2.so (include/bml_sp2.h, include/bml_chebyshev.h) — argument marshalling only.
+"""Thin ctypes binding of libbmlsp2.so (include/bml_sp2.h, include/bml_chebyshev.h, include/bml_graph.h) — argument marshalling only.
 
 Every function has the name of the C entry point it calls and takes torch CUDA tensors for device memory; all
 arithmetic of the method runs in the library's sm_100a kernels.  There is no CPU fallback: if the library is missing
@@ -29,7 +29,11 @@ EXPORTS = [
     # include/bml_chebyshev.h
     "bml_chebyshev_workspace_bytes", "bml_chebyshev_dense", "bml_symm_ab_workspace_bytes", "bml_symm_ab_dense",
     "bml_cheb_schedule", "bml_symm_work_item",
+    # include/bml_graph.h
+    "bml_graph_workspace_bytes", "bml_graph_chebyshev_ellpack", "bml_graph_core_halo", "bml_matrix2submatrix_ellpack",
+    "bml_submatrix2matrix_ellpack",
 ]
+GRAPH_MAX_PARTS = 256
 CHEB_MAX_K, CHEB_MAX_M, CHEB_MAX_TERMS, SYMM_MAX_JOBS = 32, 32, 1024, 16
 
 
@@ -96,6 +100,32 @@ class bml_cheb_stats_t(ctypes.Structure):
     ]
 
 
+class bml_graph_params_t(ctypes.Structure):
+    _fields_ = [
+        ("mu", ctypes.c_double),
+        ("beta", ctypes.c_double),
+        ("graph_tol", ctypes.c_double),
+        ("drop_tol", ctypes.c_double),
+        ("k", ctypes.c_int32),
+        ("m", ctypes.c_int32),
+        ("n_parts", ctypes.c_int32),
+        ("part_capacity", ctypes.c_int32),
+    ]
+
+
+class bml_graph_stats_t(ctypes.Structure):
+    _fields_ = [
+        ("status", ctypes.c_int32),
+        ("n_parts", ctypes.c_int32),
+        ("overflow_row", ctypes.c_int32),
+        ("max_part_size", ctypes.c_int32),
+        ("n_products", ctypes.c_int32),
+        ("pad", ctypes.c_int32),
+        ("part_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
+        ("core_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
+    ]
+
+
 _lib = None
 
 
@@ -159,6 +189,17 @@ def load(build_if_missing: bool = True):
     L.bml_cheb_schedule.argtypes = [i32, i32p, i32p, i32p]
     L.bml_symm_work_item.restype = ctypes.c_int
     L.bml_symm_work_item.argtypes = [i64, i32, i32, i32, i32, i32p]
+    L.bml_graph_workspace_bytes.restype = sz
+    L.bml_graph_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]
+    L.bml_graph_chebyshev_ellpack.restype = ctypes.c_int
+    L.bml_graph_chebyshev_ellpack.argtypes = [MP, vp, vp, ctypes.POINTER(bml_graph_params_t), MP, vp, sz,
+                                              ctypes.POINTER(bml_graph_stats_t), vp]
+    L.bml_graph_core_halo.restype = ctypes.c_int
+    L.bml_graph_core_halo.argtypes = [MP, vp, vp, i32, dbl, vp, vp, vp, vp, sz, vp]
+    L.bml_matrix2submatrix_ellpack.restype = ctypes.c_int
+    L.bml_matrix2submatrix_ellpack.argtypes = [MP, vp, i32, vp, i64, vp]
+    L.bml_submatrix2matrix_ellpack.restype = ctypes.c_int
+    L.bml_submatrix2matrix_ellpack.argtypes = [vp, i64, vp, vp, i32, dbl, MP, vp, vp]
     _lib = L
     return L
 
@@ -545,3 +586,100 @@ def bml_symm_work_items(N: int, n_jobs: int, n_ctas: int, cta: int):
             raise RuntimeError(f"bml_symm_work_item: {bml_status_string(rc)}")
         items.append(tuple(out))
         it += 1
+
+
+# ------------------------------------------------------------------------------------------------------------
+# include/bml_graph.h
+# ------------------------------------------------------------------------------------------------------------
+@dataclass
+class GraphResult:
+    status: int
+    n_parts: int
+    overflow_row: int
+    max_part_size: int
+    n_products: int
+    part_size: list
+    core_size: list
+    message: str = field(default="")
+
+
+class GraphSolver:
+    """Pre-allocated output and workspace for repeated bml_graph_chebyshev_ellpack calls."""
+
+    def __init__(self, N: int, M_out: int, n_parts: int, part_capacity: int, k: int, m: int, device="cuda"):
+        L = load()
+        self.N, self.M_out, self.n_parts, self.cap, self.k, self.m = int(N), int(M_out), int(n_parts), int(part_capacity), int(k), int(m)
+        self.device = torch.device(device)
+        self.dv = torch.zeros((N, M_out), dtype=torch.float64, device=self.device)
+        self.di = torch.zeros((N, M_out), dtype=torch.int32, device=self.device)
+        self.dn = torch.zeros((N,), dtype=torch.int32, device=self.device)
+        self.ws_bytes = L.bml_graph_workspace_bytes(self.N, self.n_parts, self.cap, self.k, self.m)
+        if self.ws_bytes == 0:
+            raise RuntimeError("bml_graph_workspace_bytes: " + bml_status_string(-1))
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, H, core_offsets: torch.Tensor, core_nodes: torch.Tensor, graph_tol: float, mu: float, beta: float,
+              drop_tol: float):
+        L = load()
+        h = ellpack_desc(*H)
+        d = ellpack_desc(self.dv, self.di, self.dn)
+        _require_cuda(core_offsets, torch.int32, "core_offsets")
+        _require_cuda(core_nodes, torch.int32, "core_nodes")
+        p = bml_graph_params_t(float(mu), float(beta), float(graph_tol), float(drop_tol), self.k, self.m, self.n_parts,
+                               self.cap)
+        st = bml_graph_stats_t()
+        rc = L.bml_graph_chebyshev_ellpack(ctypes.byref(h), core_offsets.data_ptr(), core_nodes.data_ptr(), ctypes.byref(p),
+                                           ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes, ctypes.byref(st), _stream())
+        P = self.n_parts
+        res = GraphResult(int(rc), int(st.n_parts), int(st.overflow_row), int(st.max_part_size), int(st.n_products),
+                          list(st.part_size[:P]), list(st.core_size[:P]), bml_status_string(rc))
+        return (self.dv, self.di, self.dn), res
+
+
+def bml_graph_chebyshev_ellpack(H, core_offsets, core_nodes, graph_tol, mu, beta, k, m, drop_tol, M_out, part_capacity):
+    """Graph-based D (Listing 11 with the Chebyshev local solver).  Returns ((value, index, nnz) of D, GraphResult)."""
+    N = H[0].shape[0]
+    solver = GraphSolver(N, M_out, core_offsets.numel() - 1, part_capacity, k, m, H[0].device)
+    return solver.solve(H, core_offsets, core_nodes, graph_tol, mu, beta, drop_tol)
+
+
+def bml_graph_core_halo(H, core_offsets: torch.Tensor, core_nodes: torch.Tensor, graph_tol: float):
+    """Returns (part_nodes[P, N] int32, is_core[P, N] uint8, sizes[P, 2] int32) CUDA tensors (asynchronous)."""
+    L = load()
+    h = ellpack_desc(*H)
+    P, N = core_offsets.numel() - 1, h.N
+    dev = H[0].device
+    nodes = torch.zeros((P, N), dtype=torch.int32, device=dev)
+    is_core = torch.zeros((P, N), dtype=torch.uint8, device=dev)
+    sizes = torch.zeros((P, 2), dtype=torch.int32, device=dev)
+    ws = torch.empty(P * N, dtype=torch.uint8, device=dev)
+    rc = L.bml_graph_core_halo(ctypes.byref(h), core_offsets.data_ptr(), core_nodes.data_ptr(), P, float(graph_tol),
+                               nodes.data_ptr(), is_core.data_ptr(), sizes.data_ptr(), ws.data_ptr(), P * N, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_graph_core_halo: {bml_status_string(rc)}")
+    return nodes, is_core, sizes
+
+
+def bml_matrix2submatrix_ellpack(H, nodes: torch.Tensor) -> torch.Tensor:
+    """Dense h = H[nodes, nodes] (nodes: ascending int32 CUDA tensor)."""
+    L = load()
+    h = ellpack_desc(*H)
+    s = int(nodes.numel())
+    out = torch.empty((s, s), dtype=torch.float64, device=nodes.device)
+    rc = L.bml_matrix2submatrix_ellpack(ctypes.byref(h), nodes.data_ptr(), s, out.data_ptr(), s, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_matrix2submatrix_ellpack: {bml_status_string(rc)}")
+    return out
+
+
+def bml_submatrix2matrix_ellpack(d: torch.Tensor, nodes: torch.Tensor, is_core: torch.Tensor, drop_tol: float, D):
+    """Scatter the core rows of dense d into the ELLPACK-R triple D.  Returns the overflow row tensor (INT32_MAX = none)."""
+    L = load()
+    _require_cuda(d, torch.float64, "d")
+    dd = ellpack_desc(*D)
+    ov = torch.full((1,), 2**31 - 1, dtype=torch.int32, device=d.device)
+    rc = L.bml_submatrix2matrix_ellpack(d.data_ptr(), d.stride(0), nodes.data_ptr(), is_core.data_ptr(), int(nodes.numel()),
+                                        float(drop_tol), ctypes.byref(dd), ov.data_ptr(), _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_submatrix2matrix_ellpack: {bml_status_string(rc)}")
+    return ov

@@ -4,6 +4,7 @@
 
 #include "common.cuh"
 #include "symm_ab.cuh"
+#include "../../include/bml_graph.h"
 
 namespace bmlsp2 {
 
@@ -50,6 +51,15 @@ size_t cheb_workspace_bytes(int64_t N, int k, int m);
 int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b);
 int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws,
                      bml_cheb_stats_t *stats, cudaStream_t st);
+// graph.cu
+size_t graph_workspace_bytes(int64_t N, int n_parts, int cap, int k, int m);
+int graph_chebyshev_solve(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, const bml_graph_params_t *p,
+                          bml_matrix_t *D, void *ws, bml_graph_stats_t *stats, cudaStream_t st);
+int launch_graph_core_halo(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, int n_parts, double tau,
+                           int32_t *part_nodes, uint8_t *is_core, int32_t *sizes, uint8_t *flag, cudaStream_t st);
+int launch_graph_gather(const bml_matrix_t *H, const int32_t *nodes, int s, double *h, int64_t ld, cudaStream_t st);
+int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
+                         bml_matrix_t *D, int32_t *overflow, cudaStream_t st);
 // probe.cu
 int run_fp64_tensor_probe(int iters, double *flops, double *ms, cudaStream_t st);
 
@@ -223,6 +233,7 @@ const char *bml_status_string(int status)
         case BML_ERR_CUDA: return "CUDA error";
         case BML_ERR_NOT_SYMMETRIC: return "H is not symmetric";
         case BML_ERR_ACC_CAPACITY: return "ELLPACK X^2 accumulator capacity exceeded";
+        case BML_ERR_PART_CAPACITY: return "graph solver: a core+halo part exceeds part_capacity";
         default: return "unknown status";
     }
 }
@@ -471,6 +482,76 @@ int bml_symm_work_item(int64_t N, int32_t n_jobs, int32_t n_ctas, int32_t cta, i
 {
     if (!out6) return BML_ERR_INVALID;
     return symm_ab_work_item(N, n_jobs, n_ctas, cta, it, out6);
+}
+
+// ------------------------------------------------ bml_graph.h ------------------------------------------------
+// ELLPACK-R descriptor whose row capacity may exceed the SP2 kernels' BML_ELL_MAX_M (rows of a graph-built D are as
+// long as a core+halo part unless drop_tol cuts them)
+static bool ell_ok_wide(const bml_matrix_t *A)
+{
+    return A && A->type == BML_ELLPACK && A->value && A->index && A->nnz && A->N > 0 && A->N < (1 << 29) - 1 &&
+           A->M >= 1 && A->M <= (1 << 20);
+}
+static bool graph_params_ok(const bml_graph_params_t *p, int64_t N)
+{
+    return p && p->n_parts >= 1 && p->n_parts <= BML_GRAPH_MAX_PARTS && p->part_capacity >= 1 &&
+           (int64_t)p->part_capacity <= N && p->k >= 2 && p->k <= BML_CHEB_MAX_K && p->m >= 1 && p->m <= BML_CHEB_MAX_M &&
+           p->k * p->m <= BML_CHEB_MAX_TERMS && p->beta > 0.0 && p->mu == p->mu && p->graph_tol >= 0.0 &&
+           p->drop_tol >= 0.0;
+}
+
+size_t bml_graph_workspace_bytes(int64_t N, int32_t n_parts, int32_t part_capacity, int32_t k, int32_t m)
+{
+    if (N <= 0 || n_parts < 1 || n_parts > BML_GRAPH_MAX_PARTS || part_capacity < 1 || part_capacity > N || k < 2 ||
+        k > BML_CHEB_MAX_K || m < 1 || m > BML_CHEB_MAX_M)
+        return 0;
+    return graph_workspace_bytes(N, n_parts, part_capacity, k, m);
+}
+
+int bml_graph_chebyshev_ellpack(const bml_matrix_t *H, const int32_t *d_core_offsets, const int32_t *d_core_nodes,
+                                const bml_graph_params_t *p, bml_matrix_t *D, void *d_workspace, size_t workspace_bytes,
+                                bml_graph_stats_t *stats, void *cuda_stream)
+{
+    int r;
+    if (!ell_ok_wide(H) || !ell_ok_wide(D) || D->N != H->N || !graph_params_ok(p, H->N) || !d_core_offsets ||
+        !d_core_nodes || !d_workspace || D->value == H->value || D->index == H->index || D->nnz == H->nnz ||
+        ((uintptr_t)d_workspace & 1023) != 0 ||
+        workspace_bytes < bml_graph_workspace_bytes(H->N, p->n_parts, p->part_capacity, p->k, p->m)) {
+        r = BML_ERR_INVALID;
+        if (stats) memset(stats, 0, sizeof(*stats));
+    } else {
+        r = graph_chebyshev_solve(H, d_core_offsets, d_core_nodes, p, D, d_workspace, stats, (cudaStream_t)cuda_stream);
+    }
+    if (stats) stats->status = r;
+    return r;
+}
+
+int bml_graph_core_halo(const bml_matrix_t *H, const int32_t *d_core_offsets, const int32_t *d_core_nodes, int32_t n_parts,
+                        double graph_tol, int32_t *d_part_nodes, uint8_t *d_is_core, int32_t *d_part_sizes,
+                        void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!ell_ok_wide(H) || !d_core_offsets || !d_core_nodes || n_parts < 1 || n_parts > BML_GRAPH_MAX_PARTS ||
+        !(graph_tol >= 0.0) || !d_part_nodes || !d_is_core || !d_part_sizes || !d_workspace ||
+        workspace_bytes < (size_t)n_parts * (size_t)H->N)
+        return BML_ERR_INVALID;
+    return launch_graph_core_halo(H, d_core_offsets, d_core_nodes, n_parts, graph_tol, d_part_nodes, d_is_core,
+                                  d_part_sizes, (uint8_t *)d_workspace, (cudaStream_t)cuda_stream);
+}
+
+int bml_matrix2submatrix_ellpack(const bml_matrix_t *H, const int32_t *d_nodes, int32_t s, double *d_h, int64_t ld,
+                                 void *cuda_stream)
+{
+    if (!ell_ok_wide(H) || !d_nodes || s < 1 || (int64_t)s > H->N || !d_h || ld < s) return BML_ERR_INVALID;
+    return launch_graph_gather(H, d_nodes, s, d_h, ld, (cudaStream_t)cuda_stream);
+}
+
+int bml_submatrix2matrix_ellpack(const double *d_d, int64_t ld, const int32_t *d_nodes, const uint8_t *d_is_core, int32_t s,
+                                 double drop_tol, bml_matrix_t *D, int32_t *d_overflow_row, void *cuda_stream)
+{
+    if (!ell_ok_wide(D) || !d_d || !d_nodes || !d_is_core || s < 1 || (int64_t)s > D->N || ld < s || !(drop_tol >= 0.0) ||
+        !d_overflow_row)
+        return BML_ERR_INVALID;
+    return launch_graph_scatter(d_d, ld, d_nodes, d_is_core, s, drop_tol, D, d_overflow_row, (cudaStream_t)cuda_stream);
 }
 
 int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream)

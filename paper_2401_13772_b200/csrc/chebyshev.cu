@@ -229,8 +229,10 @@ static ChebWs carve_cheb(void *ws, int64_t N, int k, int m)
 
 size_t cheb_workspace_bytes(int64_t N, int k, int m) { return carve_cheb(nullptr, N, k, m).total; }
 
-int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, bml_cheb_stats_t *stats,
-                     cudaStream_t st)
+// Enqueue one expansion (steps C0-C6), no host synchronisation.  *n_launches_out <- product-kernel launches.
+// The device-side verdict (0 or BML_ERR_DEGENERATE) is left in the int that cheb_fail_flag(ws) points to.
+int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, int *n_launches_out,
+                       cudaStream_t st)
 {
     const int64_t N = H->N;
     const int k = p->k, m = p->m;
@@ -297,7 +299,20 @@ int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matr
         return BML_ERR_CUDA;
     CK(launch_trace_dense(D->value, D->ld, (int)N, &w.ctl->trace, st));
 #undef CK
+    if (n_launches_out) *n_launches_out = n_launches;
+    return 0;
+}
 
+int *cheb_fail_flag(void *ws) { return &((ChebCtl *)ws)->fail; }
+
+int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, bml_cheb_stats_t *stats,
+                     cudaStream_t st)
+{
+    const int k = p->k, m = p->m;
+    ChebWs w = carve_cheb(ws, H->N, k, m);
+    int n_launches = 0;
+    const int r = cheb_dense_enqueue(H, p, D, ws, &n_launches, st);
+    if (r) return r;
     // the one host round trip of the call
     ChebCtl h;
     if (cudaMemcpyAsync(&h, w.ctl, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;

@@ -1,0 +1,286 @@
+// graph.cu -- the graph-based density-matrix construction (PAPER.md VIII.B, Eq. 15, Listing 11):
+// core-halo parts from the Hamiltonian's own graph, gather of the dense sub-matrices (bml_matrix2submatrix), one
+// Chebyshev expansion per part (chebyshev.cu), thresholded scatter of the core rows (bml_submatrix2matrix).
+#include <string.h>
+
+#include "common.cuh"
+#include "../../include/bml_graph.h"
+
+namespace bmlsp2 {
+
+// chebyshev.cu
+size_t cheb_workspace_bytes(int64_t N, int k, int m);
+int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, int *n_launches_out,
+                       cudaStream_t st);
+int *cheb_fail_flag(void *ws);
+
+// part that owns position q of the core-node list: largest k with offsets[k] <= q
+__device__ __forceinline__ int part_of(const int32_t *__restrict__ offs, int n_parts, int q)
+{
+    int lo = 0, hi = n_parts;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (offs[mid] <= q) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// Eq. 15 + P:494, first pass: flag[k][o] = 1 for every neighbour o of a core node of part k.  One warp per core node.
+// (All writers store the same value, so plain byte stores suffice; the core marks follow in a second launch.)
+__global__ void __launch_bounds__(256) graph_mark_halo_kernel(const double *__restrict__ hv, const int32_t *__restrict__ hi,
+                                                              const int32_t *__restrict__ hn, int N, int M,
+                                                              const int32_t *__restrict__ offs,
+                                                              const int32_t *__restrict__ core_nodes, int n_parts,
+                                                              double tau, uint8_t *__restrict__ flag)
+{
+    const int q = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (q >= N) return;
+    const int l = core_nodes[q];
+    uint8_t *row = flag + (size_t)part_of(offs, n_parts, q) * N;
+    const int n = hn[l];
+    for (int p = lane; p < n; p += 32) {
+        const int o = hi[(size_t)l * M + p];
+        if (o != l && fabs(hv[(size_t)l * M + p]) >= tau) row[o] = 1;
+    }
+}
+__global__ void __launch_bounds__(256) graph_mark_core_kernel(int N, const int32_t *__restrict__ offs,
+                                                              const int32_t *__restrict__ core_nodes, int n_parts,
+                                                              uint8_t *__restrict__ flag)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= N) return;
+    flag[(size_t)part_of(offs, n_parts, q) * N + core_nodes[q]] = 2;
+}
+
+// Ascending node list of every part (reading G2): one CTA per part compacts its flag row with a block-wide scan.
+constexpr int GC_THREADS = 1024;
+__global__ void __launch_bounds__(GC_THREADS) graph_compact_kernel(const uint8_t *__restrict__ flag, int N,
+                                                                   int32_t *__restrict__ nodes, uint8_t *__restrict__ is_core,
+                                                                   int32_t *__restrict__ sizes)
+{
+    __shared__ int s_warp[GC_THREADS / 32];
+    __shared__ int s_base, s_core;
+    const int part = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint8_t *row = flag + (size_t)part * N;
+    if (threadIdx.x == 0) { s_base = 0; s_core = 0; }
+    __syncthreads();
+    for (int j0 = 0; j0 < N; j0 += GC_THREADS) {
+        const int j = j0 + threadIdx.x;
+        const int f = j < N ? row[j] : 0;
+        const unsigned bal = __ballot_sync(0xffffffffu, f != 0), balc = __ballot_sync(0xffffffffu, f == 2);
+        if (lane == 0) s_warp[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+        for (int w = 0; w < GC_THREADS / 32; ++w) { const int c = s_warp[w]; if (w < warp) before += c; total += c; }
+        const int base = s_base;
+        if (f) {
+            const int pos = base + before + __popc(bal & ((1u << lane) - 1u));
+            nodes[(size_t)part * N + pos] = j;
+            is_core[(size_t)part * N + pos] = (uint8_t)(f == 2);
+        }
+        if (lane == 0 && balc) atomicAdd(&s_core, __popc(balc));
+        __syncthreads();
+        if (threadIdx.x == 0) s_base = base + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { sizes[2 * part] = s_base; sizes[2 * part + 1] = s_core; }
+}
+
+// bml_matrix2submatrix: h[a, b] = H[nodes[a], nodes[b]].  One warp per row a: zero the row, then place the stored
+// entries whose column is in the (ascending) node list, found by binary search.
+__global__ void __launch_bounds__(256) graph_gather_kernel(const double *__restrict__ hv, const int32_t *__restrict__ hi,
+                                                           const int32_t *__restrict__ hn, int M,
+                                                           const int32_t *__restrict__ nodes, int s, double *__restrict__ h,
+                                                           int64_t ld)
+{
+    const int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (a >= s) return;
+    double *row = h + (int64_t)a * ld;
+    for (int b = lane; b < s; b += 32) row[b] = 0.0;
+    __syncwarp();
+    const int i = nodes[a], n = hn[i];
+    for (int p = lane; p < n; p += 32) {
+        const int j = hi[(size_t)i * M + p];
+        int lo = 0, hi2 = s - 1;
+        while (lo < hi2) {
+            const int mid = (lo + hi2) >> 1;
+            if (nodes[mid] < j) lo = mid + 1; else hi2 = mid;
+        }
+        if (nodes[lo] == j) row[lo] = hv[(size_t)i * M + p];
+    }
+}
+
+// bml_submatrix2matrix: core rows of d -> ELLPACK-R rows of D with the drop rule (readings G4, G5).  One warp per row.
+__global__ void __launch_bounds__(256) graph_scatter_kernel(const double *__restrict__ d, int64_t ld,
+                                                            const int32_t *__restrict__ nodes,
+                                                            const uint8_t *__restrict__ is_core, int s, double drop_tol,
+                                                            double *__restrict__ dv, int32_t *__restrict__ di,
+                                                            int32_t *__restrict__ dn, int M, int32_t *__restrict__ overflow)
+{
+    const int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (a >= s || !is_core[a]) return;
+    const int i = nodes[a];
+    const double *row = d + (int64_t)a * ld;
+    // count first: a row that does not fit is left untouched
+    int count = 0;
+    for (int b0 = 0; b0 < s; b0 += 32) {
+        const int b = b0 + lane;
+        const bool keep = b < s && (fabs(row[b]) >= drop_tol || nodes[b] == i);
+        count += __popc(__ballot_sync(0xffffffffu, keep));
+    }
+    if (count > M) {
+        if (lane == 0) atomicMin(overflow, i);
+        return;
+    }
+    int pos = 0;
+    for (int b0 = 0; b0 < s; b0 += 32) {
+        const int b = b0 + lane;
+        const double v = b < s ? row[b] : 0.0;
+        const bool keep = b < s && (fabs(v) >= drop_tol || nodes[b] == i);
+        const unsigned bal = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+            const int q = pos + __popc(bal & ((1u << lane) - 1u));
+            dv[(size_t)i * M + q] = v;
+            di[(size_t)i * M + q] = nodes[b];
+        }
+        pos += __popc(bal);
+    }
+    for (int q = count + lane; q < M; q += 32) { dv[(size_t)i * M + q] = 0.0; di[(size_t)i * M + q] = 0; }
+    if (lane == 0) dn[i] = count;
+}
+
+// status word of the whole construction: keeps the first (most negative wins) failure of any part
+__global__ void graph_collect_kernel(const int *__restrict__ cheb_fail, int *__restrict__ status)
+{
+    if (*cheb_fail != 0 && *status == 0) *status = *cheb_fail;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------
+#define G_CHECK() do { if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA; } while (0)
+
+int launch_graph_core_halo(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, int n_parts, double tau,
+                           int32_t *part_nodes, uint8_t *is_core, int32_t *sizes, uint8_t *flag, cudaStream_t st)
+{
+    const int N = (int)H->N;
+    if (cudaMemsetAsync(flag, 0, (size_t)n_parts * N, st) != cudaSuccess) return BML_ERR_CUDA;
+    graph_mark_halo_kernel<<<(unsigned)(((size_t)N * 32 + 255) / 256), 256, 0, st>>>(H->value, H->index, H->nnz, N, H->M,
+                                                                                       offs, core_nodes, n_parts, tau, flag);
+    G_CHECK();
+    graph_mark_core_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, offs, core_nodes, n_parts, flag);
+    G_CHECK();
+    graph_compact_kernel<<<(unsigned)n_parts, GC_THREADS, 0, st>>>(flag, N, part_nodes, is_core, sizes);
+    G_CHECK();
+    return 0;
+}
+
+int launch_graph_gather(const bml_matrix_t *H, const int32_t *nodes, int s, double *h, int64_t ld, cudaStream_t st)
+{
+    graph_gather_kernel<<<(unsigned)(((size_t)s * 32 + 255) / 256), 256, 0, st>>>(H->value, H->index, H->nnz, H->M, nodes, s,
+                                                                                    h, ld);
+    G_CHECK();
+    return 0;
+}
+
+int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
+                         bml_matrix_t *D, int32_t *overflow, cudaStream_t st)
+{
+    graph_scatter_kernel<<<(unsigned)(((size_t)s * 32 + 255) / 256), 256, 0, st>>>(d, ld, nodes, is_core, s, drop_tol,
+                                                                                     D->value, D->index, D->nnz, D->M,
+                                                                                     overflow);
+    G_CHECK();
+    return 0;
+}
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct GraphWs {
+    int32_t *scal;          // [0] status, [1] overflow row, [2..] sizes (2 per part)
+    uint8_t *flag, *is_core;
+    int32_t *nodes;
+    double *h, *d;
+    void *cheb;
+    int64_t ldc;
+    size_t total;
+};
+
+static GraphWs carve_graph(void *ws, int64_t N, int n_parts, int cap, int k, int m)
+{
+    GraphWs w;
+    uint8_t *p = (uint8_t *)ws;
+    size_t off = 0;
+    w.scal = (int32_t *)(p + off); off = align_up(off + (size_t)(2 + 2 * BML_GRAPH_MAX_PARTS) * 4, 1024);
+    w.flag = p + off; off = align_up(off + (size_t)n_parts * N, 1024);
+    w.is_core = p + off; off = align_up(off + (size_t)n_parts * N, 1024);
+    w.nodes = (int32_t *)(p + off); off = align_up(off + (size_t)n_parts * N * 4, 1024);
+    w.ldc = ((int64_t)cap + 15) / 16 * 16;
+    w.h = (double *)(p + off); off = align_up(off + (size_t)cap * w.ldc * 8, 1024);
+    w.d = (double *)(p + off); off = align_up(off + (size_t)cap * w.ldc * 8, 1024);
+    w.cheb = p + off; off = align_up(off + cheb_workspace_bytes(cap, k, m), 1024);
+    w.total = off;
+    return w;
+}
+
+size_t graph_workspace_bytes(int64_t N, int n_parts, int cap, int k, int m)
+{
+    return carve_graph(nullptr, N, n_parts, cap, k, m).total;
+}
+
+int graph_chebyshev_solve(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, const bml_graph_params_t *p,
+                          bml_matrix_t *D, void *ws, bml_graph_stats_t *stats, cudaStream_t st)
+{
+    const int64_t N = H->N;
+    const int P = p->n_parts;
+    GraphWs w = carve_graph(ws, N, P, p->part_capacity, p->k, p->m);
+    int32_t h_scal[2 + 2 * BML_GRAPH_MAX_PARTS];
+    h_scal[0] = 0; h_scal[1] = INT32_MAX;
+    if (cudaMemcpyAsync(w.scal, h_scal, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return BML_ERR_CUDA;
+    int r = launch_graph_core_halo(H, offs, core_nodes, P, p->graph_tol, w.nodes, w.is_core, w.scal + 2, w.flag, st);
+    if (r) return r;
+    // the part sizes decide the launch shapes: the one host round trip before the end
+    if (cudaMemcpyAsync(h_scal + 2, w.scal + 2, (size_t)2 * P * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    int max_size = 0;
+    for (int q = 0; q < P; ++q) max_size = h_scal[2 + 2 * q] > max_size ? h_scal[2 + 2 * q] : max_size;
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->n_parts = P; stats->overflow_row = -1; stats->max_part_size = max_size;
+        for (int q = 0; q < P; ++q) { stats->part_size[q] = h_scal[2 + 2 * q]; stats->core_size[q] = h_scal[3 + 2 * q]; }
+    }
+    if (max_size > p->part_capacity) return BML_ERR_PART_CAPACITY;
+
+    bml_cheb_params_t cp;
+    memset(&cp, 0, sizeof(cp));
+    cp.mu = p->mu; cp.beta = p->beta; cp.k = p->k; cp.m = p->m;
+    int n_products = 0;
+    for (int q = 0; q < P; ++q) {
+        const int s = h_scal[2 + 2 * q];
+        if (s < 1) continue;
+        const int32_t *nodes = w.nodes + (size_t)q * N;
+        if ((r = launch_graph_gather(H, nodes, s, w.h, w.ldc, st))) return r;
+        bml_matrix_t hd = {BML_DENSE, 0, s, w.ldc, w.h, nullptr, nullptr};
+        bml_matrix_t dd = {BML_DENSE, 0, s, w.ldc, w.d, nullptr, nullptr};
+        if ((r = cheb_dense_enqueue(&hd, &cp, &dd, w.cheb, nullptr, st))) return r;
+        graph_collect_kernel<<<1, 1, 0, st>>>(cheb_fail_flag(w.cheb), w.scal);
+        G_CHECK();
+        if ((r = launch_graph_scatter(w.d, w.ldc, nodes, w.is_core + (size_t)q * N, s, p->drop_tol, D, w.scal + 1, st)))
+            return r;
+        n_products += (p->k - 1) + (p->m - 1);
+    }
+    if (cudaMemcpyAsync(h_scal, w.scal, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+        return BML_ERR_CUDA;
+    int status = BML_OK;
+    if (h_scal[0] != 0) status = h_scal[0];
+    else if (h_scal[1] != INT32_MAX) status = BML_ERR_ELL_OVERFLOW;
+    if (stats) {
+        stats->status = status;
+        stats->n_products = n_products;
+        stats->overflow_row = h_scal[1] != INT32_MAX ? h_scal[1] : -1;
+    }
+    return status;
+}
+
+}  // namespace bmlsp2

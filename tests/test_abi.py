@@ -21,7 +21,7 @@ def _declared():
 def test_header_declares_the_north_star_entry_points():
     names = _declared()
     for required in ("bml_sp2_dense", "bml_sp2_ellpack", "bml_gershgorin", "bml_trace", "bml_chebyshev_dense",
-                     "bml_symm_ab_dense"):
+                     "bml_symm_ab_dense", "bml_graph_chebyshev_ellpack"):
         assert required in names
 
 
@@ -45,9 +45,10 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     # the ctypes mirrors must have the C layout of the header (checked against gcc's sizeof)
     src = r"""
     #include <stdio.h>
-    #include "bml_chebyshev.h"
-    int main(void){ printf("%zu %zu %zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t),
-                           sizeof(bml_cheb_params_t), sizeof(bml_cheb_stats_t)); return 0; }
+    #include "bml_graph.h"
+    int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t),
+                           sizeof(bml_cheb_params_t), sizeof(bml_cheb_stats_t), sizeof(bml_graph_params_t),
+                           sizeof(bml_graph_stats_t)); return 0; }
     """
     import tempfile
 
@@ -57,7 +58,8 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     os.remove(exe)
     assert [int(x) for x in out] == [ctypes.sizeof(api.bml_matrix_t), ctypes.sizeof(api.bml_sp2_params_t),
                                     ctypes.sizeof(api.bml_sp2_stats_t), ctypes.sizeof(api.bml_cheb_params_t),
-                                    ctypes.sizeof(api.bml_cheb_stats_t)]
+                                    ctypes.sizeof(api.bml_cheb_stats_t), ctypes.sizeof(api.bml_graph_params_t),
+                                    ctypes.sizeof(api.bml_graph_stats_t)]
 
 
 def test_sass_contains_the_blackwell_instructions():
