@@ -5,7 +5,8 @@
 
 Workloads: the BASELINE.json configs (dense_n256, dense_n2048 [default], dense_n8192, mixed_n16384, mixed_bf16x3_n16384,
 ellpack_n65536) and, for the Chebyshev expansion of PAPER.md IV.B, cheby_n500 / n1000 / n2000 / n4000 / n8000 (one step =
-one bml_chebyshev_dense call; metric chebyshev_time_to_D_ms).
+one bml_chebyshev_dense call; metric chebyshev_time_to_D_ms) and, for the graph-based construction of VIII.B,
+graph_n1536 / graph_n12800 (one step = one bml_graph_chebyshev_ellpack call; metric graph_time_to_D_ms).
 
 A "step" is one whole pass of the hot path: one bml_sp2_dense (or bml_sp2_ellpack) solve = Gershgorin bounds +
 rescale + every fused X^2 product until the stop rule + output copy, on a seeded synthetic Hamiltonian.
@@ -16,6 +17,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import sys
@@ -30,6 +32,7 @@ import numpy as np  # noqa: E402
 
 METRIC = "sp2_time_to_D_ms"
 METRIC_CHEBY = "chebyshev_time_to_D_ms"     # SURVEY 8(f) item f-1 workloads (--workload cheby_n*)
+METRIC_GRAPH = "graph_time_to_D_ms"         # SURVEY 8(f) item f-2 workloads (--workload graph_n*)
 PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 64 FMA/clk/SM
 
 
@@ -215,6 +218,41 @@ def oracle_cheby_time_to_D(wname: str, H, budget_s: float):
     return ms, sample, cores, extra
 
 
+def oracle_graph_time_to_D(wname: str, H):
+    """Time the graph oracle (oracle/graph.py) on `wname`: halo lists and gathers of every part as they stand (Python
+    loops), the local Fermi operators as a bounded sample -- two steps of the plain recursion Eq. 9 at the size of the
+    first part, scaled to the L - 1 products of every part (the oracle's parity target is the plain series).
+    Returns (ms, sample, cores)."""
+    from oracle import chebyshev as och
+    from oracle import graph as og
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[wname]
+    try:
+        from threadpoolctl import threadpool_info
+
+        cores = max([int(t.get("num_threads", 1)) for t in threadpool_info()] or [1])
+    except Exception:
+        cores = os.cpu_count() or 1
+    offs, nodes = og.regular_partition(w.N, w.n_parts)
+    t0 = time.perf_counter()
+    parts = [og.core_halo(*H, nodes[offs[p]: offs[p + 1]], w.graph_tol) for p in range(w.n_parts)]
+    subs = [og.matrix2submatrix(*H, pn) for pn, _ in parts]
+    t_move = time.perf_counter() - t0
+    h = subs[0]
+    emin, emax = och.gershgorin(h)
+    Ht = och.map_to_unit(h, emin, emax)
+    t0 = time.perf_counter()
+    T2 = 2.0 * (Ht @ Ht) - np.eye(h.shape[0])
+    T3 = 2.0 * (Ht @ T2) - Ht
+    per = (time.perf_counter() - t0) / 2
+    L = w.k * w.m - 1
+    scale = sum((sub.shape[0] / h.shape[0]) ** 3 for sub in subs)
+    ms = (t_move + per * (L - 1) * scale) * 1e3
+    return ms, (f"halo lists + gathers of all {w.n_parts} parts timed in full ({t_move:.1f} s); 2 of {L - 1} recursion "
+                f"products timed at part size {h.shape[0]}, scaled to all parts"), cores
+
+
 EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30,
                      "mixed_bf16x3_n16384": 30, "ellpack_n65536": 12}
 
@@ -226,20 +264,22 @@ def run_reference(args):
     from paper_2401_13772_b200 import hamiltonians as hm
 
     w = hm.WORKLOADS[args.workload]
-    H = hm.make_dense(args.workload) if w.kind != "ellpack" else hm.make_ellpack(args.workload)
+    H = hm.make_dense(args.workload) if w.kind in ("dense", "cheby") else hm.make_ellpack(args.workload)
     total = args.steps + args.warmup
     budget = max(1.0, 200.0 / total)       # whole run within a few minutes
     times, sample, cores = [], "", 1
     for it in range(total):
         if w.kind == "cheby":
             ms, sample, cores, _ = oracle_cheby_time_to_D(args.workload, H, 0.0)
+        elif w.kind == "graph":
+            ms, sample, cores = oracle_graph_time_to_D(args.workload, H)
         else:
             ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
         if it >= args.warmup:
             times.append(ms)
     v = float(np.mean(times))
     line = {
-        "impl": "reference", "metric": METRIC_CHEBY if w.kind == "cheby" else METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": {"cheby": METRIC_CHEBY, "graph": METRIC_GRAPH}.get(w.kind, METRIC), "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": workload_config(args.workload),
@@ -261,6 +301,13 @@ def workload_config(name: str):
                  "within a step, which is part of the method"}
     if w.kind == "ellpack":
         cfg.update({"M": w.M, "drop_tol": w.drop_tol})
+    if w.kind == "graph":
+        for key in ("n_occ", "idem_tol", "max_products"):
+            cfg.pop(key)
+        cfg["l2"] = "flushed between steps (256 MiB write)"
+        cfg.update({"M": w.M, "M_out": w.M_out, "n_parts": w.n_parts, "graph_tol": w.graph_tol, "drop_tol": w.drop_tol,
+                    "mu": w.mu, "beta": w.beta, "k": w.k, "m": w.m, "L": w.k * w.m - 1,
+                    "partition": "regular index segments"})
     if w.kind == "cheby":
         for key in ("n_occ", "idem_tol", "max_products"):
             cfg.pop(key)
@@ -668,6 +715,145 @@ def run_cheby(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------------------------
+# our arm, graph-based workloads: one bml_graph_chebyshev_ellpack call per step
+# ----------------------------------------------------------------------------------------------------------
+def run_graph(args):
+    import torch
+
+    from paper_2401_13772_b200 import api, hamiltonians as hm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl")
+    api.load()
+    dev = torch.device("cuda", local)
+    w = hm.WORKLOADS[args.workload]
+    H_np = hm.make_ellpack(args.workload)
+    H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
+    H_dev = tuple(a.to(dev) for a in H_host)
+    offs_np, nodes_np = hm.regular_core_partition(w.N, w.n_parts)
+    offs, nodes = torch.from_numpy(offs_np).to(dev), torch.from_numpy(nodes_np).to(dev)
+    # part sizes are not known before the halo pass: size the workspace from one dry call of the halo kernels
+    sizes = api.bml_graph_core_halo(H_dev, offs, nodes, w.graph_tol)[2].cpu().numpy()
+    cap = int(sizes[:, 0].max())
+    solver = api.GraphSolver(w.N, w.M_out, w.n_parts, cap, w.k, w.m, dev)
+    D_host = tuple(torch.empty_like(a).pin_memory() for a in (solver.dv.cpu(), solver.di.cpu(), solver.dn.cpu()))
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def solve(Hd):
+        return solver.solve(Hd, offs, nodes, w.graph_tol, w.mu, w.beta, w.drop_tol)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    res = None
+    for _ in range(args.warmup):
+        _, res = solve(H_dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)
+            ev[k][0].record()
+            _, res = solve(H_dev)
+            ev[k][1].record()
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    ms = float(np.mean(step_ms))
+    clocks = clk.summary()
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = sum(a.numel() * a.element_size() for a in H_host)
+    d2h = sum(a.numel() * a.element_size() for a in D_host)
+    for _ in range(2):
+        solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
+        for dst, src in zip(D_host, D):
+            dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    # dominant kernel: one local-solver product at the size of the largest part, timed alone
+    g = torch.Generator().manual_seed(0)
+    A = torch.randn((cap, cap), generator=g, dtype=torch.float64) / math.sqrt(cap)
+    A = (A + A.T) / 4
+    slab, n, ld, _ = api.matrix_slab([A, A, torch.zeros_like(A)], dev)
+    ws = api._workspace(api.load().bml_symm_ab_workspace_bytes(), dev)
+    job = [(0, 1, 0, 2, 2.0, -1.0, 0.0)]
+    reps = 10
+    for _ in range(3):
+        api.bml_symm_ab_dense(slab, n, ld, job, ws)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(reps):
+        api.bml_symm_ab_dense(slab, n, ld, job, ws)
+    b.record()
+    torch.cuda.synchronize()
+    k_ms = a.elapsed_time(b) / reps
+    peak_probe = api.bml_probe_fp64_tensor_peak(40000)
+    flops = dense_flops_per_product(cap)
+    achieved = flops / (k_ms * 1e-3) / 1e12
+    n_prod = int(res.n_products)
+    step_flops = sum(dense_flops_per_product(int(sz)) for sz in res.part_size) * (w.k + w.m - 2)
+    roof = {
+        "bound": "tensor", "kernel": "symm_ab_fp64_kernel<128>", "achieved": achieved, "peak": peak_probe,
+        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+        "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
+                       "(MEASURED_PEAKS.json has no FP64 entry)",
+        "launch_ms": k_ms, "flops_per_launch": flops, "part_size": cap,
+        "in_step_tflops": step_flops / (ms * 1e-3) / 1e12,
+        "in_step_frac": step_flops / (ms * 1e-3) / 1e12 / peak_probe,
+    }
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, sample, cores = oracle_graph_time_to_D(args.workload, H_np)
+        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
+    levels = max(1, math.ceil(math.log2(w.k)))
+    per_part = 1 + 2 + 1 + 1 + levels + (w.m - 1) + 1 + 1 + 1 + 1      # gather, Gershgorin x2, coeff, map, products, sums, trace, collect, scatter
+    launches_per_step = 3 + w.n_parts * per_part
+    line = {
+        "metric": METRIC_GRAPH, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(args.workload),
+        "status": int(res.status), "n_products": n_prod, "part_size": res.part_size, "core_size": res.core_size,
+        "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
+        "aggregate_solves_per_s": replicas_per_second(world, ms),
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches_note": f"{launches_per_step} per step: 3 halo kernels + {w.n_parts} parts x {per_part} (gather, "
+                             f"2 Gershgorin, coefficients, map, {levels + w.m - 1} grouped product launches, partial sums, "
+                             "trace, status, scatter)",
+        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -684,6 +870,8 @@ def main():
 
     if hm.WORKLOADS[args.workload].kind == "cheby":
         return run_cheby(args)
+    if hm.WORKLOADS[args.workload].kind == "graph":
+        return run_graph(args)
     return run_ours(args)
 
 

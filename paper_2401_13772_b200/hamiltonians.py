@@ -164,6 +164,10 @@ class Workload:
     beta: float = 0.0
     k: int = 0
     m: int = 0
+    # graph workloads (kind "graph"): number of core parts (regular index segments), Eq. 15 threshold, D row capacity
+    n_parts: int = 0
+    graph_tol: float = 0.0
+    M_out: int = 0
 
 
 WORKLOADS = {
@@ -200,6 +204,26 @@ for _name, _L3 in (("cheby_n500", (10, 10, 5)), ("cheby_n1000", (10, 10, 10)), (
                                 note="%dx%dx%d gapless lattice, NN hopping -1, kT=1/6, L=255" % _L3)
 
 
+# Graph-based solver workloads (PAPER.md VIII.B, Table II: N = 12,972, 4 parts, core
+# 3149-3314, core+halo 5657-5810 -- the benchmark system itself is not available).  Stand-in: the 5' model of the sparse
+# SP2 path (on-site +-12 + U[-0.2, 0.2], hopping -exp(-r/0.5), r <= 3, 123 entries per row) on a 32x20x20 box, N = 12,800,
+# 4 contiguous index segments = x-slabs of 8 layers (core 3200), graph threshold 0.002 = every stored hopping, i.e. a
+# halo of 3 layers on each side (core+halo 5600); mu = 0, beta = 2 (the 22.7-wide gap makes f_mu a step to 1e-10), L = 255,
+# D kept at |v| >= 1e-6 in rows of 512 slots.  The small variant is what the oracle finishes in seconds.
+WORKLOADS["graph_n12800"] = Workload("graph_n12800", "graph", 12800, 6400, 0.0, 1e-6, M=128, lattice=(32, 20, 20), mu=0.0,
+                                     beta=2.0, k=16, m=16, n_parts=4, graph_tol=0.002, M_out=512,
+                                     note="32x20x20, -exp(-r/0.5), r<=3, delta=12; 4 x-slab parts, halo 3 layers")
+WORKLOADS["graph_n1536"] = Workload("graph_n1536", "graph", 1536, 768, 0.0, 1e-6, M=128, lattice=(24, 8, 8), mu=0.0,
+                                    beta=2.0, k=16, m=16, n_parts=3, graph_tol=0.002, M_out=512,
+                                    note="24x8x8, same model; 3 x-slab parts, halo 3 layers")
+
+
+def regular_core_partition(N: int, n_parts: int):
+    """Core partition into contiguous index segments (an INPUT of the graph path): (offsets[n_parts+1], nodes[N])."""
+    offs = np.array([(p * N) // n_parts for p in range(n_parts + 1)], dtype=np.int32)
+    return offs, np.arange(N, dtype=np.int32)
+
+
 def make_dense(name: str, seed: int = 0) -> np.ndarray:
     w = WORKLOADS[name]
     if w.kind == "cheby":
@@ -215,6 +239,8 @@ def make_dense(name: str, seed: int = 0) -> np.ndarray:
 
 def make_ellpack(name: str, seed: int = 0):
     w = WORKLOADS[name]
+    if w.kind == "graph":
+        return lattice_ellpack(w.lattice, 12.0, 0.2, 3.0, lambda r: -math.exp(-r / 0.5), w.M, seed)
     if name == "ellpack_n65536_literal":
         return lattice_ellpack(w.lattice, 1.5, 0.2, 3.0, lambda r: -math.exp(-r / 1.0), w.M, seed)
     if name == "ellpack_n65536":

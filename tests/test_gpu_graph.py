@@ -182,3 +182,42 @@ def test_graph_approaches_the_dense_expansion_as_the_halo_grows(api):
         Dg = hm.ellpack_to_dense(gv.cpu().numpy(), gi.cpu().numpy(), gn.cpu().numpy())
         errs.append(np.linalg.norm(Dg - D_full) / np.linalg.norm(D_full))
     assert errs[0] > errs[1] > errs[2] and errs[2] < 0.2 * errs[0]
+
+
+def test_graph_table2_size_workload(api):
+    """The workload bench.py times (graph_n12800: the sizes of the paper's Table II, P:527-538 -- 4 parts, core 3200,
+    core+halo 5600).  The plain-series oracle cannot finish a 5600-node part in test time, so: index work against the
+    oracle exactly (part sizes), D through properties and against the dense expansion of the WHOLE matrix computed by
+    bml_chebyshev_dense (itself oracle-checked at the sizes the oracle reaches): the difference is the graph
+    approximation, 1e-5 relative on the small variant of the same model."""
+    import torch
+
+    w = hm.WORKLOADS["graph_n12800"]
+    H = hm.make_ellpack("graph_n12800")
+    N = w.N
+    offs, nodes = hm.regular_core_partition(N, w.n_parts)
+    Hg = gpu(H)
+    sizes = api.bml_graph_core_halo(Hg, tgpu(offs), tgpu(nodes), w.graph_tol)[2].cpu().numpy()
+    ref_sizes = [og.core_halo(*H, nodes[offs[p]: offs[p + 1]], w.graph_tol)[0].size for p in range(w.n_parts)]
+    assert sizes[:, 0].tolist() == ref_sizes == [5600] * 4 and sizes[:, 1].tolist() == [3200] * 4
+    (gv, gi, gn), res = api.bml_graph_chebyshev_ellpack(Hg, tgpu(offs), tgpu(nodes), w.graph_tol, w.mu, w.beta, w.k, w.m,
+                                                       w.drop_tol, w.M_out, 5600)
+    assert res.status == 0 and res.n_products == 4 * 30
+    assert int(gn.max()) <= w.M_out and int(gn.min()) >= 1
+    # rows ascending, unused slots zero
+    mask = torch.arange(w.M_out, device="cuda").unsqueeze(0) < gn.unsqueeze(1)
+    assert bool(((gi[:, 1:] > gi[:, :-1]) | ~mask[:, 1:]).all()) and bool((gv[~mask] == 0).all())
+    # against the dense expansion of the whole matrix
+    Hd = torch.zeros((N, N), dtype=torch.float64, device="cuda")
+    hmask = torch.arange(w.M, device="cuda").unsqueeze(0) < Hg[2].unsqueeze(1)
+    rows = torch.arange(N, device="cuda").unsqueeze(1).expand(N, w.M)
+    Hd[rows[hmask], Hg[1][hmask].long()] = Hg[0][hmask]
+    D_full, r = api.bml_chebyshev_dense(Hd, w.mu, w.beta, w.k, w.m)
+    assert r.status == 0
+    Dg = torch.zeros((N, N), dtype=torch.float64, device="cuda")
+    rows = torch.arange(N, device="cuda").unsqueeze(1).expand(N, w.M_out)
+    Dg[rows[mask], gi[mask].long()] = gv[mask]
+    kept = D_full.abs() >= w.drop_tol
+    err = (torch.linalg.norm(Dg - D_full * kept) / torch.linalg.norm(D_full)).item()
+    assert err < 1e-4, err
+    assert abs(Dg.trace().item() - r.trace) < 1e-3 * N
