@@ -146,14 +146,16 @@ def x2_dense_sampled(X, rows, cols):
     return out
 
 
-def sp2_dense(H, n_occ, tol, max_products=100):
-    """Dense SP2 (Eq. 5-7, Listing 2; SURVEY 8(c) lines 1-13).  Returns (D, stats dict)."""
+def sp2_dense(H, n_occ, tol, max_products=100, bounds=None):
+    """Dense SP2 (Eq. 5-7, Listing 2; SURVEY 8(c) lines 1-13).  bounds = (e_min, e_max) replaces the Gershgorin bounds
+    (oracle/bounds.py).  Returns (D, stats dict)."""
     H = _c64(H)
     N = H.shape[0]
     D = np.zeros((N, N), dtype=np.float64)
     st = OracleStats()
-    _L().oracle_sp2_dense(_p(H, _f64p), ctypes.c_int64(N), ctypes.c_int64(H.shape[1]), ctypes.c_int32(n_occ),
-                          ctypes.c_double(tol), ctypes.c_int32(max_products), _p(D, _f64p), ctypes.byref(st))
+    b = None if bounds is None else (ctypes.c_double * 2)(float(bounds[0]), float(bounds[1]))
+    _L().oracle_sp2_dense_bounds(_p(H, _f64p), ctypes.c_int64(N), ctypes.c_int64(H.shape[1]), ctypes.c_int32(n_occ),
+                                 ctypes.c_double(tol), ctypes.c_int32(max_products), b, _p(D, _f64p), ctypes.byref(st))
     return D, _stats_dict(st)
 
 
@@ -211,14 +213,16 @@ def update_ellpack(X, P, tau):
     return ov, oi, on, int(bad), int(mx.value)
 
 
-def sp2_ellpack(value, index, nnz, n_occ, tol, tau, max_products=100):
-    """Sparse thresholded SP2 (SURVEY 8(c) sparse oracle).  Returns ((value, index, nnz) of D, stats dict)."""
+def sp2_ellpack(value, index, nnz, n_occ, tol, tau, max_products=100, bounds=None):
+    """Sparse thresholded SP2 (SURVEY 8(c) sparse oracle); bounds as in sp2_dense.
+    Returns ((value, index, nnz) of D, stats dict)."""
     value, index, nnz = _c64(value), _c32(index), _c32(nnz)
     N, M = value.shape
     dv, di, dn = np.zeros_like(value), np.zeros_like(index), np.zeros_like(nnz)
     st = OracleStats()
-    _L().oracle_sp2_ellpack(ctypes.c_int64(N), ctypes.c_int32(M), _p(value, _f64p), _p(index, _i32p), _p(nnz, _i32p),
-                            ctypes.c_int32(n_occ), ctypes.c_double(tol), ctypes.c_double(tau),
-                            ctypes.c_int32(max_products), _p(dv, _f64p), _p(di, _i32p), _p(dn, _i32p),
-                            ctypes.byref(st))
+    b = None if bounds is None else (ctypes.c_double * 2)(float(bounds[0]), float(bounds[1]))
+    _L().oracle_sp2_ellpack_bounds(ctypes.c_int64(N), ctypes.c_int32(M), _p(value, _f64p), _p(index, _i32p),
+                                   _p(nnz, _i32p), ctypes.c_int32(n_occ), ctypes.c_double(tol), ctypes.c_double(tau),
+                                   ctypes.c_int32(max_products), b, _p(dv, _f64p), _p(di, _i32p), _p(dn, _i32p),
+                                   ctypes.byref(st))
     return (dv, di, dn), _stats_dict(st)

@@ -161,8 +161,17 @@ static void dense_norms(const double *P, const double *X, int64_t N, double *e2,
  * Dense SP2, SURVEY 8(c) algorithm lines 1-13.  H: N x N row-major with leading dimension ld, exactly symmetric.
  * D: N x N, leading dimension N.  Returns the status (also in st->status).
  */
+/* bounds == NULL: Gershgorin (reading 1); else { e_min, e_max } supplied by the caller (oracle/bounds.py, the
+ * tighter-bounds option of SURVEY 8(f) f-3).  Nothing else differs. */
+int oracle_sp2_dense_bounds(const double *H, int64_t N, int64_t ld, int32_t n_occ, double tol, int32_t max_products,
+                            const double *bounds, double *D, oracle_stats_t *st);
 int oracle_sp2_dense(const double *H, int64_t N, int64_t ld, int32_t n_occ, double tol, int32_t max_products,
                      double *D, oracle_stats_t *st)
+{
+    return oracle_sp2_dense_bounds(H, N, ld, n_occ, tol, max_products, NULL, D, st);
+}
+int oracle_sp2_dense_bounds(const double *H, int64_t N, int64_t ld, int32_t n_occ, double tol, int32_t max_products,
+                            const double *bounds, double *D, oracle_stats_t *st)
 {
     stats_init(st);
     if (!H || !D || N <= 0 || ld < N || n_occ <= 0 || n_occ >= N || !(tol > 0) || max_products < 1 ||
@@ -173,6 +182,7 @@ int oracle_sp2_dense(const double *H, int64_t N, int64_t ld, int32_t n_occ, doub
             if (H[i * ld + j] != H[j * ld + i]) return st->status = -5;
     double emin, emax;
     oracle_gershgorin_dense(H, N, ld, &emin, &emax);                                          /* line 1 */
+    if (bounds) { emin = bounds[0]; emax = bounds[1]; }
     st->emin = emin; st->emax = emax;
     if (!(emax - emin > 0)) return st->status = -2;
     double *X = (double *)malloc(sizeof(double) * N * N), *P = (double *)malloc(sizeof(double) * N * N);
@@ -384,9 +394,19 @@ int64_t oracle_update_ellpack(int64_t N, int32_t M, const double *xv, const int3
  * Sparse SP2 (dense loop with lines 5, 6, 12 replaced by 5s, 6s, 12s).  Input rows may be in any
  * column order; D is returned in ascending column order in (dv, di, dn), all of size N*M / N.
  */
+int oracle_sp2_ellpack_bounds(int64_t N, int32_t M, const double *hv, const int32_t *hi, const int32_t *hn, int32_t n_occ,
+                              double tol, double tau, int32_t max_products, const double *bounds, double *dv, int32_t *di,
+                              int32_t *dn, oracle_stats_t *st);
 int oracle_sp2_ellpack(int64_t N, int32_t M, const double *hv, const int32_t *hi, const int32_t *hn, int32_t n_occ,
                        double tol, double tau, int32_t max_products, double *dv, int32_t *di, int32_t *dn,
                        oracle_stats_t *st)
+{
+    return oracle_sp2_ellpack_bounds(N, M, hv, hi, hn, n_occ, tol, tau, max_products, NULL, dv, di, dn, st);
+}
+/* bounds as in oracle_sp2_dense_bounds */
+int oracle_sp2_ellpack_bounds(int64_t N, int32_t M, const double *hv, const int32_t *hi, const int32_t *hn, int32_t n_occ,
+                              double tol, double tau, int32_t max_products, const double *bounds, double *dv, int32_t *di,
+                              int32_t *dn, oracle_stats_t *st)
 {
     stats_init(st);
     if (!hv || !hi || !hn || !dv || !di || !dn || N <= 0 || M < 1 || n_occ <= 0 || n_occ >= N || !(tol > 0) ||
@@ -395,6 +415,7 @@ int oracle_sp2_ellpack(int64_t N, int32_t M, const double *hv, const int32_t *hi
     for (int64_t i = 0; i < N; ++i) if (hn[i] < 0 || hn[i] > M) return st->status = -1;
     double emin, emax;
     oracle_gershgorin_ellpack(N, M, hv, hi, hn, &emin, &emax);
+    if (bounds) { emin = bounds[0]; emax = bounds[1]; }
     st->emin = emin; st->emax = emax;
     if (!(emax - emin > 0)) return st->status = -2;
     const size_t nm = (size_t)N * (size_t)M;
