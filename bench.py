@@ -360,6 +360,7 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     w = hm.WORKLOADS[args.workload]
     dense = w.kind == "dense"
+    sp2_flags = api.FLAG_LANCZOS_BOUNDS(args.lanczos_steps) if args.lanczos_steps else 0
 
     # ---- inputs: seeded synthetic Hamiltonian, resident in HBM; pinned host copies for the e2e leg
     if dense:
@@ -370,7 +371,7 @@ def run_ours(args):
         D_host = torch.empty((w.N, w.N), dtype=torch.float64).pin_memory()
 
         def solve(Hd):
-            return solver.solve(Hd, w.n_occ, w.idem_tol, 100)
+            return solver.solve(Hd, w.n_occ, w.idem_tol, 100, flags=sp2_flags)
     else:
         H_np = hm.make_ellpack(args.workload)
         H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
@@ -379,7 +380,7 @@ def run_ours(args):
         D_host = tuple(torch.empty_like(a).pin_memory() for a in H_host)
 
         def solve(Hd):
-            return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, 100)
+            return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, 100, flags=sp2_flags)
 
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
 
@@ -568,6 +569,8 @@ def run_ours(args):
                   2: "bf16x3 split products (fp32 TMEM chunks) + f64 accumulate/update"}[w.precision if dense else 0],
         "data": "synthetic", "config": workload_config(args.workload),
         "status": int(res.status), "n_products": n_prod, "branch": res.branch,
+        "spectral_bounds": {"emin": res.emin, "emax": res.emax,
+                            "kind": f"lanczos({args.lanczos_steps}) within gershgorin" if args.lanczos_steps else "gershgorin"},
         "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
         "ms_per_product": ms / max(n_prod, 1),
         "aggregate_solves_per_s": replicas_per_second(world, ms),
@@ -862,6 +865,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="dense_n2048")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lanczos-steps", type=int, default=0,
+                    help="SP2 workloads: tighten the Gershgorin bounds with K Lanczos steps (8..64); 0 = Gershgorin only, "
+                         "the configuration BASELINE.json names")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -21,11 +21,17 @@ ELL_ACC_SLOTS = 4096
 BML_DENSE, BML_ELLPACK = 0, 1
 FLAG_CHECK_SYMMETRY = 1
 
+
+def FLAG_LANCZOS_BOUNDS(steps: int) -> int:
+    """BML_SP2_FLAG_LANCZOS_BOUNDS(K): tighter spectral bounds from K Lanczos steps (8..64) instead of Gershgorin alone."""
+    return (int(steps) & 0xFF) << 8
+
 EXPORTS = [
     "bml_version", "bml_status_string", "bml_gershgorin_workspace_bytes", "bml_gershgorin", "bml_trace",
     "bml_sp2_workspace_bytes", "bml_sp2_dense", "bml_sp2_ellpack", "bml_x2_dense_workspace_bytes", "bml_x2_dense",
     "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_probe_fp64_tensor_peak",
     "bml_dense_work_item", "bml_dense_mixed_tile_count", "bml_dense_mixed_tile_of_cta",
+    "bml_lanczos_bounds_workspace_bytes", "bml_lanczos_bounds",
     # include/bml_chebyshev.h
     "bml_chebyshev_workspace_bytes", "bml_chebyshev_dense", "bml_symm_ab_workspace_bytes", "bml_symm_ab_dense",
     "bml_cheb_schedule", "bml_symm_work_item",
@@ -153,6 +159,10 @@ def load(build_if_missing: bool = True):
     L.bml_gershgorin.argtypes = [MP, vp, vp, sz, vp]
     L.bml_trace.restype = ctypes.c_int
     L.bml_trace.argtypes = [MP, vp, vp]
+    L.bml_lanczos_bounds_workspace_bytes.restype = sz
+    L.bml_lanczos_bounds_workspace_bytes.argtypes = [i64]
+    L.bml_lanczos_bounds.restype = ctypes.c_int
+    L.bml_lanczos_bounds.argtypes = [MP, i32, ctypes.c_uint64, vp, vp, sz, vp]
     L.bml_sp2_workspace_bytes.restype = sz
     L.bml_sp2_workspace_bytes.argtypes = [MP, PP]
     for name in ("bml_sp2_dense", "bml_sp2_ellpack"):
@@ -299,6 +309,20 @@ def bml_gershgorin(H, out: torch.Tensor | None = None) -> torch.Tensor:
     return out
 
 
+def bml_lanczos_bounds(H, steps: int, seed: int = 0) -> torch.Tensor:
+    """Tighter spectral bounds (bml_sp2.h): CUDA float64 tensor [e_min, e_max] (asynchronous)."""
+    L = load()
+    desc = dense_desc(H) if isinstance(H, torch.Tensor) else ellpack_desc(*H)
+    dev = H.device if isinstance(H, torch.Tensor) else H[0].device
+    out = torch.empty(2, dtype=torch.float64, device=dev)
+    nbytes = L.bml_lanczos_bounds_workspace_bytes(desc.N)
+    ws = torch.empty(max(nbytes, 8), dtype=torch.uint8, device=dev)
+    rc = L.bml_lanczos_bounds(ctypes.byref(desc), int(steps), int(seed), out.data_ptr(), ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_lanczos_bounds: {bml_status_string(rc)}")
+    return out
+
+
 def bml_trace(A, out: torch.Tensor | None = None) -> torch.Tensor:
     L = load()
     desc = dense_desc(A) if isinstance(A, torch.Tensor) else ellpack_desc(*A)
@@ -353,22 +377,24 @@ class EllpackSolver:
         self.ws_bytes = L.bml_sp2_workspace_bytes(ctypes.byref(d), None)
         self.ws = _workspace(self.ws_bytes, self.device)
 
-    def solve(self, value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+    def solve(self, value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100,
+              flags: int = 0):
         L = load()
         h = ellpack_desc(value, index, nnz)
         d = ellpack_desc(self.dv, self.di, self.dn)
-        p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), float(drop_tol), 0, 0)
+        p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), float(drop_tol), 0, int(flags))
         st = bml_sp2_stats_t()
         rc = L.bml_sp2_ellpack(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
                                ctypes.byref(st), _stream())
         return (self.dv, self.di, self.dn), _result(st, rc)
 
 
-def bml_sp2_ellpack(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+def bml_sp2_ellpack(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100,
+                    flags: int = 0):
     """Sparse thresholded SP2 on ELLPACK-R.  Returns ((value, index, nnz) CUDA tensors of D, Sp2Result)."""
     _require_cuda(value, torch.float64, "value")
     return EllpackSolver(value.shape[0], value.shape[1], value.device).solve(value, index, nnz, n_occ, idem_tol,
-                                                                           drop_tol, max_products)
+                                                                           drop_tol, max_products, flags)
 
 
 def padded_ld(N: int) -> int:

@@ -51,6 +51,9 @@ size_t cheb_workspace_bytes(int64_t N, int k, int m);
 int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b);
 int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws,
                      bml_cheb_stats_t *stats, cudaStream_t st);
+// bounds.cu
+size_t lanczos_workspace_doubles(int64_t N);
+int launch_lanczos_bounds(const bml_matrix_t *H, int steps, uint64_t seed, double *d_bounds, double *work, cudaStream_t st);
 // graph.cu
 size_t graph_workspace_bytes(int64_t N, int n_parts, int cap, int k, int m);
 int graph_chebyshev_solve(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, const bml_graph_params_t *p,
@@ -100,6 +103,14 @@ static inline size_t partial_slots(int64_t N)
     return (size_t)(a > b ? a : b);
 }
 
+// per-row scratch shared by the Gershgorin pass (2N doubles) and the optional Lanczos pass (3N + its control block)
+static inline size_t row_scratch_doubles(int64_t N)
+{
+    const size_t a = (size_t)2 * (size_t)N, b = lanczos_workspace_doubles(N);
+    return a > b ? a : b;
+}
+static inline int lanczos_steps(uint32_t flags) { return (int)((flags >> 8) & 0xffu); }
+
 struct DenseWs {
     Sp2Ctl *ctl;
     ScalarSlots *scal;
@@ -117,7 +128,7 @@ static DenseWs carve_dense(void *ws, int64_t N, int precision)
     size_t off = 0;
     w.ctl = (Sp2Ctl *)(p + off); off += CTL_BYTES;
     w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
-    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
+    w.rowlh = (double *)(p + off); off = align_up(off + row_scratch_doubles(N) * sizeof(double), 1024);
     w.partials = (double *)(p + off);
     off = align_up(off + partial_slots(N) * 4 * sizeof(double), 1024);
     w.sk = (void *)(p + off); off = align_up(off + dense_fp64_sk_bytes(N), 1024);
@@ -147,7 +158,7 @@ static EllWs carve_ell(void *ws, int64_t N, int M, bool with_buffers)
     size_t off = 0;
     w.ctl = (Sp2Ctl *)(p + off); off += CTL_BYTES;
     w.scal = (ScalarSlots *)(p + off); off += SCAL_BYTES;
-    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
+    w.rowlh = (double *)(p + off); off = align_up(off + row_scratch_doubles(N) * sizeof(double), 1024);
     w.rowstats = (double *)(p + off); off = align_up(off + ellpack_rowstats_bytes(N), 1024);
     w.sym = (void *)(p + off); off = align_up(off + ellpack_sym_bytes(N, M), 1024);
     w.v0 = w.v1 = nullptr; w.i0 = w.i1 = w.n0 = w.n1 = nullptr;
@@ -176,7 +187,8 @@ static bool ell_ok(const bml_matrix_t *A)
 static bool params_ok(const bml_sp2_params_t *p, int64_t N)
 {
     return p && p->n_occ > 0 && (int64_t)p->n_occ < N && p->idem_tol > 0.0 && p->max_products >= 1 &&
-           p->max_products <= BML_SP2_LOG_LEN && p->drop_tol >= 0.0 && p->precision >= 0 && p->precision <= 2;
+           p->max_products <= BML_SP2_LOG_LEN && p->drop_tol >= 0.0 && p->precision >= 0 && p->precision <= 2 &&
+           (lanczos_steps(p->flags) == 0 || (lanczos_steps(p->flags) >= 8 && lanczos_steps(p->flags) <= 64));
 }
 
 static void fill_stats(bml_sp2_stats_t *stats, const Sp2Ctl &c)
@@ -249,6 +261,23 @@ int bml_gershgorin(const bml_matrix_t *H, double *d_bounds, void *d_workspace, s
     return launch_gershgorin(H, d_bounds, (double *)d_workspace, (cudaStream_t)cuda_stream);
 }
 
+size_t bml_lanczos_bounds_workspace_bytes(int64_t N)
+{
+    return N > 0 ? row_scratch_doubles(N) * sizeof(double) : 0;
+}
+
+int bml_lanczos_bounds(const bml_matrix_t *H, int32_t steps, uint64_t seed, double *d_bounds, void *d_workspace,
+                       size_t workspace_bytes, void *cuda_stream)
+{
+    if (!H || !d_bounds || !d_workspace || steps < 8 || steps > 64) return BML_ERR_INVALID;
+    if (!(H->type == BML_DENSE ? dense_ok(H) : ell_ok(H))) return BML_ERR_INVALID;
+    if (workspace_bytes < bml_lanczos_bounds_workspace_bytes(H->N) || ((uintptr_t)d_workspace & 7) != 0)
+        return BML_ERR_INVALID;
+    int r = launch_gershgorin(H, d_bounds, (double *)d_workspace, (cudaStream_t)cuda_stream);
+    if (r) return r;
+    return launch_lanczos_bounds(H, steps, seed, d_bounds, (double *)d_workspace, (cudaStream_t)cuda_stream);
+}
+
 int bml_trace(const bml_matrix_t *A, double *d_trace, void *cuda_stream)
 {
     if (!A || !d_trace) return BML_ERR_INVALID;
@@ -281,6 +310,7 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
 
     if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
     TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // D0
+    if (lanczos_steps(p->flags)) TRY(launch_lanczos_bounds(H, lanczos_steps(p->flags), 0, w.scal->bounds, w.rowlh, st));
     if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) TRY(launch_check_symmetry(H, w.scal->fail_flag, st));
     TRY(launch_rescale_dense(H, w.scal->bounds, w.X0, w.ldx, st));                            // D1
     TRY(launch_trace_dense(w.X0, w.ldx, (int)N, &w.scal->tr0, st));
@@ -358,6 +388,7 @@ int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix
 
     if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
     TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // S0
+    if (lanczos_steps(p->flags)) TRY(launch_lanczos_bounds(H, lanczos_steps(p->flags), 0, w.scal->bounds, w.rowlh, st));
     // the Gershgorin row buffer (2N doubles) is free again: reuse it for the N diagonal values of X_0
     TRY(launch_rescale_ellpack(H, w.scal->bounds, w.v0, w.i0, w.n0, w.rowlh, &w.scal->tr0, w.scal->fail_flag, st));
     TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,

@@ -1,0 +1,103 @@
+"""GPU parity of the optional tighter spectral bounds (bml_lanczos_bounds, BML_SP2_FLAG_LANCZOS_BOUNDS)
+against oracle/bounds.py, and of SP2 run with them against the oracle run with the ORACLE's bounds.
+
+Tolerance: with full reorthogonalisation (reading B3) the recursion is stable and the two sides differ by summation
+order only; the bounds are required to agree to 1e-9 of the spectral width.  (Without reorthogonalisation the residual
+term of the unconverged end was reproducible to two digits only -- 1e-3 of the width -- which is why both sides
+reorthogonalise.)"""
+import numpy as np
+import pytest
+
+from oracle import bounds as ob
+from paper_2401_13772_b200 import hamiltonians as hm
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2401_13772_b200 import api as a
+
+    a.load()
+    return a
+
+
+def to_gpu(A):
+    import torch
+
+    return torch.from_numpy(np.ascontiguousarray(A)).cuda()
+
+
+MODELS = {
+    "ring": lambda: hm.make_dense("dense_n256"),
+    "long_range": lambda: hm.small_long_range((8, 8, 6)),
+    "planted": lambda: hm.planted_gap(333, 100, seed=3)[0],
+    "tiny": lambda: np.array([[1.0, 2.0, 0.0], [2.0, -3.0, 0.5], [0.0, 0.5, 0.25]]),
+}
+
+
+@pytest.mark.parametrize("name", list(MODELS))
+@pytest.mark.parametrize("K", [8, 24, 64])
+def test_lanczos_bounds_dense(api, name, K):
+    H = MODELS[name]()
+    w = np.linalg.eigvalsh(H)
+    for seed in (0, 7):
+        lo, hi, info = ob.lanczos_bounds(H, K, seed)
+        got = api.bml_lanczos_bounds(to_gpu(H), K, seed).cpu().numpy()
+        width = info["gershgorin"][1] - info["gershgorin"][0]
+        assert abs(got[0] - lo) <= 1e-9 * width and abs(got[1] - hi) <= 1e-9 * width
+        assert got[0] <= w[0] and got[1] >= w[-1]
+
+
+def test_lanczos_bounds_ellpack_equals_dense(api):
+    Hs = hm.small_sparse_model((8, 7, 8))
+    Hd = hm.ellpack_to_dense(*Hs)
+    lo, hi, info = ob.lanczos_bounds(Hd, 20)
+    got = api.bml_lanczos_bounds(tuple(to_gpu(a) for a in Hs), 20).cpu().numpy()
+    width = info["gershgorin"][1] - info["gershgorin"][0]
+    assert abs(got[0] - lo) <= 1e-9 * width and abs(got[1] - hi) <= 1e-9 * width
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_sp2_dense_with_lanczos_bounds(api, oracle_mod, precision):
+    H = hm.small_long_range((8, 8, 6))
+    n_occ = H.shape[0] // 2
+    tol = 1e-10 if precision == 0 else 1e-6
+    lo, hi, _ = ob.lanczos_bounds(H, 24)
+    D_ref, st = oracle_mod.sp2_dense(H, n_occ, tol, bounds=(lo, hi))
+    _, st_g = oracle_mod.sp2_dense(H, n_occ, tol)
+    D, res = api.bml_sp2_dense(to_gpu(H), n_occ, tol, 100, precision, flags=api.FLAG_LANCZOS_BOUNDS(24))
+    assert res.status == st["status"] == 0
+    assert res.branch == st["branch"] and res.n_products == st["n_products"] < st_g["n_products"] - 3
+    assert abs(res.emin - lo) <= 1e-9 * (hi - lo) and abs(res.emax - hi) <= 1e-9 * (hi - lo)
+    err = np.linalg.norm(D.cpu().numpy() - D_ref) / np.linalg.norm(D_ref)
+    assert err <= (1e-10 if precision == 0 else 1e-5)
+
+
+def test_sp2_ellpack_with_lanczos_bounds(api, oracle_mod):
+    Hs = hm.small_sparse_model((8, 7, 8))
+    n = Hs[0].shape[0]
+    tau = 1e-6
+    lo, hi, _ = ob.lanczos_bounds(hm.ellpack_to_dense(*Hs), 24)
+    Dr, st = oracle_mod.sp2_ellpack(*Hs, n // 2, 1e-8, tau, bounds=(lo, hi))
+    _, st_g = oracle_mod.sp2_ellpack(*Hs, n // 2, 1e-8, tau)
+    Dg, res = api.bml_sp2_ellpack(*(to_gpu(a) for a in Hs), n // 2, 1e-8, tau, flags=api.FLAG_LANCZOS_BOUNDS(24))
+    assert res.status == st["status"] and res.branch == st["branch"] and res.n_products == st["n_products"]
+    assert st["n_products"] < st_g["n_products"]
+    A = hm.ellpack_to_dense(*(a.cpu().numpy() for a in Dg))
+    B = hm.ellpack_to_dense(*Dr)
+    # the bounds agree to ~1e-12, not bit for bit, so entries at the drop threshold may fall on either side
+    assert np.abs(A - B).max() <= tau * 1.001
+    assert np.linalg.norm(A - B) / np.linalg.norm(B) <= 1e-5
+
+
+def test_lanczos_flag_validation(api):
+    H = to_gpu(hm.make_dense("dense_n256"))
+    assert api.bml_sp2_dense(H, 128, 1e-10, flags=api.FLAG_LANCZOS_BOUNDS(7))[1].status == -1
+    assert api.bml_sp2_dense(H, 128, 1e-10, flags=api.FLAG_LANCZOS_BOUNDS(65))[1].status == -1
+    with pytest.raises(RuntimeError):
+        api.bml_lanczos_bounds(H, 7)
