@@ -109,12 +109,13 @@ __global__ void __launch_bounds__(LZ_THREADS) lanczos_update_kernel(double *__re
     for (int i = threadIdx.x; i < N; i += LZ_THREADS) w[i] = w[i] - alpha * v[i] - (j > 0 ? beta_j * v_prev[i] : 0.0);
     for (int pass = 0; pass < 2; ++pass) {
         __syncthreads();
-        for (int q = 0; q <= j; ++q) {
+        // one warp per previous vector: c_q = v_q . w (lane-strided partial sums, then the shuffle tree: fixed order)
+        for (int q = threadIdx.x >> 5; q <= j; q += LZ_THREADS / 32) {
             const double *vq = V + (size_t)q * N;
-            acc = 0.0;
-            for (int i = threadIdx.x; i < N; i += LZ_THREADS) acc = fma(vq[i], w[i], acc);
-            const double c = lz_block_sum(acc, s_part);
-            if (threadIdx.x == 0) s_c[q] = c;
+            double a = 0.0;
+            for (int i = threadIdx.x & 31; i < N; i += 32) a = fma(vq[i], w[i], a);
+            a = warp_sum(a);
+            if ((threadIdx.x & 31) == 0) s_c[q] = a;
         }
         __syncthreads();
         for (int i = threadIdx.x; i < N; i += LZ_THREADS) {
