@@ -338,6 +338,93 @@ def replicas_per_second(world: int, ms: float) -> float:
 
 
 # ----------------------------------------------------------------------------------------------------------
+# scaffolding shared by the three arms (SP2, Chebyshev, graph): process setup, the timed loop, a kernel timed alone
+# ----------------------------------------------------------------------------------------------------------
+class Ranks:
+    """One process per GPU (torchrun env), NCCL only for the barrier and the max-over-ranks of the timings."""
+
+    def __init__(self):
+        import torch
+
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
+        torch.cuda.set_device(self.local)
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+
+            dist.init_process_group("nccl")
+            self.dist = dist
+        self.dev = torch.device("cuda", self.local)
+
+    def barrier(self):
+        import torch
+
+        if self.dist is not None:
+            self.dist.barrier()
+        torch.cuda.synchronize()
+
+    def finish(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+def timed_steps(rk: Ranks, solve, args):
+    """W untimed warm-up steps, then exactly K steps, each between CUDA events on the launch stream, L2 flushed before
+    each, barrier + synchronize on both sides, clocks sampled during the timed region.
+    Returns (per-step ms, wall seconds of the timed region, clocks summary, result of the last step)."""
+    import torch
+
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=rk.dev)
+    res = None
+    for _ in range(args.warmup):
+        _, res = solve()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    rk.barrier()
+    with ClockSampler(rk.local) as clk:
+        t0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)                     # L2 flush, outside the per-step events
+            ev[k][0].record()
+            _, res = solve()                          # synchronises the stream once, at its end (reads the stats)
+            ev[k][1].record()
+        rk.barrier()
+        t_wall = time.perf_counter() - t0
+    return [a.elapsed_time(b) for a, b in ev], t_wall, clk.summary(), res
+
+
+def time_alone(fn, reps: int, warm: int = 3) -> float:
+    """ms per call of `fn` issued back to back on the current stream, after `warm` untimed calls."""
+    import torch
+
+    for _ in range(warm):
+        fn()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def timed_e2e(rk: Ranks, step, n: int) -> float:
+    """ms per end-to-end step (`step` copies the inputs in from pinned host memory, solves, copies the result out and
+    synchronises), wall clock, after two untimed steps."""
+    for _ in range(2):
+        step()
+    rk.barrier()
+    t0 = time.perf_counter()
+    for _ in range(n):
+        step()
+    return (time.perf_counter() - t0) / n * 1e3
+
+
+# ----------------------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -345,19 +432,9 @@ def run_ours(args):
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl")
+    rk = Ranks()
     api.load()
-    dev = torch.device("cuda", local)
+    dev, dist, world, rank = rk.dev, rk.dist, rk.world, rk.rank
     w = hm.WORKLOADS[args.workload]
     dense = w.kind == "dense"
     sp2_flags = api.FLAG_LANCZOS_BOUNDS(args.lanczos_steps) if args.lanczos_steps else 0
@@ -382,53 +459,25 @@ def run_ours(args):
         def solve(Hd):
             return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, 100, flags=sp2_flags)
 
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     # ---- device-resident timing: W warm-ups, then exactly K timed steps
-    res = None
-    for _ in range(args.warmup):
-        _, res = solve(H_dev)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    with ClockSampler(local) as clk:
-        t_wall0 = time.perf_counter()
-        for k in range(args.steps):
-            flush.fill_(k & 0xFF)                     # L2 flush, outside the per-step events
-            ev[k][0].record()
-            _, res = solve(H_dev)                     # synchronises the stream once, at its end (reads the stats)
-            ev[k][1].record()
-        barrier()
-        t_wall = time.perf_counter() - t_wall0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
     ms = float(np.mean(step_ms))
-    clocks = clk.summary()
 
     # ---- e2e: host buffers through the public API; H2D of H and D2H of D inside the timed region
-    e2e_steps = max(3, min(args.steps, 10))
-    h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
-    d2h = h2d
-    for _ in range(2):
-        Hd = H_host.to(dev, non_blocking=True) if dense else tuple(a.to(dev, non_blocking=True) for a in H_host)
-        D, _ = solve(Hd)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    def e2e_step():
         if dense:
-            Hd = H_host.to(dev, non_blocking=True)
-            D, _ = solve(Hd)
+            D, _ = solve(H_host.to(dev, non_blocking=True))
             D_host.copy_(D, non_blocking=True)
         else:
-            Hd = tuple(a.to(dev, non_blocking=True) for a in H_host)
-            D, _ = solve(Hd)
+            D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
             for dst, src in zip(D_host, D):
                 dst.copy_(src, non_blocking=True)
         torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
+    d2h = h2d
+    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
 
     # ---- dominant kernel, timed alone with CUDA events on the launching stream
     pk, pk_src = peaks()
@@ -440,17 +489,7 @@ def run_ours(args):
         X0 = api.padded_dense((lo_hi[1] * torch.eye(w.N, dtype=torch.float64) - H_host) * s, dev)
         Xn = torch.empty_strided(X0.shape, X0.stride(), dtype=X0.dtype, device=dev)
         ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(w.N, 0), dev)
-        reps = 20
-        for _ in range(3):
-            api.bml_x2_dense(X0, 1, 0, Xn, ws)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        a.record()
-        for _ in range(reps):
-            api.bml_x2_dense(X0, 1, 0, Xn, ws)
-        b.record()
-        torch.cuda.synchronize()
-        k_ms = a.elapsed_time(b) / reps
+        k_ms = time_alone(lambda: api.bml_x2_dense(X0, 1, 0, Xn, ws), 20)
         peak_probe = api.bml_probe_fp64_tensor_peak(40000)
         flops = dense_flops_per_product(w.N)
         achieved = flops / (k_ms * 1e-3) / 1e12
@@ -477,17 +516,7 @@ def run_ours(args):
         X0 = api.padded_dense((lo_hi[1] * torch.eye(w.N, dtype=torch.float64) - H_host) * s, dev)
         Xn = torch.empty_strided(X0.shape, X0.stride(), dtype=X0.dtype, device=dev)
         ws = api._workspace(api.load().bml_x2_dense_workspace_bytes(w.N, w.precision), dev)
-        reps = 10
-        for _ in range(3):
-            api.bml_x2_dense(X0, 1, w.precision, Xn, ws)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        a.record()
-        for _ in range(reps):
-            api.bml_x2_dense(X0, 1, w.precision, Xn, ws)
-        b.record()
-        torch.cuda.synchronize()
-        k_ms = a.elapsed_time(b) / reps
+        k_ms = time_alone(lambda: api.bml_x2_dense(X0, 1, w.precision, Xn, ws), 10)
         flops = terms * dense_flops_per_product(w.N)      # executed 16-bit tensor flops per product
         achieved = flops / (k_ms * 1e-3) / 1e12
         roof = {
@@ -511,17 +540,7 @@ def run_ours(args):
         macs = int((nn[Xmid[1].to(torch.int64)] * mask).sum().item())     # sum_i sum_{k in row i} n_k
         out = tuple(torch.zeros_like(t) for t in Xmid)
         ws = api._workspace(api.load().bml_x2_ellpack_workspace_bytes(w.N, w.M), dev)
-        reps = 5
-        for _ in range(2):
-            api.bml_x2_ellpack(Xmid, 1, w.drop_tol, out, ws)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        a.record()
-        for _ in range(reps):
-            api.bml_x2_ellpack(Xmid, 1, w.drop_tol, out, ws)
-        b.record()
-        torch.cuda.synchronize()
-        k_ms = a.elapsed_time(b) / reps
+        k_ms = time_alone(lambda: api.bml_x2_ellpack(Xmid, 1, w.drop_tol, out, ws), 5, warm=2)
         comp_bytes = float((12 * nn + 4).sum().item() + (12 * out[2].to(torch.int64) + 4).sum().item())
         achieved = comp_bytes / (k_ms * 1e-3) / 1e9
         roof = {
@@ -541,8 +560,7 @@ def run_ours(args):
     ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
 
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+        rk.finish()
         return 0
 
     # ---- CPU oracle baseline (rank 0, N = 1 only): bounded sample, ~10-30 s
@@ -583,8 +601,7 @@ def run_ours(args):
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    rk.finish()
     return 0
 
 
@@ -596,78 +613,34 @@ def run_cheby(args):
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl")
+    rk = Ranks()
     api.load()
-    dev = torch.device("cuda", local)
+    dev = rk.dev
     w = hm.WORKLOADS[args.workload]
     H_np = hm.make_dense(args.workload)
     H_host = torch.from_numpy(H_np).pin_memory()
     H_dev = H_host.to(dev)
     solver = api.ChebyshevSolver(w.N, w.k, w.m, dev)
     D_host = torch.empty((w.N, w.N), dtype=torch.float64).pin_memory()
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    res = None
-    for _ in range(args.warmup):
-        _, res = solver.solve(H_dev, w.mu, w.beta)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    with ClockSampler(local) as clk:
-        t_wall0 = time.perf_counter()
-        for k in range(args.steps):
-            flush.fill_(k & 0xFF)
-            ev[k][0].record()
-            _, res = solver.solve(H_dev, w.mu, w.beta)
-            ev[k][1].record()
-        barrier()
-        t_wall = time.perf_counter() - t_wall0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solver.solve(H_dev, w.mu, w.beta), args)
     ms = float(np.mean(step_ms))
-    clocks = clk.summary()
 
-    e2e_steps = max(3, min(args.steps, 10))
-    h2d = d2h = H_host.numel() * 8
-    for _ in range(2):
-        solver.solve(H_host.to(dev, non_blocking=True), w.mu, w.beta)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    def e2e_step():
         D, _ = solver.solve(H_host.to(dev, non_blocking=True), w.mu, w.beta)
         D_host.copy_(D, non_blocking=True)
         torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = d2h = H_host.numel() * 8
+    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
 
     # dominant kernel: one product alpha A B + beta C + gamma I of this size, timed alone
     T1 = (2.0 * H_host - (res.emax + res.emin) * torch.eye(w.N, dtype=torch.float64)) / (res.emax - res.emin)
     slab, n, ld, _ = api.matrix_slab([T1, T1 @ T1, torch.zeros_like(T1)], dev)
     ws = api._workspace(api.load().bml_symm_ab_workspace_bytes(), dev)
     job = [(0, 1, 0, 2, 2.0, -1.0, 0.0)]
-    reps = 20
-    for _ in range(3):
-        api.bml_symm_ab_dense(slab, n, ld, job, ws)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    a.record()
-    for _ in range(reps):
-        api.bml_symm_ab_dense(slab, n, ld, job, ws)
-    b.record()
-    torch.cuda.synchronize()
-    k_ms = a.elapsed_time(b) / reps
+    k_ms = time_alone(lambda: api.bml_symm_ab_dense(slab, n, ld, job, ws), 20)
     peak_probe = api.bml_probe_fp64_tensor_peak(40000)
     flops = dense_flops_per_product(w.N)
     achieved = flops / (k_ms * 1e-3) / 1e12
@@ -686,25 +659,24 @@ def run_cheby(args):
                         "ms_at_peak": sums_bytes / (pk["hbm_gbs"] * 1e9) * 1e3, "peak": pk["hbm_gbs"],
                         "peak_source": f"{pk_src} copy bandwidth from MEASURED_PEAKS.json"},
     }
-    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], rk.dist, dev)
+    if rk.rank != 0:
+        rk.finish()
         return 0
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if rk.world == 1 and not args.no_cpu_baseline:
         v, sample, cores, extra = oracle_cheby_time_to_D(args.workload, H_np, 25.0)
         cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample, **extra}
     # gershgorin (2) + coefficients + map + product launches + partial sums + trace
     launches_per_step = 2 + 1 + 1 + int(res.n_launches) + 1 + 1
     line = {
-        "metric": METRIC_CHEBY, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC_CHEBY, "value": ms, "unit": "ms", "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": workload_config(args.workload),
         "status": int(res.status), "n_products": n_prod, "n_product_launches": int(res.n_launches),
         "trace_D": res.trace, "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)),
         "wall_s_timed_region": t_wall, "ms_per_product": ms / max(n_prod, 1),
-        "aggregate_solves_per_s": replicas_per_second(world, ms),
+        "aggregate_solves_per_s": replicas_per_second(rk.world, ms),
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps},
         "gpu_launches": launches_per_step * args.steps,
@@ -713,8 +685,7 @@ def run_cheby(args):
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    rk.finish()
     return 0
 
 
@@ -726,19 +697,9 @@ def run_graph(args):
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: libbmlsp2 has no CPU path")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl")
+    rk = Ranks()
     api.load()
-    dev = torch.device("cuda", local)
+    dev = rk.dev
     w = hm.WORKLOADS[args.workload]
     H_np = hm.make_ellpack(args.workload)
     H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
@@ -750,47 +711,23 @@ def run_graph(args):
     cap = int(sizes[:, 0].max())
     solver = api.GraphSolver(w.N, w.M_out, w.n_parts, cap, w.k, w.m, dev)
     D_host = tuple(torch.empty_like(a).pin_memory() for a in (solver.dv.cpu(), solver.di.cpu(), solver.dn.cpu()))
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
 
     def solve(Hd):
         return solver.solve(Hd, offs, nodes, w.graph_tol, w.mu, w.beta, w.drop_tol)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    res = None
-    for _ in range(args.warmup):
-        _, res = solve(H_dev)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    with ClockSampler(local) as clk:
-        t_wall0 = time.perf_counter()
-        for k in range(args.steps):
-            flush.fill_(k & 0xFF)
-            ev[k][0].record()
-            _, res = solve(H_dev)
-            ev[k][1].record()
-        barrier()
-        t_wall = time.perf_counter() - t_wall0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
     ms = float(np.mean(step_ms))
-    clocks = clk.summary()
 
-    e2e_steps = max(3, min(args.steps, 10))
-    h2d = sum(a.numel() * a.element_size() for a in H_host)
-    d2h = sum(a.numel() * a.element_size() for a in D_host)
-    for _ in range(2):
-        solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    def e2e_step():
         D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
         for dst, src in zip(D_host, D):
             dst.copy_(src, non_blocking=True)
         torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) / e2e_steps * 1e3
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = sum(a.numel() * a.element_size() for a in H_host)
+    d2h = sum(a.numel() * a.element_size() for a in D_host)
+    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
 
     # dominant kernel: one local-solver product at the size of the largest part, timed alone
     g = torch.Generator().manual_seed(0)
@@ -799,17 +736,7 @@ def run_graph(args):
     slab, n, ld, _ = api.matrix_slab([A, A, torch.zeros_like(A)], dev)
     ws = api._workspace(api.load().bml_symm_ab_workspace_bytes(), dev)
     job = [(0, 1, 0, 2, 2.0, -1.0, 0.0)]
-    reps = 10
-    for _ in range(3):
-        api.bml_symm_ab_dense(slab, n, ld, job, ws)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    a.record()
-    for _ in range(reps):
-        api.bml_symm_ab_dense(slab, n, ld, job, ws)
-    b.record()
-    torch.cuda.synchronize()
-    k_ms = a.elapsed_time(b) / reps
+    k_ms = time_alone(lambda: api.bml_symm_ab_dense(slab, n, ld, job, ws), 10)
     peak_probe = api.bml_probe_fp64_tensor_peak(40000)
     flops = dense_flops_per_product(cap)
     achieved = flops / (k_ms * 1e-3) / 1e12
@@ -824,25 +751,25 @@ def run_graph(args):
         "in_step_tflops": step_flops / (ms * 1e-3) / 1e12,
         "in_step_frac": step_flops / (ms * 1e-3) / 1e12 / peak_probe,
     }
-    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], rk.dist, dev)
+    if rk.rank != 0:
+        rk.finish()
         return 0
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if rk.world == 1 and not args.no_cpu_baseline:
         v, sample, cores = oracle_graph_time_to_D(args.workload, H_np)
         cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
     levels = max(1, math.ceil(math.log2(w.k)))
-    per_part = 1 + 2 + 1 + 1 + levels + (w.m - 1) + 1 + 1 + 1 + 1      # gather, Gershgorin x2, coeff, map, products, sums, trace, collect, scatter
+    # per part: gather, Gershgorin x2, coefficients, map, products, partial sums, trace, status, scatter
+    per_part = 1 + 2 + 1 + 1 + levels + (w.m - 1) + 1 + 1 + 1 + 1
     launches_per_step = 3 + w.n_parts * per_part
     line = {
-        "metric": METRIC_GRAPH, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC_GRAPH, "value": ms, "unit": "ms", "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": workload_config(args.workload),
         "status": int(res.status), "n_products": n_prod, "part_size": res.part_size, "core_size": res.core_size,
         "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
-        "aggregate_solves_per_s": replicas_per_second(world, ms),
+        "aggregate_solves_per_s": replicas_per_second(rk.world, ms),
         "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps},
         "gpu_launches": launches_per_step * args.steps,
@@ -852,8 +779,7 @@ def run_graph(args):
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    rk.finish()
     return 0
 
 
