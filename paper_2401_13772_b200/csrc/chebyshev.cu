@@ -122,9 +122,10 @@ __global__ void cheb_map_kernel(const double *__restrict__ H, int64_t ldh, doubl
 // computes the S_j as m separate sums on concurrent streams.  HBM-bound: (k - 1 + m) N^2 x 8 B.
 // slab: slot s holds the matrix at slab + s * slot_elems; T_i in slot i - 1, S_j in slot k + j.
 // ------------------------------------------------------------------------------------------------------------
-template <int MJ>
-__global__ void __launch_bounds__(256) cheb_sums_kernel(double *__restrict__ slab, int64_t slot_elems, int64_t ld, int N,
-                                                        int k, int m, const ChebCtl *__restrict__ ctl)
+template <int MJ, int CW>
+__global__ void __launch_bounds__(256, (MJ * CW <= 16) ? 4 : 2)
+cheb_sums_kernel(double *__restrict__ slab, int64_t slot_elems, int64_t ld, int N, int k, int m,
+                 const ChebCtl *__restrict__ ctl)
 {
     // s_d[i * MJ + j] = d_{i,j} (0 for j >= m): the MJ coefficients of one T_i are contiguous -> 128-bit broadcast loads
     __shared__ __align__(16) double s_d[BML_CHEB_MAX_K * MJ];
@@ -133,50 +134,55 @@ __global__ void __launch_bounds__(256) cheb_sums_kernel(double *__restrict__ sla
         s_d[idx] = j < m ? ctl->d[j * k + i] : 0.0;
     }
     __syncthreads();
-    // two adjacent columns per thread (ld is even and rows are 128-byte aligned, so the pair is one 16-byte access;
-    // a pair that straddles N reads a pad column and stores only its first element)
-    const int c = (blockIdx.x * blockDim.x + threadIdx.x) * 2;
+    // CW adjacent columns per thread.  CW = 2 (few sums: registers to spare) makes every access 16 bytes -- ld is even
+    // and rows are 128-byte aligned; a pair that straddles N reads a pad column and stores only its first element.
+    // CW = 1 (16 or 32 sums) keeps the accumulators at MJ registers pairs so that 4 CTAs fit an SM: the kernel is
+    // latency-bound and needs the warps more than the wider accesses.
+    const int c = (blockIdx.x * blockDim.x + threadIdx.x) * CW;
     if (c >= N) return;
-    const bool two = c + 1 < N;
+    const bool two = (CW == 2) && (c + 1 < N);
     for (int r = blockIdx.y; r < N; r += gridDim.y) {
         const int64_t off = (int64_t)r * ld + c;
-        double acc0[MJ], acc1[MJ];
+        double acc[CW][MJ];
 #pragma unroll
         for (int j = 0; j < MJ; ++j) {
-            acc0[j] = (r == c) ? s_d[j] : 0.0;
-            acc1[j] = (r == c + 1) ? s_d[j] : 0.0;
+#pragma unroll
+            for (int q = 0; q < CW; ++q) acc[q][j] = (r == c + q) ? s_d[j] : 0.0;
         }
 #pragma unroll 8
         for (int i = 1; i < k; ++i) {
-            const double2 t = __ldg((const double2 *)(slab + (int64_t)(i - 1) * slot_elems + off));
+            const double *src = slab + (int64_t)(i - 1) * slot_elems + off;
+            double t[CW];
+            if (CW == 2) { const double2 v = __ldg((const double2 *)src); t[0] = v.x; t[CW - 1] = v.y; }
+            else t[0] = __ldg(src);
 #pragma unroll
             for (int j = 0; j < MJ; ++j) {
                 const double dij = s_d[i * MJ + j];
-                acc0[j] = fma(dij, t.x, acc0[j]);
-                acc1[j] = fma(dij, t.y, acc1[j]);
+#pragma unroll
+                for (int q = 0; q < CW; ++q) acc[q][j] = fma(dij, t[q], acc[q][j]);
             }
         }
 #pragma unroll
         for (int j = 0; j < MJ; ++j) {
             if (j < m) {
                 double *dst = slab + (int64_t)(k + j) * slot_elems + off;
-                if (two) *(double2 *)dst = make_double2(acc0[j], acc1[j]);
-                else *dst = acc0[j];
+                if (two) *(double2 *)dst = make_double2(acc[0][j], acc[CW - 1][j]);
+                else *dst = acc[0][j];
             }
         }
     }
 }
 
-template <int MJ>
+template <int MJ, int CW>
 static int launch_sums_t(double *slab, int64_t slot_elems, int64_t ld, int N, int k, int m, const ChebCtl *ctl,
                          cudaStream_t st)
 {
-    // about 8 CTAs per SM in total, each walking several rows: the staging of d_{i,j} is paid once per CTA
-    const unsigned gx = (unsigned)((N + 511) / 512);
-    unsigned gy = (8u * 148u + gx - 1) / gx;
+    // a few CTAs per SM in total, each walking several rows: the staging of d_{i,j} is paid once per CTA
+    const unsigned gx = (unsigned)((N + 256 * CW - 1) / (256 * CW));
+    unsigned gy = (16u * 148u + gx - 1) / gx;
     if (gy > (unsigned)N) gy = (unsigned)N;
     const dim3 grid(gx, gy);
-    cheb_sums_kernel<MJ><<<grid, 256, 0, st>>>(slab, slot_elems, ld, N, k, m, ctl);
+    cheb_sums_kernel<MJ, CW><<<grid, 256, 0, st>>>(slab, slot_elems, ld, N, k, m, ctl);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
@@ -275,10 +281,10 @@ int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_ma
     }
 
     // S_0 .. S_{m-1} (Eq. 12)
-    if (m <= 4) CK(launch_sums_t<4>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
-    else if (m <= 8) CK(launch_sums_t<8>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
-    else if (m <= 16) CK(launch_sums_t<16>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
-    else CK(launch_sums_t<32>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st));
+    if (m <= 4) CK((launch_sums_t<4, 2>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
+    else if (m <= 8) CK((launch_sums_t<8, 2>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
+    else if (m <= 16) CK((launch_sums_t<16, 1>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
+    else CK((launch_sums_t<32, 1>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
 
     // Eq. 10, innermost bracket first: R_{m-1} = S_{m-1}; R_j = T_k R_{j+1} + S_j, written over S_j; R_0 -> D
     for (int j = m - 2; j >= 0; --j) {
