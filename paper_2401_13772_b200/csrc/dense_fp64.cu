@@ -13,6 +13,59 @@
 namespace bmlsp2 {
 
 
+// Fused epilogue (D4) of one tile held in the consumers' accumulators: X' = b ? 2X - P : P with its mirror, and this
+// thread's share of { tr P, ||P - X||^2, ||X||^2, tr X' }.  Fragment columns are first made adjacent (frag_adjacent) so
+// that X is read and X' written 16 bytes at a time; the iterates live in the workspace (ld a multiple of 16 doubles,
+// 128-byte aligned), so every pair is aligned.  Diagonal tiles use only r <= c and mirror it: X' is bitwise symmetric.
+template <int MI, int NI, int BT>
+__device__ __forceinline__ void sp2_tile_epilogue(double (&acc)[MI][NI][2], const double *__restrict__ X,
+                                                  double *__restrict__ Xn, int64_t ld, int N, int I, int J, int wm, int wn,
+                                                  int lane, int branch, double &s_trp, double &s_e, double &s_x,
+                                                  double &s_trn)
+{
+    const int g = lane >> 2, t = lane & 3;
+    const bool diag = (I == J);
+    const int row0 = I * BT + wm * (BT / 2) + perm8(g);
+    const int col0 = J * BT + wn * (BT / 4);
+    auto one = [&](int r, int c, double p) {
+        if (r < N && c < N && (!diag || r <= c)) {
+            const double x = X[(int64_t)r * ld + c];
+            const double d = p - x;
+            const double xn = branch ? (2.0 * x - p) : p;             // Eq. 7 : Eq. 6
+            Xn[(int64_t)r * ld + c] = xn;
+            if (r == c) {
+                s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
+            } else {
+                Xn[(int64_t)c * ld + r] = xn;                         // mirror
+                s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
+            }
+        }
+    };
+#pragma unroll
+    for (int i = 0; i < MI; ++i) {
+        const int r = row0 + i * 8;
+#pragma unroll
+        for (int j = 0; j < NI; ++j) {
+            double p0 = acc[i][j][0], p1 = acc[i][j][1];
+            const int c = col0 + j * 8 + frag_adjacent(p0, p1, t);
+            if (r < N && c + 1 < N && (!diag || r < c)) {
+                // both elements strictly above the diagonal: one 16-byte read of X, one 16-byte write of X'
+                const double2 x = *(const double2 *)(X + (int64_t)r * ld + c);
+                const double d0 = p0 - x.x, d1 = p1 - x.y;
+                const double xn0 = branch ? (2.0 * x.x - p0) : p0, xn1 = branch ? (2.0 * x.y - p1) : p1;
+                *(double2 *)(Xn + (int64_t)r * ld + c) = make_double2(xn0, xn1);
+                Xn[(int64_t)c * ld + r] = xn0;
+                Xn[(int64_t)(c + 1) * ld + r] = xn1;
+                s_e += 2.0 * (d0 * d0) + 2.0 * (d1 * d1);
+                s_x += 2.0 * (x.x * x.x) + 2.0 * (x.y * x.y);
+            } else {
+                one(r, c, p0);
+                one(r, c + 1, p1);
+            }
+        }
+    }
+}
+
 template <int BT>
 __global__ void __launch_bounds__(D_THREADS, 1)
 x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
@@ -76,8 +129,6 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         // ===================== DMMA consumers =====================
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(D_REGS_CONSUMER));
         const int wm = warp >> 2, wn = warp & 3;     // 2 x 4 warps; warp tile 64 x 32
-        const int g = lane >> 2, t = lane & 3;
-        const int pg = perm8(g);
         double acc[MI][NI][2];
 #pragma unroll
         for (int i = 0; i < MI; ++i)
@@ -100,36 +151,8 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
         }
 
         // ===================== fused epilogue (D4) =====================
-        // lane holds C[g][2t], C[g][2t+1] of each 8x8 fragment -> physical (row perm8(g), cols perm8(2t), perm8(2t+1))
-        const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
-        const int row0 = I * D_BM + wm * (D_BM / 2) + pg;
-        const int col0 = J * D_BN + wn * (D_BN / 4);
-#pragma unroll
-        for (int i = 0; i < MI; ++i) {
-            const int r = row0 + i * 8;
-#pragma unroll
-            for (int j = 0; j < NI; ++j) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int c = col0 + j * 8 + (h ? pc1 : pc0);
-                    // diagonal tiles: only the upper triangle (r <= c) is used and mirrored -> X' is bitwise symmetric
-                    if (r < N && c < N && (!diag || r <= c)) {
-                        const double p = acc[i][j][h];
-                        const double x = X[(int64_t)r * ld + c];
-                        const double d = p - x;
-                        const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
-                        Xn[(int64_t)r * ld + c] = xn;
-                        if (r == c) {
-                            s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
-                        } else {
-                            Xn[(int64_t)c * ld + r] = xn;                 // mirror
-                            s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
-                        }
-                    }
-                }
-            }
-        }
+        sp2_tile_epilogue<MI, NI, BT>(acc, X, Xn, ld, N, I, J, wm, wn, lane, branch, s_trp, s_e, s_x, s_trn);
         s_trp = warp_sum(s_trp); s_e = warp_sum(s_e); s_x = warp_sum(s_x); s_trn = warp_sum(s_trn);
         if (lane == 0) { s_red[warp][0] = s_trp; s_red[warp][1] = s_e; s_red[warp][2] = s_x; s_red[warp][3] = s_trn; }
     }
@@ -244,12 +267,9 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
         // ===================== DMMA consumers =====================
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(D_REGS_CONSUMER));
         const int wm = warp >> 2, wn = warp & 3;     // 2 x 4 warps; warp tile 64 x 32
-        const int g = lane >> 2, t = lane & 3;
-        const int pg = perm8(g);
         const int ctid = warp * 32 + lane;           // consumer thread id 0..255
         uint32_t koff[4];
         dmma_koff(lane, koff);
-        const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
         int slab = 0;
         StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
@@ -320,32 +340,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
             }
 
             // ===================== fused epilogue (D4) =====================
-            const int row0 = I * D_BM + wm * (D_BM / 2) + pg;
-            const int col0 = J * D_BN + wn * (D_BN / 4);
-#pragma unroll
-            for (int i = 0; i < MI; ++i) {
-                const int r = row0 + i * 8;
-#pragma unroll
-                for (int j = 0; j < NI; ++j) {
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int cc = col0 + j * 8 + (h ? pc1 : pc0);
-                        if (r < N && cc < N && (!diag || r <= cc)) {
-                            const double p = acc[i][j][h];
-                            const double x = X[(int64_t)r * ld + cc];
-                            const double d = p - x;
-                            const double xn = branch ? (2.0 * x - p) : p;     // Eq. 7 : Eq. 6
-                            Xn[(int64_t)r * ld + cc] = xn;
-                            if (r == cc) {
-                                s_trp += p; s_trn += xn; s_e += d * d; s_x += x * x;
-                            } else {
-                                Xn[(int64_t)cc * ld + r] = xn;                // mirror
-                                s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
-                            }
-                        }
-                    }
-                }
-            }
+            sp2_tile_epilogue<MI, NI, BT>(acc, X, Xn, ld, N, I, J, wm, wn, lane, branch, s_trp, s_e, s_x, s_trn);
         }
         s_trp = warp_sum(s_trp); s_e = warp_sum(s_e); s_x = warp_sum(s_x); s_trn = warp_sum(s_trn);
         if (lane == 0) { s_red[warp][0] = s_trp; s_red[warp][1] = s_e; s_red[warp][2] = s_x; s_red[warp][3] = s_trn; }

@@ -57,6 +57,18 @@ __device__ __forceinline__ void dmma_slab(double (&acc)[MI][NI][2], const uint8_
     }
 }
 
+// Exchange inside the lane pairs (t, t ^ 2) of a fragment row so that every lane ends up with two ADJACENT columns:
+// the m8n8k4 accumulator layout gives lane t the physical columns perm8(2t), perm8(2t+1) = {0,2} {4,6} {1,3} {5,7};
+// afterwards the lanes hold {0,1} {4,5} {2,3} {6,7} and the epilogues can use 16-byte loads and stores.
+// Returns the first (even) column of the pair.  Must be called by all 32 lanes.
+__device__ __forceinline__ int frag_adjacent(double &v0, double &v1, int t)
+{
+    const bool lo = t < 2;
+    const double recv = __shfl_xor_sync(0xffffffffu, lo ? v1 : v0, 2);
+    if (lo) v1 = recv; else v0 = recv;
+    return lo ? 4 * t : 4 * (t - 2) + 2;
+}
+
 // Release of a ring stage back to the TMA producer, ONE SLAB LATE.  ptxas schedules a stage's mbarrier.arrive right
 // behind the ISSUE of the slab's last fragment loads (the MMAs that consume them follow it), and the arrive does not
 // wait for those loads to have read shared memory: when the consumers run close behind the producer (short, store-only

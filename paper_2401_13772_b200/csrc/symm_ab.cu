@@ -87,7 +87,6 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
     const int ctid = warp * 32 + lane;               // consumer thread id 0..255
     uint32_t koff[4];
     dmma_koff(lane, koff);
-    const int pc0 = perm8(2 * t), pc1 = perm8(2 * t + 1);
     int slab = 0;
     StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
     SkItem w;
@@ -165,22 +164,39 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
         const double alpha = jb.alpha, beta = jb.beta, gamma = jb.gamma;
         const int row0 = I * BT + wm * (BT / 2) + pg;
         const int col0 = J * BT + wn * (BT / 4);
+        // 16-byte accesses need even leading dimensions and 16-byte aligned bases (the slab always is; a caller's D may
+        // not be): CTA-uniform choice per job
+        const bool vec = (((ldo | ldc) & 1) == 0) && ((((uintptr_t)Out | (uintptr_t)C) & 15) == 0);
+        auto one = [&](int r, int cc, double p) {
+            // diagonal tiles: only r <= cc is used and mirrored -> Out is bitwise symmetric
+            if (r < N && cc < N && (!diag || r <= cc)) {
+                double v = alpha * p;
+                if (C) v = fma(beta, C[(int64_t)r * ldc + cc], v);
+                if (r == cc) v += gamma;
+                Out[(int64_t)r * ldo + cc] = v;
+                if (r != cc) Out[(int64_t)cc * ldo + r] = v;
+            }
+        };
 #pragma unroll
         for (int i = 0; i < MI; ++i) {
             const int r = row0 + i * 8;
 #pragma unroll
             for (int j = 0; j < NI; ++j) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int cc = col0 + j * 8 + (h ? pc1 : pc0);
-                    // diagonal tiles: only r <= cc is used and mirrored -> Out is bitwise symmetric
-                    if (r < N && cc < N && (!diag || r <= cc)) {
-                        double v = alpha * acc[i][j][h];
-                        if (C) v = fma(beta, C[(int64_t)r * ldc + cc], v);
-                        if (r == cc) v += gamma;
-                        Out[(int64_t)r * ldo + cc] = v;
-                        if (r != cc) Out[(int64_t)cc * ldo + r] = v;
+                double p0 = acc[i][j][0], p1 = acc[i][j][1];
+                const int cc = col0 + j * 8 + frag_adjacent(p0, p1, t);       // columns cc, cc + 1 (cc even)
+                if (vec && r < N && cc + 1 < N && (!diag || r < cc)) {
+                    double v0 = alpha * p0, v1 = alpha * p1;
+                    if (C) {
+                        const double2 c2 = *(const double2 *)(C + (int64_t)r * ldc + cc);
+                        v0 = fma(beta, c2.x, v0);
+                        v1 = fma(beta, c2.y, v1);
                     }
+                    *(double2 *)(Out + (int64_t)r * ldo + cc) = make_double2(v0, v1);
+                    Out[(int64_t)cc * ldo + r] = v0;
+                    Out[(int64_t)(cc + 1) * ldo + r] = v1;
+                } else {
+                    one(r, cc, p0);
+                    one(r, cc + 1, p1);
                 }
             }
         }
