@@ -101,3 +101,20 @@ def test_lanczos_flag_validation(api):
     assert api.bml_sp2_dense(H, 128, 1e-10, flags=api.FLAG_LANCZOS_BOUNDS(65))[1].status == -1
     with pytest.raises(RuntimeError):
         api.bml_lanczos_bounds(H, 7)
+
+
+def test_lanczos_degenerate_and_tiny_matrices(api, oracle_mod):
+    """H = c I breaks down after one step (beta_1 = 0) and leaves a zero-width interval -> SP2 status -2 as without the
+    flag; N smaller than the number of steps runs the full-length recursion and returns (nearly) the exact spectrum."""
+    H = to_gpu(np.eye(12) * 3.0)
+    assert api.bml_sp2_dense(H, 5, 1e-10, flags=api.FLAG_LANCZOS_BOUNDS(8))[1].status == -2
+    rng = np.random.default_rng(4)
+    G = rng.normal(size=(5, 5))
+    Hs = (G + G.T) / 2
+    w = np.linalg.eigvalsh(Hs)
+    got = api.bml_lanczos_bounds(to_gpu(Hs), 8).cpu().numpy()
+    lo, hi, info = ob.lanczos_bounds(Hs, 8)
+    assert info["steps"] == 5
+    assert got[0] <= w[0] and got[1] >= w[-1]
+    assert abs(got[0] - lo) <= 1e-9 * (w[-1] - w[0]) and abs(got[1] - hi) <= 1e-9 * (w[-1] - w[0])
+    assert got[1] - got[0] <= 1.03 * (w[-1] - w[0])
