@@ -23,6 +23,8 @@ struct ChebCtl {
     double d[BML_CHEB_MAX_TERMS];      // d_{i,j} at d[j * k + i]
 };
 constexpr size_t CHEB_TAB_DOUBLES = 8 * BML_CHEB_MAX_TERMS;   // cos(pi j / (2 N_q)), j < 4 N_q, N_q = 2 (L + 1)
+constexpr size_t CHEB_CTL_BYTES = (sizeof(ChebCtl) + 1023) / 1024 * 1024;
+constexpr size_t CHEB_CTL_STRIDE = CHEB_CTL_BYTES + CHEB_TAB_DOUBLES * sizeof(double);   // control block + its table
 
 // f_mu(eps) = 1 / (1 + exp(beta (eps - mu))), written so that exp never overflows (reading C2)
 __device__ __forceinline__ double fermi_fn(double eps, double mu, double beta)
@@ -208,120 +210,158 @@ int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b)
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct ChebWs {
-    ChebCtl *ctl;
-    double *tab;
+    uint8_t *ctl0;          // P control blocks, CHEB_CTL_STRIDE bytes apart; each followed by its cosine table
     double *rowlh;
     void *sk;
-    double *slab;
+    double *slab;           // P x (k + m) slots: problem q owns slots q (k + m) .. ; T_i at +i - 1, S_j at +k + j
     int64_t ld, slot_elems;
     size_t total;
+    ChebCtl *ctl(int q) const { return (ChebCtl *)(ctl0 + (size_t)q * CHEB_CTL_STRIDE); }
+    double *tab(int q) const { return (double *)(ctl0 + (size_t)q * CHEB_CTL_STRIDE + CHEB_CTL_BYTES); }
 };
 
-static ChebWs carve_cheb(void *ws, int64_t N, int k, int m)
+static ChebWs carve_cheb(void *ws, int64_t N, int k, int m, int P)
 {
     ChebWs w;
     uint8_t *p = (uint8_t *)ws;
     size_t off = 0;
-    w.ctl = (ChebCtl *)(p + off); off = align_up(off + sizeof(ChebCtl), 1024);
-    w.tab = (double *)(p + off); off = align_up(off + CHEB_TAB_DOUBLES * sizeof(double), 1024);
+    w.ctl0 = p + off; off = align_up(off + (size_t)P * CHEB_CTL_STRIDE, 1024);
     w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * sizeof(double), 1024);
     w.sk = (void *)(p + off); off = align_up(off + symm_ab_sk_bytes(), 1024);
     w.ld = (N + 15) / 16 * 16;
     w.slot_elems = (int64_t)align_up((size_t)N * w.ld, 128);
-    w.slab = (double *)(p + off); off = align_up(off + (size_t)(k + m) * w.slot_elems * sizeof(double), 1024);
+    w.slab = (double *)(p + off); off = align_up(off + (size_t)P * (k + m) * w.slot_elems * sizeof(double), 1024);
     w.total = off;
     return w;
 }
 
-size_t cheb_workspace_bytes(int64_t N, int k, int m) { return carve_cheb(nullptr, N, k, m).total; }
+size_t cheb_workspace_bytes(int64_t N, int k, int m) { return carve_cheb(nullptr, N, k, m, 1).total; }
+size_t cheb_batch_workspace_bytes(int64_t N, int k, int m, int P) { return carve_cheb(nullptr, N, k, m, P).total; }
 
-// Enqueue one expansion (steps C0-C6), no host synchronisation.  *n_launches_out <- product-kernel launches.
-// The device-side verdict (0 or BML_ERR_DEGENERATE) is left in the int that cheb_fail_flag(ws) points to.
-int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, int *n_launches_out,
-                       cudaStream_t st)
+// Enqueue P independent expansions of the same size N (steps C0-C6 each), no host synchronisation.  The products of
+// the P problems share launches: a doubling level or a nesting step of ALL problems goes out in grouped launches of up
+// to BML_SYMM_MAX_JOBS products (this is what fills the GPU when one problem is too small to).
+// D[q] may point into the workspace (cheb_batch_result): the last nesting step then works in place.
+// The device-side verdict of problem q (0 or BML_ERR_DEGENERATE) is left in *cheb_fail_flag(ws, q).
+int cheb_dense_enqueue_batch(int P, const bml_matrix_t *H, const bml_cheb_params_t *p, const bml_matrix_t *D, void *ws,
+                             int *n_launches_out, cudaStream_t st)
 {
-    const int64_t N = H->N;
-    const int k = p->k, m = p->m;
-    ChebWs w = carve_cheb(ws, N, k, m);
-    auto slot = [&](int s) { return w.slab + (int64_t)s * w.slot_elems; };      // T_i: slot i - 1; S_j: slot k + j
+    const int64_t N = H[0].N;
+    const int k = p->k, m = p->m, SL = k + m;
+    ChebWs w = carve_cheb(ws, N, k, m, P);
+    auto slot = [&](int q, int s) { return w.slab + (int64_t)(q * SL + s) * w.slot_elems; };
 #define CK(x) do { int _r = (x); if (_r != 0) return _r; } while (0)
-    if (cudaMemsetAsync(w.ctl, 0, 64, st) != cudaSuccess) return BML_ERR_CUDA;
-    CK(launch_gershgorin(H, w.ctl->bounds, w.rowlh, st));
-    if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) CK(launch_check_symmetry(H, &w.ctl->not_symmetric, st));
-    cheb_coeff_kernel<<<1, CC_THREADS, 0, st>>>(w.ctl, w.tab, p->mu, p->beta, k, m);
-    {
+    for (int q = 0; q < P; ++q) {
+        if (cudaMemsetAsync(w.ctl(q), 0, 64, st) != cudaSuccess) return BML_ERR_CUDA;
+        CK(launch_gershgorin(&H[q], w.ctl(q)->bounds, w.rowlh, st));
+        if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) CK(launch_check_symmetry(&H[q], &w.ctl(q)->not_symmetric, st));
+        cheb_coeff_kernel<<<1, CC_THREADS, 0, st>>>(w.ctl(q), w.tab(q), p->mu, p->beta, k, m);
         const dim3 grid((unsigned)((N + 255) / 256), (unsigned)(N < 2048 ? N : 2048));
-        cheb_map_kernel<<<grid, 256, 0, st>>>(H->value, H->ld, slot(0), w.ld, (int)N, w.ctl);
+        cheb_map_kernel<<<grid, 256, 0, st>>>(H[q].value, H[q].ld, slot(q, 0), w.ld, (int)N, w.ctl(q));
+        if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
     }
-    if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
 
     CUtensorMap map;
-    CK(make_slab_map(&map, w.slab, N, w.ld, w.slot_elems, k + m));
+    CK(make_slab_map(&map, w.slab, N, w.ld, w.slot_elems, P * SL));
     CK(symm_ab_sk_reset(w.sk, st));
     unsigned int epoch = 0;
     int n_launches = 0;
+    SymmBatch batch;
+    memset(&batch, 0, sizeof(batch));
+    auto flush = [&]() -> int {
+        if (batch.n_jobs == 0) return 0;
+        const int r = launch_symm_ab(map, batch, N, w.sk, ++epoch, st);
+        ++n_launches;
+        memset(&batch, 0, sizeof(batch));
+        return r;
+    };
+    auto add = [&](const SymmJob &jb) -> int {
+        batch.job[batch.n_jobs++] = jb;
+        return batch.n_jobs == BML_SYMM_MAX_JOBS ? flush() : 0;
+    };
 
-    // T_2 .. T_k, one grouped launch per doubling level (Eq. 13-14)
+    // T_2 .. T_k of every problem, level by level (Eq. 13-14)
     int32_t level[BML_CHEB_MAX_K], ta[BML_CHEB_MAX_K], tb[BML_CHEB_MAX_K];
     const int levels = cheb_schedule(k, level, ta, tb);
     for (int lv = 1; lv <= levels; ++lv) {
-        SymmBatch batch;
-        memset(&batch, 0, sizeof(batch));
-        for (int i = 2; i <= k; ++i) {
-            if (level[i - 2] != lv) continue;
-            SymmJob &jb = batch.job[batch.n_jobs++];
-            jb.a = ta[i - 2] - 1; jb.b = tb[i - 2] - 1;
-            jb.Out = slot(i - 1); jb.ldo = w.ld; jb.ldc = w.ld;
-            jb.alpha = 2.0;
-            if (ta[i - 2] == tb[i - 2]) { jb.C = nullptr; jb.beta = 0.0; jb.gamma = -1.0; }     // - T_0
-            else { jb.C = slot(0); jb.beta = -1.0; jb.gamma = 0.0; }                            // - T_1
-        }
-        CK(launch_symm_ab(map, batch, N, w.sk, ++epoch, st));
-        ++n_launches;
+        for (int q = 0; q < P; ++q)
+            for (int i = 2; i <= k; ++i) {
+                if (level[i - 2] != lv) continue;
+                SymmJob jb;
+                memset(&jb, 0, sizeof(jb));
+                jb.a = q * SL + ta[i - 2] - 1; jb.b = q * SL + tb[i - 2] - 1;
+                jb.Out = slot(q, i - 1); jb.ldo = w.ld; jb.ldc = w.ld;
+                jb.alpha = 2.0;
+                if (ta[i - 2] == tb[i - 2]) { jb.C = nullptr; jb.beta = 0.0; jb.gamma = -1.0; }     // - T_0
+                else { jb.C = slot(q, 0); jb.beta = -1.0; jb.gamma = 0.0; }                         // - T_1
+                CK(add(jb));
+            }
+        CK(flush());                    // the next level reads this one
     }
 
     // S_0 .. S_{m-1} (Eq. 12)
-    if (m <= 4) CK((launch_sums_t<4, 2>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
-    else if (m <= 8) CK((launch_sums_t<8, 2>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
-    else if (m <= 16) CK((launch_sums_t<16, 1>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
-    else CK((launch_sums_t<32, 1>(w.slab, w.slot_elems, w.ld, (int)N, k, m, w.ctl, st)));
+    for (int q = 0; q < P; ++q) {
+        double *base = slot(q, 0);
+        if (m <= 4) CK((launch_sums_t<4, 2>(base, w.slot_elems, w.ld, (int)N, k, m, w.ctl(q), st)));
+        else if (m <= 8) CK((launch_sums_t<8, 2>(base, w.slot_elems, w.ld, (int)N, k, m, w.ctl(q), st)));
+        else if (m <= 16) CK((launch_sums_t<16, 1>(base, w.slot_elems, w.ld, (int)N, k, m, w.ctl(q), st)));
+        else CK((launch_sums_t<32, 1>(base, w.slot_elems, w.ld, (int)N, k, m, w.ctl(q), st)));
+    }
 
     // Eq. 10, innermost bracket first: R_{m-1} = S_{m-1}; R_j = T_k R_{j+1} + S_j, written over S_j; R_0 -> D
     for (int j = m - 2; j >= 0; --j) {
-        SymmBatch batch;
-        memset(&batch, 0, sizeof(batch));
-        batch.n_jobs = 1;
-        SymmJob &jb = batch.job[0];
-        jb.a = k - 1; jb.b = k + j + 1;
-        jb.C = slot(k + j); jb.ldc = w.ld;
-        jb.Out = (j == 0) ? D->value : slot(k + j);
-        jb.ldo = (j == 0) ? D->ld : w.ld;
-        jb.alpha = 1.0; jb.beta = 1.0; jb.gamma = 0.0;
-        CK(launch_symm_ab(map, batch, N, w.sk, ++epoch, st));
-        ++n_launches;
+        for (int q = 0; q < P; ++q) {
+            SymmJob jb;
+            memset(&jb, 0, sizeof(jb));
+            jb.a = q * SL + k - 1; jb.b = q * SL + k + j + 1;
+            jb.C = slot(q, k + j); jb.ldc = w.ld;
+            jb.Out = (j == 0) ? D[q].value : slot(q, k + j);
+            jb.ldo = (j == 0) ? D[q].ld : w.ld;
+            jb.alpha = 1.0; jb.beta = 1.0; jb.gamma = 0.0;
+            CK(add(jb));
+        }
+        CK(flush());
     }
-    if (m == 1 && cudaMemcpy2DAsync(D->value, (size_t)D->ld * 8, slot(k), (size_t)w.ld * 8, (size_t)N * 8, (size_t)N,
-                                    cudaMemcpyDeviceToDevice, st) != cudaSuccess)
-        return BML_ERR_CUDA;
-    CK(launch_trace_dense(D->value, D->ld, (int)N, &w.ctl->trace, st));
+    for (int q = 0; q < P; ++q) {
+        if (m == 1 && D[q].value != slot(q, k) &&
+            cudaMemcpy2DAsync(D[q].value, (size_t)D[q].ld * 8, slot(q, k), (size_t)w.ld * 8, (size_t)N * 8, (size_t)N,
+                              cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+            return BML_ERR_CUDA;
+        CK(launch_trace_dense(D[q].value, D[q].ld, (int)N, &w.ctl(q)->trace, st));
+    }
 #undef CK
     if (n_launches_out) *n_launches_out = n_launches;
     return 0;
 }
 
-int *cheb_fail_flag(void *ws) { return &((ChebCtl *)ws)->fail; }
+// where problem q of a batch leaves its result when D[q] is not supplied by the caller: its S_0 slot (leading dim ld)
+double *cheb_batch_result(void *ws, int64_t N, int k, int m, int P, int q, int64_t *ld_out)
+{
+    ChebWs w = carve_cheb(ws, N, k, m, P);
+    if (ld_out) *ld_out = w.ld;
+    return w.slab + (int64_t)(q * (k + m) + k) * w.slot_elems;
+}
+
+// Enqueue one expansion: the batch of one.
+int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, int *n_launches_out,
+                       cudaStream_t st)
+{
+    return cheb_dense_enqueue_batch(1, H, p, D, ws, n_launches_out, st);
+}
+
+int *cheb_fail_flag(void *ws, int q) { return &((ChebCtl *)((uint8_t *)ws + (size_t)q * CHEB_CTL_STRIDE))->fail; }
 
 int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, bml_cheb_stats_t *stats,
                      cudaStream_t st)
 {
     const int k = p->k, m = p->m;
-    ChebWs w = carve_cheb(ws, H->N, k, m);
+    ChebWs w = carve_cheb(ws, H->N, k, m, 1);
     int n_launches = 0;
     const int r = cheb_dense_enqueue(H, p, D, ws, &n_launches, st);
     if (r) return r;
     // the one host round trip of the call
     ChebCtl h;
-    if (cudaMemcpyAsync(&h, w.ctl, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;
+    if (cudaMemcpyAsync(&h, w.ctl(0), sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return BML_ERR_CUDA;
     if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
     int status = BML_OK;

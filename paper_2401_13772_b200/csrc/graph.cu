@@ -10,9 +10,11 @@ namespace bmlsp2 {
 
 // chebyshev.cu
 size_t cheb_workspace_bytes(int64_t N, int k, int m);
-int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, int *n_launches_out,
-                       cudaStream_t st);
-int *cheb_fail_flag(void *ws);
+size_t cheb_batch_workspace_bytes(int64_t N, int k, int m, int P);
+int cheb_dense_enqueue_batch(int P, const bml_matrix_t *H, const bml_cheb_params_t *p, const bml_matrix_t *D, void *ws,
+                             int *n_launches_out, cudaStream_t st);
+double *cheb_batch_result(void *ws, int64_t N, int k, int m, int P, int q, int64_t *ld_out);
+int *cheb_fail_flag(void *ws, int q);
 
 // part that owns position q of the core-node list: largest k with offsets[k] <= q
 __device__ __forceinline__ int part_of(const int32_t *__restrict__ offs, int n_parts, int q)
@@ -205,6 +207,15 @@ struct GraphWs {
     size_t total;
 };
 
+// Parts of EQUAL size are expanded as one batch (their products share grouped launches, which is what fills the GPU when a
+// part is too small to) if the batch's matrices fit a fixed memory budget; otherwise parts run back to back.
+constexpr size_t GRAPH_BATCH_BUDGET = (size_t)16 << 30;
+static bool graph_batch_ok(int n_parts, int size, int k, int m)
+{
+    const size_t ld = ((size_t)size + 15) / 16 * 16;
+    return n_parts >= 2 && (size_t)n_parts * (size_t)(k + m) * (size_t)size * ld * 8 <= GRAPH_BATCH_BUDGET;
+}
+
 static GraphWs carve_graph(void *ws, int64_t N, int n_parts, int cap, int k, int m)
 {
     GraphWs w;
@@ -217,7 +228,13 @@ static GraphWs carve_graph(void *ws, int64_t N, int n_parts, int cap, int k, int
     w.ldc = ((int64_t)cap + 15) / 16 * 16;
     w.h = (double *)(p + off); off = align_up(off + (size_t)cap * w.ldc * 8, 1024);
     w.d = (double *)(p + off); off = align_up(off + (size_t)cap * w.ldc * 8, 1024);
-    w.cheb = p + off; off = align_up(off + cheb_workspace_bytes(cap, k, m), 1024);
+    w.cheb = p + off;
+    size_t cheb_bytes = cheb_workspace_bytes(cap, k, m);
+    if (graph_batch_ok(n_parts, cap, k, m)) {
+        const size_t b = cheb_batch_workspace_bytes(cap, k, m, n_parts);
+        cheb_bytes = b > cheb_bytes ? b : cheb_bytes;
+    }
+    off = align_up(off + cheb_bytes, 1024);
     w.total = off;
     return w;
 }
@@ -255,19 +272,45 @@ int graph_chebyshev_solve(const bml_matrix_t *H, const int32_t *offs, const int3
     memset(&cp, 0, sizeof(cp));
     cp.mu = p->mu; cp.beta = p->beta; cp.k = p->k; cp.m = p->m;
     int n_products = 0;
-    for (int q = 0; q < P; ++q) {
-        const int s = h_scal[2 + 2 * q];
-        if (s < 1) continue;
-        const int32_t *nodes = w.nodes + (size_t)q * N;
-        if ((r = launch_graph_gather(H, nodes, s, w.h, w.ldc, st))) return r;
-        bml_matrix_t hd = {BML_DENSE, 0, s, w.ldc, w.h, nullptr, nullptr};
-        bml_matrix_t dd = {BML_DENSE, 0, s, w.ldc, w.d, nullptr, nullptr};
-        if ((r = cheb_dense_enqueue(&hd, &cp, &dd, w.cheb, nullptr, st))) return r;
-        graph_collect_kernel<<<1, 1, 0, st>>>(cheb_fail_flag(w.cheb), w.scal);
-        G_CHECK();
-        if ((r = launch_graph_scatter(w.d, w.ldc, nodes, w.is_core + (size_t)q * N, s, p->drop_tol, D, w.scal + 1, st)))
-            return r;
-        n_products += (p->k - 1) + (p->m - 1);
+    bool equal = true;
+    for (int q = 1; q < P; ++q) equal &= (h_scal[2 + 2 * q] == h_scal[2]);
+    if (equal && h_scal[2] >= 1 && graph_batch_ok(P, h_scal[2], p->k, p->m) && graph_batch_ok(P, p->part_capacity, p->k, p->m)) {
+        // ---- batched: gather each part and map it to its T_1, expand all parts together, scatter from the batch's slots
+        const int s = h_scal[2];
+        // h^k is gathered into the batch's RESULT slot of its part (S_0, free until Eq. 12 runs): it is only read to
+        // get the bounds and T_1, and the last nesting step of Eq. 10 writes d^k over it in place
+        bml_matrix_t hd[BML_GRAPH_MAX_PARTS], dd[BML_GRAPH_MAX_PARTS];
+        for (int q = 0; q < P; ++q) {
+            int64_t ldr = 0;
+            double *res = cheb_batch_result(w.cheb, s, p->k, p->m, P, q, &ldr);
+            hd[q] = bml_matrix_t{BML_DENSE, 0, s, ldr, res, nullptr, nullptr};
+            dd[q] = hd[q];
+            if ((r = launch_graph_gather(H, w.nodes + (size_t)q * N, s, res, ldr, st))) return r;
+        }
+        if ((r = cheb_dense_enqueue_batch(P, hd, &cp, dd, w.cheb, nullptr, st))) return r;
+        for (int q = 0; q < P; ++q) {
+            graph_collect_kernel<<<1, 1, 0, st>>>(cheb_fail_flag(w.cheb, q), w.scal);
+            G_CHECK();
+            if ((r = launch_graph_scatter(dd[q].value, dd[q].ld, w.nodes + (size_t)q * N, w.is_core + (size_t)q * N, s,
+                                          p->drop_tol, D, w.scal + 1, st)))
+                return r;
+            n_products += (p->k - 1) + (p->m - 1);
+        }
+    } else {
+        for (int q = 0; q < P; ++q) {
+            const int s = h_scal[2 + 2 * q];
+            if (s < 1) continue;
+            const int32_t *nodes = w.nodes + (size_t)q * N;
+            if ((r = launch_graph_gather(H, nodes, s, w.h, w.ldc, st))) return r;
+            bml_matrix_t hd = {BML_DENSE, 0, s, w.ldc, w.h, nullptr, nullptr};
+            bml_matrix_t dd = {BML_DENSE, 0, s, w.ldc, w.d, nullptr, nullptr};
+            if ((r = cheb_dense_enqueue_batch(1, &hd, &cp, &dd, w.cheb, nullptr, st))) return r;
+            graph_collect_kernel<<<1, 1, 0, st>>>(cheb_fail_flag(w.cheb, 0), w.scal);
+            G_CHECK();
+            if ((r = launch_graph_scatter(w.d, w.ldc, nodes, w.is_core + (size_t)q * N, s, p->drop_tol, D, w.scal + 1, st)))
+                return r;
+            n_products += (p->k - 1) + (p->m - 1);
+        }
     }
     if (cudaMemcpyAsync(h_scal, w.scal, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
