@@ -118,3 +118,23 @@ def test_lanczos_degenerate_and_tiny_matrices(api, oracle_mod):
     assert got[0] <= w[0] and got[1] >= w[-1]
     assert abs(got[0] - lo) <= 1e-9 * (w[-1] - w[0]) and abs(got[1] - hi) <= 1e-9 * (w[-1] - w[0])
     assert got[1] - got[0] <= 1.03 * (w[-1] - w[0])
+
+
+def test_lanczos_bounds_at_config3_size(api):
+    """BASELINE.json configs[2] (N = 8192, long-range model) with the tighter bounds, as bench.py --lanczos-steps 24 runs
+    it: the interval encloses the spectrum recorded in BASELINE.md (checked through what SP2 itself proves: it converges
+    to an idempotent matrix of the right trace, which it cannot from an interval that misses part of the spectrum), the
+    solve needs 23 products instead of 32, and D is the projector the Gershgorin path returns."""
+    import torch
+
+    w = hm.WORKLOADS["dense_n8192"]
+    H = to_gpu(hm.make_dense("dense_n8192"))
+    D0, r0 = api.bml_sp2_dense(H, w.n_occ, w.idem_tol)
+    D0 = D0.clone()
+    D1, r1 = api.bml_sp2_dense(H, w.n_occ, w.idem_tol, flags=api.FLAG_LANCZOS_BOUNDS(24))
+    assert r0.status == 0 and r1.status == 0
+    assert r0.n_products == 32 and r1.n_products == 23
+    assert r1.emin >= r0.emin and r1.emax <= r0.emax and (r1.emax - r1.emin) < 0.55 * (r0.emax - r0.emin)
+    assert r1.idem[-1] < w.idem_tol and abs(torch.trace(D1).item() - w.n_occ) < 1e-8 * w.n_occ
+    assert (torch.linalg.norm(D1 - D0) / torch.linalg.norm(D0)).item() < 1e-9
+    assert torch.equal(D1, D1.T)
