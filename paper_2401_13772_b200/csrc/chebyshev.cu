@@ -351,13 +351,92 @@ int cheb_dense_enqueue(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_ma
 
 int *cheb_fail_flag(void *ws, int q) { return &((ChebCtl *)((uint8_t *)ws + (size_t)q * CHEB_CTL_STRIDE))->fail; }
 
+// ------------------------------------------------------------------------------------------------------------
+// CUDA-graph replay of one expansion.  The launch sequence of an expansion is static -- no host decision, no
+// data-dependent launch shape -- so it is captured once per (pointers, shapes, parameters) and replayed: for small
+// matrices the ~25 launches are launch-latency bound.  A handful of instantiated graphs is kept per
+// host thread; anything that fails to capture or instantiate falls back to plain enqueueing (never to another
+// implementation).
+// ------------------------------------------------------------------------------------------------------------
+struct ChebGraphKey {
+    const void *H, *D, *ws;
+    int64_t N, ldh, ldd;
+    double mu, beta;
+    int32_t k, m;
+    uint32_t flags;
+    cudaStream_t st;
+    bool operator==(const ChebGraphKey &o) const
+    {
+        return H == o.H && D == o.D && ws == o.ws && N == o.N && ldh == o.ldh && ldd == o.ldd && mu == o.mu &&
+               beta == o.beta && k == o.k && m == o.m && flags == o.flags && st == o.st;
+    }
+};
+struct ChebGraphSlot {
+    ChebGraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    int n_launches = 0;
+    uint64_t stamp = 0;
+};
+constexpr int CHEB_GRAPH_SLOTS = 4;
+constexpr int64_t CHEB_GRAPH_MAX_N = 2048;      // above this the launches are long: nothing to gain
+
+static int cheb_enqueue_cached(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws,
+                               int *n_launches_out, cudaStream_t st)
+{
+    static thread_local ChebGraphSlot slots[CHEB_GRAPH_SLOTS];
+    static thread_local uint64_t clock_ = 0;
+    static thread_local bool warmed[3] = {false, false, false};
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const bool capturing = cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
+    const int bti = H->N <= 512 ? 0 : (H->N <= 1024 ? 1 : 2);
+    if (H->N > CHEB_GRAPH_MAX_N || capturing || st == nullptr || !warmed[bti]) {
+        // the first expansion of a tile size runs plainly: it sets the kernels' shared-memory attributes, which must
+        // not happen inside a capture; the legacy default stream cannot be captured
+        warmed[bti] = true;
+        return cheb_dense_enqueue(H, p, D, ws, n_launches_out, st);
+    }
+    const ChebGraphKey key = {H->value, D->value, ws, H->N, H->ld, D->ld, p->mu, p->beta, p->k, p->m, p->flags, st};
+    ChebGraphSlot *hit = nullptr, *victim = &slots[0];
+    for (auto &sl : slots) {
+        if (sl.exec && sl.key == key) hit = &sl;
+        if (sl.stamp < victim->stamp) victim = &sl;
+    }
+    if (!hit) {
+        cudaGraph_t graph = nullptr;
+        int nl = 0;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            return cheb_dense_enqueue(H, p, D, ws, n_launches_out, st);
+        }
+        const int r = cheb_dense_enqueue(H, p, D, ws, &nl, st);
+        const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+        cudaGraphExec_t exec = nullptr;
+        if (r != 0 || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            return cheb_dense_enqueue(H, p, D, ws, n_launches_out, st);
+        }
+        cudaGraphDestroy(graph);
+        if (victim->exec) cudaGraphExecDestroy(victim->exec);
+        victim->key = key; victim->exec = exec; victim->n_launches = nl;
+        hit = victim;
+    }
+    hit->stamp = ++clock_;
+    if (n_launches_out) *n_launches_out = hit->n_launches;
+    if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) {
+        cudaGetLastError();
+        return cheb_dense_enqueue(H, p, D, ws, n_launches_out, st);
+    }
+    return 0;
+}
+
 int cheb_dense_solve(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws, bml_cheb_stats_t *stats,
                      cudaStream_t st)
 {
     const int k = p->k, m = p->m;
     ChebWs w = carve_cheb(ws, H->N, k, m, 1);
     int n_launches = 0;
-    const int r = cheb_dense_enqueue(H, p, D, ws, &n_launches, st);
+    const int r = cheb_enqueue_cached(H, p, D, ws, &n_launches, st);
     if (r) return r;
     // the one host round trip of the call
     ChebCtl h;

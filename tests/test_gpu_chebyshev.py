@@ -259,3 +259,32 @@ def test_chebyshev_strided_input_and_repeat(api):
     assert torch.equal(D1, D2)
     D_ref, _ = och.chebyshev_serial(H, 0.2, 1.0, 31)
     assert relfro(D1.cpu().numpy(), D_ref) <= TOL_D
+
+
+def test_chebyshev_graph_replay_on_a_side_stream(api):
+    """On a non-default stream small expansions are captured once and replayed as a CUDA graph (chebyshev.cu): the
+    replays must give the bits of the plainly enqueued solve, also after the INPUT CONTENT changes under the same
+    pointers, and for several shapes alternating in one cache."""
+    import torch
+
+    H1 = hm.lattice_dense((7, 6, 5), 0.0, 0.2, 1.0, lambda r: -1.0, seed=1)
+    H2 = hm.lattice_dense((7, 6, 5), 0.3, 0.1, 1.0, lambda r: -1.0, seed=2)
+    N = H1.shape[0]
+    ref1 = api.bml_chebyshev_dense(to_gpu(H1), 0.1, 2.0, 8, 8)[0].clone()     # default stream: plain enqueue
+    ref2 = api.bml_chebyshev_dense(to_gpu(H2), 0.1, 2.0, 8, 8)[0].clone()
+    side = torch.cuda.Stream()
+    solver = api.ChebyshevSolver(N, 8, 8)
+    solver_b = api.ChebyshevSolver(N, 4, 4)
+    Hbuf = to_gpu(H1)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        for it in range(6):
+            Hbuf.copy_(to_gpu(H1 if it % 2 == 0 else H2))
+            D, res = solver.solve(Hbuf, 0.1, 2.0)
+            assert res.status == 0 and res.n_launches == 3 + 7
+            assert torch.equal(D, ref1 if it % 2 == 0 else ref2), f"replay {it}"
+            Db, rb = solver_b.solve(Hbuf, 0.1, 2.0)
+            assert rb.status == 0 and rb.n_products == 6
+    torch.cuda.synchronize()
+    D_ref_b, _ = och.chebyshev_serial(H2, 0.1, 2.0, 15)
+    assert relfro(Db.cpu().numpy(), D_ref_b) <= TOL_D
