@@ -57,7 +57,9 @@ typedef struct {
  * bitwise symmetric.  d_workspace: DEVICE scratch of >= bml_chebyshev_workspace_bytes(N, k, m) bytes, 1024-byte
  * aligned: (k + m) matrices of N x ld(N) doubles plus O(N) -- 8 GB at N = 8192, k = m = 8.
  * stats: HOST, may be NULL.  No host round trip inside the call: bounds, c_n and d_{i,j} are computed and consumed on
- * the device.  Returns BML_OK, -1 (also for k, m out of range or beta <= 0), -2, -4, -5.
+ * the device.  For N <= 2048 on a non-default stream the (static) launch sequence is captured once per argument set and
+ * replayed as a CUDA graph by later calls with the same pointers, shapes and parameters; results are identical.
+ * Returns BML_OK, -1 (also for k, m out of range or beta <= 0), -2, -4, -5.
  */
 BML_API size_t bml_chebyshev_workspace_bytes(int64_t N, int32_t k, int32_t m);
 BML_API int bml_chebyshev_dense(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *d_workspace,

@@ -10,7 +10,8 @@
  *
  * The core partition is an INPUT (graph partitioning is external: METIS etc.).  Everything else runs in the
  * library's kernels: halo construction, gather, one Chebyshev expansion per part (each on its own Gershgorin
- * interval, the whole GPU per part, parts back to back on the stream), thresholded scatter of the core rows.
+ * interval; parts of equal size are expanded as one batch whose products share grouped launches, otherwise parts run
+ * back to back with the whole GPU each), thresholded scatter of the core rows.
  * Readings of the paper fixed by this interface: DESIGN.md "Readings" G1-G6.  Conventions as in bml_sp2.h.
  */
 #ifndef BML_GRAPH_H
