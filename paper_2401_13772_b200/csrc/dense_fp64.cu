@@ -247,7 +247,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
             tma_prefetch_desc(map);
             int slab = 0;
             SkItem w;
-            for (int it = 0; sk_item(it, c, G, tiles, KT, w); ++it) {
+            for (int it = 0; sk_item(it, c, G, tiles, KT, sk_handoff_slabs(128), w); ++it) {
                 int I, J;
                 tri_decode(w.tile, I, J);
                 const bool diag = (I == J);
@@ -274,7 +274,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
         int slab = 0;
         StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
         SkItem w;
-        for (int it = 0; sk_item(it, c, G, tiles, KT, w); ++it) {
+        for (int it = 0; sk_item(it, c, G, tiles, KT, sk_handoff_slabs(128), w); ++it) {
             int I, J;
             tri_decode(w.tile, I, J);
             const bool diag = (I == J);
@@ -480,7 +480,7 @@ int dense_fp64_work_item(int64_t N, int n_ctas, int cta, int it, int32_t out[5])
     if (N <= 1024 || n_ctas < 1 || cta < 0 || cta >= n_ctas || it < 0) return BML_ERR_INVALID;
     const int T = (int)((N + 127) / 128), tiles = T * (T + 1) / 2, KT = (int)((N + D_BK - 1) / D_BK);
     SkItem w;
-    if (!sk_item(it, cta, n_ctas, tiles, KT, w)) return 1;
+    if (!sk_item(it, cta, n_ctas, tiles, KT, sk_handoff_slabs(128), w)) return 1;
     int I, J;
     tri_decode(w.tile, I, J);
     out[0] = w.tile; out[1] = I; out[2] = J; out[3] = w.kt0; out[4] = w.kt1;

@@ -93,12 +93,23 @@ struct StageRelease {
 struct SkItem {
     int tile, kt0, kt1;
 };
-// it-th work item of CTA c (identical arithmetic in every role); false when the list is exhausted
-__host__ __device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, SkItem &w)
+// Cost of one split-tile hand-off (partials to global memory, fence, flag, the owner's poll and reload) in units of
+// one k-slab of the tile's mainloop: small tiles have short slabs, so the same ~2-3 us weigh more.
+__host__ __device__ constexpr int sk_handoff_slabs(int bt) { return bt >= 128 ? 2 : (bt >= 64 ? 8 : 20); }
+
+// it-th work item of CTA c (identical arithmetic in every role); false when the list is exhausted.
+// The last, partial wave of R tiles is split along K over all G CTAs only if that is shorter than running the R tiles
+// whole on R CTAs: R KT / G + hs < KT (hs = sk_handoff_slabs).  Otherwise CTA c < R takes tile W G + c whole.
+__host__ __device__ __forceinline__ bool sk_item(int it, int c, int G, int tiles, int KT, int hs, SkItem &w)
 {
     const int W = tiles / G, R = tiles - W * G;
     if (it < W) { w.tile = it * G + c; w.kt0 = 0; w.kt1 = KT; return true; }
     if (R == 0) return false;
+    if ((int64_t)R * KT + (int64_t)hs * G >= (int64_t)KT * G) {
+        if (it > W || c >= R) return false;
+        w.tile = W * G + c; w.kt0 = 0; w.kt1 = KT;
+        return true;
+    }
     const int64_t UT = (int64_t)R * KT;
     const int64_t u0 = (int64_t)c * UT / G, u1 = (int64_t)(c + 1) * UT / G;
     const int64_t tl = u0 / KT + (it - W);

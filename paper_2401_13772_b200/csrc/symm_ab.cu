@@ -58,7 +58,7 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
             tma_prefetch_desc(&map);
             int slab = 0;
             SkItem w;
-            for (int it = 0; sk_item(it, c, G, total, KT, w); ++it) {
+            for (int it = 0; sk_item(it, c, G, total, KT, sk_handoff_slabs(BT), w); ++it) {
                 const int q = w.tile / tiles;
                 int I, J;
                 tri_decode(w.tile - q * tiles, I, J);
@@ -90,7 +90,7 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
     int slab = 0;
     StageRelease release;   // stages go back to the producer one slab late (dense_fp64_core.cuh)
     SkItem w;
-    for (int it = 0; sk_item(it, c, G, total, KT, w); ++it) {
+    for (int it = 0; sk_item(it, c, G, total, KT, sk_handoff_slabs(BT), w); ++it) {
         const int q = w.tile / tiles;
         int I, J;
         tri_decode(w.tile - q * tiles, I, J);
@@ -281,7 +281,7 @@ int symm_ab_work_item(int64_t N, int n_jobs, int n_ctas, int cta, int it, int32_
     const int bt = dense_fp64_tile(N);
     const int T = (int)((N + bt - 1) / bt), tiles = T * (T + 1) / 2, KT = (int)((N + D_BK - 1) / D_BK);
     SkItem w;
-    if (!sk_item(it, cta, n_ctas, tiles * n_jobs, KT, w)) return 1;
+    if (!sk_item(it, cta, n_ctas, tiles * n_jobs, KT, sk_handoff_slabs(bt), w)) return 1;
     const int q = w.tile / tiles;
     int I, J;
     tri_decode(w.tile - q * tiles, I, J);

@@ -91,8 +91,16 @@ def test_grouped_work_list_covers_every_unit_of_every_job_once(N, n_jobs, G):
         for cc in range(holders[0], holders[-1] + 1):
             assert cc in holders or units[cc] == W * KT
     assert sum(units) == n_jobs * T * (T + 1) // 2 * KT
+    # the last, partial wave: either split along K evenly over all CTAs, or -- when the hand-off would cost more than
+    # it saves (R KT / G + hs >= KT, hs = 2 / 8 / 20 slabs for tile edge 128 / 64 / 32) -- whole tiles on the first CTAs
     tail = [u - W * KT for u in units]
-    assert max(tail) - min(tail) <= 1
+    R = n_jobs * T * (T + 1) // 2 - W * G
+    hs = {128: 2, 64: 8, 32: 20}[bt]
+    if R * KT + hs * G >= KT * G:
+        assert tail == [KT] * R + [0] * (G - R)
+        assert all(len(p) == 1 for p in cover.values()), "no tile is split"
+    else:
+        assert max(tail) - min(tail) <= 1
 
 
 @pytest.mark.parametrize("k", list(range(2, 33)))
