@@ -22,9 +22,8 @@ struct ChebCtl {
     double c[BML_CHEB_MAX_TERMS];
     double d[BML_CHEB_MAX_TERMS];      // d_{i,j} at d[j * k + i]
 };
-constexpr size_t CHEB_TAB_DOUBLES = 8 * BML_CHEB_MAX_TERMS;   // cos(pi j / (2 N_q)), j < 4 N_q, N_q = 2 (L + 1)
 constexpr size_t CHEB_CTL_BYTES = (sizeof(ChebCtl) + 1023) / 1024 * 1024;
-constexpr size_t CHEB_CTL_STRIDE = CHEB_CTL_BYTES + CHEB_TAB_DOUBLES * sizeof(double);   // control block + its table
+constexpr size_t CHEB_CTL_STRIDE = CHEB_CTL_BYTES;
 
 // f_mu(eps) = 1 / (1 + exp(beta (eps - mu))), written so that exp never overflows (reading C2)
 __device__ __forceinline__ double fermi_fn(double eps, double mu, double beta)
@@ -40,31 +39,44 @@ __device__ __forceinline__ double fermi_fn(double eps, double mu, double beta)
 // 2k parallel chains of <= m / 2 subtractions.
 // ------------------------------------------------------------------------------------------------------------
 constexpr int CC_THREADS = 1024;
-__global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl, double *__restrict__ tab,
-                                                                   double mu, double beta, int k, int m)
+__global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl, double mu, double beta, int k, int m)
 {
-    __shared__ double s_f[2 * BML_CHEB_MAX_TERMS];     // f at the nodes
-    __shared__ double s_p[BML_CHEB_MAX_TERMS];         // dividend of the current division step
+    // dynamic shared memory, cheb_coeff_smem_bytes(k m): node values, the two division buffers and the cosine table
+    // (every lane of a warp reads a different entry of it)
+    extern __shared__ double s_dyn[];
     const int terms = k * m, Nq = 2 * terms;
+    double *s_f = s_dyn;                   // [N_q]      f at the nodes
+    double *s_p = s_f + Nq;                // [terms]    dividend of the current division step
+    double *s_q = s_p + terms;             // [terms]    its quotient
+    double *tab = s_q + terms;             // [4 N_q]    cos(pi j / (2 N_q))
     const double emin = ctl->bounds[0], emax = ctl->bounds[1];
     if (threadIdx.x == 0) ctl->fail = (emax - emin > 0.0) ? 0 : BML_ERR_DEGENERATE;
     // exact angles: every cosine needed is cos(pi j / (2 N_q)) with an integer j reduced mod 4 N_q
     for (int j = threadIdx.x; j < 4 * Nq; j += CC_THREADS) tab[j] = cospi((double)j / (double)(2 * Nq));
     __syncthreads();
-    for (int q = threadIdx.x; q < Nq; q += CC_THREADS) {
-        const double x = tab[2 * q + 1];                                // cos(pi (q + 1/2) / N_q)
-        s_f[q] = fermi_fn(0.5 * (emax - emin) * x + 0.5 * (emax + emin), mu, beta);
+    // f at the nodes, folded: cos(n pi (N_q - q - 1/2) / N_q) = (-1)^n cos(n pi (q + 1/2) / N_q), so the sum over the
+    // N_q nodes is a sum over the first N_q / 2 of f_q +- f_{N_q-1-q} (N_q is even).  This O(L N_q) loop runs on ONE SM
+    // and is issue-bound (4 schedulers): the fold halves it.  s_f[q] = f_q + f_mirror, s_f[N_q/2 + q] = f_q - f_mirror.
+    const int Nh = Nq / 2;
+    for (int q = threadIdx.x; q < Nh; q += CC_THREADS) {
+        const double x = tab[2 * q + 1];                                // cos(pi (q + 1/2) / N_q); the mirror node is -x
+        const double fa = fermi_fn(0.5 * (emax - emin) * x + 0.5 * (emax + emin), mu, beta);
+        const double fb = fermi_fn(-0.5 * (emax - emin) * x + 0.5 * (emax + emin), mu, beta);
+        s_f[q] = fa + fb;
+        s_f[Nh + q] = fa - fb;
     }
     __syncthreads();
-    // one warp per coefficient, the N_q nodes dealt out to its lanes: j = n (2 q + 1) mod 4 N_q, advanced by 64 n
+    // one warp per coefficient, the N_q / 2 nodes dealt out to its lanes: table index j = n (2 q + 1) mod 4 N_q,
+    // advanced by 64 n
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int n = warp; n < terms; n += CC_THREADS / 32) {
         const unsigned period = (unsigned)(4 * Nq);
         unsigned j = ((unsigned)n * (2u * (unsigned)lane + 1u)) % period;
         const unsigned step = (64u * (unsigned)n) % period;
+        const double *fs = s_f + ((n & 1) ? Nh : 0);
         double s = 0.0;
-        for (int q = lane; q < Nq; q += 32) {
-            s = fma(s_f[q], tab[j], s);
+        for (int q = lane; q < Nh; q += 32) {
+            s = fma(fs[q], tab[j], s);
             j += step;
             if (j >= period) j -= period;
         }
@@ -77,27 +89,30 @@ __global__ void __launch_bounds__(CC_THREADS, 1) cheb_coeff_kernel(ChebCtl *ctl,
     // Going down from the highest n, p_n is final once p_{n+2k} has been subtracted from it, so the 2k residue classes
     // of n mod 2k are independent chains (one thread each); the reflected targets |n - 2k| = 2k - n, k < n < 2k, come
     // after the chains.  Every p_i sees the same subtractions in the same order as in the one-thread loop.
+    // Only the first two warps take part (2k <= 64 chains), synchronised by a named barrier of 64 threads: a barrier of
+    // the whole 1024-thread CTA per phase was most of this kernel's time.  The quotient is built in a second buffer.
     const int tid = threadIdx.x;
+    if (tid >= 64) return;
+    auto bar64 = []() { asm volatile("bar.sync 1, 64;" ::: "memory"); };
+    double *pp = s_p, *qq = s_q;
     int len = terms;
     for (int j = 0; j < m; ++j) {
         const int qlen = len - k;
         if (tid < 2 * k && tid < len) {
             int n = tid + (len - 1 - tid) / (2 * k) * (2 * k);           // largest index of this class below len
-            double above = s_p[n];
+            double above = pp[n];
             for (n -= 2 * k; n >= 0; n -= 2 * k) {
-                above = s_p[n] - above;
-                s_p[n] = above;
+                above = pp[n] - above;
+                pp[n] = above;
             }
         }
-        __syncthreads();
-        if (tid > 0 && tid < k && 2 * k - tid < len) s_p[tid] -= s_p[2 * k - tid];
-        __syncthreads();
-        if (tid < k) ctl->d[j * k + tid] = s_p[tid];
-        double qv = 0.0;
-        if (tid < qlen) qv = (tid == 0) ? s_p[k] : 2.0 * s_p[tid + k];
-        __syncthreads();
-        if (tid < qlen) s_p[tid] = qv;
-        __syncthreads();
+        bar64();
+        if (tid > 0 && tid < k && 2 * k - tid < len) pp[tid] -= pp[2 * k - tid];
+        bar64();
+        if (tid < k) ctl->d[j * k + tid] = pp[tid];
+        for (int i = tid; i < qlen; i += 64) qq[i] = (i == 0) ? pp[k] : 2.0 * pp[i + k];
+        bar64();
+        double *t = pp; pp = qq; qq = t;
         len = qlen;
     }
 }
@@ -124,6 +139,21 @@ __global__ void cheb_map_kernel(const double *__restrict__ H, int64_t ldh, doubl
 // computes the S_j as m separate sums on concurrent streams.  HBM-bound: (k - 1 + m) N^2 x 8 B.
 // slab: slot s holds the matrix at slab + s * slot_elems; T_i in slot i - 1, S_j in slot k + j.
 // ------------------------------------------------------------------------------------------------------------
+static size_t cheb_coeff_smem_bytes(int terms) { return (size_t)(2 + 1 + 1 + 8) * (size_t)terms * sizeof(double); }
+
+static int launch_cheb_coeff(ChebCtl *ctl, double mu, double beta, int k, int m, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(cheb_coeff_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)cheb_coeff_smem_bytes(BML_CHEB_MAX_TERMS)) != cudaSuccess)
+            return BML_ERR_CUDA;
+        attr_set = true;
+    }
+    cheb_coeff_kernel<<<1, CC_THREADS, cheb_coeff_smem_bytes(k * m), st>>>(ctl, mu, beta, k, m);
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
 template <int MJ, int CW>
 __global__ void __launch_bounds__(256, (MJ * CW <= 16) ? 4 : 2)
 cheb_sums_kernel(double *__restrict__ slab, int64_t slot_elems, int64_t ld, int N, int k, int m,
@@ -210,14 +240,13 @@ int cheb_schedule(int k, int32_t *level, int32_t *a, int32_t *b)
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct ChebWs {
-    uint8_t *ctl0;          // P control blocks, CHEB_CTL_STRIDE bytes apart; each followed by its cosine table
+    uint8_t *ctl0;          // P control blocks, CHEB_CTL_STRIDE bytes apart
     double *rowlh;
     void *sk;
     double *slab;           // P x (k + m) slots: problem q owns slots q (k + m) .. ; T_i at +i - 1, S_j at +k + j
     int64_t ld, slot_elems;
     size_t total;
     ChebCtl *ctl(int q) const { return (ChebCtl *)(ctl0 + (size_t)q * CHEB_CTL_STRIDE); }
-    double *tab(int q) const { return (double *)(ctl0 + (size_t)q * CHEB_CTL_STRIDE + CHEB_CTL_BYTES); }
 };
 
 static ChebWs carve_cheb(void *ws, int64_t N, int k, int m, int P)
@@ -255,7 +284,7 @@ int cheb_dense_enqueue_batch(int P, const bml_matrix_t *H, const bml_cheb_params
         if (cudaMemsetAsync(w.ctl(q), 0, 64, st) != cudaSuccess) return BML_ERR_CUDA;
         CK(launch_gershgorin(&H[q], w.ctl(q)->bounds, w.rowlh, st));
         if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) CK(launch_check_symmetry(&H[q], &w.ctl(q)->not_symmetric, st));
-        cheb_coeff_kernel<<<1, CC_THREADS, 0, st>>>(w.ctl(q), w.tab(q), p->mu, p->beta, k, m);
+        CK(launch_cheb_coeff(w.ctl(q), p->mu, p->beta, k, m, st));
         const dim3 grid((unsigned)((N + 255) / 256), (unsigned)(N < 2048 ? N : 2048));
         cheb_map_kernel<<<grid, 256, 0, st>>>(H[q].value, H[q].ld, slot(q, 0), w.ld, (int)N, w.ctl(q));
         if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA;
