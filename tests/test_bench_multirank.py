@@ -69,3 +69,27 @@ def test_reference_arm_runs_on_rank0_only(monkeypatch, capsys):
 
     assert bench.run_reference(A) == 0
     assert capsys.readouterr().out == ""
+
+
+@pytest.mark.parametrize("workload,metric", [("dense_n256", "sp2_time_to_D_ms"), ("cheby_n500", "chebyshev_time_to_D_ms")])
+def test_reference_arm_prints_the_contract_line(monkeypatch, capsys, workload, metric):
+    """--impl reference on rank 0 (no GPU needed: it times the oracle): one JSON line with the reference-arm keys."""
+    import json
+
+    sys.path.insert(0, ROOT)
+    import bench
+
+    monkeypatch.setenv("RANK", "0")
+
+    class A:
+        steps, warmup, gpus = 1, 0, 1
+
+    A.workload = workload
+    assert bench.run_reference(A) == 0
+    lines = [l for l in capsys.readouterr().out.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == metric and d["unit"] == "ms" and d["value"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
+    assert d["e2e"] == {"value": d["value"], "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert d["config"]["workload"] == workload and d["gpu_launches"] == 0
