@@ -459,25 +459,38 @@ def run_ours(args):
         def solve(Hd):
             return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, 100, flags=sp2_flags)
 
-    # ---- device-resident timing: W warm-ups, then exactly K timed steps
-    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
-    ms = float(np.mean(step_ms))
+    # Small dense matrices run on a stream of their own: the library replays the static head of such a solve as a CUDA
+    # graph, which the legacy default stream cannot capture.  Everything else stays on the current stream.
+    import contextlib
 
-    # ---- e2e: host buffers through the public API; H2D of H and D2H of D inside the timed region
-    def e2e_step():
-        if dense:
-            D, _ = solve(H_host.to(dev, non_blocking=True))
-            D_host.copy_(D, non_blocking=True)
-        else:
-            D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
-            for dst, src in zip(D_host, D):
-                dst.copy_(src, non_blocking=True)
-        torch.cuda.synchronize()
+    side = torch.cuda.Stream(dev) if (dense and w.N <= 1024) else None
+    if side is not None:
+        side.wait_stream(torch.cuda.current_stream())
+    with (torch.cuda.stream(side) if side is not None else contextlib.nullcontext()):
+        # ---- device-resident timing: W warm-ups, then exactly K timed steps
+        step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
+        ms = float(np.mean(step_ms))
 
-    e2e_steps = max(3, min(args.steps, 10))
-    h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
-    d2h = h2d
-    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
+        # ---- e2e: host buffers through the public API; H2D of H and D2H of D inside the timed region
+        H_in = torch.empty_like(H_dev) if dense else None
+
+        def e2e_step():
+            if dense:
+                H_in.copy_(H_host, non_blocking=True)
+                D, _ = solve(H_in)
+                D_host.copy_(D, non_blocking=True)
+            else:
+                D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
+                for dst, src in zip(D_host, D):
+                    dst.copy_(src, non_blocking=True)
+            torch.cuda.synchronize()
+
+        e2e_steps = max(3, min(args.steps, 10))
+        h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
+        d2h = h2d
+        e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
+    if side is not None:
+        torch.cuda.current_stream().wait_stream(side)
 
     # ---- dominant kernel, timed alone with CUDA events on the launching stream
     pk, pk_src = peaks()

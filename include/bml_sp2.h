@@ -150,7 +150,9 @@ BML_API int bml_trace(const bml_matrix_t *A, double *d_trace, void *cuda_stream)
  * d_workspace: DEVICE scratch, >= bml_sp2_workspace_bytes(H, p) bytes, 1024-byte aligned.
  * stats: HOST, may be NULL (the status is still returned; the call still synchronises once at its end).
  * The whole solve is enqueued without any host round trip per product: the branch bit, the stop test and the
- * ping-pong buffer selection live in a device-resident control block.
+ * ping-pong buffer selection live in a device-resident control block.  Dense FP64, N <= 1024, not on the legacy default
+ * stream: the launches up to and including the first batch of products are captured once per argument set and replayed
+ * as a CUDA graph by later calls with the same pointers, shapes and parameters; results are identical.
  */
 BML_API size_t bml_sp2_workspace_bytes(const bml_matrix_t *H, const bml_sp2_params_t *p);
 BML_API int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,

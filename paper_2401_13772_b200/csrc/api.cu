@@ -223,6 +223,74 @@ static int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
     return h.status;
 }
 
+// CUDA-graph replay of the static head of a small dense FP64 solve (prelude + first batch of product launches).
+// Same rules as the Chebyshev replay (chebyshev.cu): N <= 1024, not while capturing, not on the legacy default stream,
+// the first solve of a tile size runs plainly (it sets kernel attributes), failures fall back to plain enqueueing.
+struct Sp2GraphKey {
+    const void *H, *ws;
+    int64_t N, ldh;
+    double idem_tol;
+    int32_t n_occ, max_products;
+    uint32_t flags;
+    cudaStream_t st;
+    bool operator==(const Sp2GraphKey &o) const
+    {
+        return H == o.H && ws == o.ws && N == o.N && ldh == o.ldh && idem_tol == o.idem_tol && n_occ == o.n_occ &&
+               max_products == o.max_products && flags == o.flags && st == o.st;
+    }
+};
+struct Sp2GraphSlot {
+    Sp2GraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    uint64_t stamp = 0;
+};
+
+template <class EnqueueFn>
+static int sp2_first_batch_cached(const Sp2GraphKey &key, EnqueueFn &&enqueue)
+{
+    static thread_local Sp2GraphSlot slots[4];
+    static thread_local uint64_t clock_ = 0;
+    static thread_local bool warmed[2] = {false, false};
+    cudaStream_t st = key.st;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const bool capturing = cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
+    const int bti = key.N <= 512 ? 0 : 1;
+    if (key.N > 1024 || capturing || st == nullptr || !warmed[bti]) {
+        if (key.N <= 1024) warmed[bti] = true;
+        return enqueue();
+    }
+    Sp2GraphSlot *hit = nullptr, *victim = &slots[0];
+    for (auto &sl : slots) {
+        if (sl.exec && sl.key == key) hit = &sl;
+        if (sl.stamp < victim->stamp) victim = &sl;
+    }
+    if (!hit) {
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            return enqueue();
+        }
+        const int r = enqueue();
+        const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+        cudaGraphExec_t exec = nullptr;
+        if (r != 0 || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            return enqueue();
+        }
+        cudaGraphDestroy(graph);
+        if (victim->exec) cudaGraphExecDestroy(victim->exec);
+        victim->key = key; victim->exec = exec;
+        hit = victim;
+    }
+    hit->stamp = ++clock_;
+    if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) {
+        cudaGetLastError();
+        return enqueue();
+    }
+    return 0;
+}
+
 }  // namespace bmlsp2
 
 using namespace bmlsp2;
@@ -308,24 +376,43 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
     if (workspace_bytes < w.total) TRY(BML_ERR_INVALID);
     cudaStream_t st = (cudaStream_t)cuda_stream;
 
-    if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) TRY(BML_ERR_CUDA);
-    TRY(launch_gershgorin(H, w.scal->bounds, w.rowlh, st));                                   // D0
-    if (lanczos_steps(p->flags)) TRY(launch_lanczos_bounds(H, lanczos_steps(p->flags), 0, w.scal->bounds, w.rowlh, st));
-    if (p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) TRY(launch_check_symmetry(H, w.scal->fail_flag, st));
-    TRY(launch_rescale_dense(H, w.scal->bounds, w.X0, w.ldx, st));                            // D1
-    TRY(launch_trace_dense(w.X0, w.ldx, (int)N, &w.scal->tr0, st));
-    TRY(launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
-                        w.scal->fail_flag, st));
+    // D0 + D1 + control block: everything before the first product
+    auto prelude = [&]() -> int {
+        int r;
+        if (cudaMemsetAsync(w.scal, 0, SCAL_BYTES, st) != cudaSuccess) return BML_ERR_CUDA;
+        if ((r = launch_gershgorin(H, w.scal->bounds, w.rowlh, st))) return r;                    // D0
+        if (lanczos_steps(p->flags) &&
+            (r = launch_lanczos_bounds(H, lanczos_steps(p->flags), 0, w.scal->bounds, w.rowlh, st)))
+            return r;
+        if ((p->flags & BML_SP2_FLAG_CHECK_SYMMETRY) && (r = launch_check_symmetry(H, w.scal->fail_flag, st))) return r;
+        if ((r = launch_rescale_dense(H, w.scal->bounds, w.X0, w.ldx, st))) return r;             // D1
+        if ((r = launch_trace_dense(w.X0, w.ldx, (int)N, &w.scal->tr0, st))) return r;
+        return launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
+                               w.scal->fail_flag, st);
+    };
     if (p->precision != 0) {
+        TRY(prelude());
         TRY(sp2_dense_mixed_solve(H, p, w.X0, w.X1, w.ldx, w.ctl, w.partials, w.scal->bounds, w.extra, st));
     } else {
         CUtensorMap map0, map1;
         TRY(make_dense_map(&map0, w.X0, N, w.ldx));
         TRY(make_dense_map(&map1, w.X1, N, w.ldx));
-        // D2-D5: products are enqueued ahead of the device; launches after the stop rule fired exit at once
-        TRY(dense_fp64_sk_reset(w.sk, N, st));
-        TRY(enqueue_products([&]() { return launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, w.sk, st); },
-                             w.ctl, p->max_products, st));
+        auto launch_one = [&]() { return launch_x2_dense_fp64(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, w.sk, st); };
+        // D2-D5: products are enqueued ahead of the device; launches after the stop rule fired exit at once.
+        // Small matrices: the prelude and the first batch of launches are launch-latency bound and form a static
+        // sequence, replayed as a CUDA graph when the stream allows it (sp2_first_batch_cached).
+        const int n_first = p->max_products < ENQ_FIRST ? p->max_products : ENQ_FIRST;
+        auto first_batch = [&]() -> int {
+            int r = prelude();
+            if (r) return r;
+            if ((r = dense_fp64_sk_reset(w.sk, N, st))) return r;
+            for (int l = 0; l < n_first; ++l)
+                if ((r = launch_one())) return r;
+            return 0;
+        };
+        const Sp2GraphKey key = {H->value, d_workspace, N, H->ld, p->idem_tol, p->n_occ, p->max_products, p->flags, st};
+        TRY(sp2_first_batch_cached(key, first_batch));
+        TRY(enqueue_products(launch_one, w.ctl, p->max_products, st, n_first));
     }
     TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
     return finish_solve(w.ctl, stats, st);

@@ -250,15 +250,16 @@ struct EnqueueState {
 
 EnqueueState &enqueue_state();      // api.cu: one per host thread
 
+// `already`: product launches of the first batch that are in the stream already (a replayed CUDA graph, api.cu).
 template <class LaunchFn>
-static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_products, cudaStream_t st)
+static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_products, cudaStream_t st, int already = 0)
 {
     EnqueueState &es = enqueue_state();
     if (!es.ok) {                       // no pinned memory / events: plain enqueue of everything
-        for (int l = 0; l < max_products; ++l) { int r = launch_one(); if (r) return r; }
+        for (int l = already; l < max_products; ++l) { int r = launch_one(); if (r) return r; }
         return 0;
     }
-    int enq = 0, batch = 0;
+    int enq = already, batch = 0;
     auto enqueue_batch = [&](int n) -> int {
         for (int l = 0; l < n && enq < max_products; ++l, ++enq) { int r = launch_one(); if (r) return r; }
         const int slot = batch % ENQ_RING;
@@ -268,7 +269,7 @@ static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_produc
         ++batch;
         return 0;
     };
-    int r = enqueue_batch(ENQ_FIRST);
+    int r = enqueue_batch(ENQ_FIRST - already);
     if (r) return r;
     while (enq < max_products) {
         if ((r = enqueue_batch(ENQ_BATCH))) return r;          // one batch ahead ...

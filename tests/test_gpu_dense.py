@@ -291,3 +291,37 @@ def test_sp2_square_kernel_many_launches_bit_reproducible(api):
         for it in range(300):
             _, sums = api.bml_x2_dense(X, 0, 0, Xn, ws)
             assert torch.equal(Xn, ref), f"N={N}: launch {it} differs"
+
+
+def test_sp2_small_matrix_graph_replay_on_a_side_stream(api, oracle_mod):
+    """On a non-default stream the prelude and the first batch of product launches of a small dense solve are captured
+    once and replayed as a CUDA graph (api.cu): replays give the bits of the plainly enqueued solve, also when the
+    input content changes under the same pointers, with and without the Lanczos flag, and for solves that need more
+    products than the first batch holds."""
+    import torch
+
+    cases = [(hm.make_dense("dense_n256"), 128, 1e-10), (hm.small_long_range((8, 8, 6)), 192, 1e-10)]
+    side = torch.cuda.Stream()
+    for H1, n_occ, tol in cases:
+        H2 = H1 + np.diag(np.linspace(-0.05, 0.05, H1.shape[0]))
+        refs = []
+        for Hx in (H1, H2):
+            D, r = api.bml_sp2_dense(to_gpu(Hx), n_occ, tol)          # default stream: plain enqueue
+            refs.append((D.clone(), r))
+        assert refs[1][1].n_products > 16 or H1.shape[0] == 256      # the long-range case outlasts the first batch
+        solver = api.DenseSolver(H1.shape[0], "cuda", 0)
+        Hbuf = to_gpu(H1)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            for it in range(6):
+                Hbuf.copy_(to_gpu(H1 if it % 2 == 0 else H2))
+                D, r = solver.solve(Hbuf, n_occ, tol)
+                D0, r0 = refs[it % 2]
+                assert r.status == r0.status == 0 and r.branch == r0.branch and r.n_products == r0.n_products
+                assert np.array_equal(r.idem, r0.idem)
+                assert torch.equal(D, D0), f"replay {it}"
+            Dl, rl = solver.solve(Hbuf, n_occ, tol, flags=api.FLAG_LANCZOS_BOUNDS(16))
+            Dl2, rl2 = solver.solve(Hbuf, n_occ, tol, flags=api.FLAG_LANCZOS_BOUNDS(16))
+            assert rl.status == 0 and rl.branch == rl2.branch and (rl.emin, rl.emax) == (rl2.emin, rl2.emax)
+            assert rl.n_products <= refs[1][1].n_products
+        torch.cuda.synchronize()
