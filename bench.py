@@ -55,6 +55,8 @@ NCU_TRAFFIC_BYTES = {
     "mixed_n16384": 20.4e9,         # 17.2 GB read + 3.2 GB written (FP16 x 2 planes, super-block tile order)
     "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (capture quoted in DESIGN.md 5.3)
     "cheby_n2000": 98.1e6,          # grouped product kernel, one Eq. 10 step: 85.3 MB read + 12.8 MB written
+    "cheby_n4000": 891.3e6,         # one Eq. 10 step: 766.1 MB read + 125.2 MB written (512 MB algorithmic)
+    "graph_n12800": 1.84e9,         # per product at part size 5600 (captured launch: 4 products, 6.36 GB + 1.00 GB)
     "ellpack_n65536": 1.25e9,       # kernel 1: 0.246 + 0.190 GB; kernel 2: 0.451 + 0.363 GB (read + written)
 }
 
