@@ -72,6 +72,11 @@ def test_sass_contains_the_blackwell_instructions():
     # the mixed-precision path must be tcgen05 MMAs with TMEM accumulators read back by tcgen05.ld
     assert "UTCHMMA" in sass
     assert "LDTM" in sass
+    # every kernel family of the three headers is in the image
+    for kernel in ("x2_dense_fp64_sk_kernel", "x2_dense_mixed_kernel", "x2_ellpack_upper_kernel", "symm_ab_fp64_kernel",
+                   "cheb_coeff_kernel", "cheb_sums_kernel", "graph_gather_kernel", "graph_scatter_kernel",
+                   "lanczos_update_kernel"):
+        assert kernel in sass, kernel
 
 
 def test_product_and_oracle_do_not_import_each_other():
