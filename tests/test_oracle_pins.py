@@ -341,3 +341,26 @@ def test_config5_literal_overflows_at_product0_with_fill_829(oracle_mod):
     assert bad == -1
     pv, pi, pn, bad, mx = oracle_mod.x2_ellpack(xv, xi, xn, 1e-6)
     assert bad == 0 and mx == 829
+
+
+# ------------------------------------------------------------------ rule R1 == variant R2 -------------
+@pytest.mark.parametrize("seed,N,n_occ", [(21, 48, 7), (22, 48, 24), (23, 61, 50)])
+def test_rule_R1_picks_the_candidate_whose_trace_is_nearer_n_occ(oracle_mod, seed, N, n_occ):
+    """DESIGN.md reading 4: with a = tr X - n_occ and d = tr X - tr X^2 >= 0 the two candidates of Eq. 6-7 have traces
+    n_occ + a - d (X^2) and n_occ + a + d (2X - X^2), so "take the candidate whose trace is nearer n_occ" (variant R2 of
+    P:169's "other variants") is a < 0 => 2X - X^2, a > 0 => X^2: Listing 2's rule except on the tie a = 0.
+    Brute force: replay the oracle's branch string with numpy and form BOTH candidates at every step."""
+    H, _ = hm.planted_gap(N, n_occ, gap=0.6, width=4.0, seed=seed)
+    D, st = oracle_mod.sp2_dense(H, n_occ, 1e-10)
+    assert st["status"] == 0
+    X = (st["emax"] * np.eye(N) - H) / (st["emax"] - st["emin"])
+    for m in range(st["m_star"]):
+        P = X @ X
+        cand = (P, 2.0 * X - P)                        # b = 0, b = 1
+        dist = [abs(np.trace(c) - n_occ) for c in cand]
+        b = int(st["branch"][m])
+        assert dist[b] <= dist[1 - b]
+        assert abs(np.trace(X) - st["trace"][m]) <= 1e-10
+        assert np.trace(X) - np.trace(P) >= -1e-12     # d >= 0: the spectrum of X lies in [0, 1]
+        X = cand[b]
+    assert relfro(X, D) <= 1e-10
