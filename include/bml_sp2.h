@@ -129,7 +129,8 @@ BML_API int bml_gershgorin(const bml_matrix_t *H, double *d_bounds, void *d_work
  * seed tried (with 2-4 steps an outlying band can be missed, so steps < 8 is rejected); if it fails SP2 does not
  * converge and ends with BML_MAX_PRODUCTS.  steps in 8..64.  H dense or ellpack.
  * d_bounds: DEVICE double[2] <- {e_min, e_max}.  d_workspace >= bml_lanczos_bounds_workspace_bytes(N), 8-byte aligned.
- * Asynchronous.  Returns 0, -1 or -4.
+ * One persistent cooperative launch (one CTA per SM) runs the whole recursion; the device must support cooperative
+ * launches (else -4).  Asynchronous.  Returns 0, -1 or -4.
  */
 BML_API size_t bml_lanczos_bounds_workspace_bytes(int64_t N);
 BML_API int bml_lanczos_bounds(const bml_matrix_t *H, int32_t steps, uint64_t seed, double *d_bounds, void *d_workspace,

@@ -1,10 +1,15 @@
 // bounds.cu -- optional tighter spectral bounds for Eq. 5 (readings B1-B3): K steps of
 // the Lanczos recursion on H from a counter-based start vector, the extreme Ritz values of the K x K tridiagonal matrix
 // widened by their residual norms and a 1% pad, intersected with the Gershgorin bounds already in d_bounds.
-// Two launches per step (matrix-vector product; one-CTA vector update with full reorthogonalisation and fixed-order
-// reductions), one finishing
-// thread for the tridiagonal eigenproblem.  Everything stays on the device.
+// One persistent cooperative launch runs the whole recursion (matrix-vector products, vector updates with full
+// reorthogonalisation, every scalar product as fixed-order per-CTA partials behind a grid barrier); one finishing
+// thread then solves the tridiagonal eigenproblem.  Everything stays on the device.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+#include "dense_fp64_core.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace bmlsp2 {
 
@@ -29,114 +34,132 @@ __device__ __forceinline__ double lz_uniform(uint64_t x)
     return 2.0 * ((double)(z >> 11) * 0x1.0p-53) - 1.0;
 }
 
-// fixed-order block sum (all threads get the result)
-__device__ __forceinline__ double lz_block_sum(double v, double *s_part)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    v = warp_sum(v);
-    __syncthreads();
-    if (lane == 0) s_part[warp] = v;
-    __syncthreads();
-    double t = 0.0;
-#pragma unroll
-    for (int w = 0; w < LZ_THREADS / 32; ++w) t += s_part[w];
-    return t;
-}
+// ------------------------------------------------------------------------------------------------------------
+// The whole recursion is ONE persistent cooperative launch (one CTA per SM).  CTA c owns the contiguous index range
+// [c chunk, (c + 1) chunk) of every vector; a scalar product is per-CTA partial sums -> grid barrier -> every CTA adds
+// the G partials in the same fixed order, so all CTAs hold bitwise identical alpha, c_q, beta and take the same
+// branches (no broadcast, no atomics; results are bit-reproducible).  Each phase writes its partials to a region
+// of its own (a fast CTA may already write the next phase's while a slow one still reads this one's).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int LZ_REG_ALPHA = 0, LZ_REG_PASS0 = 1, LZ_REG_PASS1 = 1 + LZ_MAX_STEPS, LZ_REG_NORM = 1 + 2 * LZ_MAX_STEPS;
+constexpr int LZ_PART_ROWS = 2 + 2 * LZ_MAX_STEPS;          // rows of G partials each
+constexpr int LZ_MAX_GRID = 256;
 
-__global__ void __launch_bounds__(LZ_THREADS) lanczos_start_kernel(double *__restrict__ v, int N, uint64_t seed,
-                                                                   LanczosCtl *__restrict__ ctl)
+// part[(row0 + q) G + cta] = sum over this CTA's index range of V[q][i] w[i], q = q0 .. q1: one warp per q
+__device__ __forceinline__ void lz_partial_dots(const double *V, const double *w, int N, int q0, int q1, int i0, int i1,
+                                                double *part, int row0, int G)
 {
-    __shared__ double s_part[LZ_THREADS / 32];
-    double acc = 0.0;
-    for (int i = threadIdx.x; i < N; i += LZ_THREADS) {
-        const double u = lz_uniform(seed + (uint64_t)i);
-        v[i] = u;
-        acc += u * u;
+    const int lane = threadIdx.x & 31;
+    for (int q = q0 + (threadIdx.x >> 5); q <= q1; q += LZ_THREADS / 32) {
+        const double *vq = V + (size_t)q * N;
+        double a = 0.0;
+        for (int i = i0 + lane; i < i1; i += 32) a = fma(vq[i], w[i], a);
+        a = warp_sum(a);
+        if (lane == 0) part[(size_t)(row0 + q) * G + blockIdx.x] = a;
     }
-    const double inv = 1.0 / sqrt(lz_block_sum(acc, s_part));
-    for (int i = threadIdx.x; i < N; i += LZ_THREADS) v[i] *= inv;
-    if (threadIdx.x == 0) { ctl->steps = 0; ctl->stopped = 0; ctl->beta[0] = 0.0; }
+}
+// s_c[q] = sum over CTAs (lane-strided, then the shuffle tree: the same order in every CTA), q = q0 .. q1
+__device__ __forceinline__ void lz_gather(const double *part, int row0, int q0, int q1, int G, double *s_c)
+{
+    const int lane = threadIdx.x & 31;
+    for (int q = q0 + (threadIdx.x >> 5); q <= q1; q += LZ_THREADS / 32) {
+        double a = 0.0;
+        for (int c = lane; c < G; c += 32) a += part[(size_t)(row0 + q) * G + c];
+        a = warp_sum(a);
+        if (lane == 0) s_c[q] = a;
+    }
+    __syncthreads();
 }
 
-// w = H v, one warp per row
-__global__ void __launch_bounds__(256) lanczos_matvec_dense_kernel(const double *__restrict__ H, int64_t ld, int N,
-                                                                   const double *__restrict__ V, double *__restrict__ w,
-                                                                   const LanczosCtl *__restrict__ ctl)
+// Recursion per step j (the oracle's order, oracle/bounds.py): w = H v_j;  alpha_j = v_j.w;
+// w -= alpha_j v_j + beta_j v_{j-1};  two passes of classical Gram-Schmidt against v_0 .. v_j (reading B3: without them
+// the recursion loses orthogonality once an extreme Ritz value converges and the residual term of the other end is
+// reproducible to two digits only);  beta_{j+1} = ||w||;  v_{j+1} = w / beta_{j+1}.  V holds the Lanczos vectors,
+// row j = v_j.  H is dense (hi == nullptr: hv = values, ld) or ELLPACK-R (hv, hi, hn, ld = M).
+__global__ void __launch_bounds__(LZ_THREADS, 1)
+lanczos_run_kernel(const double *__restrict__ hv, const int32_t *__restrict__ hi, const int32_t *__restrict__ hn, int64_t ld,
+                   int N, int steps, uint64_t seed, double *V, double *w, double *part, LanczosCtl *ctl)
 {
-    if (ctl->stopped) return;
-    const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (r >= N) return;
-    const double *__restrict__ v = V + (size_t)ctl->steps * N;
-    const double *row = H + (int64_t)r * ld;
-    double acc = 0.0;
-    for (int j = lane; j < N; j += 32) acc = fma(row[j], v[j], acc);
-    acc = warp_sum(acc);
-    if (lane == 0) w[r] = acc;
-}
-__global__ void __launch_bounds__(256) lanczos_matvec_ellpack_kernel(const double *__restrict__ hv,
-                                                                     const int32_t *__restrict__ hi,
-                                                                     const int32_t *__restrict__ hn, int N, int M,
-                                                                     const double *__restrict__ V, double *__restrict__ w,
-                                                                     const LanczosCtl *__restrict__ ctl)
-{
-    if (ctl->stopped) return;
-    const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (r >= N) return;
-    const double *__restrict__ v = V + (size_t)ctl->steps * N;
-    const int n = hn[r];
-    double acc = 0.0;
-    for (int p = lane; p < n; p += 32) acc = fma(hv[(size_t)r * M + p], v[hi[(size_t)r * M + p]], acc);
-    acc = warp_sum(acc);
-    if (lane == 0) w[r] = acc;
-}
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double s_c[LZ_MAX_STEPS + 1];
+    const int G = gridDim.x, lane = threadIdx.x & 31;
+    const int chunk = (N + G - 1) / G;
+    const int i0 = min(N, (int)blockIdx.x * chunk), i1 = min(N, i0 + chunk);
+    const int gwarp = (blockIdx.x * LZ_THREADS + threadIdx.x) >> 5, nwarps = G * (LZ_THREADS / 32);
 
-// alpha_j = v_j.w;  w -= alpha_j v_j + beta_j v_{j-1};  two passes of classical Gram-Schmidt against v_0 .. v_j (reading
-// B3: without them the recursion loses orthogonality once an extreme Ritz value converges and the residual term of the
-// other end is reproducible to two digits only);  beta_{j+1} = ||w||;  v_{j+1} = w / beta_{j+1}.
-// V holds the Lanczos vectors, row j = v_j.  One CTA; every reduction in a fixed order.
-__global__ void __launch_bounds__(LZ_THREADS) lanczos_update_kernel(double *__restrict__ V, double *__restrict__ w, int N,
-                                                                    LanczosCtl *__restrict__ ctl)
-{
-    __shared__ double s_part[LZ_THREADS / 32];
-    __shared__ double s_c[LZ_MAX_STEPS];
-    if (ctl->stopped) return;
-    const int j = ctl->steps;
-    const double beta_j = ctl->beta[j];
-    const double *v = V + (size_t)j * N, *v_prev = V + (size_t)(j > 0 ? j - 1 : 0) * N;
-    double acc = 0.0;
-    for (int i = threadIdx.x; i < N; i += LZ_THREADS) acc = fma(v[i], w[i], acc);
-    const double alpha = lz_block_sum(acc, s_part);
-    for (int i = threadIdx.x; i < N; i += LZ_THREADS) w[i] = w[i] - alpha * v[i] - (j > 0 ? beta_j * v_prev[i] : 0.0);
-    for (int pass = 0; pass < 2; ++pass) {
-        __syncthreads();
-        // one warp per previous vector: c_q = v_q . w (lane-strided partial sums, then the shuffle tree: fixed order)
-        for (int q = threadIdx.x >> 5; q <= j; q += LZ_THREADS / 32) {
-            const double *vq = V + (size_t)q * N;
-            double a = 0.0;
-            for (int i = threadIdx.x & 31; i < N; i += 32) a = fma(vq[i], w[i], a);
-            a = warp_sum(a);
-            if ((threadIdx.x & 31) == 0) s_c[q] = a;
+    // start vector: counter-based uniform numbers, normalised
+    for (int i = i0 + threadIdx.x; i < i1; i += LZ_THREADS) V[i] = lz_uniform(seed + (uint64_t)i);
+    __syncthreads();
+    lz_partial_dots(V, V, N, 0, 0, i0, i1, part, LZ_REG_NORM, G);
+    grid.sync();
+    lz_gather(part, LZ_REG_NORM, 0, 0, G, s_c);
+    {
+        const double inv = 1.0 / sqrt(s_c[0]);
+        for (int i = i0 + threadIdx.x; i < i1; i += LZ_THREADS) V[i] *= inv;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) { ctl->steps = 0; ctl->stopped = 0; ctl->beta[0] = 0.0; }
+    grid.sync();
+
+    double beta_j = 0.0;
+    for (int j = 0; j < steps; ++j) {
+        const double *v = V + (size_t)j * N, *v_prev = V + (size_t)(j > 0 ? j - 1 : 0) * N;
+        // w = H v_j: one warp per row, rows dealt round-robin over all warps of the grid
+        if (hi == nullptr) {
+            for (int r = gwarp; r < N; r += nwarps) {
+                const double *__restrict__ row = hv + (int64_t)r * ld;
+                double acc = 0.0;
+#pragma unroll 8
+                for (int c = lane; c < N; c += 32) acc = fma(row[c], v[c], acc);
+                acc = warp_sum(acc);
+                if (lane == 0) w[r] = acc;
+            }
+        } else {
+            for (int r = gwarp; r < N; r += nwarps) {
+                const int n = hn[r];
+                double acc = 0.0;
+                for (int p = lane; p < n; p += 32) acc = fma(hv[(size_t)r * ld + p], v[hi[(size_t)r * ld + p]], acc);
+                acc = warp_sum(acc);
+                if (lane == 0) w[r] = acc;
+            }
+        }
+        grid.sync();
+        lz_partial_dots(V, w, N, j, j, i0, i1, part, LZ_REG_ALPHA - j, G);      // row0 + q = LZ_REG_ALPHA
+        grid.sync();
+        lz_gather(part, LZ_REG_ALPHA - j, j, j, G, s_c);
+        const double alpha = s_c[j];
+        for (int i = i0 + threadIdx.x; i < i1; i += LZ_THREADS)
+            w[i] = w[i] - alpha * v[i] - (j > 0 ? beta_j * v_prev[i] : 0.0);
+        for (int pass = 0; pass < 2; ++pass) {
+            const int row0 = pass ? LZ_REG_PASS1 : LZ_REG_PASS0;
+            __syncthreads();
+            lz_partial_dots(V, w, N, 0, j, i0, i1, part, row0, G);
+            grid.sync();
+            lz_gather(part, row0, 0, j, G, s_c);
+            for (int i = i0 + threadIdx.x; i < i1; i += LZ_THREADS) {
+                double x = w[i];
+                for (int q = 0; q <= j; ++q) x -= s_c[q] * V[(size_t)q * N + i];
+                w[i] = x;
+            }
         }
         __syncthreads();
-        for (int i = threadIdx.x; i < N; i += LZ_THREADS) {
-            double x = w[i];
-            for (int q = 0; q <= j; ++q) x -= s_c[q] * V[(size_t)q * N + i];
-            w[i] = x;
+        lz_partial_dots(w, w, N, 0, 0, i0, i1, part, LZ_REG_NORM, G);
+        grid.sync();
+        lz_gather(part, LZ_REG_NORM, 0, 0, G, s_c);
+        const double beta = sqrt(s_c[0]);
+        if (beta > 0.0 && j + 1 < LZ_MAX_STEPS) {
+            const double inv = 1.0 / beta;
+            double *vn = V + (size_t)(j + 1) * N;
+            for (int i = i0 + threadIdx.x; i < i1; i += LZ_THREADS) vn[i] = w[i] * inv;
         }
-    }
-    acc = 0.0;
-    for (int i = threadIdx.x; i < N; i += LZ_THREADS) acc = fma(w[i], w[i], acc);
-    const double beta = sqrt(lz_block_sum(acc, s_part));
-    if (beta > 0.0 && j + 1 < LZ_MAX_STEPS) {
-        const double inv = 1.0 / beta;
-        double *vn = V + (size_t)(j + 1) * N;
-        for (int i = threadIdx.x; i < N; i += LZ_THREADS) vn[i] = w[i] * inv;
-    }
-    if (threadIdx.x == 0) {
-        ctl->alpha[j] = alpha;
-        ctl->beta[j + 1] = beta;
-        ctl->steps = j + 1;
-        if (!(beta > 0.0)) ctl->stopped = 1;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            ctl->alpha[j] = alpha;
+            ctl->beta[j + 1] = beta;
+            ctl->steps = j + 1;
+            if (!(beta > 0.0)) ctl->stopped = 1;
+        }
+        if (!(beta > 0.0)) break;           // exact breakdown; every CTA holds the same beta
+        beta_j = beta;
+        grid.sync();                        // v_{j+1} complete before the next product reads it
     }
 }
 
@@ -198,29 +221,30 @@ __global__ void lanczos_finish_kernel(const LanczosCtl *__restrict__ ctl, double
 // ------------------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------------------
-// V (LZ_MAX_STEPS Lanczos vectors), w, the control block
+// V (LZ_MAX_STEPS Lanczos vectors), w, the per-CTA partial sums, the control block
 size_t lanczos_workspace_doubles(int64_t N)
 {
-    return (size_t)(LZ_MAX_STEPS + 1) * (size_t)N + (sizeof(LanczosCtl) + 7) / 8 + 16;
+    return (size_t)(LZ_MAX_STEPS + 1) * (size_t)N + (size_t)LZ_PART_ROWS * LZ_MAX_GRID + (sizeof(LanczosCtl) + 7) / 8 + 16;
 }
 
 // d_bounds: IN the Gershgorin bounds, OUT the tightened ones.  work: lanczos_workspace_doubles(N) doubles.
 int launch_lanczos_bounds(const bml_matrix_t *H, int steps, uint64_t seed, double *d_bounds, double *work, cudaStream_t st)
 {
     if (steps < 8 || steps > LZ_MAX_STEPS) return BML_ERR_INVALID;      // fewer steps do not see outlying bands
-    const int N = (int)H->N;
-    double *V = work, *w = work + (size_t)LZ_MAX_STEPS * N;
-    LanczosCtl *ctl = (LanczosCtl *)(work + (size_t)(LZ_MAX_STEPS + 1) * N + 8);
+    int N = (int)H->N;
+    double *V = work, *w = work + (size_t)LZ_MAX_STEPS * N, *part = w + N;
+    LanczosCtl *ctl = (LanczosCtl *)(part + (size_t)LZ_PART_ROWS * LZ_MAX_GRID + 8);
     if (steps > N) steps = N;
-    lanczos_start_kernel<<<1, LZ_THREADS, 0, st>>>(V, N, seed, ctl);
-    const unsigned grid = (unsigned)(((size_t)N * 32 + 255) / 256);
-    for (int j = 0; j < steps; ++j) {
-        if (H->type == BML_DENSE)
-            lanczos_matvec_dense_kernel<<<grid, 256, 0, st>>>(H->value, H->ld, N, V, w, ctl);
-        else
-            lanczos_matvec_ellpack_kernel<<<grid, 256, 0, st>>>(H->value, H->index, H->nnz, N, H->M, V, w, ctl);
-        lanczos_update_kernel<<<1, LZ_THREADS, 0, st>>>(V, w, N, ctl);
-    }
+    int G = sk_grid();                                                   // one CTA per SM, cooperative launch
+    if (G <= 0) return BML_ERR_CUDA;
+    if (G > LZ_MAX_GRID) G = LZ_MAX_GRID;
+    const double *hv = H->value;
+    const int32_t *hi = H->type == BML_DENSE ? nullptr : H->index, *hn = H->type == BML_DENSE ? nullptr : H->nnz;
+    int64_t ld = H->type == BML_DENSE ? H->ld : (int64_t)H->M;
+    void *args[] = {&hv, &hi, &hn, &ld, &N, &steps, &seed, &V, &w, &part, &ctl};
+    if (cudaLaunchCooperativeKernel((const void *)lanczos_run_kernel, dim3((unsigned)G), dim3(LZ_THREADS), args, 0, st) !=
+        cudaSuccess)
+        return BML_ERR_CUDA;
     lanczos_finish_kernel<<<1, 32, 0, st>>>(ctl, d_bounds);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }

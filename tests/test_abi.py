@@ -75,7 +75,7 @@ def test_sass_contains_the_blackwell_instructions():
     # every kernel family of the three headers is in the image
     for kernel in ("x2_dense_fp64_sk_kernel", "x2_dense_mixed_kernel", "x2_ellpack_upper_kernel", "symm_ab_fp64_kernel",
                    "cheb_coeff_kernel", "cheb_sums_kernel", "graph_gather_kernel", "graph_scatter_kernel",
-                   "lanczos_update_kernel"):
+                   "lanczos_run_kernel"):
         assert kernel in sass, kernel
 
 
