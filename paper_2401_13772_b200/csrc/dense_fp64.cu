@@ -61,15 +61,17 @@ __device__ __forceinline__ void sp2_tile_epilogue(double (&acc)[MI][NI][2], cons
             }
         };
 #pragma unroll
-        for (int i = 0; i < MI; i += 2) {
-            double2 xv[2][NI];
+        constexpr int RB = MI >= 4 ? 4 : 2;                            // fragment rows read ahead
 #pragma unroll
-            for (int ii = 0; ii < 2; ++ii)
+        for (int i = 0; i < MI; i += RB) {
+            double2 xv[RB][NI];
+#pragma unroll
+            for (int ii = 0; ii < RB; ++ii)
 #pragma unroll
                 for (int j = 0; j < NI; ++j)
                     xv[ii][j] = *(const double2 *)(X + (int64_t)(row0 + (i + ii) * 8) * ld + col0 + j * 8 + cadj);
 #pragma unroll
-            for (int ii = 0; ii < 2; ++ii) {
+            for (int ii = 0; ii < RB; ++ii) {
                 const int r = row0 + (i + ii) * 8;
 #pragma unroll
                 for (int j = 0; j < NI; ++j) {

@@ -177,6 +177,50 @@ symm_ab_fp64_kernel(const __grid_constant__ CUtensorMap map, const __grid_consta
                 if (r != cc) Out[(int64_t)cc * ldo + r] = v;
             }
         };
+        if (vec && C != nullptr && I * BT + BT <= N && J * BT + BT <= N) {
+            // Tile entirely inside the matrix (CTA-uniform): C is read RB fragment rows ahead of its use instead of
+            // inside the per-element conditions below (one L2 round trip per step, see sp2_tile_epilogue).  Same
+            // arithmetic, element by element.
+            const int cadj = (t < 2) ? 4 * t : 4 * (t - 2) + 2;               // frag_adjacent's column of this lane
+            auto one_c = [&](int r, int cc, double p, double cv) {
+                if (r <= cc) {                                                // only reached on diagonal tiles
+                    double v = fma(beta, cv, alpha * p);
+                    if (r == cc) v += gamma;
+                    Out[(int64_t)r * ldo + cc] = v;
+                    if (r != cc) Out[(int64_t)cc * ldo + r] = v;
+                }
+            };
+            constexpr int RB = MI >= 4 ? 4 : 2;
+#pragma unroll
+            for (int i = 0; i < MI; i += RB) {
+                double2 cv[RB][NI];
+#pragma unroll
+                for (int ii = 0; ii < RB; ++ii)
+#pragma unroll
+                    for (int j = 0; j < NI; ++j)
+                        cv[ii][j] = *(const double2 *)(C + (int64_t)(row0 + (i + ii) * 8) * ldc + col0 + j * 8 + cadj);
+#pragma unroll
+                for (int ii = 0; ii < RB; ++ii) {
+                    const int r = row0 + (i + ii) * 8;
+#pragma unroll
+                    for (int j = 0; j < NI; ++j) {
+                        double p0 = acc[i + ii][j][0], p1 = acc[i + ii][j][1];
+                        const int cc = col0 + j * 8 + frag_adjacent(p0, p1, t);
+                        const double2 c2 = cv[ii][j];
+                        if (!diag || r < cc) {
+                            const double v0 = fma(beta, c2.x, alpha * p0), v1 = fma(beta, c2.y, alpha * p1);
+                            *(double2 *)(Out + (int64_t)r * ldo + cc) = make_double2(v0, v1);
+                            Out[(int64_t)cc * ldo + r] = v0;
+                            Out[(int64_t)(cc + 1) * ldo + r] = v1;
+                        } else {
+                            one_c(r, cc, p0, c2.x);
+                            one_c(r, cc + 1, p1, c2.y);
+                        }
+                    }
+                }
+            }
+            continue;
+        }
 #pragma unroll
         for (int i = 0; i < MI; ++i) {
             const int r = row0 + i * 8;
