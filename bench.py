@@ -50,8 +50,8 @@ def dense_flops_per_product(N: int) -> float:
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r01_ncu_kernels.md names the commands); None = no capture of this workload.
 NCU_TRAFFIC_BYTES = {
-    "dense_n2048": 41.8e6,          # 33.9 MB read (= N^2 x 8 B: X read once) + 7.9 MB written (X' mostly stays in L2)
-    "dense_n8192": 6.08e9,          # 5.55 GB read (row panels re-read) + 0.53 GB written
+    "dense_n2048": 43.2e6,          # 33.9 MB read (= N^2 x 8 B: X read once) + 9.2 MB written (X' mostly stays in L2)
+    "dense_n8192": 6.09e9,          # 5.56 GB read (row panels re-read) + 0.53 GB written
     "mixed_n16384": 20.4e9,         # 17.2 GB read + 3.2 GB written (FP16 x 2 planes, super-block tile order)
     "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (capture quoted in DESIGN.md 5.3)
     "cheby_n2000": 98.1e6,          # grouped product kernel, one Eq. 10 step: 85.3 MB read + 12.8 MB written
