@@ -327,13 +327,35 @@ x2_dense_mixed_kernel(const __grid_constant__ CUtensorMap map0, const __grid_con
         const int r = I * M_BM + rl;
         const int64_t plane = (int64_t)N * ld;
         // (1) rows e, e + 8, ... of the X tile; lane covers 4 consecutive columns (ld is a multiple of 16: in bounds)
-        for (int rr = e; rr < M_BM; rr += M_EPI_WARPS) {
-            const int gr = I * M_BM + rr, gc = J * M_BN + lane * 4;
-            if (gr < N && gc < N) {
-                const double2 *src = (const double2 *)(X + (int64_t)gr * ld + gc);
-                const double2 a = src[0], bb = src[1];
-                double *dst = S + rr * SS + lane * 4;
-                dst[0] = a.x; dst[1] = a.y; dst[2] = bb.x; dst[3] = bb.y;
+        if (I * M_BM + M_BM <= N && J * M_BN + M_BN <= N) {
+            // tile entirely inside the matrix: no bounds test, so the reads of 8 rows are in flight together (with the
+            // loads inside the condition below, each of a warp's 16 rows costs one L2 round trip)
+            constexpr int RA = 8;
+            static_assert((M_BM / M_EPI_WARPS) % RA == 0, "read-ahead depth must divide the rows per warp");
+            const double *xt = X + (int64_t)(I * M_BM + e) * ld + J * M_BN + lane * 4;
+#pragma unroll
+            for (int k = 0; k < M_BM / M_EPI_WARPS; k += RA) {
+                double2 a[RA], bb[RA];
+#pragma unroll
+                for (int u = 0; u < RA; ++u) {
+                    const double2 *src = (const double2 *)(xt + (int64_t)((k + u) * M_EPI_WARPS) * ld);
+                    a[u] = src[0]; bb[u] = src[1];
+                }
+#pragma unroll
+                for (int u = 0; u < RA; ++u) {
+                    double *dst = S + (e + (k + u) * M_EPI_WARPS) * SS + lane * 4;
+                    dst[0] = a[u].x; dst[1] = a[u].y; dst[2] = bb[u].x; dst[3] = bb[u].y;
+                }
+            }
+        } else {
+            for (int rr = e; rr < M_BM; rr += M_EPI_WARPS) {
+                const int gr = I * M_BM + rr, gc = J * M_BN + lane * 4;
+                if (gr < N && gc < N) {
+                    const double2 *src = (const double2 *)(X + (int64_t)gr * ld + gc);
+                    const double2 a = src[0], bb = src[1];
+                    double *dst = S + rr * SS + lane * 4;
+                    dst[0] = a.x; dst[1] = a.y; dst[2] = bb.x; dst[3] = bb.y;
+                }
             }
         }
         asm volatile("bar.sync 1, %0;" ::"n"(M_EPI_WARPS * 32) : "memory");
