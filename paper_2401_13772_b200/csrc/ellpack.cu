@@ -296,20 +296,47 @@ x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict
             for (int s = tg; s < E_SLOTS / 4; s += E_GT) k4[s] = e4;
         }
         int nk_max = 0;
-        for (int p = tg; p < n_i; p += E_GT) {
-            const int k = xi[rbase + p];
-            const int n_k = min(xn[k], M);
-            // first slot of row k whose column is >= row (rows are in ascending column order)
-            const int32_t *rk = xi + (int64_t)k * M;
-            int lo = 0, hi = n_k;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (__ldg(rk + mid) < row) lo = mid + 1; else hi = mid;
+        // Four entries of row i per thread at a time (one pass for n_i <= 4 E_GT): their binary searches -- about
+        // log2(n_k) dependent L2 loads each -- advance in lock step with unconditional loads, so a round costs one
+        // round trip for all four instead of one each.
+        constexpr int SU = 4;
+        for (int p0 = tg; p0 < n_i; p0 += SU * E_GT) {
+            int k[SU], nk[SU], lo[SU], hi[SU];
+#pragma unroll
+            for (int u = 0; u < SU; ++u) k[u] = (p0 + u * E_GT < n_i) ? xi[rbase + p0 + u * E_GT] : row;
+#pragma unroll
+            for (int u = 0; u < SU; ++u) {
+                nk[u] = (p0 + u * E_GT < n_i) ? min(xn[k[u]], M) : 0;
+                lo[u] = 0; hi[u] = nk[u];
             }
-            sk[p] = k;
-            sa[p] = xv[rbase + p];
-            sn[p] = (lo << 16) | (n_k - lo);
-            nk_max = max(nk_max, n_k - lo);
+            // first slot of row k whose column is >= row (rows are in ascending column order)
+            bool more = true;
+            while (more) {
+                int v[SU], mid[SU];
+#pragma unroll
+                for (int u = 0; u < SU; ++u) {
+                    mid[u] = (lo[u] < hi[u]) ? ((lo[u] + hi[u]) >> 1) : 0;      // slot 0 always exists: a safe read
+                    v[u] = __ldg(xi + (int64_t)k[u] * M + mid[u]);
+                }
+                more = false;
+#pragma unroll
+                for (int u = 0; u < SU; ++u) {
+                    if (lo[u] < hi[u]) {
+                        if (v[u] < row) lo[u] = mid[u] + 1; else hi[u] = mid[u];
+                    }
+                    more |= lo[u] < hi[u];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < SU; ++u) {
+                const int p = p0 + u * E_GT;
+                if (p < n_i) {
+                    sk[p] = k[u];
+                    sa[p] = xv[rbase + p];
+                    sn[p] = (lo[u] << 16) | (nk[u] - lo[u]);
+                    nk_max = max(nk_max, nk[u] - lo[u]);
+                }
+            }
         }
         nk_max = __reduce_max_sync(0xffffffffu, nk_max);
         if (lane == 0) atomicMax(&s_nkmax[grp][it & 1], nk_max);
