@@ -482,16 +482,19 @@ x2_ellpack_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, in
         // ---- lower part: sort the appended (row j, value) pairs by column
         int n2 = 32;
         while (n2 < n_l) n2 <<= 1;
+#pragma unroll 4
         for (int q = lane; q < n2; q += 32)
             sortbuf[q] = q < n_l ? (((unsigned long long)(unsigned)li[rbase + q] << 32) | (unsigned)q) : ~0ull;
         __syncwarp();
         if (n_l > 1) warp_bitonic_sort(sortbuf, n2, lane);
+#pragma unroll 4
         for (int q = lane; q < n_l; q += 32) {
             const unsigned long long e = sortbuf[q];
             pc[q] = (int)(e >> 32);
             pv[q] = lv[rbase + (int)(e & 0xffffffffu)];
             pf[q] = 0;
         }
+#pragma unroll 4
         for (int q = lane; q < u; q += 32) {
             pc[n_l + q] = ti[rbase + q];
             pv[n_l + q] = tv[rbase + q];
