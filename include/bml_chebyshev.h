@@ -82,16 +82,6 @@ BML_API int bml_symm_ab_dense(double *base, int64_t N, int64_t ld, int64_t slot_
                               const int32_t *out_slot, const double *alpha, const double *beta, const double *gamma,
                               void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
-/*
- * Host-computable parts of the path, exported so that they can be tested exhaustively without a GPU:
- * bml_cheb_schedule: the doubling schedule of reading C5.  For i = 2..k: level[i-2] (1-based doubling level),
- *   a[i-2], b[i-2] with T_i = 2 T_a T_b - T_{a-b}.  Returns the number of levels, or -1.
- * bml_symm_work_item: the it-th work item of CTA `cta` (of n_ctas) of a grouped launch of n_jobs products of size N:
- *   out6 <- { job, I, J, kt_begin, kt_end, tile_edge }.  Returns 0, 1 when the list is exhausted, or -1.
- */
-BML_API int bml_cheb_schedule(int32_t k, int32_t *level, int32_t *a, int32_t *b);
-BML_API int bml_symm_work_item(int64_t N, int32_t n_jobs, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out6);
-
 #ifdef __cplusplus
 }
 #endif

@@ -27,7 +27,7 @@
  *   -5  BML_ERR_NOT_SYMMETRIC H is not bitwise symmetric (checked only with BML_SP2_FLAG_CHECK_SYMMETRY)
  *   -6  BML_ERR_ACC_CAPACITY  ELLPACK: a row of X*X touched more distinct columns BEFORE thresholding than the
  *                             on-chip accumulator holds (BML_ELL_ACC_SLOTS); stats->overflow_row = that row.
- * On a negative return D is undefined.
+ * On a negative return D is undefined (bml_sp2_*: left untouched).
  */
 #ifndef BML_SP2_H
 #define BML_SP2_H
@@ -149,23 +149,39 @@ BML_API int bml_trace(const bml_matrix_t *A, double *d_trace, void *cuda_stream)
  *   D = X_{m*}, the iterate that was tested.
  * H: input, never written.  D: output, same type (and for ellpack the same M) as H; must not alias H.
  * d_workspace: DEVICE scratch, >= bml_sp2_workspace_bytes(H, p) bytes, 1024-byte aligned.
- * stats: HOST, may be NULL (the status is still returned; the call still synchronises once at its end).
+ * stats: HOST.  Non-NULL: the call synchronises the stream once, at its end, to read the control block back, and returns
+ *   the solve's status.  While it enqueues, the host also waits on an event behind every batch of 8 product launches, one
+ *   batch BEHIND the one in flight (this only bounds how many launches are issued after the stop rule fired; the device
+ *   never waits for the host).  NULL: the call is FULLY ASYNCHRONOUS -- all max_products launches are enqueued (those
+ *   behind the device-side stop flag exit at once), the host never waits, nothing is copied back, and the return value
+ *   is 0 / -1 / -4 for "enqueued" only; the verdict stays in the control block at the start of d_workspace and is read
+ *   later with bml_sp2_read_stats (which synchronises).  On a negative status D is left untouched.
  * The whole solve is enqueued without any host round trip per product: the branch bit, the stop test and the
- * ping-pong buffer selection live in a device-resident control block.  Dense FP64, N <= 1024, not on the legacy default
- * stream: the launches up to and including the first batch of products are captured once per argument set and replayed
- * as a CUDA graph by later calls with the same pointers, shapes and parameters; results are identical.
+ * ping-pong buffer selection live in a device-resident control block.
+ * Cached state.  Dense FP64, N <= 1024, not on the legacy default stream: the launches up to and including the first
+ *   batch of products are captured once per argument set and replayed as a CUDA graph by later calls with the same
+ *   device, pointers, shapes and parameters; results are identical.  The cache (4 graphs per host thread; the same
+ *   holds for bml_chebyshev_dense) remembers the caller's H / workspace POINTERS as lookup keys -- they are compared,
+ *   never dereferenced by the host, and a replay only touches the arrays of the call that replays it -- until
+ *   bml_sp2_release_cached() is called on that thread.  Nothing else outlives a call.
  */
 BML_API size_t bml_sp2_workspace_bytes(const bml_matrix_t *H, const bml_sp2_params_t *p);
 BML_API int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,
                   size_t workspace_bytes, bml_sp2_stats_t *stats, void *cuda_stream);
 BML_API int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,
                     size_t workspace_bytes, bml_sp2_stats_t *stats, void *cuda_stream);
+/* Fill `stats` from the control block of the last bml_sp2_* call that used `d_workspace` (for calls made with
+ * stats == NULL).  Synchronises `cuda_stream`.  Returns the solve's status, or -1 / -4. */
+BML_API int bml_sp2_read_stats(const void *d_workspace, bml_sp2_stats_t *stats, void *cuda_stream);
+/* Destroy the calling thread's cached CUDA graphs (see "Cached state" above).  Safe to call at any time. */
+BML_API void bml_sp2_release_cached(void);
 
 /*
  * One product of the hot loop, exported for per-kernel parity tests and per-kernel timing.
  *
  * bml_x2_dense: the fused symmetric-square kernel (steps D3 + D4 of DESIGN.md) on a caller-supplied iterate.
- *   X: dense N x N, bitwise symmetric, ld a multiple of 16 elements, value 128-byte aligned.  Xnext: same shape/ld
+ *   X: dense N x N, bitwise symmetric, ld a multiple of 16 elements (precision 1, 2: ld == 16 * ceil(N / 16) exactly,
+ *   the 16-bit planes in the workspace are sized for that pitch; anything else is -1), value 128-byte aligned.  Xnext: same shape/ld
  *   <- branch ? 2X - X*X : X*X  (Eq. 7 / Eq. 6), both triangles written.  d_sums: DEVICE double[4] <-
  *   { tr(X*X), ||X*X - X||_F^2, ||X||_F^2, tr(Xnext) }.  precision (0, 1, 2) as in bml_sp2_params_t.
  *   d_workspace >= bml_x2_dense_workspace_bytes(N, precision).
@@ -183,28 +199,6 @@ BML_API int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t bra
 BML_API size_t bml_x2_ellpack_workspace_bytes(int64_t N, int32_t M);
 BML_API int bml_x2_ellpack(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, double drop_tol, double *d_sums,
                    int32_t *d_info, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
-
-/*
- * Measurement helper (not part of the method): issue `iters` back-to-back register-resident FP64 tensor-core
- * instructions (mma.sync m8n8k4 f64 = SASS DMMA.8x8x4) per warp on every SM and return the elapsed device time.
- * bench.py divides the flops by it to get the FP64 tensor-pipe peak at the clocks of the same run (the driver's
- * MEASURED_PEAKS.json has no FP64 entry).  *flops_out <- total flops issued, *ms_out <- CUDA-event milliseconds.
- * Synchronises the stream.  Returns 0 or -4.
- */
-BML_API int bml_probe_fp64_tensor_peak(int32_t iters, double *flops_out, double *ms_out, void *cuda_stream);
-
-/*
- * Introspection of the host-computable work distribution of the dense kernels (pure host functions, no GPU needed;
- * they run the same arithmetic as the kernels and exist so that the partition can be tested exhaustively on a CPU).
- * bml_dense_work_item: the it-th work item of CTA `cta` (of n_ctas) of the persistent FP64 kernel for an N x N product
- *   (N > 1024).  out5 <- { tile, I, J, kt_begin, kt_end }: tile (I, J), I <= J, of 128 x 128, k-slabs [kt_begin, kt_end)
- *   of ceil(N / 16).  Returns 0, 1 when the CTA's list has fewer than it + 1 items, or -1.
- * bml_dense_mixed_tile_count / bml_dense_mixed_tile_of_cta: grid size of the mixed kernel and the tile of a CTA
- *   (out2 <- { I, J }); returns 1 for the empty slots of the super-block order.
- */
-BML_API int bml_dense_work_item(int64_t N, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out5);
-BML_API int bml_dense_mixed_tile_count(int64_t N);
-BML_API int bml_dense_mixed_tile_of_cta(int64_t N, int32_t cta, int32_t *out2);
 
 BML_API const char *bml_status_string(int status);
 /* "major.minor.patch (sm_100a)" */

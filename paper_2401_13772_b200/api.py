@@ -29,9 +29,10 @@ def FLAG_LANCZOS_BOUNDS(steps: int) -> int:
 EXPORTS = [
     "bml_version", "bml_status_string", "bml_gershgorin_workspace_bytes", "bml_gershgorin", "bml_trace",
     "bml_sp2_workspace_bytes", "bml_sp2_dense", "bml_sp2_ellpack", "bml_x2_dense_workspace_bytes", "bml_x2_dense",
-    "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_probe_fp64_tensor_peak",
-    "bml_dense_work_item", "bml_dense_mixed_tile_count", "bml_dense_mixed_tile_of_cta",
+    "bml_x2_ellpack_workspace_bytes", "bml_x2_ellpack", "bml_sp2_read_stats", "bml_sp2_release_cached",
     "bml_lanczos_bounds_workspace_bytes", "bml_lanczos_bounds",
+    # include/bml_sp2_testing.h (test / measurement hooks, not the product interface)
+    "bml_probe_fp64_tensor_peak", "bml_dense_work_item", "bml_dense_mixed_tile_count", "bml_dense_mixed_tile_of_cta",
     # include/bml_chebyshev.h
     "bml_chebyshev_workspace_bytes", "bml_chebyshev_dense", "bml_symm_ab_workspace_bytes", "bml_symm_ab_dense",
     "bml_cheb_schedule", "bml_symm_work_item",
@@ -169,6 +170,10 @@ def load(build_if_missing: bool = True):
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [MP, PP, MP, vp, sz, SP, vp]
+    L.bml_sp2_read_stats.restype = ctypes.c_int
+    L.bml_sp2_read_stats.argtypes = [vp, SP, vp]
+    L.bml_sp2_release_cached.restype = None
+    L.bml_sp2_release_cached.argtypes = []
     L.bml_x2_dense_workspace_bytes.restype = sz
     L.bml_x2_dense_workspace_bytes.argtypes = [i64, i32]
     L.bml_x2_dense.restype = ctypes.c_int
@@ -348,14 +353,23 @@ class DenseSolver:
         self.ws_bytes = L.bml_sp2_workspace_bytes(ctypes.byref(d), ctypes.byref(p))
         self.ws = _workspace(self.ws_bytes, self.device)
 
-    def solve(self, H: torch.Tensor, n_occ: int, idem_tol: float, max_products: int = 100, flags: int = 0):
+    def solve(self, H: torch.Tensor, n_occ: int, idem_tol: float, max_products: int = 100, flags: int = 0,
+              asynchronous: bool = False):
+        """asynchronous=True passes stats = NULL: nothing is synchronised, the result is read later by read_stats()."""
         L = load()
         h, d = dense_desc(H), dense_desc(self.D)
         p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), 0.0, self.precision, int(flags))
         st = bml_sp2_stats_t()
         rc = L.bml_sp2_dense(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
-                             ctypes.byref(st), _stream())
+                             None if asynchronous else ctypes.byref(st), _stream())
+        if asynchronous:
+            if rc != 0:
+                raise RuntimeError(f"bml_sp2_dense: {bml_status_string(rc)}")
+            return self.D, None
         return self.D, _result(st, rc)
+
+    def read_stats(self) -> "Sp2Result":
+        return bml_sp2_read_stats(self.ws)
 
 
 def bml_sp2_dense(H: torch.Tensor, n_occ: int, idem_tol: float, max_products: int = 100, precision: int = 0,
@@ -378,15 +392,22 @@ class EllpackSolver:
         self.ws = _workspace(self.ws_bytes, self.device)
 
     def solve(self, value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100,
-              flags: int = 0):
+              flags: int = 0, asynchronous: bool = False):
         L = load()
         h = ellpack_desc(value, index, nnz)
         d = ellpack_desc(self.dv, self.di, self.dn)
         p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), float(drop_tol), 0, int(flags))
         st = bml_sp2_stats_t()
         rc = L.bml_sp2_ellpack(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
-                               ctypes.byref(st), _stream())
+                               None if asynchronous else ctypes.byref(st), _stream())
+        if asynchronous:
+            if rc != 0:
+                raise RuntimeError(f"bml_sp2_ellpack: {bml_status_string(rc)}")
+            return (self.dv, self.di, self.dn), None
         return (self.dv, self.di, self.dn), _result(st, rc)
+
+    def read_stats(self) -> "Sp2Result":
+        return bml_sp2_read_stats(self.ws)
 
 
 def bml_sp2_ellpack(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100,
@@ -395,6 +416,17 @@ def bml_sp2_ellpack(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: fl
     _require_cuda(value, torch.float64, "value")
     return EllpackSolver(value.shape[0], value.shape[1], value.device).solve(value, index, nnz, n_occ, idem_tol,
                                                                            drop_tol, max_products, flags)
+
+
+def bml_sp2_read_stats(ws: torch.Tensor) -> Sp2Result:
+    """Result of the last bml_sp2_* call on workspace `ws` (for calls made with stats = NULL); synchronises."""
+    st = bml_sp2_stats_t()
+    rc = load().bml_sp2_read_stats(ws.data_ptr(), ctypes.byref(st), _stream())
+    return _result(st, rc)
+
+
+def bml_sp2_release_cached() -> None:
+    load().bml_sp2_release_cached()
 
 
 def padded_ld(N: int) -> int:

@@ -5,6 +5,7 @@
 #include "common.cuh"
 #include "symm_ab.cuh"
 #include "../../include/bml_graph.h"
+#include "../../include/bml_sp2_testing.h"
 
 namespace bmlsp2 {
 
@@ -21,7 +22,8 @@ int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, doubl
 int dense_mixed_num_tiles(int64_t N);
 size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx);
 int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, double *X0, double *X1, int64_t ldx,
-                          Sp2Ctl *ctl, double *partials, const double *d_bounds, void *extra, cudaStream_t st);
+                          Sp2Ctl *ctl, double *partials, const double *d_bounds, void *extra, cudaStream_t st,
+                          bool no_host_wait);
 int x2_dense_mixed_once(const bml_matrix_t *X, bml_matrix_t *Xn, int precision, Sp2Ctl *ctl, double *partials,
                         void *extra, cudaStream_t st);
 // reductions.cu
@@ -63,6 +65,7 @@ int launch_graph_core_halo(const bml_matrix_t *H, const int32_t *offs, const int
 int launch_graph_gather(const bml_matrix_t *H, const int32_t *nodes, int s, double *h, int64_t ld, cudaStream_t st);
 int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
                          bml_matrix_t *D, int32_t *overflow, cudaStream_t st);
+void cheb_graph_cache_release();
 // probe.cu
 int run_fp64_tensor_probe(int iters, double *flops, double *ms, cudaStream_t st);
 
@@ -213,8 +216,12 @@ EnqueueState &enqueue_state()
     return es;
 }
 
+// stats == NULL: the call is fully asynchronous -- nothing is copied back, the stream is not synchronised and the
+// return value only says that everything was enqueued (the verdict of the solve stays in the device control block,
+// whose first words bml_sp2_read_status copies out later).
 static int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
 {
+    if (!stats) return cudaGetLastError() == cudaSuccess ? BML_OK : BML_ERR_CUDA;
     Sp2Ctl h;
     if (cudaMemcpyAsync(&h, d_ctl, sizeof(Sp2Ctl), cudaMemcpyDeviceToHost, st) != cudaSuccess) return BML_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return BML_ERR_CUDA;
@@ -233,10 +240,11 @@ struct Sp2GraphKey {
     int32_t n_occ, max_products;
     uint32_t flags;
     cudaStream_t st;
+    int dev;            // device ordinal: a graph exec belongs to the device it was instantiated on
     bool operator==(const Sp2GraphKey &o) const
     {
         return H == o.H && ws == o.ws && N == o.N && ldh == o.ldh && idem_tol == o.idem_tol && n_occ == o.n_occ &&
-               max_products == o.max_products && flags == o.flags && st == o.st;
+               max_products == o.max_products && flags == o.flags && st == o.st && dev == o.dev;
     }
 };
 struct Sp2GraphSlot {
@@ -245,16 +253,31 @@ struct Sp2GraphSlot {
     uint64_t stamp = 0;
 };
 
+// The cache is per host thread and holds the caller's H / workspace pointers as KEYS only (they are compared, never
+// dereferenced by the host); bml_sp2_release_cached() drops it.
+static thread_local Sp2GraphSlot g_sp2_slots[4];
+static thread_local uint64_t g_sp2_clock = 0;
+static thread_local bool g_sp2_warmed[MAX_DEVICES][2] = {};
+
+void sp2_graph_cache_release()
+{
+    for (auto &sl : g_sp2_slots) {
+        if (sl.exec) cudaGraphExecDestroy(sl.exec);
+        sl = Sp2GraphSlot();
+    }
+}
+
 template <class EnqueueFn>
 static int sp2_first_batch_cached(const Sp2GraphKey &key, EnqueueFn &&enqueue)
 {
-    static thread_local Sp2GraphSlot slots[4];
-    static thread_local uint64_t clock_ = 0;
-    static thread_local bool warmed[2] = {false, false};
+    Sp2GraphSlot (&slots)[4] = g_sp2_slots;
+    uint64_t &clock_ = g_sp2_clock;
     cudaStream_t st = key.st;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     const bool capturing = cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
     const int bti = key.N <= 512 ? 0 : 1;
+    if (key.dev < 0) return enqueue();
+    bool *warmed = g_sp2_warmed[key.dev];
     if (key.N > 1024 || capturing || st == nullptr || !warmed[bti]) {
         if (key.N <= 1024) warmed[bti] = true;
         return enqueue();
@@ -392,7 +415,8 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
     };
     if (p->precision != 0) {
         TRY(prelude());
-        TRY(sp2_dense_mixed_solve(H, p, w.X0, w.X1, w.ldx, w.ctl, w.partials, w.scal->bounds, w.extra, st));
+        TRY(sp2_dense_mixed_solve(H, p, w.X0, w.X1, w.ldx, w.ctl, w.partials, w.scal->bounds, w.extra, st,
+                                  stats == nullptr));
     } else {
         CUtensorMap map0, map1;
         TRY(make_dense_map(&map0, w.X0, N, w.ldx));
@@ -410,12 +434,25 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
                 if ((r = launch_one())) return r;
             return 0;
         };
-        const Sp2GraphKey key = {H->value, d_workspace, N, H->ld, p->idem_tol, p->n_occ, p->max_products, p->flags, st};
+        const Sp2GraphKey key = {H->value, d_workspace, N, H->ld, p->idem_tol, p->n_occ, p->max_products, p->flags, st,
+                                 current_device()};
         TRY(sp2_first_batch_cached(key, first_batch));
-        TRY(enqueue_products(launch_one, w.ctl, p->max_products, st, n_first));
+        TRY(enqueue_products(launch_one, w.ctl, p->max_products, st, n_first, stats == nullptr));
     }
     TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
     return finish_solve(w.ctl, stats, st);
+}
+
+void bml_sp2_release_cached(void)
+{
+    sp2_graph_cache_release();
+    cheb_graph_cache_release();
+}
+
+int bml_sp2_read_stats(const void *d_workspace, bml_sp2_stats_t *stats, void *cuda_stream)
+{
+    if (!d_workspace || !stats || ((uintptr_t)d_workspace & 1023) != 0) return BML_ERR_INVALID;
+    return finish_solve((Sp2Ctl *)d_workspace, stats, (cudaStream_t)cuda_stream);
 }
 
 size_t bml_x2_dense_workspace_bytes(int64_t N, int32_t precision)
@@ -436,6 +473,9 @@ int bml_x2_dense(const bml_matrix_t *X, bml_matrix_t *Xnext, int32_t branch, int
         !d_sums || !d_workspace || ((uintptr_t)d_workspace & 1023) != 0 || precision < 0 || precision > 2 ||
         workspace_bytes < bml_x2_dense_workspace_bytes(X->N, precision))
         return BML_ERR_INVALID;
+    // the 16-bit planes and the FP64 diagonal in the workspace are sized by bml_x2_dense_workspace_bytes for the pitch
+    // padded_ld(N), and the mixed kernel carves them with the iterate's own ld: any wider ld would run past the end
+    if (precision != 0 && X->ld != padded_ld(X->N)) return BML_ERR_INVALID;
     const int64_t N = X->N;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     uint8_t *p = (uint8_t *)d_workspace;
@@ -483,7 +523,7 @@ int bml_sp2_ellpack(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix
     TRY(ellpack_sym_reset(w.sym, N, M, st));
     TRY(enqueue_products([&]() { return launch_x2_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, p->drop_tol, w.ctl,
                                                           w.rowstats, w.sym, st); },
-                         w.ctl, p->max_products, st));                                            // S2-S5
+                         w.ctl, p->max_products, st, 0, stats == nullptr));                       // S2-S5
     TRY(launch_copy_out_ellpack(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, N, M, w.ctl, D->value, D->index, D->nnz, st));
     return finish_solve(w.ctl, stats, st);
 }

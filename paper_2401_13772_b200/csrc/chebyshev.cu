@@ -143,13 +143,8 @@ static size_t cheb_coeff_smem_bytes(int terms) { return (size_t)(2 + 1 + 1 + 8) 
 
 static int launch_cheb_coeff(ChebCtl *ctl, double mu, double beta, int k, int m, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(cheb_coeff_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)cheb_coeff_smem_bytes(BML_CHEB_MAX_TERMS)) != cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
-    }
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(cheb_coeff_kernel, cheb_coeff_smem_bytes(BML_CHEB_MAX_TERMS), have)) return BML_ERR_CUDA;
     cheb_coeff_kernel<<<1, CC_THREADS, cheb_coeff_smem_bytes(k * m), st>>>(ctl, mu, beta, k, m);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
@@ -394,10 +389,11 @@ struct ChebGraphKey {
     int32_t k, m;
     uint32_t flags;
     cudaStream_t st;
+    int dev;            // device ordinal the graph was instantiated on
     bool operator==(const ChebGraphKey &o) const
     {
         return H == o.H && D == o.D && ws == o.ws && N == o.N && ldh == o.ldh && ldd == o.ldd && mu == o.mu &&
-               beta == o.beta && k == o.k && m == o.m && flags == o.flags && st == o.st;
+               beta == o.beta && k == o.k && m == o.m && flags == o.flags && st == o.st && dev == o.dev;
     }
 };
 struct ChebGraphSlot {
@@ -409,12 +405,27 @@ struct ChebGraphSlot {
 constexpr int CHEB_GRAPH_SLOTS = 4;
 constexpr int64_t CHEB_GRAPH_MAX_N = 2048;      // above this the launches are long: nothing to gain
 
+// per host thread; the caller's pointers are keys only.  bml_sp2_release_cached() drops it.
+static thread_local ChebGraphSlot g_cheb_slots[CHEB_GRAPH_SLOTS];
+static thread_local uint64_t g_cheb_clock = 0;
+static thread_local bool g_cheb_warmed[MAX_DEVICES][3] = {};
+
+void cheb_graph_cache_release()
+{
+    for (auto &sl : g_cheb_slots) {
+        if (sl.exec) cudaGraphExecDestroy(sl.exec);
+        sl = ChebGraphSlot();
+    }
+}
+
 static int cheb_enqueue_cached(const bml_matrix_t *H, const bml_cheb_params_t *p, bml_matrix_t *D, void *ws,
                                int *n_launches_out, cudaStream_t st)
 {
-    static thread_local ChebGraphSlot slots[CHEB_GRAPH_SLOTS];
-    static thread_local uint64_t clock_ = 0;
-    static thread_local bool warmed[3] = {false, false, false};
+    ChebGraphSlot (&slots)[CHEB_GRAPH_SLOTS] = g_cheb_slots;
+    uint64_t &clock_ = g_cheb_clock;
+    const int dev = current_device();
+    if (dev < 0) return BML_ERR_CUDA;
+    bool *warmed = g_cheb_warmed[dev];
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     const bool capturing = cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
     const int bti = H->N <= 512 ? 0 : (H->N <= 1024 ? 1 : 2);
@@ -424,7 +435,7 @@ static int cheb_enqueue_cached(const bml_matrix_t *H, const bml_cheb_params_t *p
         warmed[bti] = true;
         return cheb_dense_enqueue(H, p, D, ws, n_launches_out, st);
     }
-    const ChebGraphKey key = {H->value, D->value, ws, H->N, H->ld, D->ld, p->mu, p->beta, p->k, p->m, p->flags, st};
+    const ChebGraphKey key = {H->value, D->value, ws, H->N, H->ld, D->ld, p->mu, p->beta, p->k, p->m, p->flags, st, dev};
     ChebGraphSlot *hit = nullptr, *victim = &slots[0];
     for (auto &sl : slots) {
         if (sl.exec && sl.key == key) hit = &sl;

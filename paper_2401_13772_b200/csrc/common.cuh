@@ -223,6 +223,38 @@ __host__ __device__ __forceinline__ bool tile_sb_decode(int bid, int T, int &I, 
     return I <= J && J < T;
 }
 
+// One-time host state (kernel attributes, SM counts, cooperative grid sizes) is kept PER DEVICE ORDINAL: a process may
+// drive several GPUs, and cudaFuncSetAttribute / the SM count belong to the device that is current at the call.
+constexpr int MAX_DEVICES = 64;
+static inline int current_device()
+{
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= MAX_DEVICES) return -1;
+    return d;
+}
+// raise a kernel's dynamic shared-memory limit to `bytes` once per device (`have` = per-device high-water mark)
+template <class Kernel>
+static inline int ensure_smem_attr(Kernel kernel, size_t bytes, size_t (&have)[MAX_DEVICES], size_t floor_bytes = 0)
+{
+    const int dev = current_device();
+    if (dev < 0) return BML_ERR_CUDA;
+    if (have[dev] < floor_bytes) have[dev] = floor_bytes;
+    if (bytes > have[dev]) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+            return BML_ERR_CUDA;
+        have[dev] = bytes;
+    }
+    return 0;
+}
+static inline int device_sm_count()
+{
+    static int sms[MAX_DEVICES] = {};
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    if (!sms[dev] && cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms[dev] = 0;
+    return sms[dev];
+}
+
 // Host-side helpers (api.cu)
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -233,7 +265,8 @@ PFN_encodeTiled get_encode_tiled();
 // batch AHEAD are always queued; after each batch the device-side stop flag is copied to pinned host memory and the
 // host waits on an event recorded behind the batch BEFORE the one in flight.  Launches behind the stop flag exit at
 // once on the device, so correctness never depends on the host seeing the flag; batching only bounds how many of
-// them are issued (at most two batches instead of max_products - n_products).
+// them are issued (at most two batches instead of max_products - n_products).  These event waits are the only host
+// synchronisation of a solve besides the final read of the control block, and they trail the device by a batch.
 constexpr int ENQ_FIRST = 16, ENQ_BATCH = 8, ENQ_RING = 4;
 struct EnqueueState {
     int32_t *h_done = nullptr;          // pinned, ENQ_RING slots
@@ -251,11 +284,14 @@ struct EnqueueState {
 EnqueueState &enqueue_state();      // api.cu: one per host thread
 
 // `already`: product launches of the first batch that are in the stream already (a replayed CUDA graph, api.cu).
+// `no_host_wait`: the caller asked for a fully asynchronous solve (stats == NULL): every one of the max_products
+// launches is enqueued and the host never waits; the launches behind the stop flag cost a few microseconds each.
 template <class LaunchFn>
-static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_products, cudaStream_t st, int already = 0)
+static int enqueue_products(LaunchFn &&launch_one, Sp2Ctl *d_ctl, int max_products, cudaStream_t st, int already = 0,
+                            bool no_host_wait = false)
 {
     EnqueueState &es = enqueue_state();
-    if (!es.ok) {                       // no pinned memory / events: plain enqueue of everything
+    if (!es.ok || no_host_wait) {       // (or no pinned memory / events): plain enqueue of everything
         for (int l = already; l < max_products; ++l) { int r = launch_one(); if (r) return r; }
         return 0;
     }

@@ -453,16 +453,17 @@ int make_dense_map(CUtensorMap *map, const double *base, int64_t N, int64_t ld)
 
 int sk_grid()
 {
-    static int g = 0;
-    if (!g) {
-        int dev = 0, sms = 0, coop = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+    static int g[MAX_DEVICES] = {};
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    if (!g[dev]) {
+        int sms = 0, coop = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop)
             return 0;
-        g = sms < SK_MAX_GRID ? sms : SK_MAX_GRID;      // one CTA per SM (198 KB of shared memory each)
+        g[dev] = sms < SK_MAX_GRID ? sms : SK_MAX_GRID;      // one CTA per SM (198 KB of shared memory each)
     }
-    return g;
+    return g[dev];
 }
 
 // number of CTAs (= per-CTA partial-sum slots) of one product
@@ -493,13 +494,8 @@ static int launch_x2_dense_fp64_sk(const CUtensorMap &map0, const CUtensorMap &m
 {
     const int G = sk_grid();
     if (G <= 0 || !sk) return BML_ERR_CUDA;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(x2_dense_fp64_sk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)d_smem_bytes(128)) != cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
-    }
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(x2_dense_fp64_sk_kernel, d_smem_bytes(128), have)) return BML_ERR_CUDA;
     double *scratch = (double *)sk;
     unsigned int *flags = (unsigned int *)((uint8_t *)sk + (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double));
     int n = (int)N;
@@ -515,13 +511,8 @@ template <int BT>
 static int launch_x2_dense_fp64_t(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1,
                                   int64_t ld, int64_t N, Sp2Ctl *ctl, double *partials, cudaStream_t stream)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(x2_dense_fp64_kernel<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)d_smem_bytes(BT)) != cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
-    }
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(x2_dense_fp64_kernel<BT>, d_smem_bytes(BT), have)) return BML_ERR_CUDA;
     x2_dense_fp64_kernel<BT><<<dense_fp64_num_tiles(N), D_THREADS, d_smem_bytes(BT), stream>>>(map0, map1, buf0, buf1, ld,
                                                                                               (int)N, ctl, partials);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;

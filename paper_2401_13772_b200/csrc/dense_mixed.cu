@@ -516,13 +516,8 @@ static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double 
 {
     constexpr size_t smem = (size_t)MixedCfg<V>::STAGES * 2 * MixedCfg<V>::PLANES * (M_BM * MixedCfg<V>::BK * 2) +
                             1024 /*align*/ + 1024 /*barriers, scratch*/;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(x2_dense_mixed_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
-            cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
-    }
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(x2_dense_mixed_kernel<V>, smem, have)) return BML_ERR_CUDA;
     diag_x2_fp64_kernel<<<(unsigned)((N + 7) / 8), 256, 0, st>>>(b0, b1, ld, (int)N, ctl, dsq);
     x2_dense_mixed_kernel<V><<<dense_mixed_num_tiles(N), M_THREADS, smem, st>>>(m0, m1, b0, b1, p0, p1, ld, (int)N, ctl,
                                                                                 partials, dsq);
@@ -531,7 +526,7 @@ static int launch_x2_mixed(const CUtensorMap &m0, const CUtensorMap &m1, double 
 
 template <int V>
 static int solve_v(int64_t N, int max_products, double *X0, double *X1, int64_t ldx, Sp2Ctl *ctl, double *partials,
-                   void *extra, cudaStream_t st)
+                   void *extra, cudaStream_t st, bool no_host_wait = false)
 {
     uint16_t *p0 = (uint16_t *)extra;
     uint16_t *p1 = (uint16_t *)((uint8_t *)extra + plane_set_bytes(N, ldx));
@@ -543,15 +538,16 @@ static int solve_v(int64_t N, int max_products, double *X0, double *X1, int64_t 
     if ((r = launch_split<V>(X0, ldx, N, p0, st))) return r;
     if (max_products == 1) return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, dsq, st);
     return enqueue_products([&]() { return launch_x2_mixed<V>(m0, m1, X0, X1, p0, p1, ldx, N, ctl, partials, dsq, st); },
-                            ctl, max_products, st);
+                            ctl, max_products, st, 0, no_host_wait);
 }
 
 // X0 (already rescaled, in buffer 0) -> planes of buffer 0, then the fused products
 int sp2_dense_mixed_solve(const bml_matrix_t *H, const bml_sp2_params_t *p, double *X0, double *X1, int64_t ldx,
-                          Sp2Ctl *ctl, double *partials, const double *, void *extra, cudaStream_t st)
+                          Sp2Ctl *ctl, double *partials, const double *, void *extra, cudaStream_t st, bool no_host_wait)
 {
-    if (p->precision == MV_BF16X3) return solve_v<MV_BF16X3>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st);
-    return solve_v<MV_F16X2>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st);
+    if (p->precision == MV_BF16X3)
+        return solve_v<MV_BF16X3>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st, no_host_wait);
+    return solve_v<MV_F16X2>(H->N, p->max_products, X0, X1, ldx, ctl, partials, extra, st, no_host_wait);
 }
 
 // one product on a caller-supplied iterate (the control block was initialised in standalone mode)

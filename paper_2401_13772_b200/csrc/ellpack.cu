@@ -709,6 +709,7 @@ copy_out_ellpack_kernel(const double *__restrict__ v0, const int32_t *__restrict
                         int64_t N, int M, const Sp2Ctl *__restrict__ ctl, double *__restrict__ dv,
                         int32_t *__restrict__ di, int32_t *__restrict__ dn)
 {
+    if (ctl->done && ctl->status < 0) return;       // failed solve: D is left untouched
     const int parity = ctl->parity;
     const double *__restrict__ sv = parity ? v1 : v0;
     const int32_t *__restrict__ si = parity ? i1 : i0;
@@ -737,16 +738,7 @@ __global__ void x2_ellpack_info_kernel(const Sp2Ctl *__restrict__ ctl, int32_t *
 // ------------------------------------------------------------------------------------------------------------
 #define BML_CHECK_LAUNCH() do { if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA; } while (0)
 
-static int sm_count()
-{
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            sms = 0;
-    }
-    return sms;
-}
+static int sm_count() { return device_sm_count(); }
 
 // bytes of the scratch the symmetric product needs: upper parts (tv, ti, tn) and lower lists (lv, li, lcnt)
 size_t ellpack_sym_bytes(int64_t N, int M)
@@ -787,13 +779,8 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
     if (ngroups > E_MAX_GROUPS) ngroups = E_MAX_GROUPS;
     if (ngroups < 1 || M > 8 * E_GT) return BML_ERR_INVALID;
     const size_t smem1 = (size_t)ngroups * e_group_bytes(M);
-    static size_t attr1 = 0;
-    if (smem1 > attr1) {
-        if (cudaFuncSetAttribute(x2_ellpack_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1) !=
-            cudaSuccess)
-            return BML_ERR_CUDA;
-        attr1 = smem1;
-    }
+    static size_t attr1[MAX_DEVICES] = {};
+    if (ensure_smem_attr(x2_ellpack_upper_kernel, smem1, attr1)) return BML_ERR_CUDA;
     int64_t grid1 = (N + ngroups - 1) / ngroups;
     if (grid1 > sms) grid1 = sms;
     x2_ellpack_upper_kernel<<<(unsigned)grid1, ngroups * E_GT, smem1, st>>>(
@@ -806,13 +793,8 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
     if (nwarps > A_MAX_WARPS) nwarps = A_MAX_WARPS;
     if (nwarps < 1) return BML_ERR_INVALID;
     const size_t smem2 = (size_t)nwarps * wbytes;
-    static size_t attr2 = 48 * 1024;
-    if (smem2 > attr2) {
-        if (cudaFuncSetAttribute(x2_ellpack_assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2) !=
-            cudaSuccess)
-            return BML_ERR_CUDA;
-        attr2 = smem2;
-    }
+    static size_t attr2[MAX_DEVICES] = {};
+    if (ensure_smem_attr(x2_ellpack_assemble_kernel, smem2, attr2, 48 * 1024)) return BML_ERR_CUDA;
     int64_t grid2 = (N + nwarps - 1) / nwarps;
     const int64_t per_sm = (int64_t)(smem_cap / smem2) > 0 ? (int64_t)(smem_cap / smem2) : 1;
     if (grid2 > sms * per_sm) grid2 = sms * per_sm;
@@ -832,12 +814,8 @@ int launch_rescale_ellpack(const bml_matrix_t *H, const double *d_bounds, double
     const int cap = next_pow2(M + 1) < 32 ? 32 : next_pow2(M + 1);
     const int nwarps = 4;
     const size_t smem = (size_t)nwarps * cap * 8;
-    static size_t attr_smem = 48 * 1024;
-    if (smem > attr_smem) {
-        if (cudaFuncSetAttribute(rescale_ellpack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_smem = smem;
-    }
+    static size_t attr_smem[MAX_DEVICES] = {};
+    if (ensure_smem_attr(rescale_ellpack_kernel, smem, attr_smem, 48 * 1024)) return BML_ERR_CUDA;
     rescale_ellpack_kernel<<<(N + nwarps - 1) / nwarps, nwarps * 32, smem, st>>>(H->value, H->index, H->nnz, N, M,
                                                                                   d_bounds, xv, xi, xn, diag,
                                                                                   fail_flag, cap);

@@ -178,6 +178,7 @@ __global__ void __launch_bounds__(256) copy_out_dense_kernel(const double *__res
                                                              const Sp2Ctl *__restrict__ ctl, double *__restrict__ D,
                                                              int64_t ldd)
 {
+    if (ctl->done && ctl->status < 0) return;       // failed solve: D is left untouched (X_0 may hold Inf / NaN)
     const double *__restrict__ X = ctl->parity ? buf1 : buf0;
     const int row = blockIdx.x;
     for (int j = blockIdx.y * blockDim.x + threadIdx.x; j < N; j += gridDim.y * blockDim.x)

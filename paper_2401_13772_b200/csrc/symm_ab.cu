@@ -286,13 +286,8 @@ static int launch_symm_t(const CUtensorMap &map, const SymmBatch &batch, int64_t
 {
     const int G = sk_grid();
     if (G <= 0 || !sk) return BML_ERR_CUDA;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(symm_ab_fp64_kernel<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)d_smem_bytes(BT)) != cudaSuccess)
-            return BML_ERR_CUDA;
-        attr_set = true;
-    }
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(symm_ab_fp64_kernel<BT>, d_smem_bytes(BT), have)) return BML_ERR_CUDA;
     double *scratch = (double *)sk;
     unsigned int *flags = symm_flags(sk);
     int n = (int)N;
