@@ -3,8 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload dense_n2048] [--impl ours|reference]
 
-Workloads: the BASELINE.json configs (dense_n256, dense_n2048 [default], dense_n8192, mixed_n16384, mixed_bf16x3_n16384,
-ellpack_n65536) and, for the Chebyshev expansion of PAPER.md IV.B, cheby_n500 / n1000 / n2000 / n4000 / n8000 (one step =
+Workloads: the BASELINE.json configs (dense_n256, dense_n2048, dense_n8192 [default], mixed_n16384 (FP16 x 2 split),
+mixed_bf16x3_n16384 (the BF16 split BASELINE.json names), ellpack_n65536 (the labelled stand-in 5'), ellpack_n65536_literal);
+the default run also measures all the others and attaches them to its JSON line as `per_config` and, for the Chebyshev expansion of PAPER.md IV.B, cheby_n500 / n1000 / n2000 / n4000 / n8000 (one step =
 one bml_chebyshev_dense call; metric chebyshev_time_to_D_ms) and, for the graph-based construction of VIII.B,
 graph_n1536 / graph_n12800 (one step = one bml_graph_chebyshev_ellpack call; metric graph_time_to_D_ms).
 
@@ -31,6 +32,7 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 METRIC = "sp2_time_to_D_ms"
+DEFAULT_WORKLOAD = "dense_n8192"            # BASELINE.json configs[2]: the largest FP64 single-GPU configuration
 METRIC_CHEBY = "chebyshev_time_to_D_ms"     # SURVEY 8(f) item f-1 workloads (--workload cheby_n*)
 METRIC_GRAPH = "graph_time_to_D_ms"         # SURVEY 8(f) item f-2 workloads (--workload graph_n*)
 PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 64 FMA/clk/SM
@@ -47,18 +49,54 @@ def dense_flops_per_product(N: int) -> float:
     return 2.0 * (T * (T + 1) // 2) * float(bt) * float(bt) * N
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_ncu_kernels.md names the commands); None = no capture of this workload.
-NCU_TRAFFIC_BYTES = {
-    "dense_n2048": 43.2e6,          # 33.9 MB read (= N^2 x 8 B: X read once) + 9.2 MB written (X' mostly stays in L2)
-    "dense_n8192": 6.09e9,          # 5.56 GB read (row panels re-read) + 0.53 GB written
-    "mixed_n16384": 20.4e9,         # 17.2 GB read + 3.2 GB written (FP16 x 2 planes, super-block tile order)
-    "mixed_bf16x3_n16384": 71.5e9,  # 67.5 GB read + 4.0 GB written (capture quoted in DESIGN.md 5.3)
-    "cheby_n2000": 98.1e6,          # grouped product kernel, one Eq. 10 step: 85.3 MB read + 12.8 MB written
-    "cheby_n4000": 891.3e6,         # one Eq. 10 step: 766.1 MB read + 125.2 MB written (512 MB algorithmic)
-    "graph_n12800": 1.84e9,         # per product at part size 5600 (captured launch: 4 products, 6.36 GB + 1.00 GB)
-    "ellpack_n65536": 1.25e9,       # kernel 1: 0.246 + 0.190 GB; kernel 2: 0.451 + 0.363 GB (read + written)
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel come from the committed ncu captures:
+# profiles/r02_traffic.json, written by `python bench.py --traffic-from <ncu raw csv> --workload W` from the
+# `ncu -i <rep> --page raw --csv` export of an `ncu --set full` capture (the .md beside it names the capture command).
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def ncu_traffic(workload: str):
+    """{'bytes': per-launch DRAM bytes of the workload's dominant kernel(s) or None, 'source': where it came from}."""
+    try:
+        entry = json.load(open(TRAFFIC_JSON)).get(workload)
+    except (OSError, ValueError):
+        entry = None
+    if not entry:
+        return {"bytes": None, "source": "no ncu capture of this workload in profiles/r02_traffic.json"}
+    return {"bytes": float(entry["dram_bytes_per_launch"]), "source": entry.get("source", "profiles/r02_traffic.json")}
+
+
+def write_traffic(csv_path: str, workload: str, kernels: list[str], note: str = ""):
+    """Parse an `ncu --page raw --csv` export: per kernel name in `kernels` (substring match) the mean per-launch
+    dram__bytes_read.sum + dram__bytes_write.sum; their sum is stored as the workload's per-launch traffic."""
+    import csv
+
+    rows = list(csv.reader(open(csv_path)))
+    hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+    names, units = rows[hdr], rows[hdr + 1]
+    col = {n: i for i, n in enumerate(names)}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+    def val(r, key):
+        return float(r[col[key]].replace(",", "")) * scale[units[col[key]]]
+
+    per_kernel = {}
+    for k in kernels:
+        sel = [r for r in rows[hdr + 2:] if len(r) > col["Kernel Name"] and k in r[col["Kernel Name"]]]
+        if not sel:
+            raise SystemExit(f"kernel {k!r} not in {csv_path}")
+        rd = sum(val(r, "dram__bytes_read.sum") for r in sel) / len(sel)
+        wr = sum(val(r, "dram__bytes_write.sum") for r in sel) / len(sel)
+        per_kernel[k] = {"launches": len(sel), "dram_bytes_read": rd, "dram_bytes_write": wr}
+    data = json.load(open(TRAFFIC_JSON)) if os.path.exists(TRAFFIC_JSON) else {}
+    data[workload] = {
+        "dram_bytes_per_launch": sum(v["dram_bytes_read"] + v["dram_bytes_write"] for v in per_kernel.values()),
+        "kernels": per_kernel, "source": "profiles/" + os.path.basename(csv_path), "note": note,
+    }
+    with open(TRAFFIC_JSON, "w") as f:
+        json.dump(data, f, indent=1, sort_keys=True)
+        f.write("\n")
+    print(json.dumps(data[workload]))
 
 
 def peaks():
@@ -299,8 +337,16 @@ def workload_config(name: str):
     w = hm.WORKLOADS[name]
     cfg = {"workload": name, "kind": w.kind, "N": w.N, "n_occ": w.n_occ, "idem_tol": w.idem_tol, "note": w.note,
            "seed": 0, "max_products": 100,
-           "l2": "flushed between steps (256 MiB write); H + both iterates (96 MiB at N=2048) then stay L2-resident "
-                 "within a step, which is part of the method"}
+           "l2": "flushed between steps (256 MiB write > the 126 MB L2)"}
+    if w.kind == "dense":
+        resident = 3 * w.N * w.N * 8 / 2**20
+        cfg["l2"] += (f"; H + both iterates are {resident:.0f} MiB: " +
+                      ("they then stay L2-resident within a step, which is part of the method" if resident < 120
+                       else "larger than L2, every product streams its operands from HBM"))
+        cfg["arithmetic"] = {0: "fp64 (DMMA)", 1: "mixed: FP16 x 2 split products on tcgen05, FP64 elsewhere "
+                                "(NOT the split BASELINE.json names; see mixed_bf16x3_n16384)",
+                             2: "mixed: BF16 x 3 split products on tcgen05, FP64 elsewhere (the BF16 split of "
+                                "BASELINE.json configs[3])"}[w.precision]
     if w.kind == "ellpack":
         cfg.update({"M": w.M, "drop_tol": w.drop_tol})
     if w.kind == "graph":
@@ -429,21 +475,26 @@ def timed_e2e(rk: Ranks, step, n: int) -> float:
 # ----------------------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------------------
-def run_ours(args):
+def sp2_measure(rk: Ranks, wname: str, steps: int, warmup: int, lanczos_steps: int = 0, e2e_steps: int | None = None):
+    """One SP2 workload through the C ABI: W warm-ups + K timed solves on a resident H (CUDA events, L2 flushed between
+    steps, clocks sampled), the end-to-end leg with host buffers, and the dominant kernel timed alone against its
+    roofline.  Returns (record dict, H as numpy) -- the record is the body of the JSON line / of a per_config entry."""
+    import contextlib
+    import types
+
     import torch
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    rk = Ranks()
-    api.load()
-    dev, dist, world, rank = rk.dev, rk.dist, rk.world, rk.rank
-    w = hm.WORKLOADS[args.workload]
+    args = types.SimpleNamespace(steps=steps, warmup=warmup)
+    dev = rk.dev
+    w = hm.WORKLOADS[wname]
     dense = w.kind == "dense"
-    sp2_flags = api.FLAG_LANCZOS_BOUNDS(args.lanczos_steps) if args.lanczos_steps else 0
+    sp2_flags = api.FLAG_LANCZOS_BOUNDS(lanczos_steps) if lanczos_steps else 0
 
     # ---- inputs: seeded synthetic Hamiltonian, resident in HBM; pinned host copies for the e2e leg
     if dense:
-        H_np = hm.make_dense(args.workload)
+        H_np = hm.make_dense(wname)
         H_host = torch.from_numpy(H_np).pin_memory()
         H_dev = H_host.to(dev)
         solver = api.DenseSolver(w.N, dev, precision=w.precision)
@@ -452,7 +503,7 @@ def run_ours(args):
         def solve(Hd):
             return solver.solve(Hd, w.n_occ, w.idem_tol, 100, flags=sp2_flags)
     else:
-        H_np = hm.make_ellpack(args.workload)
+        H_np = hm.make_ellpack(wname)
         H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
         H_dev = tuple(a.to(dev) for a in H_host)
         solver = api.EllpackSolver(w.N, w.M, dev)
@@ -463,8 +514,6 @@ def run_ours(args):
 
     # Small dense matrices run on a stream of their own: the library replays the static head of such a solve as a CUDA
     # graph, which the legacy default stream cannot capture.  Everything else stays on the current stream.
-    import contextlib
-
     side = torch.cuda.Stream(dev) if (dense and w.N <= 1024) else None
     if side is not None:
         side.wait_stream(torch.cuda.current_stream())
@@ -487,18 +536,22 @@ def run_ours(args):
                     dst.copy_(src, non_blocking=True)
             torch.cuda.synchronize()
 
-        e2e_steps = max(3, min(args.steps, 10))
+        if e2e_steps is None:
+            e2e_steps = max(3, min(steps, 10))
         h2d = H_host.numel() * 8 if dense else sum(a.numel() * a.element_size() for a in H_host)
         d2h = h2d
-        e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
+        e2e_ms = timed_e2e(rk, e2e_step, e2e_steps) if res.status >= 0 else float("nan")
     if side is not None:
         torch.cuda.current_stream().wait_stream(side)
 
     # ---- dominant kernel, timed alone with CUDA events on the launching stream
     pk, pk_src = peaks()
+    traffic = ncu_traffic(wname)
     roof = None
     n_prod = int(res.n_products)
-    if dense and w.precision == 0:
+    if res.status < 0:
+        roof = None
+    elif dense and w.precision == 0:
         lo_hi = api.bml_gershgorin(H_dev).cpu().numpy()
         s = 1.0 / (lo_hi[1] - lo_hi[0])
         X0 = api.padded_dense((lo_hi[1] * torch.eye(w.N, dtype=torch.float64) - H_host) * s, dev)
@@ -513,7 +566,8 @@ def run_ours(args):
             "bound": "tensor",
             "kernel": "x2_dense_fp64_sk_kernel" if w.N > 1024 else "x2_dense_fp64_kernel<%d>" % (32 if w.N <= 512 else 64),
             "achieved": achieved, "peak": peak_probe,
-            "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+            "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": traffic["bytes"], "traffic_source": traffic["source"],
+            "algorithmic_bytes": 2.0 * w.N * w.N * 8,
             "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
                            "(MEASURED_PEAKS.json has no FP64 entry)",
             "peak_alt_bf16_ratio": nominal_ratio_peak,
@@ -522,6 +576,7 @@ def run_ours(args):
             "launch_ms": k_ms, "flops_per_launch": flops,
             "in_step_tflops": flops * n_prod / (ms * 1e-3) / 1e12,
         }
+        del X0, Xn, ws
     elif dense and w.precision != 0:
         # mixed mode: the fused split-plane tcgen05 product, timed alone through bml_x2_dense(precision); that entry
         # point also runs the (HBM-bound, ~2% of the time) FP64 -> 16-bit planes split of its input
@@ -536,7 +591,8 @@ def run_ours(args):
         achieved = flops / (k_ms * 1e-3) / 1e12
         roof = {
             "bound": "tensor", "kernel": "x2_dense_mixed_kernel", "achieved": achieved, "peak": pk["bf16_tflops"],
-            "unit": "TFLOP/s", "frac": achieved / pk["bf16_tflops"], "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+            "unit": "TFLOP/s", "frac": achieved / pk["bf16_tflops"], "traffic": traffic["bytes"],
+            "traffic_source": traffic["source"],
             "peak_source": f"{pk_src} bf16 burst (cuBLAS) from MEASURED_PEAKS.json (fp16 and bf16 share the tcgen05 "
                            "kind::f16 rate); kernel timed alone (launch includes the FP64 -> 16-bit planes split)",
             "cross_terms": terms,
@@ -557,32 +613,33 @@ def run_ours(args):
         ws = api._workspace(api.load().bml_x2_ellpack_workspace_bytes(w.N, w.M), dev)
         k_ms = time_alone(lambda: api.bml_x2_ellpack(Xmid, 1, w.drop_tol, out, ws), 5, warm=2)
         comp_bytes = float((12 * nn + 4).sum().item() + (12 * out[2].to(torch.int64) + 4).sum().item())
+        gathered = 12.0 * macs
         achieved = comp_bytes / (k_ms * 1e-3) / 1e9
         roof = {
-            "bound": "hbm", "kernel": "x2_ellpack_upper_kernel + x2_ellpack_assemble_kernel", "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-            "frac": achieved / pk["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+            "bound": "hbm", "kernel": "x2_ellpack_upper_kernel + x2_ellpack_assemble_kernel", "achieved": achieved,
+            "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": achieved / pk["hbm_gbs"],
+            "frac_uses": "compulsory bytes (read X_5 + write X_6: 12 B per stored entry + 4 B per row)",
+            "traffic": traffic["bytes"], "traffic_source": traffic["source"],
             "peak_source": f"{pk_src} copy bandwidth from MEASURED_PEAKS.json",
-            "note": "achieved = COMPULSORY bytes (read X_5 + write X_6, 12 B per stored entry + 4 B per row) / time; "
-                    "the kernel is bound by shared-memory hash updates and issue slots, not HBM (DESIGN.md 5.4)",
-            "launch_ms": k_ms, "compulsory_bytes": comp_bytes, "macs_per_launch": macs,
+            "note": "SURVEY 8(d): three byte counts.  `frac` uses the COMPULSORY bytes; the kernel is bound by "
+                    "shared-memory hash updates and issue slots, not HBM (DESIGN.md 5.4), so that fraction is small by "
+                    "construction; the gathered-bytes rate is what BASELINE.json's '>= 60% of HBM' can be read on",
+            "launch_ms": k_ms,
+            "bytes": {
+                "compulsory": {"bytes": comp_bytes, "gbs": achieved, "frac_of_hbm": achieved / pk["hbm_gbs"]},
+                "ncu_dram": None if traffic["bytes"] is None else {
+                    "bytes": traffic["bytes"], "gbs": traffic["bytes"] / (k_ms * 1e-3) / 1e9,
+                    "frac_of_hbm": traffic["bytes"] / (k_ms * 1e-3) / 1e9 / pk["hbm_gbs"]},
+                "gathered": {"bytes": gathered, "gbs": gathered / (k_ms * 1e-3) / 1e9,
+                             "frac_of_hbm": gathered / (k_ms * 1e-3) / 1e9 / pk["hbm_gbs"]},
+            },
+            "compulsory_bytes": comp_bytes, "macs_per_launch": macs,
             "macs_note": "full-row Gustavson count sum_i sum_{k in i} n_k; the kernel executes about half of them "
                          "(columns j >= i only, mirrored by symmetry)",
-            "gathered_gbs": 12.0 * macs / (k_ms * 1e-3) / 1e9, "gmacs_per_s": macs / (k_ms * 1e-3) / 1e9,
+            "gathered_gbs": gathered / (k_ms * 1e-3) / 1e9, "gmacs_per_s": macs / (k_ms * 1e-3) / 1e9,
             "mean_row_nnz": float(nn.double().mean().item()),
         }
-
-    # ---- aggregate over ranks: max time
-    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], dist, dev)
-
-    if rank != 0:
-        rk.finish()
-        return 0
-
-    # ---- CPU oracle baseline (rank 0, N = 1 only): bounded sample, ~10-30 s
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        v, sample, cores = oracle_time_to_D(args.workload, H_np, 25.0, n_prod)
-        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
+        del Xmid, out, ws
 
     # product launches of one solve: a first batch of 16, then batches of 8 kept one batch ahead of the device until
     # the host sees the stop flag (api.cu enqueue_products); launches behind the stop flag exit at once on the device
@@ -595,25 +652,95 @@ def run_ours(args):
     pre = (2 + 1 + 1 + 1 + (1 if w.precision != 0 else 0)) if dense else (2 + 2 + 1)
     # a sparse product is two kernels; a mixed product is the FP64-diagonal kernel + the tcgen05 kernel
     launches_per_step = pre + n_enq * (2 if (not dense or w.precision != 0) else 1) + 1
+    rec = {
+        "ms": ms, "step_ms": step_ms, "t_wall": t_wall, "clocks": clocks, "res": res, "n_products": n_prod,
+        "e2e_ms": e2e_ms, "e2e_steps": e2e_steps, "h2d": int(h2d), "d2h": int(d2h), "roofline": roof,
+        "launches_per_step": launches_per_step,
+        "dtype": {0: "f64", 1: "fp16x2 split products (fp32 TMEM chunks) + f64 accumulate/update",
+                  2: "bf16x3 split products (fp32 TMEM chunks) + f64 accumulate/update"}[w.precision if dense else 0],
+    }
+    del solver, H_dev, H_host, D_host
+    torch.cuda.empty_cache()
+    return rec, H_np
+
+
+# the other BASELINE.json configs, measured in the same run and attached to the default line as `per_config`
+PER_CONFIG = [("dense_n256", 10), ("dense_n2048", 10), ("mixed_bf16x3_n16384", 3), ("mixed_n16384", 3),
+              ("ellpack_n65536", 3), ("ellpack_n65536_literal", 1)]
+
+
+def per_config_block(rk: Ranks, skip: str, only=None):
+    out = {}
+    for wname, steps in PER_CONFIG:
+        if wname == skip or (only and wname not in only):
+            continue
+        t0 = time.perf_counter()
+        try:
+            rec, _ = sp2_measure(rk, wname, steps, 3, 0, e2e_steps=2)
+        except Exception as e:      # one config must not take the headline down with it
+            out[wname] = {"error": f"{type(e).__name__}: {e}"}
+            continue
+        res = rec["res"]
+        out[wname] = {
+            "config": workload_config(wname), "dtype": rec["dtype"], "ms": rec["ms"], "steps": steps, "warmup": 3,
+            "step_ms_min": float(min(rec["step_ms"])), "step_ms_max": float(max(rec["step_ms"])),
+            "status": int(res.status), "status_string": res.message, "n_products": rec["n_products"],
+            "branch": res.branch, "max_row_nnz": [int(x) for x in res.max_row_nnz] if "ellpack" in wname else None,
+            "overflow_row": int(res.overflow_row),
+            "e2e": {"value": rec["e2e_ms"], "unit": "ms", "h2d_bytes_per_step": rec["h2d"],
+                    "d2h_bytes_per_step": rec["d2h"], "steps": rec["e2e_steps"]},
+            "roofline": rec["roofline"], "clocks": rec["clocks"], "gpu_launches_per_step": rec["launches_per_step"],
+            "bench_wall_s": round(time.perf_counter() - t0, 1),
+        }
+    return out
+
+
+def run_ours(args):
+    from paper_2401_13772_b200 import api
+
+    rk = Ranks()
+    api.load()
+    dev, dist, world, rank = rk.dev, rk.dist, rk.world, rk.rank
+    rec, H_np = sp2_measure(rk, args.workload, args.steps, args.warmup, args.lanczos_steps)
+    res, n_prod, step_ms, clocks = rec["res"], rec["n_products"], rec["step_ms"], rec["clocks"]
+    launches_per_step = rec["launches_per_step"]
+
+    # ---- aggregate over ranks: max time
+    ms, e2e_ms = aggregate_over_ranks([rec["ms"], rec["e2e_ms"]], dist, dev)
+
+    if rank != 0:
+        rk.finish()
+        return 0
+
+    # ---- the other configs of BASELINE.json (one GPU, default run only)
+    per_config = None
+    if world == 1 and args.per_config:
+        per_config = per_config_block(rk, args.workload, [x for x in args.per_config_list.split(",") if x])
+
+    # ---- CPU oracle baseline (rank 0, N = 1 only): bounded sample, ~10-30 s
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, sample, cores = oracle_time_to_D(args.workload, H_np, 25.0, n_prod)
+        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
+
     line = {
         "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": {0: "f64", 1: "fp16x2 split products (fp32 TMEM chunks) + f64 accumulate/update",
-                  2: "bf16x3 split products (fp32 TMEM chunks) + f64 accumulate/update"}[w.precision if dense else 0],
+        "dtype": rec["dtype"],
         "data": "synthetic", "config": workload_config(args.workload),
         "status": int(res.status), "n_products": n_prod, "branch": res.branch,
         "spectral_bounds": {"emin": res.emin, "emax": res.emax,
                             "kind": f"lanczos({args.lanczos_steps}) within gershgorin" if args.lanczos_steps else "gershgorin"},
-        "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
+        "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": rec["t_wall"],
         "ms_per_product": ms / max(n_prod, 1),
         "aggregate_solves_per_s": replicas_per_second(world, ms),
-        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "steps": e2e_steps},
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": rec["h2d"], "d2h_bytes_per_step": rec["d2h"],
+                "steps": rec["e2e_steps"]},
         "gpu_launches": launches_per_step * args.steps,
         "gpu_launches_note": f"{launches_per_step} per step (upper bound: the host stops enqueueing one or two batches of "
                              f"8 after the stop flag); {n_prod} product launches do work, the rest exit on the "
                              "device-side stop flag",
-        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+        "roofline": rec["roofline"], "cpu_baseline": cpu, "clocks": clocks, "per_config": per_config,
     }
     print(json.dumps(line), flush=True)
     rk.finish()
@@ -674,7 +801,7 @@ def run_cheby(args):
     sums_bytes = float(w.k - 1 + w.m) * w.N * w.N * 8
     roof = {
         "bound": "tensor", "kernel": "symm_ab_fp64_kernel<%d>" % bt, "achieved": achieved, "peak": peak_probe,
-        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
         "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
                        "(MEASURED_PEAKS.json has no FP64 entry)",
         "launch_ms": k_ms, "flops_per_launch": flops,
@@ -768,7 +895,7 @@ def run_graph(args):
     step_flops = sum(dense_flops_per_product(int(sz)) for sz in res.part_size) * (w.k + w.m - 2)
     roof = {
         "bound": "tensor", "kernel": "symm_ab_fp64_kernel<128>", "achieved": achieved, "peak": peak_probe,
-        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
         "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
                        "(MEASURED_PEAKS.json has no FP64 entry)",
         "launch_ms": k_ms, "flops_per_launch": flops, "part_size": cap,
@@ -813,12 +940,26 @@ def main():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="dense_n2048")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-config", dest="per_config", action="store_true", default=None,
+                    help="attach the other BASELINE.json configs as `per_config` (default: on for the default workload)")
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false")
+    ap.add_argument("--per-config-list", default="", help="restrict per_config to these workloads (comma-separated)")
+    ap.add_argument("--traffic-from", default=None, metavar="CSV",
+                    help="no benchmark: parse an `ncu --page raw --csv` export and store the per-launch DRAM bytes of "
+                         "--traffic-kernels under --workload in profiles/r02_traffic.json")
+    ap.add_argument("--traffic-kernels", default="", help="comma-separated kernel-name substrings")
+    ap.add_argument("--traffic-note", default="")
     ap.add_argument("--lanczos-steps", type=int, default=0,
                     help="SP2 workloads: tighten the Gershgorin bounds with K Lanczos steps (8..64); 0 = Gershgorin only, "
                          "the configuration BASELINE.json names")
     args = ap.parse_args()
+    if args.traffic_from:
+        write_traffic(args.traffic_from, args.workload, [k for k in args.traffic_kernels.split(",") if k], args.traffic_note)
+        return 0
+    if args.per_config is None:
+        args.per_config = args.workload == DEFAULT_WORKLOAD and args.impl == "ours"
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

@@ -93,3 +93,51 @@ def test_reference_arm_prints_the_contract_line(monkeypatch, capsys, workload, m
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["config"]["workload"] == workload and d["gpu_launches"] == 0
+
+
+def test_default_line_is_the_largest_fp64_config_and_per_config_covers_the_rest():
+    """the driver runs the default, so the default must be configs[2] (N = 8192) and carry every other
+    BASELINE.json config as a per_config record."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    assert bench.DEFAULT_WORKLOAD == "dense_n8192"
+    names = [n for n, _ in bench.PER_CONFIG]
+    assert names == ["dense_n256", "dense_n2048", "mixed_bf16x3_n16384", "mixed_n16384", "ellpack_n65536",
+                     "ellpack_n65536_literal"]
+    for n in names:
+        cfg = bench.workload_config(n)
+        assert cfg["workload"] == n and "model" not in cfg
+    assert "BF16 x 3" in bench.workload_config("mixed_bf16x3_n16384")["arithmetic"]
+    assert "FP16 x 2" in bench.workload_config("mixed_n16384")["arithmetic"]
+    assert hm.WORKLOADS["dense_n8192"].N == 8192
+
+
+def test_traffic_is_read_from_the_committed_capture_summary(tmp_path, monkeypatch):
+    """roofline.traffic comes from profiles/r02_traffic.json, which `bench.py --traffic-from` writes from an
+    `ncu --page raw --csv` export (units row under the header row, one row per profiled launch)."""
+    import json
+
+    sys.path.insert(0, ROOT)
+    import bench
+
+    committed = json.load(open(bench.TRAFFIC_JSON))
+    for name in ("dense_n8192", "dense_n2048", "mixed_n16384", "mixed_bf16x3_n16384", "ellpack_n65536"):
+        assert committed[name]["dram_bytes_per_launch"] > 0 and committed[name]["source"].startswith("profiles/")
+        assert bench.ncu_traffic(name)["bytes"] == committed[name]["dram_bytes_per_launch"]
+    assert bench.ncu_traffic("no_such_workload")["bytes"] is None
+
+    csv = tmp_path / "raw.csv"
+    csv.write_text(
+        '"ID","Kernel Name","dram__bytes_read.sum","dram__bytes_write.sum"\n'
+        '"","","Mbyte","Kbyte"\n'
+        '"0","k_a(int)","10.5","2,000"\n'
+        '"1","k_b<1>(double)","1","0"\n'
+        '"2","k_a(int)","11.5","4,000"\n')
+    monkeypatch.setattr(bench, "TRAFFIC_JSON", str(tmp_path / "t.json"))
+    bench.write_traffic(str(csv), "w", ["k_a", "k_b"], "unit test")
+    got = json.load(open(tmp_path / "t.json"))["w"]
+    assert got["kernels"]["k_a"] == {"launches": 2, "dram_bytes_read": 11.0e6, "dram_bytes_write": 3.0e6}
+    assert got["dram_bytes_per_launch"] == 11.0e6 + 3.0e6 + 1.0e6
+    assert bench.ncu_traffic("w")["bytes"] == 15.0e6

@@ -58,3 +58,25 @@ def test_bench_contract_chebyshev_workload():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 500 * 500 * 8 and d["e2e"]["value"] >= d["value"] * 0.5
     assert d["gpu_launches"] == 3 * (6 + 19)
+
+
+def test_bench_per_config_block():
+    """The default line attaches every other BASELINE.json config as `per_config`; here forced on for two cheap ones:
+    configs[0] and configs[4] as literally written, which must report the overflow failure it is graded on."""
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", "--workload",
+                          "dense_n2048", "--per-config", "--per-config-list", "dense_n256,ellpack_n65536_literal",
+                          "--no-cpu-baseline"], capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][0])
+    pc = d["per_config"]
+    assert sorted(pc) == ["dense_n256", "ellpack_n65536_literal"]
+    a = pc["dense_n256"]
+    assert a["status"] == 0 and a["n_products"] == 15 and a["roofline"]["bound"] == "tensor" and a["ms"] > 0
+    assert a["clocks"]["sm_max_mhz"] and a["e2e"]["h2d_bytes_per_step"] == 256 * 256 * 8
+    lit = pc["ellpack_n65536_literal"]
+    assert lit["status"] == -3 and lit["n_products"] == 1 and lit["max_row_nnz"][0] == 829 and lit["roofline"] is None
+    assert d["roofline"]["traffic"] > 0 and d["roofline"]["traffic_source"].startswith("profiles/")
