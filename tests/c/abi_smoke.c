@@ -58,7 +58,7 @@ int main(int argc, char **argv)
         tr_ref += a - a;
     }
     double *dH, *dD, *dS;
-    void *ws;
+    void *ws_raw, *ws;
     CHECK(cudaMalloc((void **)&dH, bytes) == cudaSuccess && cudaMalloc((void **)&dD, bytes) == cudaSuccess &&
           cudaMalloc((void **)&dS, 4 * sizeof(double)) == cudaSuccess);
     CHECK(cudaMemcpy(dH, h, bytes, cudaMemcpyHostToDevice) == cudaSuccess);
@@ -66,7 +66,8 @@ int main(int argc, char **argv)
     bml_sp2_params_t p = {N / 2, 100, 1e-10, 0.0, 0, 0};
     bml_sp2_stats_t st;
     const size_t wsb = bml_sp2_workspace_bytes(&H, &p);
-    CHECK(wsb > 0 && cudaMalloc(&ws, wsb) == cudaSuccess && ((size_t)ws & 1023) == 0);
+    CHECK(wsb > 0 && cudaMalloc(&ws_raw, wsb + 1024) == cudaSuccess);
+    ws = (void *)(((size_t)ws_raw + 1023) & ~(size_t)1023);           /* the workspace must be 1024-byte aligned */
 
     double s[4];
     CHECK(bml_gershgorin(&H, dS, ws, wsb, NULL) == BML_OK);

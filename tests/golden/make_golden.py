@@ -17,7 +17,8 @@ tests/golden/<case>_Dv.txt (one value per line, repr precision).  The full-size 
 
 Cost on 8 cores: dense_n8192 (32 naive N^3 products) and mixed_n16384_first4 (the FP64 oracle stopped after 4 products
 at N=16384: the reference for the mixed-precision kernel's X_3) ~15-30 min each; ellpack_n65536 (the 12-product 5'
-solve) ~1-2 min; the others seconds.
+solve) ~1-2 min; the others seconds.  `mixed_n16384` (not in the default list: the full 30-product FP64 oracle solve of
+configs[3], 1.3e14 multiply-adds) takes hours.
 """
 from __future__ import annotations
 
@@ -132,6 +133,8 @@ def run_case(name):
     if name == "mixed_n16384_first4":
         # the FP64 oracle on configs[3]'s input, stopped by S3 after 4 products: D = X_3 (reading 6), status 2
         return dense_case(name, max_products=4, workload="mixed_n16384")
+    # "mixed_n16384": reading 17 -- the oracle of the mixed-precision mode is the FP64 oracle at the mixed config's
+    # tolerance (1e-6); ~30 naive products at N = 16384, hours on 8 cores: run on request only
     return dense_case(name)
 
 

@@ -48,7 +48,9 @@ def test_oracle_reproduces_golden_ellpack_small(oracle_mod, gold):
 
 
 def test_golden_covers_the_dense_configs(gold):
-    for name in ("dense_n256", "dense_n2048"):
+    for name in ("dense_n256", "dense_n2048", "dense_n8192"):
+        if name not in gold:
+            pytest.skip(f"{name} not written yet")
         w = hm.WORKLOADS[name]
         g = gold[name]
         assert (g["N"], g["n_occ"], g["idem_tol"]) == (w.N, w.n_occ, w.idem_tol)
@@ -89,6 +91,79 @@ def test_gpu_matches_golden_dense(api, gold, name):
         assert abs(D[i, j].item() - v) <= TOL_D * g["D_fro"]
     assert abs(torch.trace(D).item() - g["D_trace"]) <= 1e-8
     assert abs(torch.linalg.norm(D).item() - g["D_fro"]) <= TOL_D * g["D_fro"]
+    if "Dv_file" in g:
+        # whole-matrix check: y = D_oracle v for the seeded Gaussian probe v; E ||A v||^2 = ||A||_F^2, so
+        # ||D_gpu v - y|| estimates ||D_gpu - D_oracle||_F over every entry (3 x: the estimate's spread)
+        y = torch.from_numpy(np.loadtxt(os.path.join(os.path.dirname(GOLD), g["Dv_file"]))).cuda()
+        v = torch.from_numpy(np.random.default_rng(g["probe_seed"]).standard_normal(g["N"])).cuda()
+        assert (torch.linalg.norm(D @ v - y) / g["D_fro"]).item() <= 3 * TOL_D
+
+
+def _ell_digest(dv, di, dn):
+    """Same digest as tests/golden/make_golden.py ell_digest (restated: the tests do not import the golden writer)."""
+    import hashlib
+
+    h = hashlib.sha256()
+    h.update(np.ascontiguousarray(dn, dtype=np.int32).tobytes())
+    keep = np.arange(dv.shape[1])[None, :] < dn[:, None]
+    h.update(np.ascontiguousarray(di[keep], dtype=np.int32).tobytes())
+    h.update(np.ascontiguousarray(dv[keep], dtype=np.float64).tobytes())
+    return h.hexdigest()
+
+
+@pytest.mark.gpu
+def test_gpu_matches_golden_ellpack_n65536_full_solve_bit_exact(api, gold):
+    """The labelled stand-in 5' at full size (N = 65536, M = 512, tau = 1e-6): the whole 12-product solve against the
+    oracle's -- status, branch string, traces, per-product row fill, and EVERY stored (column, value) of D bit for bit
+    (SHA-256 over nnz, columns and value bit patterns) plus 16 whole rows for a readable failure."""
+    import torch
+
+    g = gold["ellpack_n65536"]
+    w = hm.WORKLOADS["ellpack_n65536"]
+    assert (g["N"], g["M"], g["n_occ"], g["idem_tol"], g["drop_tol"]) == (w.N, w.M, w.n_occ, w.idem_tol, w.drop_tol)
+    H = hm.make_ellpack("ellpack_n65536")
+    (dv, di, dn), res = api.bml_sp2_ellpack(*(torch.from_numpy(a).cuda() for a in H), w.n_occ, w.idem_tol, w.drop_tol)
+    assert res.status == g["status"] == 1 and res.n_products == g["n_products"] and res.m_star == g["m_star"]
+    assert res.branch == g["branch"]
+    assert (res.emin, res.emax) == (g["emin"], g["emax"])
+    assert [int(x) for x in res.max_row_nnz] == g["max_row_nnz"]
+    np.testing.assert_allclose(res.trace, g["trace"], rtol=0, atol=1e-7)
+    np.testing.assert_allclose(res.idem, g["idem"], rtol=1e-6, atol=1e-14)
+    dv, di, dn = dv.cpu().numpy(), di.cpu().numpy(), dn.cpu().numpy()
+    assert int(dn.sum()) == g["D_nnz_total"] and int(dn.max()) == g["D_nnz_max"]
+    for r in g["D_rows"]:
+        n = int(dn[r["row"]])
+        assert di[r["row"], :n].tolist() == r["index"], r["row"]
+        assert dv[r["row"], :n].tolist() == r["value"], r["row"]
+    assert _ell_digest(dv, di, dn) == g["D_sha256"]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", [1, 2])
+def test_gpu_mixed_n16384_first_products_match_the_fp64_oracle(api, gold, precision):
+    """configs[3] against the ORACLE (not against this library's FP64 path): the FP64 oracle stopped by S3 after 4
+    products returns X_3; the mixed-precision kernels must reach the same iterate within the per-product error bound
+    of DESIGN.md 5.3 (3e-6 relative Frobenius per product, 4 products), with the same branch bits and traces."""
+    import torch
+
+    name = "mixed_n16384_first4"
+    if name not in gold:
+        pytest.skip(f"{name} not in the golden file yet (run tests/golden/make_golden.py {name})")
+    g = gold[name]
+    H = torch.from_numpy(hm.make_dense(g["workload"])).cuda()
+    D, res = api.bml_sp2_dense(H, g["n_occ"], g["idem_tol"], g["max_products"], precision)
+    del H
+    assert res.status == g["status"] == 2 and res.n_products == g["n_products"] == 4 and res.m_star == g["m_star"]
+    assert res.branch == g["branch"]
+    assert (res.emin, res.emax) == (g["emin"], g["emax"])
+    np.testing.assert_allclose(res.trace, g["trace"], rtol=2e-6, atol=0)
+    tol = 4 * 3e-6
+    for i, j, v in g["D_samples"]:
+        assert abs(D[i, j].item() - v) <= tol * g["D_fro"]
+    assert abs(torch.linalg.norm(D).item() - g["D_fro"]) <= tol * g["D_fro"]
+    y = torch.from_numpy(np.loadtxt(os.path.join(os.path.dirname(GOLD), g["Dv_file"]))).cuda()
+    v = torch.from_numpy(np.random.default_rng(g["probe_seed"]).standard_normal(g["N"])).cuda()
+    assert (torch.linalg.norm(D @ v - y) / g["D_fro"]).item() <= 3 * tol
 
 
 @pytest.mark.gpu

@@ -364,3 +364,82 @@ def test_rule_R1_picks_the_candidate_whose_trace_is_nearer_n_occ(oracle_mod, see
         assert np.trace(X) - np.trace(P) >= -1e-12     # d >= 0: the spectrum of X lies in [0, 1]
         X = cand[b]
     assert relfro(X, D) <= 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Pins added in round 2 ("parity unpinned" items i and ii)
+# ---------------------------------------------------------------------------------------------------------------
+def test_rescale_ellpack_inserts_a_missing_diagonal_hand_example(oracle_mod):
+    """Eq. 5 on ELLPACK-R with a row whose diagonal is NOT stored (H_11 = 0): the diagonal slot must appear,
+    in ascending-column position, with value s (e_max - 0).  Every expected slot and value is written out by hand:
+    e_min = -2, e_max = 3, s = 1 / 5."""
+    M = 4
+    hv = np.zeros((3, M)); hi = np.zeros((3, M), dtype=np.int32); hn = np.zeros(3, dtype=np.int32)
+    # row 0: (0, 2.0), (1, 1.0)      row 1 (unsorted, no diagonal): (2, -0.5), (0, 1.0)      row 2: (1, -0.5), (2, -1.0)
+    hv[0, :2] = [2.0, 1.0]; hi[0, :2] = [0, 1]; hn[0] = 2
+    hv[1, :2] = [-0.5, 1.0]; hi[1, :2] = [2, 0]; hn[1] = 2
+    hv[2, :2] = [-0.5, -1.0]; hi[2, :2] = [1, 2]; hn[2] = 2
+    xv, xi, xn, bad = oracle_mod.rescale_ellpack(hv, hi, hn, -2.0, 3.0)
+    assert bad < 0
+    assert xn.tolist() == [2, 3, 2]
+    assert xi.tolist() == [[0, 1, 0, 0], [0, 1, 2, 0], [1, 2, 0, 0]]
+    s = 1.0 / (3.0 - -2.0)
+    want = [[s * (3.0 - 2.0), -s * 1.0, 0.0, 0.0],           # X_00 = s (e_max - H_00), X_01 = -s H_01
+            [-s * 1.0, s * (3.0 - 0.0), -s * -0.5, 0.0],     # inserted X_11 = s e_max = 0.6 between columns 0 and 2
+            [-s * -0.5, s * (3.0 - -1.0), 0.0, 0.0]]
+    assert xv.tolist() == want
+    assert want[1][1] == 0.6000000000000001 and want[1][2] == 0.1           # the literal numbers
+    assert oracle_mod.trace_ellpack(xv, xi, xn) == pytest.approx(0.2 + 0.6 + 0.8, abs=1e-15)
+    # a full row without its diagonal cannot take the inserted slot: that row is reported, lowest first
+    hv2 = np.ones((2, 2)); hi2 = np.array([[1, 0], [0, 0]], dtype=np.int32); hn2 = np.array([2, 1], dtype=np.int32)
+    hi2[1, 0] = 0                                             # row 1 = {(0, 1.0)}: one free slot, diagonal fits
+    hv3 = np.ones((2, 1)); hi3 = np.array([[1], [0]], dtype=np.int32); hn3 = np.array([1, 1], dtype=np.int32)
+    assert oracle_mod.rescale_ellpack(hv2, hi2, hn2, -2.0, 3.0)[3] < 0
+    assert oracle_mod.rescale_ellpack(hv3, hi3, hn3, -2.0, 3.0)[3] == 0      # M = 1, both rows lack the diagonal
+
+
+def test_idempotency_norm_over_the_union_of_two_different_patterns(oracle_mod):
+    """Reading 8: e_m = ||thr(X X) - X||_F / ||X||_F runs over the UNION of the two patterns, an absent entry counting as
+    0.  A small random sparse H and a large tau give entries that are in X only (their product entry was dropped) and
+    entries in thr(X X) only (fill-in); the expected value is computed in exact rational arithmetic from the definition
+    on the dense 8 x 8 matrices -- no sparse merge, no floating point."""
+    from fractions import Fraction
+
+    N, M, tau = 8, 8, 0.02
+    rng = np.random.default_rng(11)
+    A = np.zeros((N, N))
+    for i in range(N):
+        A[i, i] = rng.uniform(-1, 1)
+        for j in (i + 1, i + 3):
+            if j < N:
+                A[i, j] = A[j, i] = rng.uniform(-1, 1)
+    H = hm.ellpack_from_dense(A, M)
+    lo, hi = oracle_mod.gershgorin_ellpack(*H)
+    xv, xi, xn, bad = oracle_mod.rescale_ellpack(*H, lo, hi)
+    assert bad < 0
+    X = [[Fraction(0)] * N for _ in range(N)]
+    inX = [[False] * N for _ in range(N)]
+    for i in range(N):
+        for p in range(xn[i]):
+            X[i][xi[i, p]] = Fraction(float(xv[i, p]))
+            inX[i][xi[i, p]] = True
+    e2 = x2 = Fraction(0)
+    only_x = only_p = 0
+    for i in range(N):
+        for j in range(N):
+            touched = any(inX[i][k] and inX[k][j] for k in range(N))
+            pij = sum(X[i][k] * X[k][j] for k in range(N))
+            keep = touched and (abs(pij) >= Fraction(tau) or i == j)
+            only_x += inX[i][j] and not keep
+            only_p += keep and not inX[i][j]
+            e2 += ((pij if keep else 0) - X[i][j]) ** 2
+            x2 += X[i][j] ** 2
+    assert only_x >= 2 and only_p >= 2          # the case exercises both kinds of mismatch
+    _, st = oracle_mod.sp2_ellpack(*H, N // 2, 1e-12, tau, max_products=1)
+    assert st["n_products"] == 1
+    want = float(e2) ** 0.5 / float(x2) ** 0.5
+    assert st["idem"][0] == pytest.approx(want, rel=1e-13)
+    # and the two norms move the value: ignoring either kind of one-sided entry would miss by far more than 1e-13
+    e2_wrong = sum(((sum(X[i][k] * X[k][j] for k in range(N)) - X[i][j]) ** 2 for i in range(N) for j in range(N)
+                    if inX[i][j]), Fraction(0))
+    assert abs(float(e2_wrong) ** 0.5 / float(x2) ** 0.5 - want) > 1e-6
