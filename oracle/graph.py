@@ -23,6 +23,18 @@ Readings of the paper (items G1-G6):
       other cores).  D is therefore assembled row by row and is symmetric only up to the method's own error.
   G5. D is stored in ELLPACK-R with the SP2 path's drop rule: keep |v| >= drop_tol or the diagonal; a row that needs
       more than M slots is the overflow failure of P:47-49 (status -3).
+  G3'. SP2 as the local solver (``graph_sp2``; "prg_build_DM" of Listing 11 is any DM solver, and SP2 is the
+      paper's, section IV.A).  The graph theory behind the method needs the SAME matrix function on every part (P:456:
+      "the same functions applied to only certain graph-restricted domains"), and SP2's function is fixed by its
+      spectral bounds and its branch sequence.  Reading: ONE SP2 polynomial for all parts --
+        * one Eq. 5 map: e_min, e_max = Gershgorin bounds of the whole H (they enclose the spectrum of every
+          principal sub-matrix h^k by interlacing), X_0^k = (e_max I - h^k) / (e_max - e_min);
+        * one branch bit per product, b_m = [t_m - N_occ <= 0] with the occupation counted where the result is read:
+          t_m = sum_k sum_{a core of k} (X_m^k)_aa  (every orbital is a core node of exactly one part);
+        * one stop test, e_m = sqrt(sum_k ||(X_m^k)^2 - X_m^k||_F^2) / sqrt(sum_k ||X_m^k||_F^2), rules S1-S3 of
+          the SP2 path with the same constants; D rows = core rows of X_{m*}^k.
+      A partition whose single part is the whole matrix reproduces the dense SP2 oracle exactly; on disconnected
+      parts (no halo) it reproduces it up to the order of the trace / norm sums.
   G6. The core partition is an INPUT (partitioning "stays external": METIS etc.); ``regular_partition`` is the
       paper's "simply divide the matrix index list into relatively regular segments" (P:486).
 
@@ -112,3 +124,65 @@ def graph_fermi(value, index, nnz, core_offsets, core_nodes, graph_tol, mu, beta
             bad = b if bad < 0 else min(bad, b)
         sizes.append(int(nodes.size))
     return (dv, di, dn), {"part_sizes": sizes, "overflow_row": bad, "status": -3 if bad >= 0 else 0}
+
+
+def graph_sp2(value, index, nnz, core_offsets, core_nodes, graph_tol, n_occ, idem_tol, drop_tol, max_products=100,
+              M_out=None):
+    """Listing 11 with SP2 (Eq. 5-7, Listing 2) as the local solver, reading G3': one Eq. 5 map, one branch sequence
+    and one stop test shared by all parts.  Step by step in the order of Listing 2: trace, product, test, branch.
+    Returns ((dv, di, dn), info) with info = status, m_star, n_products, branch string, trace[], idem[], emin, emax,
+    part_sizes, core_sizes, overflow_row.  Status as in the SP2 path: 0 S1, 1 S2, 2 S3, -2 degenerate bounds, -3 overflow
+    of a row of D.  The products are the plain triple loop of the dense SP2 oracle (sp2_oracle.c oracle_x2_dense)."""
+    import math
+
+    import oracle as osp2                      # the C SP2 oracle: Gershgorin, Eq. 5 rescale, triple-loop product
+
+    N = value.shape[0]
+    M = value.shape[1] if M_out is None else int(M_out)
+    dv, di, dn = np.zeros((N, M)), np.zeros((N, M), dtype=np.int32), np.zeros(N, dtype=np.int32)
+    emin, emax = osp2.gershgorin_ellpack(value, index, nnz)                       # one map for every part (Eq. 5)
+    info = {"emin": emin, "emax": emax, "overflow_row": -1, "branch": "", "trace": [], "idem": [], "m_star": 0,
+            "n_products": 0, "part_sizes": [], "core_sizes": []}
+    if not emax - emin > 0:
+        info["status"] = -2
+        return (dv, di, dn), info
+    parts = []
+    for p in range(len(core_offsets) - 1):
+        core = core_nodes[core_offsets[p]: core_offsets[p + 1]]
+        nodes, is_core = core_halo(value, index, nnz, core, graph_tol)
+        h = matrix2submatrix(value, index, nnz, nodes)
+        parts.append([nodes, is_core, osp2.rescale_dense(h, emin, emax)])         # X_0^k
+        info["part_sizes"].append(int(nodes.size))
+        info["core_sizes"].append(int(is_core.sum()))
+    status, m = 2, 0
+    while True:
+        t = math.fsum(float(X[a, a]) for _, is_core, X in parts for a in np.nonzero(is_core)[0])   # core trace
+        P = [osp2.x2_dense(X) for _, _, X in parts]                                               # products
+        e2 = math.fsum(float(v) for (_, _, X), Pk in zip(parts, P) for v in ((Pk - X) ** 2).ravel())
+        x2 = math.fsum(float(v) for _, _, X in parts for v in (X ** 2).ravel())
+        info["trace"].append(t)
+        info["idem"].append(math.sqrt(e2) / math.sqrt(x2))
+        e = info["idem"]
+        if e[m] < idem_tol:                                       # S1
+            status = 0
+            break
+        if m >= 2 and e[m] < 1e-2 and e[m] >= e[m - 2]:           # S2
+            status = 1
+            break
+        if m + 1 == max_products:                                 # S3
+            status = 2
+            break
+        b = t - float(n_occ) <= 0.0                               # Eq. 6-7, "<=" of Listing 2 (P:204)
+        info["branch"] += "1" if b else "0"
+        for part, Pk in zip(parts, P):
+            part[2] = 2.0 * part[2] - Pk if b else Pk
+        m += 1
+    info["m_star"], info["n_products"] = m, m + 1
+    bad = -1
+    for nodes, is_core, X in parts:
+        r = submatrix2matrix(X, nodes, is_core, drop_tol, dv, di, dn)
+        if r >= 0:
+            bad = r if bad < 0 else min(bad, r)
+    info["overflow_row"] = bad
+    info["status"] = -3 if bad >= 0 else status
+    return (dv, di, dn), info

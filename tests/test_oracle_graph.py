@@ -134,3 +134,97 @@ def test_chebyshev_local_solver_matches_the_exact_one_within_truncation():
     assert ia["status"] == 0 and ib["status"] == 0
     assert np.allclose(hm.ellpack_to_dense(*a), hm.ellpack_to_dense(*b), atol=1e-8)
     assert np.array_equal(a[2], b[2]) and np.array_equal(a[1], b[1])        # drop_tol = 0: same pattern
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# graph_sp2: SP2 as the local solver (reading G3'; Listing 11 with prg_build_DM = SP2, one polynomial for all parts)
+# ---------------------------------------------------------------------------------------------------------------
+def gapped_model(L=(8, 6, 5), M=64, seed=0):
+    """The 5'-like insulator (on-site +-12, hopping -exp(-r / 0.5), r <= 2): wide gap, D decays fast."""
+    return hm.lattice_ellpack(L, 12.0, 0.2, 2.0, lambda r: -math.exp(-r / 0.5), M, seed)
+
+
+def test_graph_sp2_single_part_is_the_dense_sp2_oracle():
+    """One part that is the whole matrix (halo = nothing to add): graph_sp2 must walk exactly the dense SP2 oracle's
+    iterates -- same bounds, same branch string, same product count, D equal entry by entry.  Catches a wrong Eq. 5 map
+    (per-part bounds), a trace over the wrong node set, a branch / stop test out of Listing 2's order."""
+    import oracle
+
+    H = gapped_model()
+    Hd = dense_of(H)
+    N = Hd.shape[0]
+    D_ref, st = oracle.sp2_dense(Hd, N // 2, 1e-10)
+    offs, nodes = og.regular_partition(N, 1)
+    (dv, di, dn), info = og.graph_sp2(*H, offs, nodes, 0.0, N // 2, 1e-10, 0.0, M_out=N)
+    assert info["status"] == st["status"] == 0
+    assert (info["emin"], info["emax"]) == (st["emin"], st["emax"])
+    assert info["branch"] == st["branch"] and info["n_products"] == st["n_products"]
+    np.testing.assert_allclose(info["trace"], st["trace"], rtol=0, atol=1e-11)
+    np.testing.assert_allclose(info["idem"], st["idem"], rtol=1e-9, atol=1e-16)
+    assert np.array_equal(hm.ellpack_to_dense(dv, di, dn), D_ref)
+
+
+def test_graph_sp2_disconnected_parts_equal_the_global_solve():
+    """H block diagonal with the blocks as parts (no halo at any threshold): the global X_m stays block diagonal, the
+    traces and squared norms add up over the blocks, so the shared branch sequence is the global one and every block
+    of D is the global D's block.  Catches per-part branch decisions and per-part occupation counts."""
+    import oracle
+
+    rng = np.random.default_rng(5)
+    sizes = [7, 12, 9]
+    N = sum(sizes)
+    Hd = np.zeros((N, N))
+    o = 0
+    for s, shift in zip(sizes, (-0.8, 0.1, 0.9)):          # different fillings per block: the split of N_occ is not N/2 each
+        A = rng.normal(size=(s, s))
+        Hd[o:o + s, o:o + s] = (A + A.T) / 2 + shift * np.eye(s)
+        o += s
+    eps = np.linalg.eigvalsh(Hd)
+    n_occ = 13
+    assert eps[n_occ] - eps[n_occ - 1] > 0.05              # a gap at the chosen filling
+    H = hm.ellpack_from_dense(Hd, N)
+    offs = np.array([0, 7, 19, 28], dtype=np.int32)
+    nodes = np.arange(N, dtype=np.int32)
+    D_ref, st = oracle.sp2_dense(Hd, n_occ, 1e-10)
+    (dv, di, dn), info = og.graph_sp2(*H, offs, nodes, 0.0, n_occ, 1e-10, 0.0, M_out=N)
+    assert info["part_sizes"] == sizes and info["core_sizes"] == sizes
+    assert info["status"] == st["status"] == 0 and info["branch"] == st["branch"]
+    D = hm.ellpack_to_dense(dv, di, dn)
+    assert np.abs(D - D_ref).max() <= 1e-13
+    # the occupations of the blocks are what the global Fermi level gives them, not N_occ / parts
+    occ = [np.trace(D[a:b, a:b]) for a, b in zip(offs[:-1], offs[1:])]
+    want = [int((np.linalg.eigvalsh(Hd[a:b, a:b]) < (eps[n_occ - 1] + eps[n_occ]) / 2).sum()) for a, b in zip(offs[:-1], offs[1:])]
+    assert np.allclose(occ, want, atol=1e-8) and len(set(want)) > 1
+
+
+def test_graph_sp2_approaches_the_dense_projector_as_the_halo_grows():
+    """With real halos the result is the graph approximation of the dense projector (LAPACK, Eq. 2 with the step
+    function): the error must fall as graph_tol falls (Fig. 8's trend), tr D must stay near N_occ, and core rows only
+    are written.  Catches halo rows leaking into D and a scatter that uses part-local column numbers."""
+    H = gapped_model((12, 6, 5))
+    Hd = dense_of(H)
+    N = Hd.shape[0]
+    w, U = np.linalg.eigh(Hd)
+    n_occ = N // 2
+    D_exact = U[:, :n_occ] @ U[:, :n_occ].T
+    offs, nodes = og.regular_partition(N, 4)
+    errs = []
+    for tol in (0.2, 0.02, 0.002):                          # hopping -exp(-r/0.5): 0.135 (r=1), 0.059, 0.031, 0.018 (r=2)
+        (dv, di, dn), info = og.graph_sp2(*H, offs, nodes, tol, n_occ, 1e-9, 0.0, M_out=N)
+        assert info["status"] in (0, 1)
+        D = hm.ellpack_to_dense(dv, di, dn)
+        errs.append(np.linalg.norm(D - D_exact) / np.linalg.norm(D_exact))
+        assert abs(np.trace(D) - n_occ) < 50 * errs[-1] * n_occ ** 0.5 + 1e-8
+        assert np.all(dn >= 1)
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 2e-3
+    assert info["part_sizes"][0] > info["core_sizes"][0]
+
+
+def test_graph_sp2_overflow_and_degenerate_bounds():
+    H = gapped_model()
+    N = H[0].shape[0]
+    offs, nodes = og.regular_partition(N, 2)
+    (_, _, dn), info = og.graph_sp2(*H, offs, nodes, 0.02, N // 2, 1e-9, 0.0, M_out=8)      # rows of D need > 8 slots
+    assert info["status"] == -3 and info["overflow_row"] == 0
+    I = hm.ellpack_from_dense(2.0 * np.eye(6), 4)
+    assert og.graph_sp2(*I, np.array([0, 6], dtype=np.int32), np.arange(6, dtype=np.int32), 0.0, 3, 1e-9, 0.0)[1]["status"] == -2
