@@ -84,6 +84,45 @@ BML_API int bml_submatrix2matrix_ellpack(const double *d_d, int64_t ld, const in
                                          int32_t s, double drop_tol, bml_matrix_t *D, int32_t *d_overflow_row,
                                          void *cuda_stream);
 
+/*
+ * Listing 11 with SP2 (section IV.A, Eq. 5-7) as the local solver `prg_build_DM`.  The graph theory of the
+ * method applies the SAME matrix function to every part, and SP2's function is fixed by its spectral bounds
+ * and its branch sequence, so all parts share one SP2 polynomial (reading G3'):
+ *   X_0^k = (e_max I - h^k) / (e_max - e_min)     with the Gershgorin bounds of the WHOLE H (bml_gershgorin), Eq. 5
+ *   b_m = [ t_m - n_occ <= 0 ],  t_m = sum_k sum_{a in core of k} (X_m^k)_aa          one branch bit, Eq. 6-7
+ *   e_m = sqrt(sum_k ||(X_m^k)^2 - X_m^k||_F^2) / sqrt(sum_k ||X_m^k||_F^2)           one stop test, rules S1-S3
+ *   D[l, :] <- X_{m*}^k[l, :] for the core nodes l of part k.
+ * A product of ALL parts is one persistent launch over the parts' upper-triangle tiles (parts may differ in size); the
+ * branch bit and the stop test stay on the device as in bml_sp2_dense.  One host synchronisation after the halo pass
+ * (part sizes decide buffer offsets) and one at the end.  n_parts <= BML_GRAPH_MAX_PARTS.
+ * d_workspace >= bml_graph_sp2_workspace_bytes(N, n_parts, part_capacity), 1024-byte aligned.
+ * Returns the SP2 status (0, 1, 2) or -1, -2, -3 (a row of D needs more than D->M slots), -4, -7.
+ */
+typedef struct {
+    double  graph_tol;      /* tau of Eq. 15                                                                        */
+    double  drop_tol;       /* D keeps |v| >= drop_tol or the diagonal                                              */
+    double  idem_tol;       /* tolerance on e_m                                                                     */
+    int32_t n_occ;          /* occupied orbitals of the WHOLE system, 0 < n_occ < N                                 */
+    int32_t max_products;   /* 1 .. BML_SP2_LOG_LEN                                                                 */
+    int32_t n_parts;        /* 1 .. BML_GRAPH_MAX_PARTS                                                             */
+    int32_t part_capacity;  /* largest core+halo size the workspace is provisioned for (<= N)                       */
+} bml_graph_sp2_params_t;
+
+typedef struct {
+    bml_sp2_stats_t sp2;    /* the shared SP2 record: status, products, branch bits, traces (over core orbitals), e_m */
+    int32_t status;         /* = return value                                                                       */
+    int32_t n_parts;
+    int32_t overflow_row;   /* status -3: lowest row of D needing more than D->M slots, else -1                     */
+    int32_t max_part_size;
+    int32_t part_size[BML_GRAPH_MAX_PARTS];
+    int32_t core_size[BML_GRAPH_MAX_PARTS];
+} bml_graph_sp2_stats_t;
+
+BML_API size_t bml_graph_sp2_workspace_bytes(int64_t N, int32_t n_parts, int32_t part_capacity);
+BML_API int bml_graph_sp2_ellpack(const bml_matrix_t *H, const int32_t *d_core_offsets, const int32_t *d_core_nodes,
+                                  const bml_graph_sp2_params_t *p, bml_matrix_t *D, void *d_workspace,
+                                  size_t workspace_bytes, bml_graph_sp2_stats_t *stats, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

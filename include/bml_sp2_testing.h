@@ -45,6 +45,13 @@ BML_API int bml_dense_mixed_tile_of_cta(int64_t N, int32_t cta, int32_t *out2);
 BML_API int bml_cheb_schedule(int32_t k, int32_t *level, int32_t *a, int32_t *b);
 BML_API int bml_symm_work_item(int64_t N, int32_t n_jobs, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out6);
 
+/*
+ * bml_dense_batch_work_item: the it-th work item of CTA `cta` (of n_ctas) of the batched symmetric-square kernel of the
+ * graph-based SP2 solver, for parts of sizes n[0 .. n_jobs): out5 <- { part, tile (upper-triangle index of 128 x 128
+ * tiles, column by column), kt_begin, kt_end, KT = ceil(n / 16) }.  Pure host arithmetic.  Returns 0, 1 past the end, -1.
+ */
+BML_API int bml_dense_batch_work_item(int32_t n_jobs, const int32_t *n, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out5);
+
 #ifdef __cplusplus
 }
 #endif

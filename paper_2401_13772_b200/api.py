@@ -38,7 +38,8 @@ EXPORTS = [
     "bml_cheb_schedule", "bml_symm_work_item",
     # include/bml_graph.h
     "bml_graph_workspace_bytes", "bml_graph_chebyshev_ellpack", "bml_graph_core_halo", "bml_matrix2submatrix_ellpack",
-    "bml_submatrix2matrix_ellpack",
+    "bml_submatrix2matrix_ellpack", "bml_graph_sp2_workspace_bytes", "bml_graph_sp2_ellpack",
+    "bml_dense_batch_work_item",
 ]
 GRAPH_MAX_PARTS = 256
 CHEB_MAX_K, CHEB_MAX_M, CHEB_MAX_TERMS, SYMM_MAX_JOBS = 32, 32, 1024, 16
@@ -133,6 +134,30 @@ class bml_graph_stats_t(ctypes.Structure):
     ]
 
 
+class bml_graph_sp2_params_t(ctypes.Structure):
+    _fields_ = [
+        ("graph_tol", ctypes.c_double),
+        ("drop_tol", ctypes.c_double),
+        ("idem_tol", ctypes.c_double),
+        ("n_occ", ctypes.c_int32),
+        ("max_products", ctypes.c_int32),
+        ("n_parts", ctypes.c_int32),
+        ("part_capacity", ctypes.c_int32),
+    ]
+
+
+class bml_graph_sp2_stats_t(ctypes.Structure):
+    _fields_ = [
+        ("sp2", bml_sp2_stats_t),
+        ("status", ctypes.c_int32),
+        ("n_parts", ctypes.c_int32),
+        ("overflow_row", ctypes.c_int32),
+        ("max_part_size", ctypes.c_int32),
+        ("part_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
+        ("core_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
+    ]
+
+
 _lib = None
 
 
@@ -209,6 +234,13 @@ def load(build_if_missing: bool = True):
     L.bml_graph_chebyshev_ellpack.restype = ctypes.c_int
     L.bml_graph_chebyshev_ellpack.argtypes = [MP, vp, vp, ctypes.POINTER(bml_graph_params_t), MP, vp, sz,
                                               ctypes.POINTER(bml_graph_stats_t), vp]
+    L.bml_graph_sp2_workspace_bytes.restype = sz
+    L.bml_graph_sp2_workspace_bytes.argtypes = [i64, i32, i32]
+    L.bml_graph_sp2_ellpack.restype = ctypes.c_int
+    L.bml_graph_sp2_ellpack.argtypes = [MP, vp, vp, ctypes.POINTER(bml_graph_sp2_params_t), MP, vp, sz,
+                                        ctypes.POINTER(bml_graph_sp2_stats_t), vp]
+    L.bml_dense_batch_work_item.restype = ctypes.c_int
+    L.bml_dense_batch_work_item.argtypes = [i32, i32p, i32, i32, i32, i32p]
     L.bml_graph_core_halo.restype = ctypes.c_int
     L.bml_graph_core_halo.argtypes = [MP, vp, vp, i32, dbl, vp, vp, vp, vp, sz, vp]
     L.bml_matrix2submatrix_ellpack.restype = ctypes.c_int
@@ -699,6 +731,75 @@ def bml_graph_chebyshev_ellpack(H, core_offsets, core_nodes, graph_tol, mu, beta
     N = H[0].shape[0]
     solver = GraphSolver(N, M_out, core_offsets.numel() - 1, part_capacity, k, m, H[0].device)
     return solver.solve(H, core_offsets, core_nodes, graph_tol, mu, beta, drop_tol)
+
+
+@dataclass
+class GraphSp2Result:
+    status: int
+    sp2: Sp2Result
+    n_parts: int
+    overflow_row: int
+    max_part_size: int
+    part_size: list
+    core_size: list
+    message: str = field(default="")
+
+
+class GraphSp2Solver:
+    """Pre-allocated output and workspace for repeated bml_graph_sp2_ellpack calls (SP2 as the local solver)."""
+
+    def __init__(self, N: int, M_out: int, n_parts: int, part_capacity: int, device="cuda"):
+        L = load()
+        self.N, self.M_out, self.n_parts, self.cap = int(N), int(M_out), int(n_parts), int(part_capacity)
+        self.device = torch.device(device)
+        self.dv = torch.zeros((N, M_out), dtype=torch.float64, device=self.device)
+        self.di = torch.zeros((N, M_out), dtype=torch.int32, device=self.device)
+        self.dn = torch.zeros((N,), dtype=torch.int32, device=self.device)
+        self.ws_bytes = L.bml_graph_sp2_workspace_bytes(self.N, self.n_parts, self.cap)
+        if self.ws_bytes == 0:
+            raise RuntimeError("bml_graph_sp2_workspace_bytes: " + bml_status_string(-1))
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, H, core_offsets: torch.Tensor, core_nodes: torch.Tensor, graph_tol: float, n_occ: int,
+              idem_tol: float, drop_tol: float, max_products: int = 100):
+        L = load()
+        h = ellpack_desc(*H)
+        d = ellpack_desc(self.dv, self.di, self.dn)
+        _require_cuda(core_offsets, torch.int32, "core_offsets")
+        _require_cuda(core_nodes, torch.int32, "core_nodes")
+        p = bml_graph_sp2_params_t(float(graph_tol), float(drop_tol), float(idem_tol), int(n_occ), int(max_products),
+                                   self.n_parts, self.cap)
+        st = bml_graph_sp2_stats_t()
+        rc = L.bml_graph_sp2_ellpack(ctypes.byref(h), core_offsets.data_ptr(), core_nodes.data_ptr(), ctypes.byref(p),
+                                     ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes, ctypes.byref(st), _stream())
+        P = self.n_parts
+        res = GraphSp2Result(int(rc), _result(st.sp2, rc), int(st.n_parts), int(st.overflow_row), int(st.max_part_size),
+                             list(st.part_size[:P]), list(st.core_size[:P]), bml_status_string(rc))
+        return (self.dv, self.di, self.dn), res
+
+
+def bml_graph_sp2_ellpack(H, core_offsets, core_nodes, graph_tol, n_occ, idem_tol, drop_tol, M_out, part_capacity,
+                          max_products: int = 100):
+    """Graph-based D with SP2 as the local solver (one shared polynomial).  Returns ((value, index, nnz), GraphSp2Result)."""
+    N = H[0].shape[0]
+    solver = GraphSp2Solver(N, M_out, core_offsets.numel() - 1, part_capacity, H[0].device)
+    return solver.solve(H, core_offsets, core_nodes, graph_tol, n_occ, idem_tol, drop_tol, max_products)
+
+
+def bml_dense_batch_work_items(sizes, n_ctas: int, cta: int):
+    """Work list of one CTA of the batched symmetric-square kernel: [(part, tile, kt_begin, kt_end, KT), ...]."""
+    L = load()
+    n = (ctypes.c_int32 * len(sizes))(*[int(x) for x in sizes])
+    out = (ctypes.c_int32 * 5)()
+    items, it = [], 0
+    while True:
+        rc = L.bml_dense_batch_work_item(len(sizes), n, int(n_ctas), int(cta), it, out)
+        if rc == 1:
+            return items
+        if rc != 0:
+            raise RuntimeError(f"bml_dense_batch_work_item: {bml_status_string(rc)}")
+        items.append(tuple(out))
+        it += 1
 
 
 def bml_graph_core_halo(H, core_offsets: torch.Tensor, core_nodes: torch.Tensor, graph_tol: float):

@@ -66,6 +66,10 @@ int launch_graph_gather(const bml_matrix_t *H, const int32_t *nodes, int s, doub
 int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
                          bml_matrix_t *D, int32_t *overflow, cudaStream_t st);
 void cheb_graph_cache_release();
+size_t graph_sp2_workspace_bytes(int64_t N, int n_parts, int cap);
+int graph_sp2_solve(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, const bml_graph_sp2_params_t *p,
+                    bml_matrix_t *D, void *ws, bml_graph_sp2_stats_t *stats, cudaStream_t st);
+int dense_batch_work_item(int n_jobs, const int32_t *n, int n_ctas, int cta, int it, int32_t out[5]);
 // probe.cu
 int run_fp64_tensor_probe(int iters, double *flops, double *ms, cudaStream_t st);
 
@@ -682,6 +686,38 @@ int bml_graph_chebyshev_ellpack(const bml_matrix_t *H, const int32_t *d_core_off
     }
     if (stats) stats->status = r;
     return r;
+}
+
+size_t bml_graph_sp2_workspace_bytes(int64_t N, int32_t n_parts, int32_t part_capacity)
+{
+    if (N <= 0 || n_parts < 1 || n_parts > BML_GRAPH_MAX_PARTS || part_capacity < 1 || part_capacity > N) return 0;
+    return graph_sp2_workspace_bytes(N, n_parts, part_capacity);
+}
+
+int bml_graph_sp2_ellpack(const bml_matrix_t *H, const int32_t *d_core_offsets, const int32_t *d_core_nodes,
+                          const bml_graph_sp2_params_t *p, bml_matrix_t *D, void *d_workspace, size_t workspace_bytes,
+                          bml_graph_sp2_stats_t *stats, void *cuda_stream)
+{
+    int r;
+    if (!ell_ok_wide(H) || !ell_ok_wide(D) || D->N != H->N || !p || p->n_parts < 1 || p->n_parts > BML_GRAPH_MAX_PARTS ||
+        p->part_capacity < 1 || (int64_t)p->part_capacity > H->N || p->n_occ <= 0 || (int64_t)p->n_occ >= H->N ||
+        !(p->idem_tol > 0.0) || !(p->graph_tol >= 0.0) || !(p->drop_tol >= 0.0) || p->max_products < 1 ||
+        p->max_products > BML_SP2_LOG_LEN || !d_core_offsets || !d_core_nodes || !d_workspace || D->value == H->value ||
+        D->index == H->index || D->nnz == H->nnz || ((uintptr_t)d_workspace & 1023) != 0 ||
+        workspace_bytes < bml_graph_sp2_workspace_bytes(H->N, p->n_parts, p->part_capacity)) {
+        r = BML_ERR_INVALID;
+        if (stats) memset(stats, 0, sizeof(*stats));
+    } else {
+        r = graph_sp2_solve(H, d_core_offsets, d_core_nodes, p, D, d_workspace, stats, (cudaStream_t)cuda_stream);
+    }
+    if (stats) { stats->status = r; stats->sp2.status = r; }
+    return r;
+}
+
+int bml_dense_batch_work_item(int32_t n_jobs, const int32_t *n, int32_t n_ctas, int32_t cta, int32_t it, int32_t *out5)
+{
+    if (!n || !out5) return BML_ERR_INVALID;
+    return dense_batch_work_item(n_jobs, n, n_ctas, cta, it, out5);
 }
 
 int bml_graph_core_halo(const bml_matrix_t *H, const int32_t *d_core_offsets, const int32_t *d_core_nodes, int32_t n_parts,

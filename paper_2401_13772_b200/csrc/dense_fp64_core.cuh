@@ -69,6 +69,117 @@ __device__ __forceinline__ int frag_adjacent(double &v0, double &v1, int t)
     return lo ? 4 * t : 4 * (t - 2) + 2;
 }
 
+// Fused epilogue (D4) of one tile held in the consumers' accumulators: X' = b ? 2X - P : P with its mirror, and this
+// thread's share of { tr P, ||P - X||^2, ||X||^2, tr X' }.  `core` (may be NULL): per-row flags; the two TRACES then
+// count only the rows whose flag is set (the graph-based solver's occupation is counted over core orbitals, bml_graph.h);
+// the norms always run over the whole tile.  Fragment columns are first made adjacent (frag_adjacent) so
+// that X is read and X' written 16 bytes at a time; the iterates live in the workspace (ld a multiple of 16 doubles,
+// 128-byte aligned), so every pair is aligned.  Diagonal tiles use only r <= c and mirror it: X' is bitwise symmetric.
+template <int MI, int NI, int BT>
+__device__ __forceinline__ void sp2_tile_epilogue(double (&acc)[MI][NI][2], const double *__restrict__ X,
+                                                  double *__restrict__ Xn, int64_t ld, int N, int I, int J, int wm, int wn,
+                                                  int lane, int branch, double &s_trp, double &s_e, double &s_x,
+                                                  double &s_trn, const uint8_t *__restrict__ core = nullptr)
+{
+    const int g = lane >> 2, t = lane & 3;
+    const bool diag = (I == J);
+    const int row0 = I * BT + wm * (BT / 2) + perm8(g);
+    const int col0 = J * BT + wn * (BT / 4);
+    auto one = [&](int r, int c, double p) {
+        if (r < N && c < N && (!diag || r <= c)) {
+            const double x = X[(int64_t)r * ld + c];
+            const double d = p - x;
+            const double xn = branch ? (2.0 * x - p) : p;             // Eq. 7 : Eq. 6
+            Xn[(int64_t)r * ld + c] = xn;
+            if (r == c) {
+                if (!core || core[r]) { s_trp += p; s_trn += xn; }
+                s_e += d * d; s_x += x * x;
+            } else {
+                Xn[(int64_t)c * ld + r] = xn;                         // mirror
+                s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
+            }
+        }
+    };
+    if (I * BT + BT <= N && J * BT + BT <= N) {
+        // Tile entirely inside the matrix (CTA-uniform): the reads of X need no bounds test, so they are issued two
+        // fragment rows (2 x NI 16-byte loads) ahead of their use.  With the loads inside the per-element conditions
+        // below every (i, j) step costs one L2 round trip (8 warps per SM: nothing else hides it).  Same arithmetic in
+        // the same order as the general path: the sums are bitwise the same.
+        const int cadj = (t < 2) ? 4 * t : 4 * (t - 2) + 2;             // frag_adjacent's column of this lane
+        auto one_x = [&](int r, int c, double p, double x) {
+            if (r <= c) {                                               // only reached on diagonal tiles
+                const double d = p - x;
+                const double xn = branch ? (2.0 * x - p) : p;
+                Xn[(int64_t)r * ld + c] = xn;
+                if (r == c) {
+                    if (!core || core[r]) { s_trp += p; s_trn += xn; }
+                    s_e += d * d; s_x += x * x;
+                } else {
+                    Xn[(int64_t)c * ld + r] = xn;
+                    s_e += 2.0 * (d * d); s_x += 2.0 * (x * x);
+                }
+            }
+        };
+#pragma unroll
+        constexpr int RB = MI >= 4 ? 4 : 2;                            // fragment rows read ahead
+#pragma unroll
+        for (int i = 0; i < MI; i += RB) {
+            double2 xv[RB][NI];
+#pragma unroll
+            for (int ii = 0; ii < RB; ++ii)
+#pragma unroll
+                for (int j = 0; j < NI; ++j)
+                    xv[ii][j] = *(const double2 *)(X + (int64_t)(row0 + (i + ii) * 8) * ld + col0 + j * 8 + cadj);
+#pragma unroll
+            for (int ii = 0; ii < RB; ++ii) {
+                const int r = row0 + (i + ii) * 8;
+#pragma unroll
+                for (int j = 0; j < NI; ++j) {
+                    double p0 = acc[i + ii][j][0], p1 = acc[i + ii][j][1];
+                    const int c = col0 + j * 8 + frag_adjacent(p0, p1, t);
+                    const double2 x = xv[ii][j];
+                    if (!diag || r < c) {
+                        const double d0 = p0 - x.x, d1 = p1 - x.y;
+                        const double xn0 = branch ? (2.0 * x.x - p0) : p0, xn1 = branch ? (2.0 * x.y - p1) : p1;
+                        *(double2 *)(Xn + (int64_t)r * ld + c) = make_double2(xn0, xn1);
+                        Xn[(int64_t)c * ld + r] = xn0;
+                        Xn[(int64_t)(c + 1) * ld + r] = xn1;
+                        s_e += 2.0 * (d0 * d0) + 2.0 * (d1 * d1);
+                        s_x += 2.0 * (x.x * x.x) + 2.0 * (x.y * x.y);
+                    } else {
+                        one_x(r, c, p0, x.x);
+                        one_x(r, c + 1, p1, x.y);
+                    }
+                }
+            }
+        }
+        return;
+    }
+#pragma unroll
+    for (int i = 0; i < MI; ++i) {
+        const int r = row0 + i * 8;
+#pragma unroll
+        for (int j = 0; j < NI; ++j) {
+            double p0 = acc[i][j][0], p1 = acc[i][j][1];
+            const int c = col0 + j * 8 + frag_adjacent(p0, p1, t);
+            if (r < N && c + 1 < N && (!diag || r < c)) {
+                // both elements strictly above the diagonal: one 16-byte read of X, one 16-byte write of X'
+                const double2 x = *(const double2 *)(X + (int64_t)r * ld + c);
+                const double d0 = p0 - x.x, d1 = p1 - x.y;
+                const double xn0 = branch ? (2.0 * x.x - p0) : p0, xn1 = branch ? (2.0 * x.y - p1) : p1;
+                *(double2 *)(Xn + (int64_t)r * ld + c) = make_double2(xn0, xn1);
+                Xn[(int64_t)c * ld + r] = xn0;
+                Xn[(int64_t)(c + 1) * ld + r] = xn1;
+                s_e += 2.0 * (d0 * d0) + 2.0 * (d1 * d1);
+                s_x += 2.0 * (x.x * x.x) + 2.0 * (x.y * x.y);
+            } else {
+                one(r, c, p0);
+                one(r, c + 1, p1);
+            }
+        }
+    }
+}
+
 // Release of a ring stage back to the TMA producer, ONE SLAB LATE.  ptxas schedules a stage's mbarrier.arrive right
 // behind the ISSUE of the slab's last fragment loads (the MMAs that consume them follow it), and the arrive does not
 // wait for those loads to have read shared memory: when the consumers run close behind the producer (short, store-only

@@ -3,7 +3,7 @@
 // Chebyshev expansion per part (chebyshev.cu), thresholded scatter of the core rows (bml_submatrix2matrix).
 #include <string.h>
 
-#include "common.cuh"
+#include "dense_fp64_core.cuh"
 #include "../../include/bml_graph.h"
 
 namespace bmlsp2 {
@@ -15,6 +15,18 @@ int cheb_dense_enqueue_batch(int P, const bml_matrix_t *H, const bml_cheb_params
                              int *n_launches_out, cudaStream_t st);
 double *cheb_batch_result(void *ws, int64_t N, int k, int m, int P, int q, int64_t *ld_out);
 int *cheb_fail_flag(void *ws, int q);
+// reductions.cu
+int launch_gershgorin(const bml_matrix_t *H, double *d_bounds, double *rowlh, cudaStream_t st);
+int launch_rescale_dense(const bml_matrix_t *H, const double *d_bounds, double *X, int64_t ldx, cudaStream_t st);
+int launch_init_ctl(Sp2Ctl *ctl, const double *d_bounds, const double *d_tr0, int n_occ, int max_products,
+                    double idem_tol, int loop_mode, int branch0, const int *fail_flag, cudaStream_t st);
+// dense_batch.cu
+size_t dense_batch_table_bytes();
+int dense_batch_fill(void *h_table, int n_jobs, const int32_t *n, double *const *buf0, double *const *buf1,
+                     const int64_t *ld, const uint8_t *const *core);
+int launch_x2_dense_fp64_batch(const void *d_table, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream);
+int launch_batch_core_trace(const void *d_table, double *d_out, cudaStream_t st);
+int launch_batch_final_buffers(const void *d_table, const Sp2Ctl *ctl, const double **d_out, int n_jobs, cudaStream_t st);
 
 // part that owns position q of the core-node list: largest k with offsets[k] <= q
 __device__ __forceinline__ int part_of(const int32_t *__restrict__ offs, int n_parts, int q)
@@ -113,14 +125,18 @@ __global__ void __launch_bounds__(256) graph_gather_kernel(const double *__restr
 }
 
 // bml_submatrix2matrix: core rows of d -> ELLPACK-R rows of D with the drop rule (readings G4, G5).  One warp per row.
+// dsel (may be NULL): the matrix is *dsel instead of d (the SP2 local solver's final iterate sits in the ping-pong
+// buffer the device-side control block selected).
 __global__ void __launch_bounds__(256) graph_scatter_kernel(const double *__restrict__ d, int64_t ld,
                                                             const int32_t *__restrict__ nodes,
                                                             const uint8_t *__restrict__ is_core, int s, double drop_tol,
                                                             double *__restrict__ dv, int32_t *__restrict__ di,
-                                                            int32_t *__restrict__ dn, int M, int32_t *__restrict__ overflow)
+                                                            int32_t *__restrict__ dn, int M, int32_t *__restrict__ overflow,
+                                                            const double *const *__restrict__ dsel)
 {
     const int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (a >= s || !is_core[a]) return;
+    if (dsel) d = *dsel;
     const int i = nodes[a];
     const double *row = d + (int64_t)a * ld;
     // count first: a row that does not fit is left untouched
@@ -185,14 +201,21 @@ int launch_graph_gather(const bml_matrix_t *H, const int32_t *nodes, int s, doub
     return 0;
 }
 
-int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
-                         bml_matrix_t *D, int32_t *overflow, cudaStream_t st)
+static int launch_graph_scatter_sel(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s,
+                                    double drop_tol, bml_matrix_t *D, int32_t *overflow, cudaStream_t st,
+                                    const double *const *dsel)
 {
     graph_scatter_kernel<<<(unsigned)(((size_t)s * 32 + 255) / 256), 256, 0, st>>>(d, ld, nodes, is_core, s, drop_tol,
                                                                                      D->value, D->index, D->nnz, D->M,
-                                                                                     overflow);
+                                                                                     overflow, dsel);
     G_CHECK();
     return 0;
+}
+
+int launch_graph_scatter(const double *d, int64_t ld, const int32_t *nodes, const uint8_t *is_core, int s, double drop_tol,
+                         bml_matrix_t *D, int32_t *overflow, cudaStream_t st)
+{
+    return launch_graph_scatter_sel(d, ld, nodes, is_core, s, drop_tol, D, overflow, st, nullptr);
 }
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -321,6 +344,151 @@ int graph_chebyshev_solve(const bml_matrix_t *H, const int32_t *offs, const int3
     if (stats) {
         stats->status = status;
         stats->n_products = n_products;
+        stats->overflow_row = h_scal[1] != INT32_MAX ? h_scal[1] : -1;
+    }
+    return status;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Listing 11 with SP2 as the local solver (reading G3'): ONE SP2 polynomial for all parts -- the Gershgorin bounds of
+// the whole H define Eq. 5 for every part, the branch bit comes from the trace summed over the core orbitals of all
+// parts, the stop test from the norms summed over all parts.  A product of the whole batch is one launch of
+// x2_dense_fp64_batch_kernel (dense_batch.cu); nothing but the part sizes (launch shapes) goes through the host.
+// ------------------------------------------------------------------------------------------------------------
+constexpr size_t GS_CTL_BYTES = 4096;
+static_assert(sizeof(Sp2Ctl) <= GS_CTL_BYTES, "control block does not fit its slot");
+
+struct GraphSp2Ws {
+    int32_t *scal;          // [0] unused, [1] overflow row, [2..] sizes (2 per part)
+    uint8_t *flag, *is_core;
+    int32_t *nodes;
+    Sp2Ctl *ctl;
+    double *bounds;         // [0..1] e_min, e_max; [2] tr X_0 over the core orbitals
+    double *rowlh, *partials;
+    void *sk, *table;
+    const double **final_buf;
+    double *iter;           // the parts' ping-pong iterates, packed
+    size_t iter_doubles, total;
+};
+
+static size_t gs_sk_bytes() { return (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double) + 1024; }
+
+static GraphSp2Ws carve_graph_sp2(void *ws, int64_t N, int n_parts, int cap)
+{
+    GraphSp2Ws w;
+    uint8_t *p = (uint8_t *)ws;
+    size_t off = 0;
+    w.scal = (int32_t *)(p + off); off = align_up(off + (size_t)(2 + 2 * BML_GRAPH_MAX_PARTS) * 4, 1024);
+    w.flag = p + off; off = align_up(off + (size_t)n_parts * N, 1024);
+    w.is_core = p + off; off = align_up(off + (size_t)n_parts * N, 1024);
+    w.nodes = (int32_t *)(p + off); off = align_up(off + (size_t)n_parts * N * 4, 1024);
+    w.ctl = (Sp2Ctl *)(p + off); off += GS_CTL_BYTES;
+    w.bounds = (double *)(p + off); off += 1024;
+    w.rowlh = (double *)(p + off); off = align_up(off + (size_t)2 * N * 8, 1024);
+    w.partials = (double *)(p + off); off = align_up(off + (size_t)SK_MAX_GRID * 4 * 8, 1024);
+    w.sk = p + off; off = align_up(off + gs_sk_bytes(), 1024);
+    w.table = p + off; off = align_up(off + dense_batch_table_bytes(), 1024);
+    w.final_buf = (const double **)(p + off); off = align_up(off + (size_t)BML_GRAPH_MAX_PARTS * 8, 1024);
+    const size_t ldc = ((size_t)cap + 15) / 16 * 16;
+    w.iter = (double *)(p + off);
+    w.iter_doubles = (size_t)n_parts * 2 * (align_up((size_t)cap * ldc * 8, 1024) / 8);
+    off = align_up(off + w.iter_doubles * 8, 1024);
+    w.total = off;
+    return w;
+}
+
+size_t graph_sp2_workspace_bytes(int64_t N, int n_parts, int cap) { return carve_graph_sp2(nullptr, N, n_parts, cap).total; }
+
+int graph_sp2_solve(const bml_matrix_t *H, const int32_t *offs, const int32_t *core_nodes, const bml_graph_sp2_params_t *p,
+                    bml_matrix_t *D, void *ws, bml_graph_sp2_stats_t *stats, cudaStream_t st)
+{
+    const int64_t N = H->N;
+    const int P = p->n_parts;
+    GraphSp2Ws w = carve_graph_sp2(ws, N, P, p->part_capacity);
+    int32_t h_scal[2 + 2 * BML_GRAPH_MAX_PARTS];
+    h_scal[0] = 0; h_scal[1] = INT32_MAX;
+    if (cudaMemcpyAsync(w.scal, h_scal, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return BML_ERR_CUDA;
+    int r = launch_graph_core_halo(H, offs, core_nodes, P, p->graph_tol, w.nodes, w.is_core, w.scal + 2, w.flag, st);
+    if (r) return r;
+    if ((r = launch_gershgorin(H, w.bounds, w.rowlh, st))) return r;           // one Eq. 5 map for every part
+    // the part sizes decide the launch shapes: the one host round trip before the end
+    if (cudaMemcpyAsync(h_scal + 2, w.scal + 2, (size_t)2 * P * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    int max_size = 0;
+    for (int q = 0; q < P; ++q) max_size = h_scal[2 + 2 * q] > max_size ? h_scal[2 + 2 * q] : max_size;
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->n_parts = P; stats->overflow_row = -1; stats->max_part_size = max_size;
+        for (int q = 0; q < P; ++q) { stats->part_size[q] = h_scal[2 + 2 * q]; stats->core_size[q] = h_scal[3 + 2 * q]; }
+    }
+    if (max_size > p->part_capacity) return BML_ERR_PART_CAPACITY;
+
+    // ---- gather h^k and rescale it in place to X_0^k (Eq. 5 with the bounds of H); build the job table
+    int32_t n[BML_GRAPH_MAX_PARTS], job_of[BML_GRAPH_MAX_PARTS];
+    double *b0[BML_GRAPH_MAX_PARTS], *b1[BML_GRAPH_MAX_PARTS];
+    int64_t ld[BML_GRAPH_MAX_PARTS];
+    const uint8_t *core[BML_GRAPH_MAX_PARTS];
+    int nj = 0;
+    size_t used = 0;
+    for (int q = 0; q < P; ++q) {
+        const int s = h_scal[2 + 2 * q];
+        if (s < 1) continue;
+        const int64_t l = ((int64_t)s + 15) / 16 * 16;
+        const size_t one = align_up((size_t)s * l * 8, 1024) / 8;
+        if (used + 2 * one > w.iter_doubles) return BML_ERR_INVALID;
+        n[nj] = s; ld[nj] = l; b0[nj] = w.iter + used; b1[nj] = w.iter + used + one; core[nj] = w.is_core + (size_t)q * N;
+        job_of[nj] = q;
+        used += 2 * one;
+        if ((r = launch_graph_gather(H, w.nodes + (size_t)q * N, s, b0[nj], l, st))) return r;
+        const bml_matrix_t hd = {BML_DENSE, 0, s, l, b0[nj], nullptr, nullptr};
+        if ((r = launch_rescale_dense(&hd, w.bounds, b0[nj], l, st))) return r;
+        ++nj;
+    }
+    if (nj < 1) return BML_ERR_INVALID;
+    {
+        void *h_table = malloc(dense_batch_table_bytes());
+        if (!h_table) return BML_ERR_CUDA;
+        r = dense_batch_fill(h_table, nj, n, b0, b1, ld, core);
+        // pageable source: the copy is staged before cudaMemcpyAsync returns, so the buffer may be freed right away
+        if (!r && cudaMemcpyAsync(w.table, h_table, dense_batch_table_bytes(), cudaMemcpyHostToDevice, st) != cudaSuccess)
+            r = BML_ERR_CUDA;
+        if (!r && cudaStreamSynchronize(st) != cudaSuccess) r = BML_ERR_CUDA;
+        free(h_table);
+        if (r) return r;
+    }
+    if ((r = launch_batch_core_trace(w.table, w.bounds + 2, st))) return r;
+    if ((r = launch_init_ctl(w.ctl, w.bounds, w.bounds + 2, p->n_occ, p->max_products, p->idem_tol, 1, 0, nullptr, st)))
+        return r;
+    if (cudaMemsetAsync((uint8_t *)w.sk + (size_t)SK_MAX_GRID * SK_SLOT_DOUBLES * sizeof(double), 0, 1024, st) != cudaSuccess)
+        return BML_ERR_CUDA;
+    // ---- products: enqueued ahead of the device, launches behind the stop flag exit at once
+    if ((r = enqueue_products([&]() { return launch_x2_dense_fp64_batch(w.table, w.ctl, w.partials, w.sk, st); }, w.ctl,
+                              p->max_products, st)))
+        return r;
+    // ---- D rows of the core orbitals from X_{m*}^k
+    if ((r = launch_batch_final_buffers(w.table, w.ctl, w.final_buf, nj, st))) return r;
+    for (int j = 0; j < nj; ++j) {
+        const int q = job_of[j];
+        if ((r = launch_graph_scatter_sel(nullptr, ld[j], w.nodes + (size_t)q * N, w.is_core + (size_t)q * N, n[j],
+                                          p->drop_tol, D, w.scal + 1, st, w.final_buf + j)))
+            return r;
+    }
+    Sp2Ctl h;
+    if (cudaMemcpyAsync(&h, w.ctl, sizeof(Sp2Ctl), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(h_scal, w.scal, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+        return BML_ERR_CUDA;
+    int status = h.status;
+    if (status >= 0 && h_scal[1] != INT32_MAX) status = BML_ERR_ELL_OVERFLOW;
+    if (stats) {
+        bml_sp2_stats_t &s2 = stats->sp2;
+        s2.status = status; s2.m_star = h.m; s2.n_products = h.n_done; s2.overflow_row = -1;
+        s2.emin = h.emin; s2.emax = h.emax;
+        memcpy(s2.branch, h.branch, sizeof(h.branch));
+        memcpy(s2.trace, h.trace, sizeof(h.trace));
+        memcpy(s2.idem, h.idem, sizeof(h.idem));
+        stats->status = status;
         stats->overflow_row = h_scal[1] != INT32_MAX ? h_scal[1] : -1;
     }
     return status;

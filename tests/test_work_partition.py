@@ -126,3 +126,38 @@ def test_schedule_rejects_bad_k():
     assert L.bml_cheb_schedule(1, None, None, None) == -1
     assert L.bml_cheb_schedule(33, None, None, None) == -1
     assert L.bml_cheb_schedule(16, None, None, None) == 4
+
+
+@pytest.mark.parametrize("sizes,G", [([5600, 5600, 5600, 5600], 148), ([896, 896, 896], 148), ([5657, 5810, 300, 1, 129], 148),
+                                     ([200], 148), ([1500, 64], 7), ([128] * 40, 148), ([3000, 2000, 1000], 1)])
+def test_batched_work_list_covers_every_unit_of_every_part_once(sizes, G):
+    """The batched symmetric-square kernel of the graph-based SP2 solver (dense_batch.cu): pure stream-K over the units
+    (part, upper-triangle tile, 16-column k-slab) of parts of UNEQUAL sizes.  Every unit exactly once; a tile cut by a
+    range boundary has one owner (the piece starting at k-slab 0) followed by contributors on the next CTAs; a CTA
+    contributes to at most one tile and that piece is the FIRST item of its range (so hand-offs cannot cycle)."""
+    cover = {}
+    units = []
+    for c in range(G):
+        items = api.bml_dense_batch_work_items(sizes, G, c)
+        units.append(sum(k1 - k0 for _, _, k0, k1, _ in items))
+        for pos, (job, tile, k0, k1, KT) in enumerate(items):
+            T = (sizes[job] + 127) // 128
+            assert 0 <= job < len(sizes) and 0 <= tile < T * (T + 1) // 2 and KT == (sizes[job] + 15) // 16
+            assert 0 <= k0 < k1 <= KT
+            if k0 > 0:
+                assert pos == 0, "a contributed piece must come first in the CTA's range"
+            if k1 < KT:
+                assert pos == len(items) - 1, "only the last item of a range may be cut short"
+            cover.setdefault((job, tile), []).append((k0, k1, c))
+    want = {(j, t) for j, n in enumerate(sizes) for t in range(((n + 127) // 128) * ((n + 127) // 128 + 1) // 2)}
+    assert set(cover) == want
+    for (job, tile), parts in cover.items():
+        KT = (sizes[job] + 15) // 16
+        parts.sort()
+        assert parts[0][0] == 0 and parts[-1][1] == KT
+        for (a0, a1, ca), (b0, b1, cb) in zip(parts, parts[1:]):
+            assert a1 == b0 and cb > ca
+        # contributors are consecutive CTAs, up to CTAs whose range is empty (tiny batches on many CTAs)
+        ctas = [p[2] for p in parts]
+        assert all(units[c] == 0 for c in range(ctas[0], ctas[-1] + 1) if c not in ctas)
+    assert max(units) - min(units) <= 1
