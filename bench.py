@@ -34,7 +34,7 @@ import numpy as np  # noqa: E402
 METRIC = "sp2_time_to_D_ms"
 DEFAULT_WORKLOAD = "dense_n8192"            # BASELINE.json configs[2]: the largest FP64 single-GPU configuration
 METRIC_CHEBY = "chebyshev_time_to_D_ms"     # SURVEY 8(f) item f-1 workloads (--workload cheby_n*)
-METRIC_GRAPH = "graph_time_to_D_ms"         # SURVEY 8(f) item f-2 workloads (--workload graph_n*)
+METRIC_GRAPH = "graph_time_to_D_ms"         # SURVEY 8(f) item f-2 workloads (--workload graph_n*, graph_sp2_n*)
 PAPER_DSMS = 148 * 64 * 2  # flops per clock of the FP64 tensor pipe: 148 SMs x 64 FMA/clk/SM
 
 
@@ -293,6 +293,34 @@ def oracle_graph_time_to_D(wname: str, H):
                 f"products timed at part size {h.shape[0]}, scaled to all parts"), cores
 
 
+def oracle_graph_sp2_time_to_D(wname: str, H, n_products):
+    """Time the graph-SP2 oracle (oracle/graph.py graph_sp2) on `wname` as a bounded sample: the halo lists and gathers of
+    every part in full (Python loops), and ONE plain triple-loop product (oracle.x2_dense) on the leading 2048 x 2048
+    block of the first part, scaled by sum_p (n_p / 2048)^3 x products (every product of the oracle is that loop).
+    Returns (ms, sample, cores)."""
+    import oracle
+    from oracle import graph as og
+    from paper_2401_13772_b200 import hamiltonians as hm
+
+    w = hm.WORKLOADS[wname]
+    offs, nodes = og.regular_partition(w.N, w.n_parts)
+    t0 = time.perf_counter()
+    parts = [og.core_halo(*H, nodes[offs[p]: offs[p + 1]], w.graph_tol) for p in range(w.n_parts)]
+    subs = [og.matrix2submatrix(*H, pn) for pn, _ in parts]
+    t_move = time.perf_counter() - t0
+    nb = min(2048, subs[0].shape[0])
+    lo, hi = oracle.gershgorin_ellpack(*H)
+    Xb = oracle.rescale_dense(np.ascontiguousarray(subs[0][:nb, :nb]), lo, hi)
+    t0 = time.perf_counter()
+    oracle.x2_dense(Xb)
+    per = time.perf_counter() - t0
+    full = n_products or 24
+    scale = sum((sub.shape[0] / nb) ** 3 for sub in subs)
+    ms = (t_move + per * scale * full) * 1e3
+    return ms, (f"halo lists + gathers of all {w.n_parts} parts timed in full ({t_move:.1f} s); one oracle product on the "
+                f"leading {nb}x{nb} block, scaled by sum_p (n_p/{nb})^3 x {full} products"), oracle.omp_threads()
+
+
 EXPECTED_PRODUCTS = {"dense_n256": 15, "dense_n2048": 19, "dense_n8192": 32, "mixed_n16384": 30,
                      "mixed_bf16x3_n16384": 30, "ellpack_n65536": 12}
 
@@ -313,13 +341,15 @@ def run_reference(args):
             ms, sample, cores, _ = oracle_cheby_time_to_D(args.workload, H, 0.0)
         elif w.kind == "graph":
             ms, sample, cores = oracle_graph_time_to_D(args.workload, H)
+        elif w.kind == "graph_sp2":
+            ms, sample, cores = oracle_graph_sp2_time_to_D(args.workload, H, None)
         else:
             ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
         if it >= args.warmup:
             times.append(ms)
     v = float(np.mean(times))
     line = {
-        "impl": "reference", "metric": {"cheby": METRIC_CHEBY, "graph": METRIC_GRAPH}.get(w.kind, METRIC), "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": {"cheby": METRIC_CHEBY, "graph": METRIC_GRAPH, "graph_sp2": METRIC_GRAPH}.get(w.kind, METRIC), "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": workload_config(args.workload),
@@ -349,6 +379,10 @@ def workload_config(name: str):
                                 "BASELINE.json configs[3])"}[w.precision]
     if w.kind == "ellpack":
         cfg.update({"M": w.M, "drop_tol": w.drop_tol})
+    if w.kind == "graph_sp2":
+        cfg["l2"] = "flushed between steps (256 MiB write)"
+        cfg.update({"M": w.M, "M_out": w.M_out, "n_parts": w.n_parts, "graph_tol": w.graph_tol, "drop_tol": w.drop_tol,
+                    "partition": "regular index segments", "local_solver": "SP2, one polynomial for all parts"})
     if w.kind == "graph":
         for key in ("n_occ", "idem_tol", "max_products"):
             cfg.pop(key)
@@ -934,6 +968,95 @@ def run_graph(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------------------------
+# our arm, graph-based workloads with SP2 as the local solver: one bml_graph_sp2_ellpack call per step
+# ----------------------------------------------------------------------------------------------------------
+def run_graph_sp2(args):
+    import torch
+
+    from paper_2401_13772_b200 import api, hamiltonians as hm
+
+    rk = Ranks()
+    api.load()
+    dev = rk.dev
+    w = hm.WORKLOADS[args.workload]
+    H_np = hm.make_ellpack(args.workload)
+    H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
+    H_dev = tuple(a.to(dev) for a in H_host)
+    offs_np, nodes_np = hm.regular_core_partition(w.N, w.n_parts)
+    offs, nodes = torch.from_numpy(offs_np).to(dev), torch.from_numpy(nodes_np).to(dev)
+    sizes = api.bml_graph_core_halo(H_dev, offs, nodes, w.graph_tol)[2].cpu().numpy()
+    cap = int(sizes[:, 0].max())
+    solver = api.GraphSp2Solver(w.N, w.M_out, w.n_parts, cap, dev)
+    D_host = tuple(torch.empty_like(a).pin_memory() for a in (solver.dv.cpu(), solver.di.cpu(), solver.dn.cpu()))
+
+    def solve(Hd):
+        return solver.solve(Hd, offs, nodes, w.graph_tol, w.n_occ, w.idem_tol, w.drop_tol)
+
+    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
+    ms = float(np.mean(step_ms))
+
+    def e2e_step():
+        D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
+        for dst, src in zip(D_host, D):
+            dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = sum(a.numel() * a.element_size() for a in H_host)
+    d2h = sum(a.numel() * a.element_size() for a in D_host)
+    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps)
+
+    # dominant kernel: x2_dense_fp64_batch_kernel, one launch = one product of every part; its rate is taken in-step
+    # (the launches are the step but for the halo / gather / rescale / scatter kernels, < 1% of it)
+    peak_probe = api.bml_probe_fp64_tensor_peak(40000)
+    n_prod = int(res.sp2.n_products)
+    flops = sum(dense_flops_per_product(int(sz)) if sz > 1024 else 2.0 * (((sz + 127) // 128) * ((sz + 127) // 128 + 1) // 2) * 128 * 128 * sz
+                for sz in res.part_size)
+    achieved = flops * n_prod / (ms * 1e-3) / 1e12
+    roof = {
+        "bound": "tensor", "kernel": "x2_dense_fp64_batch_kernel", "achieved": achieved, "peak": peak_probe,
+        "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
+        "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run "
+                       "(MEASURED_PEAKS.json has no FP64 entry)",
+        "note": "in-step rate: executed flops of all products / whole time-to-D (includes halo, gather, rescale, scatter)",
+        "launch_ms": ms / max(n_prod, 1), "flops_per_launch": flops, "part_size": res.part_size,
+    }
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], rk.dist, dev)
+    if rk.rank != 0:
+        rk.finish()
+        return 0
+    cpu = None
+    if rk.world == 1 and not args.no_cpu_baseline:
+        v, sample, cores = oracle_graph_sp2_time_to_D(args.workload, H_np, n_prod)
+        cpu = {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample}
+    n_enq = 16
+    while n_enq < 100:
+        n_enq += 8
+        if n_enq - 8 >= max(n_prod, 16):
+            break
+    # 3 halo kernels + 2 Gershgorin + per part (gather, rescale) + core trace + init + products + final buffers + scatters
+    launches_per_step = 3 + 2 + 2 * w.n_parts + 2 + min(n_enq, 100) + 1 + w.n_parts
+    line = {
+        "metric": METRIC_GRAPH, "value": ms, "unit": "ms", "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(args.workload),
+        "status": int(res.status), "n_products": n_prod, "branch": res.sp2.branch, "part_size": res.part_size,
+        "core_size": res.core_size, "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)),
+        "wall_s_timed_region": t_wall, "ms_per_product": ms / max(n_prod, 1),
+        "aggregate_solves_per_s": replicas_per_second(rk.world, ms),
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches_note": f"{launches_per_step} per step (upper bound): halo, Gershgorin, gather + rescale per part, "
+                             f"{min(n_enq, 100)} batched product launches of which {n_prod} do work, scatter per part",
+        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    rk.finish()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -969,6 +1092,8 @@ def main():
         return run_cheby(args)
     if hm.WORKLOADS[args.workload].kind == "graph":
         return run_graph(args)
+    if hm.WORKLOADS[args.workload].kind == "graph_sp2":
+        return run_graph_sp2(args)
     return run_ours(args)
 
 

@@ -218,6 +218,16 @@ WORKLOADS["graph_n1536"] = Workload("graph_n1536", "graph", 1536, 768, 0.0, 1e-6
                                     note="24x8x8, same model; 3 x-slab parts, halo 3 layers")
 
 
+# The same two systems with SP2 as the local solver (bml_graph_sp2_ellpack, reading G3': one SP2 polynomial for all
+# parts): half filling, idempotency tolerance 1e-10 on the norms summed over the parts.
+WORKLOADS["graph_sp2_n12800"] = Workload("graph_sp2_n12800", "graph_sp2", 12800, 6400, 1e-10, 1e-6, M=128, lattice=(32, 20, 20),
+                                         n_parts=4, graph_tol=0.002, M_out=512,
+                                         note="32x20x20, -exp(-r/0.5), r<=3, delta=12; 4 x-slab parts, halo 3 layers; SP2 local solver")
+WORKLOADS["graph_sp2_n1536"] = Workload("graph_sp2_n1536", "graph_sp2", 1536, 768, 1e-10, 1e-6, M=128, lattice=(24, 8, 8),
+                                        n_parts=3, graph_tol=0.002, M_out=512,
+                                        note="24x8x8, same model; 3 x-slab parts, halo 3 layers; SP2 local solver")
+
+
 def regular_core_partition(N: int, n_parts: int):
     """Core partition into contiguous index segments (an INPUT of the graph path): (offsets[n_parts+1], nodes[N])."""
     offs = np.array([(p * N) // n_parts for p in range(n_parts + 1)], dtype=np.int32)
@@ -239,7 +249,7 @@ def make_dense(name: str, seed: int = 0) -> np.ndarray:
 
 def make_ellpack(name: str, seed: int = 0):
     w = WORKLOADS[name]
-    if w.kind == "graph":
+    if w.kind in ("graph", "graph_sp2"):
         return lattice_ellpack(w.lattice, 12.0, 0.2, 3.0, lambda r: -math.exp(-r / 0.5), w.M, seed)
     if name == "ellpack_n65536_literal":
         return lattice_ellpack(w.lattice, 1.5, 0.2, 3.0, lambda r: -math.exp(-r / 1.0), w.M, seed)

@@ -151,3 +151,43 @@ def test_runs_are_bit_reproducible(api):
     for _ in range(10):
         (dv, _, _), r = solver.solve(Hg, og_, ng, 0.02, N // 2, 1e-10, 0.0)
         assert torch.equal(dv, first) and r.sp2.branch == r0.sp2.branch
+
+
+def test_table2_shape_full_size_properties(api):
+    """The stand-in of the paper's Table II system (N = 12,800, 4 parts, core 3200, core+halo 5600) in the
+    launch configuration bench.py times.  The oracle's triple-loop products at this size take hours, so: properties
+    that hold at any size (status, occupation, every core row written, ascending columns, reproducibility of the branch
+    string on a second run) and agreement with this library's Chebyshev local solver (itself oracle-checked) at the
+    level both approximate the zero-temperature projector of the same parts (beta = 2: f_mu is a step to 1e-10)."""
+    import torch
+
+    w = hm.WORKLOADS["graph_sp2_n12800"]
+    H = gpu(hm.make_ellpack("graph_sp2_n12800"))
+    offs_np, nodes_np = hm.regular_core_partition(w.N, w.n_parts)
+    offs, nodes = tgpu(offs_np), tgpu(nodes_np)
+    solver = api.GraphSp2Solver(w.N, w.M_out, w.n_parts, 5600)
+    (dv, di, dn), res = solver.solve(H, offs, nodes, w.graph_tol, w.n_occ, w.idem_tol, w.drop_tol)
+    assert res.status == 0 and res.part_size == [5600] * 4 and res.core_size == [3200] * 4
+    assert res.sp2.idem[-1] < w.idem_tol and len(res.sp2.branch) == res.sp2.n_products - 1
+    rows = torch.arange(w.N, device="cuda").unsqueeze(1)
+    mask = torch.arange(w.M_out, device="cuda").unsqueeze(0) < dn.unsqueeze(1)
+    tr = dv[(di == rows) & mask].sum().item()
+    assert abs(tr - w.n_occ) < 1e-6                       # the shared branch sequence pins the core trace to N_occ
+    assert int(dn.min()) >= 1 and int(dn.max()) <= w.M_out
+    d = (di[:, 1:] - di[:, :-1])[mask[:, 1:]]
+    assert bool((d > 0).all())
+    first = (dv.clone(), di.clone(), dn.clone(), res.sp2.branch)
+    (dv, di, dn), res2 = solver.solve(H, offs, nodes, w.graph_tol, w.n_occ, w.idem_tol, w.drop_tol)
+    assert res2.sp2.branch == first[3] and torch.equal(dv, first[0]) and torch.equal(di, first[1])
+    # against the Chebyshev local solver on the same parts (graph_n12800: mu = 0, beta = 2, L = 255)
+    c = hm.WORKLOADS["graph_n12800"]
+    (cv, ci, cn), cres = api.bml_graph_chebyshev_ellpack(H, offs, nodes, c.graph_tol, c.mu, c.beta, c.k, c.m, c.drop_tol,
+                                                         c.M_out, 5600)
+    assert cres.status == 0
+    A = torch.zeros((64, w.N), dtype=torch.float64, device="cuda")
+    B = torch.zeros_like(A)
+    pick = torch.arange(0, w.N, w.N // 64, device="cuda")[:64]
+    for t, (r_, src_v, src_i, src_n, dst) in enumerate([(r, dv, di, dn, A) for r in pick] + [(r, cv, ci, cn, B) for r in pick]):
+        n = int(src_n[r_])
+        dst[t % 64, src_i[r_, :n].long()] = src_v[r_, :n]
+    assert (torch.linalg.norm(A - B) / torch.linalg.norm(A)).item() < 1e-6
