@@ -59,7 +59,9 @@ def _L():
         lib = ctypes.CDLL(build())
         lib.oracle_trace_dense.restype = ctypes.c_double
         lib.oracle_trace_ellpack.restype = ctypes.c_double
-        for name in ("oracle_rescale_ellpack", "oracle_x2_ellpack", "oracle_update_ellpack"):
+        lib.oracle_trace_ellblock.restype = ctypes.c_double
+        for name in ("oracle_rescale_ellpack", "oracle_x2_ellpack", "oracle_update_ellpack", "oracle_rescale_ellblock",
+                     "oracle_x2_ellblock", "oracle_update_ellblock"):
             getattr(lib, name).restype = ctypes.c_int64
         lib.oracle_x2_dense.restype = None
         lib.oracle_x2_dense_sampled.restype = None
@@ -225,4 +227,73 @@ def sp2_ellpack(value, index, nnz, n_occ, tol, tau, max_products=100, bounds=Non
                                    _p(nnz, _i32p), ctypes.c_int32(n_occ), ctypes.c_double(tol), ctypes.c_double(tau),
                                    ctypes.c_int32(max_products), b, _p(dv, _f64p), _p(di, _i32p), _p(dn, _i32p),
                                    ctypes.byref(st))
+    return (dv, di, dn), _stats_dict(st)
+
+
+# ----------------------------------------------- ELLBLOCK -----------------------------------------------
+# value[NB, MB, bs, bs] float64, index[NB, MB] int32 (block columns), nnz[NB] int32 (readings E1-E4 in sp2_oracle.c)
+def _blk(value, index, nnz):
+    value, index, nnz = _c64(value), _c32(index), _c32(nnz)
+    NB, MB, bs, bs2 = value.shape
+    assert bs == bs2 and index.shape == (NB, MB) and nnz.shape == (NB,)
+    return value, index, nnz, NB, MB, bs
+
+
+def gershgorin_ellblock(value, index, nnz):
+    value, index, nnz, NB, MB, bs = _blk(value, index, nnz)
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    rc = _L().oracle_gershgorin_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(value, _f64p),
+                                         _p(index, _i32p), _p(nnz, _i32p), ctypes.byref(lo), ctypes.byref(hi))
+    assert rc == 0
+    return lo.value, hi.value
+
+
+def trace_ellblock(value, index, nnz):
+    value, index, nnz, NB, MB, bs = _blk(value, index, nnz)
+    return float(_L().oracle_trace_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(value, _f64p),
+                                            _p(index, _i32p), _p(nnz, _i32p)))
+
+
+def rescale_ellblock(value, index, nnz, emin, emax):
+    """Eq. 5 on ELLBLOCK; returns (value, index, nnz, overflow block row)."""
+    value, index, nnz, NB, MB, bs = _blk(value, index, nnz)
+    xv, xi, xn = np.zeros_like(value), np.zeros_like(index), np.zeros_like(nnz)
+    bad = _L().oracle_rescale_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(value, _f64p),
+                                       _p(index, _i32p), _p(nnz, _i32p), ctypes.c_double(emin), ctypes.c_double(emax),
+                                       _p(xv, _f64p), _p(xi, _i32p), _p(xn, _i32p))
+    return xv, xi, xn, int(bad)
+
+
+def x2_ellblock(value, index, nnz, tau):
+    """P = thr_tau(X X) on blocks (a block is kept iff its Frobenius norm >= tau or it is diagonal).
+    Returns (value, index, nnz, overflow block row, max blocks per block row)."""
+    value, index, nnz, NB, MB, bs = _blk(value, index, nnz)
+    pv, pi, pn = np.zeros_like(value), np.zeros_like(index), np.zeros_like(nnz)
+    mx = ctypes.c_int32()
+    bad = _L().oracle_x2_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(value, _f64p),
+                                  _p(index, _i32p), _p(nnz, _i32p), ctypes.c_double(tau), _p(pv, _f64p), _p(pi, _i32p),
+                                  _p(pn, _i32p), ctypes.byref(mx))
+    return pv, pi, pn, int(bad), int(mx.value)
+
+
+def update_ellblock(X, P, tau):
+    """X' = thr_tau(2X - P) on the union of the block patterns."""
+    xv, xi, xn, NB, MB, bs = _blk(*X)
+    pv, pi, pn, _, _, _ = _blk(*P)
+    ov, oi, on = np.zeros_like(xv), np.zeros_like(xi), np.zeros_like(xn)
+    mx = ctypes.c_int32()
+    bad = _L().oracle_update_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(xv, _f64p),
+                                      _p(xi, _i32p), _p(xn, _i32p), _p(pv, _f64p), _p(pi, _i32p), _p(pn, _i32p),
+                                      ctypes.c_double(tau), _p(ov, _f64p), _p(oi, _i32p), _p(on, _i32p), ctypes.byref(mx))
+    return ov, oi, on, int(bad), int(mx.value)
+
+
+def sp2_ellblock(value, index, nnz, n_occ, tol, tau, max_products=100):
+    """Thresholded SP2 on ELLBLOCK.  Returns ((value, index, nnz) of D, stats dict)."""
+    value, index, nnz, NB, MB, bs = _blk(value, index, nnz)
+    dv, di, dn = np.zeros_like(value), np.zeros_like(index), np.zeros_like(nnz)
+    st = OracleStats()
+    _L().oracle_sp2_ellblock(ctypes.c_int64(NB), ctypes.c_int32(MB), ctypes.c_int32(bs), _p(value, _f64p), _p(index, _i32p),
+                             _p(nnz, _i32p), ctypes.c_int32(n_occ), ctypes.c_double(tol), ctypes.c_double(tau),
+                             ctypes.c_int32(max_products), _p(dv, _f64p), _p(di, _i32p), _p(dn, _i32p), ctypes.byref(st))
     return (dv, di, dn), _stats_dict(st)

@@ -463,6 +463,274 @@ done:
     return st->status = status;
 }
 
+/* =============================================== ELLBLOCK ============================================= */
+/*
+ * ELLBLOCK ("a generalization of ELLPACK-R where each element is a block"): N = NB * bs rows in NB block rows of
+ * bs x bs dense blocks, MB block slots per block row: block p of block row I is value[((I*MB + p)*bs + r)*bs + c],
+ * r, c < bs (row-major inside the block), at block column index[I*MB + p]; nnz[I] blocks are stored.
+ * Readings (items E1-E4 -- the paper gives the format's one-line definition only):
+ *   E1. one uniform block size bs; N is a multiple of bs;
+ *   E2. the threshold acts on BLOCKS: a block of thr(A) is kept iff its Frobenius norm sqrt(sum v^2) >= tau or it is a
+ *       diagonal block (I == J) -- for bs = 1 this is the scalar rule |v| >= tau or j == i (sqrt(v*v) == |v| exactly);
+ *   E3. accumulation order of a block product chain: blocks K of block row I ascending, and inside one block product
+ *       acc[r][c] = fma(A[r][k], B[k][c], acc[r][c]) for k = 0 .. bs-1 ascending -- for bs = 1 the scalar oracle's
+ *       order, so bs = 1 must reproduce oracle_x2_ellpack / oracle_sp2_ellpack bit for bit (pinned);
+ *   E4. everything else (Gershgorin over stored entries, Eq. 5 with a missing diagonal BLOCK inserted, union-pattern
+ *       norms, stop rules, D = X_{m*}, overflow of MB = failure -3) is the ELLPACK-R oracle's, applied per element.
+ */
+static double blk_norm(const double *b, int32_t bs)
+{
+    double s = 0.0;
+    for (int32_t q = 0; q < bs * bs; ++q) s += b[q] * b[q];
+    return sqrt(s);
+}
+
+int oracle_gershgorin_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *value, const int32_t *index,
+                               const int32_t *nnz, double *emin, double *emax)
+{
+    if (!value || !index || !nnz || NB <= 0 || MB < 1 || bs < 1) return -1;
+    const int64_t bb = (int64_t)bs * bs;
+    double lo = INFINITY, hi = -INFINITY;
+    for (int64_t I = 0; I < NB; ++I)
+        for (int32_t r = 0; r < bs; ++r) {
+            nsum_t rad = {0, 0};
+            double d = 0.0;
+            for (int32_t p = 0; p < nnz[I]; ++p) {
+                const double *b = value + (I * MB + p) * bb + (int64_t)r * bs;
+                for (int32_t c = 0; c < bs; ++c) {
+                    if (index[I * MB + p] == I && c == r) d = b[c];
+                    else nsum_add(&rad, fabs(b[c]));
+                }
+            }
+            const double g = nsum_get(&rad);
+            if (d - g < lo) lo = d - g;
+            if (d + g > hi) hi = d + g;
+        }
+    *emin = lo; *emax = hi;
+    return 0;
+}
+
+double oracle_trace_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *value, const int32_t *index,
+                             const int32_t *nnz)
+{
+    const int64_t bb = (int64_t)bs * bs;
+    nsum_t t = {0, 0};
+    for (int64_t I = 0; I < NB; ++I)
+        for (int32_t p = 0; p < nnz[I]; ++p)
+            if (index[I * MB + p] == I)
+                for (int32_t r = 0; r < bs; ++r) nsum_add(&t, value[(I * MB + p) * bb + (int64_t)r * bs + r]);
+    return nsum_get(&t);
+}
+
+/* Eq. 5 per element; a missing diagonal block is inserted (H_II = 0); blocks in ascending block-column order.
+ * Returns -1 if ok else the lowest block row that needs more than MB slots. */
+int64_t oracle_rescale_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *hv, const int32_t *hi, const int32_t *hn,
+                                double emin, double emax, double *xv, int32_t *xi, int32_t *xn)
+{
+    const double s = 1.0 / (emax - emin);
+    const int64_t bb = (int64_t)bs * bs;
+    int64_t bad = -1;
+    for (int64_t I = 0; I < NB; ++I) {
+        const int32_t n = hn[I];
+        int32_t have = 0, cnt = 0;
+        for (int32_t p = 0; p < n; ++p) if (hi[I * MB + p] == I) have = 1;
+        if (n + (have ? 0 : 1) > MB) { if (bad < 0) bad = I; xn[I] = 0; continue; }
+        for (int32_t p = 0; p < n; ++p) xi[I * MB + cnt++] = hi[I * MB + p];
+        if (!have) xi[I * MB + cnt++] = (int32_t)I;
+        qsort(xi + I * MB, (size_t)cnt, sizeof(int32_t), cmp_i32);
+        for (int32_t q = 0; q < cnt; ++q) {
+            const int32_t J = xi[I * MB + q];
+            const double *src = NULL;
+            for (int32_t p = 0; p < n; ++p) if (hi[I * MB + p] == J) src = hv + (I * MB + p) * bb;
+            double *dst = xv + (I * MB + q) * bb;
+            for (int32_t r = 0; r < bs; ++r)
+                for (int32_t c = 0; c < bs; ++c) {
+                    const double h = src ? src[(int64_t)r * bs + c] : 0.0;
+                    dst[(int64_t)r * bs + c] = (J == I && r == c) ? s * (emax - h) : -s * h;
+                }
+        }
+        for (int32_t q = cnt; q < MB; ++q) { xi[I * MB + q] = 0; memset(xv + (I * MB + q) * bb, 0, sizeof(double) * bb); }
+        xn[I] = cnt;
+    }
+    return bad;
+}
+
+/* P = thr_tau(X X) on blocks (readings E2, E3): Gustavson over block rows with a dense array of accumulator blocks. */
+int64_t oracle_x2_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *xv, const int32_t *xi, const int32_t *xn,
+                           double tau, double *pv, int32_t *pi, int32_t *pn, int32_t *max_nnz)
+{
+    const int64_t bb = (int64_t)bs * bs;
+    int64_t bad = -1;
+    int32_t mx = 0;
+#pragma omp parallel
+    {
+        double *acc = (double *)calloc((size_t)NB * (size_t)bb, sizeof(double));
+        uint8_t *seen = (uint8_t *)calloc((size_t)NB, 1);
+        int32_t *touched = (int32_t *)malloc(sizeof(int32_t) * (size_t)NB);
+#pragma omp for schedule(dynamic, 16) reduction(max : mx)
+        for (int64_t I = 0; I < NB; ++I) {
+            int32_t nt = 0;
+            for (int32_t p = 0; p < xn[I]; ++p) {
+                const int32_t K = xi[I * MB + p];
+                const double *A = xv + (I * MB + p) * bb;
+                for (int32_t q = 0; q < xn[K]; ++q) {
+                    const int32_t J = xi[(int64_t)K * MB + q];
+                    const double *Bk = xv + ((int64_t)K * MB + q) * bb;
+                    double *C = acc + (int64_t)J * bb;
+                    if (!seen[J]) { seen[J] = 1; memset(C, 0, sizeof(double) * bb); touched[nt++] = J; }
+                    for (int32_t r = 0; r < bs; ++r)
+                        for (int32_t c = 0; c < bs; ++c) {
+                            double v = C[(int64_t)r * bs + c];
+                            for (int32_t k = 0; k < bs; ++k) v = fma(A[(int64_t)r * bs + k], Bk[(int64_t)k * bs + c], v);
+                            C[(int64_t)r * bs + c] = v;
+                        }
+                }
+            }
+            qsort(touched, (size_t)nt, sizeof(int32_t), cmp_i32);
+            int32_t cnt = 0;
+            for (int32_t u = 0; u < nt; ++u) {
+                const int32_t J = touched[u];
+                const double *C = acc + (int64_t)J * bb;
+                if (blk_norm(C, bs) >= tau || J == I) {
+                    if (cnt < MB) { pi[I * MB + cnt] = J; memcpy(pv + (I * MB + cnt) * bb, C, sizeof(double) * bb); }
+                    ++cnt;
+                }
+                seen[J] = 0;
+            }
+            if (cnt > mx) mx = cnt;
+            if (cnt > MB) {
+#pragma omp critical
+                { if (bad < 0 || I < bad) bad = I; }
+                cnt = MB;
+            }
+            for (int32_t q = cnt; q < MB; ++q) { pi[I * MB + q] = 0; memset(pv + (I * MB + q) * bb, 0, sizeof(double) * bb); }
+            pn[I] = cnt;
+        }
+        free(acc); free(seen); free(touched);
+    }
+    if (max_nnz) *max_nnz = mx;
+    return bad;
+}
+
+/* ||P - X||_F^2 over the union of the two block patterns (an absent block = 0) and ||X||_F^2 */
+static void ellblock_norms(int64_t NB, int32_t MB, int32_t bs, const double *pv, const int32_t *pi, const int32_t *pn,
+                           const double *xv, const int32_t *xi, const int32_t *xn, double *e2, double *x2)
+{
+    const int64_t bb = (int64_t)bs * bs;
+    nsum_t a = {0, 0}, b = {0, 0};
+    for (int64_t I = 0; I < NB; ++I) {
+        nsum_t ra = {0, 0}, rb = {0, 0};
+        int32_t p = 0, q = 0;
+        while (p < pn[I] || q < xn[I]) {
+            const int32_t jp = p < pn[I] ? pi[I * MB + p] : INT32_MAX, jx = q < xn[I] ? xi[I * MB + q] : INT32_MAX;
+            const double *P = (jp <= jx) ? pv + (I * MB + p) * bb : NULL, *X = (jx <= jp) ? xv + (I * MB + q) * bb : NULL;
+            for (int64_t t = 0; t < bb; ++t) {
+                const double d = (P ? P[t] : 0.0) - (X ? X[t] : 0.0);
+                nsum_add(&ra, d * d);
+            }
+            if (P) ++p;
+            if (X) ++q;
+        }
+        for (q = 0; q < xn[I]; ++q)
+            for (int64_t t = 0; t < bb; ++t) nsum_add(&rb, xv[(I * MB + q) * bb + t] * xv[(I * MB + q) * bb + t]);
+        nsum_add(&a, nsum_get(&ra));
+        nsum_add(&b, nsum_get(&rb));
+    }
+    *e2 = nsum_get(&a); *x2 = nsum_get(&b);
+}
+
+/* X' = thr_tau(2X - P) on the union of the block patterns; diagonal blocks always kept. */
+int64_t oracle_update_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *xv, const int32_t *xi, const int32_t *xn,
+                               const double *pv, const int32_t *pi, const int32_t *pn, double tau, double *ov, int32_t *oi,
+                               int32_t *on, int32_t *max_nnz)
+{
+    const int64_t bb = (int64_t)bs * bs;
+    int64_t bad = -1;
+    int32_t mx = 0;
+    double *tmp = (double *)malloc(sizeof(double) * (size_t)bb);
+    for (int64_t I = 0; I < NB; ++I) {
+        int32_t p = 0, q = 0, cnt = 0;
+        while (p < pn[I] || q < xn[I]) {
+            const int32_t jp = p < pn[I] ? pi[I * MB + p] : INT32_MAX, jx = q < xn[I] ? xi[I * MB + q] : INT32_MAX;
+            const double *P = (jp <= jx) ? pv + (I * MB + p) * bb : NULL, *X = (jx <= jp) ? xv + (I * MB + q) * bb : NULL;
+            const int32_t J = jp < jx ? jp : jx;
+            for (int64_t t = 0; t < bb; ++t) tmp[t] = X ? (P ? 2.0 * X[t] - P[t] : 2.0 * X[t]) : -P[t];
+            if (P) ++p;
+            if (X) ++q;
+            if (blk_norm(tmp, bs) >= tau || J == I) {
+                if (cnt < MB) { oi[I * MB + cnt] = J; memcpy(ov + (I * MB + cnt) * bb, tmp, sizeof(double) * bb); }
+                ++cnt;
+            }
+        }
+        if (cnt > mx) mx = cnt;
+        if (cnt > MB) { if (bad < 0) bad = I; cnt = MB; }
+        for (int32_t u = cnt; u < MB; ++u) { oi[I * MB + u] = 0; memset(ov + (I * MB + u) * bb, 0, sizeof(double) * bb); }
+        on[I] = cnt;
+    }
+    free(tmp);
+    if (max_nnz) *max_nnz = mx;
+    return bad;
+}
+
+/* SP2 on ELLBLOCK: the ELLPACK-R loop (oracle_sp2_ellpack_bounds) with the block operations above. */
+int oracle_sp2_ellblock(int64_t NB, int32_t MB, int32_t bs, const double *hv, const int32_t *hi, const int32_t *hn,
+                        int32_t n_occ, double tol, double tau, int32_t max_products, double *dv, int32_t *di, int32_t *dn,
+                        oracle_stats_t *st)
+{
+    stats_init(st);
+    if (!hv || !hi || !hn || !dv || !di || !dn || NB <= 0 || MB < 1 || bs < 1 || n_occ <= 0 || n_occ >= NB * bs ||
+        !(tol > 0) || !(tau >= 0) || max_products < 1 || max_products > ORACLE_LOG_LEN)
+        return st->status = -1;
+    for (int64_t I = 0; I < NB; ++I) if (hn[I] < 0 || hn[I] > MB) return st->status = -1;
+    double emin, emax;
+    oracle_gershgorin_ellblock(NB, MB, bs, hv, hi, hn, &emin, &emax);
+    st->emin = emin; st->emax = emax;
+    if (!(emax - emin > 0)) return st->status = -2;
+    const size_t nm = (size_t)NB * (size_t)MB, nv = nm * (size_t)bs * (size_t)bs;
+    double *xv = (double *)malloc(sizeof(double) * nv), *pv = (double *)malloc(sizeof(double) * nv),
+           *yv = (double *)malloc(sizeof(double) * nv);
+    int32_t *xi = (int32_t *)malloc(sizeof(int32_t) * nm), *pi = (int32_t *)malloc(sizeof(int32_t) * nm),
+            *yi = (int32_t *)malloc(sizeof(int32_t) * nm);
+    int32_t *xn = (int32_t *)malloc(sizeof(int32_t) * (size_t)NB), *pn = (int32_t *)malloc(sizeof(int32_t) * (size_t)NB),
+            *yn = (int32_t *)malloc(sizeof(int32_t) * (size_t)NB);
+    int status = 2, m = 0;
+    int64_t bad = oracle_rescale_ellblock(NB, MB, bs, hv, hi, hn, emin, emax, xv, xi, xn);
+    if (bad >= 0) { st->overflow_row = (int32_t)bad; status = -3; goto done; }
+    for (m = 0;; ++m) {
+        const double t = oracle_trace_ellblock(NB, MB, bs, xv, xi, xn);
+        int32_t mxp = 0, mxu = 0;
+        bad = oracle_x2_ellblock(NB, MB, bs, xv, xi, xn, tau, pv, pi, pn, &mxp);
+        st->max_row_nnz[m] = mxp;
+        st->trace[m] = t;
+        if (bad >= 0) { st->overflow_row = (int32_t)bad; status = -3; break; }
+        double e2, x2;
+        ellblock_norms(NB, MB, bs, pv, pi, pn, xv, xi, xn, &e2, &x2);
+        st->idem[m] = sqrt(e2) / sqrt(x2);
+        const int s = stop_rule(m, st->idem, tol, max_products);
+        if (s >= 0) { status = s; break; }
+        const int b = (t - (double)n_occ <= 0.0);
+        st->branch[m] = (uint8_t)b;
+        if (b) {
+            bad = oracle_update_ellblock(NB, MB, bs, xv, xi, xn, pv, pi, pn, tau, yv, yi, yn, &mxu);
+            if (mxu > st->max_row_nnz[m]) st->max_row_nnz[m] = mxu;
+            if (bad >= 0) { st->overflow_row = (int32_t)bad; status = -3; break; }
+            memcpy(xv, yv, sizeof(double) * nv); memcpy(xi, yi, sizeof(int32_t) * nm);
+            memcpy(xn, yn, sizeof(int32_t) * (size_t)NB);
+        } else {
+            memcpy(xv, pv, sizeof(double) * nv); memcpy(xi, pi, sizeof(int32_t) * nm);
+            memcpy(xn, pn, sizeof(int32_t) * (size_t)NB);
+        }
+    }
+    if (status >= 0) {
+        memcpy(dv, xv, sizeof(double) * nv); memcpy(di, xi, sizeof(int32_t) * nm);
+        memcpy(dn, xn, sizeof(int32_t) * (size_t)NB);
+    }
+done:
+    st->m_star = m; st->n_products = m + 1;
+    free(xv); free(pv); free(yv); free(xi); free(pi); free(yi); free(xn); free(pn); free(yn);
+    return st->status = status;
+}
+
 int oracle_omp_threads(void)
 {
     int n = 1;

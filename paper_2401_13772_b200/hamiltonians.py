@@ -147,6 +147,62 @@ def ellpack_to_dense(value, index, nnz, N=None):
 # ----------------------------------------------------------------------------------------------
 # the BASELINE.json configs
 # ----------------------------------------------------------------------------------------------
+def ellblock_from_dense(A, bs, MB, tol=0.0):
+    """Pack a dense matrix into ELLBLOCK: value[NB, MB, bs, bs], index[NB, MB] int32 block columns
+    (ascending), nnz[NB]; a block is stored iff one of its entries has |a| > tol, or it is a diagonal block.
+    N must be a multiple of bs.  Layout only: no method arithmetic."""
+    N = A.shape[0]
+    assert N % bs == 0
+    NB = N // bs
+    blocks = np.ascontiguousarray(A.reshape(NB, bs, NB, bs).transpose(0, 2, 1, 3))
+    keep = (np.abs(blocks) > tol).any(axis=(2, 3)) | np.eye(NB, dtype=bool)
+    value = np.zeros((NB, MB, bs, bs), dtype=np.float64)
+    index = np.zeros((NB, MB), dtype=np.int32)
+    nnz = np.zeros(NB, dtype=np.int32)
+    for I in range(NB):
+        cols = np.nonzero(keep[I])[0]
+        assert cols.size <= MB, "block row does not fit MB slots"
+        nnz[I] = cols.size
+        index[I, : cols.size] = cols
+        value[I, : cols.size] = blocks[I, cols]
+    return value, index, nnz
+
+
+def ellblock_to_dense(value, index, nnz):
+    NB, MB, bs, _ = value.shape
+    A = np.zeros((NB, bs, NB, bs), dtype=np.float64)
+    for I in range(NB):
+        for p in range(int(nnz[I])):
+            A[I, :, int(index[I, p]), :] = value[I, p]
+    return A.reshape(NB * bs, NB * bs)
+
+
+def ellblock_from_ellpack(value, index, nnz, bs, MB):
+    """The same matrix in ELLBLOCK: every block that holds a stored scalar entry (and every diagonal block) is stored."""
+    N, M = value.shape
+    assert N % bs == 0
+    NB = N // bs
+    bv = np.zeros((NB, MB, bs, bs), dtype=np.float64)
+    bi = np.zeros((NB, MB), dtype=np.int32)
+    bn = np.zeros(NB, dtype=np.int32)
+    for I in range(NB):
+        cols = set([I])
+        for r in range(bs):
+            i = I * bs + r
+            cols.update((index[i, : nnz[i]] // bs).tolist())
+        cols = np.array(sorted(cols), dtype=np.int32)
+        assert cols.size <= MB, "block row does not fit MB slots"
+        pos = {int(c): q for q, c in enumerate(cols)}
+        bn[I] = cols.size
+        bi[I, : cols.size] = cols
+        for r in range(bs):
+            i = I * bs + r
+            for p in range(int(nnz[i])):
+                j = int(index[i, p])
+                bv[I, pos[j // bs], r, j % bs] = value[i, p]
+    return bv, bi, bn
+
+
 @dataclasses.dataclass
 class Workload:
     name: str
