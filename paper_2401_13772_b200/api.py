@@ -40,6 +40,9 @@ EXPORTS = [
     "bml_graph_workspace_bytes", "bml_graph_chebyshev_ellpack", "bml_graph_core_halo", "bml_matrix2submatrix_ellpack",
     "bml_submatrix2matrix_ellpack", "bml_graph_sp2_workspace_bytes", "bml_graph_sp2_ellpack",
     "bml_dense_batch_work_item",
+    # include/bml_ellblock.h
+    "bml_gershgorin_ellblock_workspace_bytes", "bml_gershgorin_ellblock", "bml_trace_ellblock",
+    "bml_sp2_ellblock_workspace_bytes", "bml_sp2_ellblock", "bml_x2_ellblock_workspace_bytes", "bml_x2_ellblock",
 ]
 GRAPH_MAX_PARTS = 256
 CHEB_MAX_K, CHEB_MAX_M, CHEB_MAX_TERMS, SYMM_MAX_JOBS = 32, 32, 1024, 16
@@ -131,6 +134,17 @@ class bml_graph_stats_t(ctypes.Structure):
         ("pad", ctypes.c_int32),
         ("part_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
         ("core_size", ctypes.c_int32 * GRAPH_MAX_PARTS),
+    ]
+
+
+class bml_ellblock_t(ctypes.Structure):
+    _fields_ = [
+        ("bs", ctypes.c_int32),
+        ("MB", ctypes.c_int32),
+        ("NB", ctypes.c_int64),
+        ("value", ctypes.c_void_p),
+        ("index", ctypes.c_void_p),
+        ("nnz", ctypes.c_void_p),
     ]
 
 
@@ -241,6 +255,20 @@ def load(build_if_missing: bool = True):
                                         ctypes.POINTER(bml_graph_sp2_stats_t), vp]
     L.bml_dense_batch_work_item.restype = ctypes.c_int
     L.bml_dense_batch_work_item.argtypes = [i32, i32p, i32, i32, i32, i32p]
+    EP = ctypes.POINTER(bml_ellblock_t)
+    L.bml_gershgorin_ellblock_workspace_bytes.restype = sz
+    L.bml_gershgorin_ellblock_workspace_bytes.argtypes = [i64, i32]
+    L.bml_gershgorin_ellblock.restype = ctypes.c_int
+    L.bml_gershgorin_ellblock.argtypes = [EP, vp, vp, sz, vp]
+    L.bml_trace_ellblock.restype = ctypes.c_int
+    L.bml_trace_ellblock.argtypes = [EP, vp, vp]
+    for name in ("bml_sp2_ellblock_workspace_bytes", "bml_x2_ellblock_workspace_bytes"):
+        getattr(L, name).restype = sz
+        getattr(L, name).argtypes = [i64, i32, i32]
+    L.bml_sp2_ellblock.restype = ctypes.c_int
+    L.bml_sp2_ellblock.argtypes = [EP, PP, EP, vp, sz, SP, vp]
+    L.bml_x2_ellblock.restype = ctypes.c_int
+    L.bml_x2_ellblock.argtypes = [EP, EP, i32, dbl, vp, vp, vp, sz, vp]
     L.bml_graph_core_halo.restype = ctypes.c_int
     L.bml_graph_core_halo.argtypes = [MP, vp, vp, i32, dbl, vp, vp, vp, vp, sz, vp]
     L.bml_matrix2submatrix_ellpack.restype = ctypes.c_int
@@ -784,6 +812,96 @@ def bml_graph_sp2_ellpack(H, core_offsets, core_nodes, graph_tol, n_occ, idem_to
     N = H[0].shape[0]
     solver = GraphSp2Solver(N, M_out, core_offsets.numel() - 1, part_capacity, H[0].device)
     return solver.solve(H, core_offsets, core_nodes, graph_tol, n_occ, idem_tol, drop_tol, max_products)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# ELLBLOCK (include/bml_ellblock.h): value[NB, MB, bs, bs] float64, index[NB, MB] int32, nnz[NB] int32
+# ------------------------------------------------------------------------------------------------------------
+def ellblock_desc(value: torch.Tensor, index: torch.Tensor, nnz: torch.Tensor) -> bml_ellblock_t:
+    _require_cuda(value, torch.float64, "ellblock value")
+    _require_cuda(index, torch.int32, "ellblock index")
+    _require_cuda(nnz, torch.int32, "ellblock nnz")
+    if value.dim() != 4 or value.shape[2] != value.shape[3] or index.shape != value.shape[:2] or nnz.shape != (value.shape[0],):
+        raise ValueError("ellblock: value[NB,MB,bs,bs], index[NB,MB], nnz[NB] expected")
+    if not (value.is_contiguous() and index.is_contiguous() and nnz.is_contiguous()):
+        raise ValueError("ellblock arrays must be contiguous")
+    NB, MB, bs, _ = value.shape
+    return bml_ellblock_t(bs, MB, NB, value.data_ptr(), index.data_ptr(), nnz.data_ptr())
+
+
+def bml_gershgorin_ellblock(H) -> torch.Tensor:
+    L = load()
+    d = ellblock_desc(*H)
+    out = torch.empty(2, dtype=torch.float64, device=H[0].device)
+    nbytes = L.bml_gershgorin_ellblock_workspace_bytes(d.NB, d.bs)
+    ws = torch.empty(max(nbytes, 8), dtype=torch.uint8, device=H[0].device)
+    rc = L.bml_gershgorin_ellblock(ctypes.byref(d), out.data_ptr(), ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_gershgorin_ellblock: {bml_status_string(rc)}")
+    return out
+
+
+def bml_trace_ellblock(A) -> torch.Tensor:
+    d = ellblock_desc(*A)
+    out = torch.empty(1, dtype=torch.float64, device=A[0].device)
+    rc = load().bml_trace_ellblock(ctypes.byref(d), out.data_ptr(), _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_trace_ellblock: {bml_status_string(rc)}")
+    return out
+
+
+class EllblockSolver:
+    def __init__(self, NB: int, MB: int, bs: int, device="cuda"):
+        L = load()
+        self.NB, self.MB, self.bs = int(NB), int(MB), int(bs)
+        self.device = torch.device(device)
+        self.dv = torch.zeros((NB, MB, bs, bs), dtype=torch.float64, device=self.device)
+        self.di = torch.zeros((NB, MB), dtype=torch.int32, device=self.device)
+        self.dn = torch.zeros((NB,), dtype=torch.int32, device=self.device)
+        self.ws_bytes = L.bml_sp2_ellblock_workspace_bytes(self.NB, self.MB, self.bs)
+        if self.ws_bytes == 0:
+            raise RuntimeError("bml_sp2_ellblock_workspace_bytes: " + bml_status_string(-1))
+        self.ws = _workspace(self.ws_bytes, self.device)
+
+    def solve(self, value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+        L = load()
+        h = ellblock_desc(value, index, nnz)
+        d = ellblock_desc(self.dv, self.di, self.dn)
+        p = bml_sp2_params_t(int(n_occ), int(max_products), float(idem_tol), float(drop_tol), 0, 0)
+        st = bml_sp2_stats_t()
+        rc = L.bml_sp2_ellblock(ctypes.byref(h), ctypes.byref(p), ctypes.byref(d), self.ws.data_ptr(), self.ws_bytes,
+                                ctypes.byref(st), _stream())
+        return (self.dv, self.di, self.dn), _result(st, rc)
+
+
+def bml_sp2_ellblock(value, index, nnz, n_occ: int, idem_tol: float, drop_tol: float, max_products: int = 100):
+    """Thresholded SP2 on ELLBLOCK.  Returns ((value, index, nnz) CUDA tensors of D, Sp2Result)."""
+    _require_cuda(value, torch.float64, "value")
+    NB, MB, bs, _ = value.shape
+    return EllblockSolver(NB, MB, bs, value.device).solve(value, index, nnz, n_occ, idem_tol, drop_tol, max_products)
+
+
+def bml_x2_ellblock(X, branch: int, drop_tol: float, out=None, ws=None):
+    """One fused block product on an ELLBLOCK iterate (block rows ascending, X symmetric).
+    Returns ((value, index, nnz), sums[4], info[4]) -- all CUDA tensors."""
+    L = load()
+    value, index, nnz = X
+    x = ellblock_desc(value, index, nnz)
+    if out is None:
+        out = (torch.zeros_like(value), torch.zeros_like(index), torch.zeros_like(nnz))
+    o = ellblock_desc(*out)
+    sums = torch.empty(4, dtype=torch.float64, device=value.device)
+    info = torch.empty(4, dtype=torch.int32, device=value.device)
+    nbytes = L.bml_x2_ellblock_workspace_bytes(x.NB, x.MB, x.bs)
+    if nbytes == 0:
+        raise RuntimeError("bml_x2_ellblock_workspace_bytes: " + bml_status_string(-1))
+    if ws is None:
+        ws = _workspace(nbytes, value.device)
+    rc = L.bml_x2_ellblock(ctypes.byref(x), ctypes.byref(o), int(branch), float(drop_tol), sums.data_ptr(), info.data_ptr(),
+                           ws.data_ptr(), nbytes, _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_x2_ellblock: {bml_status_string(rc)}")
+    return out, sums, info
 
 
 def bml_dense_batch_work_items(sizes, n_ctas: int, cta: int):

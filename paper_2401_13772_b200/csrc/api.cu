@@ -223,7 +223,7 @@ EnqueueState &enqueue_state()
 // stats == NULL: the call is fully asynchronous -- nothing is copied back, the stream is not synchronised and the
 // return value only says that everything was enqueued (the verdict of the solve stays in the device control block,
 // whose first words bml_sp2_read_status copies out later).
-static int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
+int finish_solve(Sp2Ctl *d_ctl, bml_sp2_stats_t *stats, cudaStream_t st)
 {
     if (!stats) return cudaGetLastError() == cudaSuccess ? BML_OK : BML_ERR_CUDA;
     Sp2Ctl h;

@@ -825,6 +825,13 @@ int launch_rescale_ellpack(const bml_matrix_t *H, const double *d_bounds, double
     return 0;
 }
 
+int launch_sum_vector(const double *v, int N, double *d_out, cudaStream_t st)
+{
+    sum_vector_kernel<<<1, 1024, 0, st>>>(v, N, d_out);
+    BML_CHECK_LAUNCH();
+    return 0;
+}
+
 int launch_copy_out_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, const double *v1,
                             const int32_t *i1, const int32_t *n1, int64_t N, int M, const Sp2Ctl *ctl, double *dv,
                             int32_t *di, int32_t *dn, cudaStream_t st)

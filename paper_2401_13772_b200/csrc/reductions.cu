@@ -205,6 +205,13 @@ int launch_gershgorin(const bml_matrix_t *H, double *d_bounds, double *rowlh, cu
     return 0;
 }
 
+int launch_gershgorin_reduce(const double *rowlh, int N, double *d_bounds, cudaStream_t st)
+{
+    gershgorin_reduce_kernel<<<1, 1024, 0, st>>>(rowlh, N, d_bounds);
+    BML_CHECK_LAUNCH();
+    return 0;
+}
+
 int launch_trace_dense(const double *A, int64_t ld, int N, double *d_out, cudaStream_t st)
 {
     trace_dense_kernel<<<1, 1024, 0, st>>>(A, ld, N, d_out);

@@ -21,7 +21,7 @@ def _declared():
 def test_header_declares_the_north_star_entry_points():
     names = _declared()
     for required in ("bml_sp2_dense", "bml_sp2_ellpack", "bml_gershgorin", "bml_trace", "bml_chebyshev_dense",
-                     "bml_symm_ab_dense", "bml_graph_chebyshev_ellpack", "bml_graph_sp2_ellpack"):
+                     "bml_symm_ab_dense", "bml_graph_chebyshev_ellpack", "bml_graph_sp2_ellpack", "bml_sp2_ellblock"):
         assert required in names
 
 
@@ -46,9 +46,11 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
     src = r"""
     #include <stdio.h>
     #include "bml_graph.h"
-    int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t),
+    #include "bml_ellblock.h"
+    int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(bml_matrix_t), sizeof(bml_sp2_params_t), sizeof(bml_sp2_stats_t),
                            sizeof(bml_cheb_params_t), sizeof(bml_cheb_stats_t), sizeof(bml_graph_params_t),
-                           sizeof(bml_graph_stats_t), sizeof(bml_graph_sp2_params_t), sizeof(bml_graph_sp2_stats_t)); return 0; }
+                           sizeof(bml_graph_stats_t), sizeof(bml_graph_sp2_params_t), sizeof(bml_graph_sp2_stats_t),
+                           sizeof(bml_ellblock_t)); return 0; }
     """
     import tempfile
 
@@ -60,7 +62,7 @@ def test_binding_lists_the_same_exports_and_struct_sizes():
                                     ctypes.sizeof(api.bml_sp2_stats_t), ctypes.sizeof(api.bml_cheb_params_t),
                                     ctypes.sizeof(api.bml_cheb_stats_t), ctypes.sizeof(api.bml_graph_params_t),
                                     ctypes.sizeof(api.bml_graph_stats_t), ctypes.sizeof(api.bml_graph_sp2_params_t),
-                                    ctypes.sizeof(api.bml_graph_sp2_stats_t)]
+                                    ctypes.sizeof(api.bml_graph_sp2_stats_t), ctypes.sizeof(api.bml_ellblock_t)]
 
 
 def test_sass_contains_the_blackwell_instructions():
@@ -76,7 +78,8 @@ def test_sass_contains_the_blackwell_instructions():
     # every kernel family of the three headers is in the image
     for kernel in ("x2_dense_fp64_sk_kernel", "x2_dense_mixed_kernel", "x2_ellpack_upper_kernel", "symm_ab_fp64_kernel",
                    "cheb_coeff_kernel", "cheb_sums_kernel", "graph_gather_kernel", "graph_scatter_kernel",
-                   "lanczos_run_kernel", "x2_dense_fp64_batch_kernel"):
+                   "lanczos_run_kernel", "x2_dense_fp64_batch_kernel", "x2_ellblock_upper_kernel",
+                   "x2_ellblock_assemble_kernel"):
         assert kernel in sass, kernel
 
 
