@@ -332,7 +332,10 @@ def run_reference(args):
     from paper_2401_13772_b200 import hamiltonians as hm
 
     w = hm.WORKLOADS[args.workload]
-    H = hm.make_dense(args.workload) if w.kind in ("dense", "cheby") else hm.make_ellpack(args.workload)
+    if w.kind == "ellblock":
+        H = hm.make_ellblock(args.workload)
+    else:
+        H = hm.make_dense(args.workload) if w.kind in ("dense", "cheby") else hm.make_ellpack(args.workload)
     total = args.steps + args.warmup
     budget = max(1.0, 200.0 / total)       # whole run within a few minutes
     times, sample, cores = [], "", 1
@@ -343,6 +346,15 @@ def run_reference(args):
             ms, sample, cores = oracle_graph_time_to_D(args.workload, H)
         elif w.kind == "graph_sp2":
             ms, sample, cores = oracle_graph_sp2_time_to_D(args.workload, H, None)
+        elif w.kind == "ellblock":
+            import oracle
+
+            lo, hi = oracle.gershgorin_ellblock(*H)
+            X0 = oracle.rescale_ellblock(*H, lo, hi)[:3]
+            t0 = time.perf_counter()
+            oracle.x2_ellblock(*X0, w.drop_tol)
+            ms = (time.perf_counter() - t0) * 12 * 1e3
+            sample, cores = "one oracle block product on X_0 timed, x 12 products", oracle.omp_threads()
         else:
             ms, sample, cores = oracle_time_to_D(args.workload, H, budget, EXPECTED_PRODUCTS.get(args.workload))
         if it >= args.warmup:
@@ -379,6 +391,9 @@ def workload_config(name: str):
                                 "BASELINE.json configs[3])"}[w.precision]
     if w.kind == "ellpack":
         cfg.update({"M": w.M, "drop_tol": w.drop_tol})
+    if w.kind == "ellblock":
+        cfg["l2"] = "flushed between steps (256 MiB write)"
+        cfg.update({"bs": w.bs, "MB": w.MB, "drop_tol": w.drop_tol, "drop_rule": "block Frobenius norm >= drop_tol or diagonal block"})
     if w.kind == "graph_sp2":
         cfg["l2"] = "flushed between steps (256 MiB write)"
         cfg.update({"M": w.M, "M_out": w.M_out, "n_parts": w.n_parts, "graph_tol": w.graph_tol, "drop_tol": w.drop_tol,
@@ -1057,6 +1072,124 @@ def run_graph_sp2(args):
     return 0
 
 
+# ----------------------------------------------------------------------------------------------------------
+# our arm, ELLBLOCK workloads: one bml_sp2_ellblock call per step
+# ----------------------------------------------------------------------------------------------------------
+def ellblock_block_macs(index, nnz, bs: int) -> int:
+    """Executed multiply-adds of one upper-triangle block product: for every stored block (I, K), the blocks (K, J) with
+    J >= I, bs^3 each (what kernel 1's DMMA chains execute for bs >= 8).  torch, chunked over block rows."""
+    import torch
+
+    NB, MB = index.shape
+    live = torch.arange(MB, device=index.device).unsqueeze(0) < nnz.unsqueeze(1)
+    total = 0
+    for I0 in range(0, NB, 256):
+        I1 = min(NB, I0 + 256)
+        K = index[I0:I1].long()                                   # [r, MB]
+        rows = index[K]                                           # [r, MB, MB] block columns of row K
+        ok = live[K] & (rows >= torch.arange(I0, I1, device=index.device).view(-1, 1, 1))
+        total += int((ok.sum(dim=2) * live[I0:I1]).sum().item())
+    return total * bs ** 3
+
+
+def run_ellblock(args):
+    import torch
+
+    from paper_2401_13772_b200 import api, hamiltonians as hm
+
+    rk = Ranks()
+    api.load()
+    dev = rk.dev
+    w = hm.WORKLOADS[args.workload]
+    H_np = hm.make_ellblock(args.workload)
+    H_host = tuple(torch.from_numpy(a).pin_memory() for a in H_np)
+    H_dev = tuple(a.to(dev) for a in H_host)
+    NB = w.N // w.bs
+    solver = api.EllblockSolver(NB, w.MB, w.bs, dev)
+    D_host = tuple(torch.empty_like(a).pin_memory() for a in H_host)
+
+    def solve(Hd, mp=100):
+        return solver.solve(*Hd, w.n_occ, w.idem_tol, w.drop_tol, mp)
+
+    step_ms, t_wall, clocks, res = timed_steps(rk, lambda: solve(H_dev), args)
+    ms = float(np.mean(step_ms))
+
+    def e2e_step():
+        D, _ = solve(tuple(a.to(dev, non_blocking=True) for a in H_host))
+        for dst, src in zip(D_host, D):
+            dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_steps = max(3, min(args.steps, 10))
+    h2d = sum(a.numel() * a.element_size() for a in H_host)
+    e2e_ms = timed_e2e(rk, e2e_step, e2e_steps) if res.status >= 0 else float("nan")
+
+    # dominant kernels: one fused product on a mid-sequence iterate (X_5), timed alone
+    roof, n_prod = None, int(res.n_products)
+    if res.status >= 0:
+        Xmid, _ = solve(H_dev, 6)
+        Xmid = tuple(t.clone() for t in Xmid)
+        out = tuple(torch.zeros_like(t) for t in Xmid)
+        ws = api._workspace(api.load().bml_x2_ellblock_workspace_bytes(NB, w.MB, w.bs), dev)
+        k_ms = time_alone(lambda: api.bml_x2_ellblock(Xmid, 1, w.drop_tol, out, ws), 5, warm=2)
+        macs = ellblock_block_macs(Xmid[1], Xmid[2], w.bs)
+        peak_probe = api.bml_probe_fp64_tensor_peak(40000)
+        achieved = 2.0 * macs / (k_ms * 1e-3) / 1e12
+        blocks = int(Xmid[2].sum().item())
+        pk, pk_src = peaks()
+        gathered = 2.0 * (macs / w.bs ** 3) * w.bs * w.bs * 8        # two operand blocks per block product
+        roof = {
+            "bound": "tensor", "kernel": "x2_ellblock_upper_kernel + x2_ellblock_assemble_kernel", "achieved": achieved,
+            "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
+            "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run",
+            "note": "executed DMMA flops of the upper-triangle block products (2 bs^3 per block pair) / time of the two "
+                    "kernels; the operand blocks come from L2 (2 flop per byte at bs = 8), so the L2 -> SM fabric, not "
+                    "the tensor pipe, bounds this kernel",
+            "launch_ms": k_ms, "flops_per_launch": 2.0 * macs, "mean_blocks_per_block_row": blocks / NB,
+            "stored_fill": None, "gathered_bytes": gathered, "gathered_gbs": gathered / (k_ms * 1e-3) / 1e9,
+            "compulsory_bytes": 2.0 * blocks * (w.bs * w.bs * 8 + 4),
+            "compulsory_frac_of_hbm": 2.0 * blocks * (w.bs * w.bs * 8 + 4) / (k_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+        }
+    ms, e2e_ms = aggregate_over_ranks([ms, e2e_ms], rk.dist, dev)
+    if rk.rank != 0:
+        rk.finish()
+        return 0
+    cpu = None
+    if rk.world == 1 and not args.no_cpu_baseline:
+        import oracle
+
+        lo, hi = oracle.gershgorin_ellblock(*H_np)
+        X0 = oracle.rescale_ellblock(*H_np, lo, hi)[:3]
+        t0 = time.perf_counter()
+        oracle.x2_ellblock(*X0, w.drop_tol)
+        per = time.perf_counter() - t0
+        cpu = {"value": per * max(n_prod, 1) * 1e3, "unit": "ms", "cores": oracle.omp_threads(), "kind": "oracle",
+               "sample": f"one oracle block product (the first, on X_0: the sparsest of the solve) timed, x {n_prod} products"}
+    n_enq = 16
+    while n_enq < 100:
+        n_enq += 8
+        if n_enq - 8 >= max(n_prod, 16):
+            break
+    launches_per_step = 2 + 1 + 1 + 1 + 2 * min(n_enq, 100) + 1
+    line = {
+        "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": workload_config(args.workload),
+        "status": int(res.status), "n_products": n_prod, "branch": res.branch,
+        "max_blocks_per_block_row": [int(x) for x in res.max_row_nnz],
+        "step_ms_min": float(min(step_ms)), "step_ms_max": float(max(step_ms)), "wall_s_timed_region": t_wall,
+        "ms_per_product": ms / max(n_prod, 1), "aggregate_solves_per_s": replicas_per_second(rk.world, ms),
+        "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h2d),
+                "steps": e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "gpu_launches_note": f"{launches_per_step} per step (upper bound); a product is two kernels",
+        "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    rk.finish()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -1094,6 +1227,8 @@ def main():
         return run_graph(args)
     if hm.WORKLOADS[args.workload].kind == "graph_sp2":
         return run_graph_sp2(args)
+    if hm.WORKLOADS[args.workload].kind == "ellblock":
+        return run_ellblock(args)
     return run_ours(args)
 
 

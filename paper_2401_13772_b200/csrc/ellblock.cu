@@ -28,6 +28,7 @@ namespace bmlsp2 {
 constexpr int EB_THREADS = 512;
 constexpr int EB_WARPS = EB_THREADS / 32;
 constexpr int EB_MAX_GRID = 1024;
+constexpr int EB_PIPE = 4;               // block pairs whose operand loads are in flight together (kernel 1)
 
 __device__ __forceinline__ int eb_find(const int *__restrict__ list, int n, int key)
 {
@@ -145,27 +146,53 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                     const int q = q0 + lane;
                     const int pI = q < nJ ? eb_find(sI, nI, rowJ[q]) : -1;
                     unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
-                    while (bal) {                          // matches in ascending K (row J is in ascending order)
-                        const int src = __ffs(bal) - 1;
-                        bal &= bal - 1;
-                        const int pA = __shfl_sync(0xffffffffu, pI, src);
-                        const double *A = sA + (size_t)pA * BB;
-                        const double *B = valJ + (size_t)(q0 + src) * BB;
+                    // matches in ascending K (row J is in ascending order), EB_PIPE at a time: the operand blocks of row
+                    // J come from L2 and their loads are issued for the whole group before the first DMMA needs them
+                    // (one match at a time left every warp waiting a full L2 round trip per block pair)
+                    while (bal) {
+                        int pA[EB_PIPE];
+                        const double *Bp[EB_PIPE];
+                        double bq[EB_PIPE][KS][MT];
+                        int nm = 0;
 #pragma unroll
-                        for (int s = 0; s < KS; ++s) {
-                            double a[MT], b[MT];
-                            const int col = 4 * s + t;
-#pragma unroll
-                            for (int m = 0; m < MT; ++m) {
-                                const int r = m * 8 + g;
-                                const bool ok = r < BS && col < BS;
-                                a[m] = ok ? A[r * BS + col] : 0.0;
-                                b[m] = ok ? __ldg(B + r * BS + col) : 0.0;
+                        for (int u = 0; u < EB_PIPE; ++u) {
+                            pA[u] = -1; Bp[u] = valJ;
+                            if (bal) {
+                                const int src = __ffs(bal) - 1;
+                                bal &= bal - 1;
+                                pA[u] = __shfl_sync(0xffffffffu, pI, src);
+                                Bp[u] = valJ + (size_t)(q0 + src) * BB;
+                                nm = u + 1;
                             }
+                        }
 #pragma unroll
-                            for (int m = 0; m < MT; ++m)
+                        for (int u = 0; u < EB_PIPE; ++u)
 #pragma unroll
-                                for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], b[n]);
+                            for (int s = 0; s < KS; ++s)
+#pragma unroll
+                                for (int m = 0; m < MT; ++m) {
+                                    const int r = m * 8 + g, col = 4 * s + t;
+                                    bq[u][s][m] = (u < nm && r < BS && col < BS) ? __ldg(Bp[u] + r * BS + col) : 0.0;
+                                }
+#pragma unroll
+                        for (int u = 0; u < EB_PIPE; ++u) {
+                            if (u < nm) {                  // warp-uniform
+                                const double *A = sA + (size_t)pA[u] * BB;
+#pragma unroll
+                                for (int s = 0; s < KS; ++s) {
+                                    double a[MT];
+                                    const int col = 4 * s + t;
+#pragma unroll
+                                    for (int m = 0; m < MT; ++m) {
+                                        const int r = m * 8 + g;
+                                        a[m] = (r < BS && col < BS) ? A[r * BS + col] : 0.0;
+                                    }
+#pragma unroll
+                                    for (int m = 0; m < MT; ++m)
+#pragma unroll
+                                        for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], bq[u][s][n]);
+                                }
+                            }
                         }
                     }
                 }

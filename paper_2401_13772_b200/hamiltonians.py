@@ -222,6 +222,9 @@ class Workload:
     n_parts: int = 0
     graph_tol: float = 0.0
     M_out: int = 0
+    # ELLBLOCK workloads (kind "ellblock"): block edge and block slots per block row
+    bs: int = 0
+    MB: int = 0
 
 
 WORKLOADS = {
@@ -280,6 +283,22 @@ WORKLOADS["graph_sp2_n12800"] = Workload("graph_sp2_n12800", "graph_sp2", 12800,
 WORKLOADS["graph_sp2_n1536"] = Workload("graph_sp2_n1536", "graph_sp2", 1536, 768, 1e-10, 1e-6, M=128, lattice=(24, 8, 8),
                                         n_parts=3, graph_tol=0.002, M_out=512,
                                         note="24x8x8, same model; 3 x-slab parts, halo 3 layers; SP2 local solver")
+
+
+# ELLBLOCK: the 5' sparse workload of the scalar ELLPACK path stored in 8 x 8 blocks
+# (z runs fastest in the site index, so a block is 8 consecutive z sites of one lattice column); same N, N_occ, tol, tau --
+# tau now acts on the Frobenius norm of a block (reading E2), so the block path keeps a superset of the scalar path's
+# entries.  256 block slots per block row (the iterates reach ~190).  The small variant is what the oracle finishes in seconds.
+WORKLOADS["ellblock_n65536"] = Workload("ellblock_n65536", "ellblock", 65536, 32768, 1e-8, 1e-6, M=512, lattice=(64, 32, 32),
+                                        bs=8, MB=256, note="5' model (64x32x32, -exp(-r/0.5), r<=3, delta=12) in 8x8 blocks")
+WORKLOADS["ellblock_n8192"] = Workload("ellblock_n8192", "ellblock", 8192, 4096, 1e-8, 1e-6, M=512, lattice=(16, 16, 32),
+                                       bs=8, MB=256, note="same model on 16x16x32, 8x8 blocks")
+
+
+def make_ellblock(name: str, seed: int = 0):
+    w = WORKLOADS[name]
+    ell = lattice_ellpack(w.lattice, 12.0, 0.2, 3.0, lambda r: -math.exp(-r / 0.5), w.M, seed)
+    return ellblock_from_ellpack(*ell, w.bs, w.MB)
 
 
 def regular_core_partition(N: int, n_parts: int):
