@@ -701,6 +701,8 @@ def sp2_measure(rk: Ranks, wname: str, steps: int, warmup: int, lanczos_steps: i
     pre = (2 + 1 + 1 + 1 + (1 if w.precision != 0 else 0)) if dense else (2 + 2 + 1)
     # a sparse product is two kernels; a mixed product is the FP64-diagonal kernel + the tcgen05 kernel
     launches_per_step = pre + n_enq * (2 if (not dense or w.precision != 0) else 1) + 1
+    if dense and w.precision == 0 and w.N <= 1024:
+        launches_per_step = pre + 1 + 1           # all products run inside ONE cooperative launch (whole-solve kernel)
     rec = {
         "ms": ms, "step_ms": step_ms, "t_wall": t_wall, "clocks": clocks, "res": res, "n_products": n_prod,
         "e2e_ms": e2e_ms, "e2e_steps": e2e_steps, "h2d": int(h2d), "d2h": int(d2h), "roofline": roof,

@@ -18,6 +18,9 @@ size_t dense_fp64_sk_bytes(int64_t N);
 int dense_fp64_sk_reset(void *sk, int64_t N, cudaStream_t st);
 int launch_x2_dense_fp64(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
                          int64_t N, Sp2Ctl *ctl, double *partials, void *sk, cudaStream_t stream);
+bool dense_fp64_loop_available(int64_t N);
+int launch_sp2_dense_fp64_loop(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
+                               int64_t N, Sp2Ctl *ctl, double *partials, int max_products, cudaStream_t stream);
 // dense_mixed.cu
 int dense_mixed_num_tiles(int64_t N);
 size_t dense_mixed_extra_bytes(int64_t N, int64_t ldx);
@@ -106,7 +109,8 @@ static_assert(sizeof(ScalarSlots) <= SCAL_BYTES, "scalar slots");
 // per-CTA partial-sum slots: enough for the grid of either dense product kernel
 static inline size_t partial_slots(int64_t N)
 {
-    const int a = dense_fp64_num_tiles(N), b = dense_mixed_num_tiles(N);
+    // the whole-solve kernel of small matrices (N <= 1024) alternates between two sets of per-CTA partial sums
+    const int a = dense_fp64_num_tiles(N) * (N <= 1024 ? 2 : 1), b = dense_mixed_num_tiles(N);
     return (size_t)(a > b ? a : b);
 }
 
@@ -429,19 +433,24 @@ int bml_sp2_dense(const bml_matrix_t *H, const bml_sp2_params_t *p, bml_matrix_t
         // D2-D5: products are enqueued ahead of the device; launches after the stop rule fired exit at once.
         // Small matrices: the prelude and the first batch of launches are launch-latency bound and form a static
         // sequence, replayed as a CUDA graph when the stream allows it (sp2_first_batch_cached).
-        const int n_first = p->max_products < ENQ_FIRST ? p->max_products : ENQ_FIRST;
-        auto first_batch = [&]() -> int {
+        // Small matrices (N <= 1024): a product is a few microseconds of work, so ALL products run inside one
+        // cooperative launch (sp2_dense_fp64_loop_kernel: grid barrier + device-side stop test between products); the
+        // prelude and that launch form a static sequence, replayed as a CUDA graph when the stream allows it.
+        auto small_solve = [&]() -> int {
             int r = prelude();
             if (r) return r;
-            if ((r = dense_fp64_sk_reset(w.sk, N, st))) return r;
-            for (int l = 0; l < n_first; ++l)
-                if ((r = launch_one())) return r;
-            return 0;
+            r = launch_sp2_dense_fp64_loop(map0, map1, w.X0, w.X1, w.ldx, N, w.ctl, w.partials, p->max_products, st);
+            return r == 1 ? BML_ERR_CUDA : r;
         };
-        const Sp2GraphKey key = {H->value, d_workspace, N, H->ld, p->idem_tol, p->n_occ, p->max_products, p->flags, st,
-                                 current_device()};
-        TRY(sp2_first_batch_cached(key, first_batch));
-        TRY(enqueue_products(launch_one, w.ctl, p->max_products, st, n_first, stats == nullptr));
+        if (dense_fp64_loop_available(N)) {
+            const Sp2GraphKey key = {H->value, d_workspace, N, H->ld, p->idem_tol, p->n_occ, p->max_products, p->flags, st,
+                                     current_device()};
+            TRY(sp2_first_batch_cached(key, small_solve));
+        } else {
+            TRY(prelude());
+            TRY(dense_fp64_sk_reset(w.sk, N, st));
+            TRY(enqueue_products(launch_one, w.ctl, p->max_products, st, 0, stats == nullptr));
+        }
     }
     TRY(launch_copy_out_dense(w.X0, w.X1, w.ldx, (int)N, w.ctl, D->value, D->ld, st));        // D6
     return finish_solve(w.ctl, stats, st);

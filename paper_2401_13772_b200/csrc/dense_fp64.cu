@@ -8,7 +8,11 @@
 // Pipeline: one producer thread issues TMA (cp.async.bulk.tensor, 128B swizzle, FP64 tensor map) into a STAGES-deep
 // ring of { A panel 128 x 16, B panel 128 x 16 } tiles guarded by full/empty mbarriers; 8 consumer warps (2 x 4, warp
 // tile 64 x 32) read fragments with conflict-free LDS.64 and issue mma.sync m8n8k4 f64 (SASS DMMA.8x8x4).
+#include <cooperative_groups.h>
+
 #include "dense_fp64_core.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace bmlsp2 {
 
@@ -132,6 +136,138 @@ x2_dense_fp64_kernel(const __grid_constant__ CUtensorMap map0, const __grid_cons
 #pragma unroll
         for (int q = 0; q < 4; ++q) s[q] = warp_sum(s[q]);
         if (lane == 0) sp2_finalise(ctl, s);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Whole-solve variant for small matrices (N <= 1024: one CTA per tile fits one wave of co-resident CTAs): ALL products of
+// an SP2 solve in ONE cooperative launch.  A product there is 5-40 us of work against ~18 us per kernel launch + drain, so
+// the launch sequence, not the arithmetic, set time-to-D (0.27 ms at N = 256 for 15 products; "fast
+// time-to-solution" at about a thousand orbitals is the paper's use case).  Between products: the last CTA's finaliser
+// (stop rules, next branch bit), then a grid barrier; the epilogue's global writes are fenced for the async proxy because
+// the next product's TMA loads read them.  The TMA ring and its mbarrier phases run on across products.
+// ------------------------------------------------------------------------------------------------------------
+// ring depth of the whole-solve kernel: small tiles have small stages (8 KB at BT = 32, 16 KB at BT = 64)
+constexpr int loop_stages(int BT) { return BT == 32 ? 16 : 12; }
+constexpr size_t loop_smem_bytes(int BT) { return (size_t)loop_stages(BT) * d_stage_bytes(BT) + 1024 + 1024; }
+
+template <int BT>
+__global__ void __launch_bounds__(D_THREADS, 1)
+sp2_dense_fp64_loop_kernel(const __grid_constant__ CUtensorMap map0, const __grid_constant__ CUtensorMap map1,
+                           double *__restrict__ buf0, double *__restrict__ buf1, int64_t ld, int N,
+                           Sp2Ctl *__restrict__ ctl, double *__restrict__ partials, int max_products)
+{
+    constexpr int D_BM = BT, D_BN = BT, D_PANEL_BYTES = d_panel_bytes(BT), D_STAGE_BYTES = d_stage_bytes(BT);
+    constexpr int MI = BT / 16, NI = BT / 32;
+    constexpr int ST = loop_stages(BT);          // deep ring: (almost) a whole row panel pair in flight
+    cg::grid_group grid = cg::this_grid();
+
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t *full_bar = (uint64_t *)(smem + (size_t)ST * D_STAGE_BYTES);
+    uint64_t *empty_bar = full_bar + ST;
+    double (*s_red)[4] = (double (*)[4])(empty_bar + ST);
+    int *s_last = (int *)(s_red + D_CONSUMER_WARPS);
+
+    const int warp_all = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = warp_all - D_PRODUCER_WARPS;
+    int I, J;
+    const bool valid = tile_sb_decode((int)blockIdx.x, (N + D_BM - 1) / D_BM, I, J);
+    const bool diag = (I == J);
+    const int KT = (N + D_BK - 1) / D_BK;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < ST; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], D_CONSUMER_WARPS); }
+        mbar_fence_init();
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (warp < 0) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(D_REGS_PRODUCER));
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(D_REGS_CONSUMER));
+
+    int slab = 0;                       // runs on across products (both roles count the same slabs)
+    StageRelease release;
+    uint32_t koff[4];
+    dmma_koff(lane, koff);
+    // Every CTA keeps its own copy of the loop state and takes the stop / branch decision itself from the same per-CTA
+    // partial sums added in the same order (bitwise identical in every CTA), so a product costs ONE grid barrier and one
+    // read of the partials; CTA 0 alone writes the control block (logs, parity, status) for the host and the copy-out.
+    int m = ctl->m, parity = ctl->parity, branch = ctl->branch_cur;
+    bool done = ctl->done != 0;
+    const int loop_mode = ctl->loop_mode, n_occ = ctl->n_occ;
+    const double idem_tol = ctl->idem_tol;
+    double e_prev1 = 0.0, e_prev2 = 0.0;          // e_{m-1}, e_{m-2}
+    for (int it = 0; it < max_products && !done; ++it) {
+        const CUtensorMap *map = parity ? &map1 : &map0;
+        const double *__restrict__ X = parity ? buf1 : buf0;
+        double *__restrict__ Xn = parity ? buf0 : buf1;
+        double *part = partials + (size_t)(it & 1) * gridDim.x * 4;      // two sets: a fast CTA may already write the next
+        if (threadIdx.x < D_CONSUMER_WARPS * 4) ((double *)s_red)[threadIdx.x] = 0.0;
+        __syncthreads();
+        if (!valid) {
+        } else if (warp < 0) {
+            if (warp_all == 0 && lane == 0) {
+                const uint32_t tx = diag ? D_PANEL_BYTES : D_STAGE_BYTES;
+                for (int kt = 0; kt < KT; ++kt, ++slab) {
+                    const int s = slab % ST;
+                    const uint32_t ph = (uint32_t)(slab / ST) & 1u;
+                    mbar_wait(&empty_bar[s], ph ^ 1u);
+                    mbar_expect_tx(&full_bar[s], tx);
+                    uint8_t *dst = smem + (size_t)s * D_STAGE_BYTES;
+                    tma_load_2d(dst, map, kt * D_BK, I * D_BM, &full_bar[s]);
+                    if (!diag) tma_load_2d(dst + D_PANEL_BYTES, map, kt * D_BK, J * D_BN, &full_bar[s]);
+                }
+            }
+        } else {
+            const int wm = warp >> 2, wn = warp & 3;
+            double acc[MI][NI][2];
+#pragma unroll
+            for (int i = 0; i < MI; ++i)
+#pragma unroll
+                for (int j = 0; j < NI; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+            const uint8_t *a_base = smem + wm * (D_BM / 2) * 128;
+            const uint8_t *b_base = smem + (diag ? 0 : D_PANEL_BYTES) + wn * (D_BN / 4) * 128;
+            for (int kt = 0; kt < KT; ++kt, ++slab) {
+                const int s = slab % ST;
+                const uint32_t ph = (uint32_t)(slab / ST) & 1u;
+                mbar_wait(&full_bar[s], ph);
+                const uint8_t *sa = a_base + (size_t)s * D_STAGE_BYTES, *sb = b_base + (size_t)s * D_STAGE_BYTES;
+                dmma_slab<MI, NI>(acc, sa, sb, koff);
+                release.after_slab(empty_bar, s, lane);
+            }
+            double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
+            sp2_tile_epilogue<MI, NI, BT>(acc, X, Xn, ld, N, I, J, wm, wn, lane, branch, s_trp, s_e, s_x, s_trn);
+            s_trp = warp_sum(s_trp); s_e = warp_sum(s_e); s_x = warp_sum(s_x); s_trn = warp_sum(s_trn);
+            if (lane == 0) { s_red[warp][0] = s_trp; s_red[warp][1] = s_e; s_red[warp][2] = s_x; s_red[warp][3] = s_trn; }
+            // X' is read by the next product's TMA loads (async proxy): order this thread's global writes before them
+            asm volatile("fence.proxy.async;" ::: "memory");
+        }
+        __syncthreads();
+        if (threadIdx.x < 4) {
+            double v = 0.0;
+#pragma unroll
+            for (int w = 0; w < D_CONSUMER_WARPS; ++w) v += s_red[w][threadIdx.x];
+            __stcg(&part[(size_t)blockIdx.x * 4 + threadIdx.x], v);
+        }
+        __threadfence();
+        grid.sync();
+        // every warp adds the partials in the same fixed order: all threads of all CTAs hold identical sums
+        double sm[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int tI = lane; tI < (int)gridDim.x; tI += 32) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sm[q] += __ldcg(&part[(size_t)tI * 4 + q]);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sm[q] = warp_sum(sm[q]);
+        if (blockIdx.x == 0 && threadIdx.x == 0) sp2_finalise(ctl, sm);       // the record: same rules, same numbers
+        if (!loop_mode) { done = true; break; }
+        // the decision of sp2_finalise (common.cuh), taken locally
+        const double e = sqrt(sm[1]) / sqrt(sm[2]);
+        if (e < idem_tol || (m >= 2 && e < 1e-2 && e >= e_prev2) || m + 1 == max_products) { done = true; break; }
+        e_prev2 = e_prev1; e_prev1 = e;
+        parity ^= 1;
+        m += 1;
+        branch = (sm[3] - (double)n_occ <= 0.0) ? 1 : 0;
     }
 }
 
@@ -409,6 +545,41 @@ static int launch_x2_dense_fp64_t(const CUtensorMap &map0, const CUtensorMap &ma
     x2_dense_fp64_kernel<BT><<<dense_fp64_num_tiles(N), D_THREADS, d_smem_bytes(BT), stream>>>(map0, map1, buf0, buf1, ld,
                                                                                               (int)N, ctl, partials);
     return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+// The whole product loop of a small solve in one cooperative launch.  Returns 1 if this device / size cannot run it (the
+// caller then enqueues the products one launch each), 0 when enqueued, or a negative status.
+template <int BT>
+static int launch_sp2_loop_t(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
+                             int64_t N, Sp2Ctl *ctl, double *partials, int max_products, cudaStream_t stream)
+{
+    static size_t have[MAX_DEVICES] = {};
+    if (ensure_smem_attr(sp2_dense_fp64_loop_kernel<BT>, loop_smem_bytes(BT), have)) return BML_ERR_CUDA;
+    const int tiles = dense_fp64_num_tiles(N);
+    if (sk_grid() <= 0 || tiles > sk_grid()) return 1;          // all CTAs must be co-resident (one per SM)
+    int n = (int)N;
+    CUtensorMap m0 = map0, m1 = map1;
+    void *args[] = {&m0, &m1, &buf0, &buf1, &ld, &n, &ctl, &partials, &max_products};
+    if (cudaLaunchCooperativeKernel((const void *)sp2_dense_fp64_loop_kernel<BT>, dim3((unsigned)tiles), dim3(D_THREADS), args,
+                                    loop_smem_bytes(BT), stream) != cudaSuccess)
+        return BML_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? 0 : BML_ERR_CUDA;
+}
+
+// one CTA per tile, all co-resident (one per SM): N <= 1024 on a device with cooperative launch and enough SMs
+bool dense_fp64_loop_available(int64_t N)
+{
+    return dense_fp64_tile(N) != 128 && sk_grid() > 0 && dense_fp64_num_tiles(N) <= sk_grid();
+}
+
+int launch_sp2_dense_fp64_loop(const CUtensorMap &map0, const CUtensorMap &map1, double *buf0, double *buf1, int64_t ld,
+                               int64_t N, Sp2Ctl *ctl, double *partials, int max_products, cudaStream_t stream)
+{
+    switch (dense_fp64_tile(N)) {
+        case 32: return launch_sp2_loop_t<32>(map0, map1, buf0, buf1, ld, N, ctl, partials, max_products, stream);
+        case 64: return launch_sp2_loop_t<64>(map0, map1, buf0, buf1, ld, N, ctl, partials, max_products, stream);
+        default: return 1;
+    }
 }
 
 // Enqueue one product.  buf0/buf1: ping-pong iterates (leading dimension ld, multiple of 16, 128-byte aligned).

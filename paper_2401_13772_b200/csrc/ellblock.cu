@@ -28,6 +28,7 @@ namespace bmlsp2 {
 constexpr int EB_THREADS = 512;
 constexpr int EB_WARPS = EB_THREADS / 32;
 constexpr int EB_MAX_GRID = 1024;
+constexpr int EB_CHUNKS = 8;             // 32-entry chunks of a block row's index list fetched together (kernel 1)
 constexpr int EB_PIPE = 4;               // block pairs whose operand loads are in flight together (kernel 1)
 
 __device__ __forceinline__ int eb_find(const int *__restrict__ list, int n, int key)
@@ -35,6 +36,22 @@ __device__ __forceinline__ int eb_find(const int *__restrict__ list, int n, int 
     int lo = 0, hi = n;
     while (lo < hi) { const int mid = (lo + hi) >> 1; if (list[mid] < key) lo = mid + 1; else hi = mid; }
     return (lo < n && list[lo] == key) ? lo : -1;
+}
+
+// the same search done by a whole warp on a list in GLOBAL memory: every lane tests the slots lane, lane + 32, ... (one
+// round of independent, coalesced loads instead of log2(n) dependent ones); all lanes return the position or -1
+__device__ __forceinline__ int eb_find_warp(const int *__restrict__ list, int n, int key, int lane)
+{
+    int hit = -1;
+    for (int q0 = 0; q0 < n; q0 += 128) {
+        int v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int q = q0 + u * 32 + lane; v[u] = q < n ? __ldg(list + q) : -1; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) if (v[u] == key) hit = q0 + u * 32 + lane;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, hit >= 0);
+    return bal ? __shfl_sync(0xffffffffu, hit, __ffs(bal) - 1) : -1;
 }
 
 // Candidate block columns of block row I: every J (>= jmin) stored in some row K with K stored in row I.  Sets the bits,
@@ -142,9 +159,15 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 const int nJ = min(xn[J], MB);
                 const int32_t *rowJ = xi + (int64_t)J * MB;
                 const double *valJ = xv + (int64_t)J * MB * BB;
-                for (int q0 = 0; q0 < nJ; q0 += 32) {
-                    const int q = q0 + lane;
-                    const int pI = q < nJ ? eb_find(sI, nI, rowJ[q]) : -1;
+                for (int qg = 0; qg < nJ; qg += 32 * EB_CHUNKS) {
+                  int kq[EB_CHUNKS];                       // block columns of row J, EB_CHUNKS x 32 at a time (one round trip)
+#pragma unroll
+                  for (int u = 0; u < EB_CHUNKS; ++u) { const int q = qg + u * 32 + lane; kq[u] = q < nJ ? __ldg(rowJ + q) : -1; }
+#pragma unroll
+                  for (int u = 0; u < EB_CHUNKS; ++u) {
+                    const int q0 = qg + u * 32;
+                    if (q0 >= nJ) break;
+                    const int pI = kq[u] >= 0 ? eb_find(sI, nI, kq[u]) : -1;
                     unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
                     // matches in ascending K (row J is in ascending order), EB_PIPE at a time: the operand blocks of row
                     // J come from L2 and their loads are issued for the whole group before the first DMMA needs them
@@ -195,6 +218,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                             }
                         }
                     }
+                }
                 }
                 double nrm2 = 0.0;
 #pragma unroll
@@ -289,11 +313,11 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                 const double *P = nullptr;
                 bool transposed = false;
                 if (C >= J) {
-                    const int pos = eb_find(ti + (int64_t)J * MB, min(nU, MB), C);
+                    const int pos = eb_find_warp(ti + (int64_t)J * MB, min(nU, MB), C, lane);
                     if (pos >= 0) P = tv + ((int64_t)J * MB + pos) * BB;
                 } else {
                     const int nC = min(tn[C], MB);
-                    const int pos = eb_find(ti + (int64_t)C * MB, nC, J);
+                    const int pos = eb_find_warp(ti + (int64_t)C * MB, nC, J, lane);
                     if (pos >= 0) { P = tv + ((int64_t)C * MB + pos) * BB; transposed = true; }
                 }
                 const int px = eb_find(sX, nX, C);
