@@ -249,7 +249,7 @@ def oracle_cheby_time_to_D(wname: str, H, budget_s: float):
         axpy = (time.perf_counter() - t0) / 2
         ms = (per * (w.k + w.m - 2) + axpy * w.k * w.m) * 1e3
         sample = (f"2 of {w.k + w.m - 2} oracle products and 2 of {w.k * w.m} scaled additions timed at full size, "
-                  "scaled")
+                  "scaled; the oracle's products are numpy matmul (BLAS threads), not plain loops")
     if w.N <= 4000 and budget_s >= 20.0:
         t0 = time.perf_counter()
         och.fermi_exact(H, w.mu, w.beta)
@@ -290,7 +290,8 @@ def oracle_graph_time_to_D(wname: str, H):
     scale = sum((sub.shape[0] / h.shape[0]) ** 3 for sub in subs)
     ms = (t_move + per * (L - 1) * scale) * 1e3
     return ms, (f"halo lists + gathers of all {w.n_parts} parts timed in full ({t_move:.1f} s); 2 of {L - 1} recursion "
-                f"products timed at part size {h.shape[0]}, scaled to all parts"), cores
+                f"products timed at part size {h.shape[0]}, scaled to all parts; products are numpy matmul (BLAS threads), "
+                "not plain loops"), cores
 
 
 def oracle_graph_sp2_time_to_D(wname: str, H, n_products):

@@ -255,6 +255,29 @@ static inline int device_sm_count()
     return sms[dev];
 }
 
+// The same super-block order WITHOUT empty slots, for the persistent kernels that walk a dense list of tile numbers:
+// t in [0, T (T + 1) / 2) -> (I, J), I <= J.  Super-blocks column by column; inside an off-diagonal super-block row by
+// row, inside a diagonal one the triangular order.  At most S (S + 1) / 2 (~20) steps per work item of ~1 ms.
+__host__ __device__ __forceinline__ void tri_sb_decode(int t, int T, int &I, int &J)
+{
+    if (tile_sb_plain(T)) { tri_decode(t, I, J); return; }
+    const int S = (T + TILE_SB - 1) / TILE_SB;
+    for (int bj = 0; bj < S; ++bj) {
+        const int c0 = bj * TILE_SB, nc = (T - c0 < TILE_SB) ? T - c0 : TILE_SB;
+        for (int bi = 0; bi <= bj; ++bi) {
+            const int r0 = bi * TILE_SB, nr = (T - r0 < TILE_SB) ? T - r0 : TILE_SB;
+            const int cnt = (bi == bj) ? nr * (nr + 1) / 2 : nr * nc;
+            if (t < cnt) {
+                if (bi == bj) { int i, j; tri_decode(t, i, j); I = r0 + i; J = c0 + j; }
+                else { I = r0 + t / nc; J = c0 + t % nc; }
+                return;
+            }
+            t -= cnt;
+        }
+    }
+    I = J = T - 1;      // not reached for t < T (T + 1) / 2
+}
+
 // Host-side helpers (api.cu)
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,

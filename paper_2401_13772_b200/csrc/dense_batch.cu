@@ -95,7 +95,7 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
                 batch_next(tb, u, r1, job, w);
                 const CUtensorMap *map = &tb->map[parity][w.job];
                 int I, J;
-                tri_decode(w.tile, I, J);
+                tri_sb_decode(w.tile, (tb->job[w.job].N + 127) / 128, I, J);
                 const bool diag = (I == J);
                 const uint32_t tx = diag ? D_PANEL_BYTES : D_STAGE_BYTES;
                 for (int kt = w.kt0; kt < w.kt1; ++kt, ++slab) {
@@ -126,7 +126,7 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
             const BatchJob &jb = tb->job[w.job];
             const int KT = jb.KT;
             int I, J;
-            tri_decode(w.tile, I, J);
+            tri_sb_decode(w.tile, (jb.N + 127) / 128, I, J);
             const bool diag = (I == J);
             double acc[MI][NI][2];
 #pragma unroll

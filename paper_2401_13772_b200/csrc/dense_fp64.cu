@@ -332,7 +332,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
             SkItem w;
             for (int it = 0; sk_item(it, c, G, tiles, KT, sk_handoff_slabs(128), w); ++it) {
                 int I, J;
-                tri_decode(w.tile, I, J);
+                tri_sb_decode(w.tile, T, I, J);
                 const bool diag = (I == J);
                 const uint32_t tx = diag ? D_PANEL_BYTES : D_STAGE_BYTES;
                 for (int kt = w.kt0; kt < w.kt1; ++kt, ++slab) {
@@ -359,7 +359,7 @@ x2_dense_fp64_sk_kernel(const __grid_constant__ CUtensorMap map0, const __grid_c
         SkItem w;
         for (int it = 0; sk_item(it, c, G, tiles, KT, sk_handoff_slabs(128), w); ++it) {
             int I, J;
-            tri_decode(w.tile, I, J);
+            tri_sb_decode(w.tile, T, I, J);
             const bool diag = (I == J);
             double acc[MI][NI][2];
 #pragma unroll
@@ -591,7 +591,7 @@ int dense_fp64_work_item(int64_t N, int n_ctas, int cta, int it, int32_t out[5])
     SkItem w;
     if (!sk_item(it, cta, n_ctas, tiles, KT, sk_handoff_slabs(128), w)) return 1;
     int I, J;
-    tri_decode(w.tile, I, J);
+    tri_sb_decode(w.tile, T, I, J);
     out[0] = w.tile; out[1] = I; out[2] = J; out[3] = w.kt0; out[4] = w.kt1;
     return 0;
 }

@@ -14,17 +14,25 @@ def test_persistent_fp64_work_list_covers_every_unit_once(N, G):
     tiles = T * (T + 1) // 2
     cover = {}
     per_cta = []
+    where = {}
     for c in range(G):
         items = api.bml_dense_work_items(N, G, c)
         per_cta.append(items)
         n_contrib = 0
         for tile, I, J, k0, k1 in items:
-            assert 0 <= I <= J < T and tile == J * (J + 1) // 2 + I
+            # tile number -> (I, J) is a bijection onto the upper triangle (super-block order above 24 tile rows)
+            assert 0 <= I <= J < T and where.setdefault(tile, (I, J)) == (I, J)
+            if T <= 24:
+                assert tile == J * (J + 1) // 2 + I
             assert 0 <= k0 < k1 <= KT
             cover.setdefault(tile, []).append((k0, k1, c))
             n_contrib += k0 > 0
         assert n_contrib <= 1, "a CTA has one scratch slot: at most one contributed partial per launch"
     assert sorted(cover) == list(range(tiles))
+    assert len(set(where.values())) == tiles
+    if T > 24:      # a wave of consecutive tiles shares few row panels: at most 2 x 12 + a super-block boundary
+        wave = [where[t] for t in range(min(G, tiles))]
+        assert len({i for i, _ in wave} | {j for _, j in wave}) <= 50
     for tile, parts in cover.items():
         parts.sort()
         assert parts[0][0] == 0 and parts[-1][1] == KT
