@@ -21,6 +21,8 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
     "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr", "-fmad=true",
 ]
+# extra nvcc flags for kernel experiments (e.g. BML_NVCC_EXTRA="-DBML_ELL_BUCKET_LOG2=3"); empty in normal builds
+NVCC_FLAGS += os.environ.get("BML_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

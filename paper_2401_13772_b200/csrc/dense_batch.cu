@@ -25,32 +25,67 @@ struct BatchJob {
     const uint8_t *core;     // [N] 1 = core orbital (its diagonal counts in the traces); NULL = every row
     int64_t ld;
     int64_t unit0;           // index of the part's first work unit in the batch's unit list
-    int32_t N, KT, tiles, pad;
+    int32_t N, KT, tiles, tile0;   // tile0: index of the part's first tile in the batch's tile list
 };
 constexpr int BATCH_MAX_JOBS = 256;
 struct alignas(128) BatchTable {
     CUtensorMap map[2][BATCH_MAX_JOBS];      // [buffer][job]: FP64 tensor map of that iterate buffer (box 16 x 128)
     BatchJob job[BATCH_MAX_JOBS];
     int64_t units;
-    int32_t n_jobs, pad;
+    int32_t n_jobs, tiles_total;
 };
 size_t dense_batch_table_bytes() { return sizeof(BatchTable); }
 
 struct BatchItem {
     int job, tile, kt0, kt1;
 };
-// next work item of a range [u, u1): advances u; `job` is a cursor that only moves forward
-__device__ __forceinline__ void batch_next(const BatchTable *__restrict__ tb, int64_t &u, int64_t u1, int &job, BatchItem &w)
+// Work list of CTA c: first W = tiles_total / G WHOLE tiles, dealt in waves (tile w G + c of wave w: the CTAs resident
+// at any time work on ~G consecutive tiles of one part, i.e. on one super-block, and share its row panels in L2 -- with
+// contiguous ranges per CTA every tile pulled both its panels from HBM: 42.5 GB per product at 4 x 5600 against 2 GB
+// algorithmic); then the units of the remaining tiles_total - W G tiles are cut into G equal contiguous ranges
+// (stream-K with unequal KT).  Identical arithmetic in the producer, the consumers and the host-side test hook.
+struct BatchWalk {
+    int wv, W, job;
+    int64_t u, u1;
+};
+__host__ __device__ __forceinline__ void batch_walk_init(BatchWalk &k, const BatchJob *jobs, int n_jobs, int tiles_total,
+                                                         int64_t units, int G, int c, int64_t &tail_unit0)
 {
-    while (u >= tb->job[job].unit0 + (int64_t)tb->job[job].tiles * tb->job[job].KT) ++job;
-    const int KT = tb->job[job].KT;
-    const int64_t rel = u - tb->job[job].unit0;
-    w.job = job;
+    k.W = tiles_total / G;
+    k.wv = 0;
+    k.job = 0;
+    const int t_tail = k.W * G;                       // first tile of the split tail
+    tail_unit0 = units;
+    for (int p = 0; p < n_jobs; ++p)
+        if (t_tail < jobs[p].tile0 + jobs[p].tiles) { tail_unit0 = jobs[p].unit0 + (int64_t)(t_tail - jobs[p].tile0) * jobs[p].KT; break; }
+    const int64_t UT = units - tail_unit0;
+    k.u = tail_unit0 + (int64_t)c * UT / G;
+    k.u1 = tail_unit0 + (int64_t)(c + 1) * UT / G;
+}
+// next item; u_item = first unit of the item (meaningful for tail items); false when the list is exhausted
+__host__ __device__ __forceinline__ bool batch_walk_next(BatchWalk &k, const BatchJob *jobs, int G, int c, BatchItem &w,
+                                                         int64_t &u_item)
+{
+    if (k.wv < k.W) {
+        const int q = k.wv * G + c;
+        ++k.wv;
+        while (q >= jobs[k.job].tile0 + jobs[k.job].tiles) ++k.job;
+        w.job = k.job; w.tile = q - jobs[k.job].tile0; w.kt0 = 0; w.kt1 = jobs[k.job].KT;
+        u_item = jobs[k.job].unit0 + (int64_t)w.tile * w.kt1;
+        return true;
+    }
+    if (k.u >= k.u1) return false;
+    while (k.u >= jobs[k.job].unit0 + (int64_t)jobs[k.job].tiles * jobs[k.job].KT) ++k.job;
+    const int KT = jobs[k.job].KT;
+    const int64_t rel = k.u - jobs[k.job].unit0;
+    u_item = k.u;
+    w.job = k.job;
     w.tile = (int)(rel / KT);
     w.kt0 = (int)(rel - (int64_t)w.tile * KT);
-    const int64_t left = u1 - u;
+    const int64_t left = k.u1 - k.u;
     w.kt1 = (int64_t)(KT - w.kt0) <= left ? KT : w.kt0 + (int)left;
-    u += w.kt1 - w.kt0;
+    k.u += w.kt1 - w.kt0;
+    return true;
 }
 
 __global__ void __launch_bounds__(D_THREADS, 1)
@@ -75,7 +110,6 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
     const int warp = warp_all - D_PRODUCER_WARPS;
     const int G = (int)gridDim.x, c = (int)blockIdx.x;
     const int64_t U = tb->units;
-    const int64_t r0 = (int64_t)c * U / G, r1 = (int64_t)(c + 1) * U / G;      // this CTA's range of work units
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < D_STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], D_CONSUMER_WARPS); }
@@ -89,10 +123,12 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
         // ===================== TMA producer warpgroup (one elected lane works) =====================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(D_REGS_PRODUCER));
         if (warp_all == 0 && lane == 0) {
-            int slab = 0, job = 0;
+            int slab = 0;
             BatchItem w;
-            for (int64_t u = r0; u < r1;) {
-                batch_next(tb, u, r1, job, w);
+            BatchWalk walk;
+            int64_t tail0, u_item;
+            batch_walk_init(walk, tb->job, tb->n_jobs, tb->tiles_total, U, G, c, tail0);
+            while (batch_walk_next(walk, tb->job, G, c, w, u_item)) {
                 const CUtensorMap *map = &tb->map[parity][w.job];
                 int I, J;
                 tri_sb_decode(w.tile, (tb->job[w.job].N + 127) / 128, I, J);
@@ -117,12 +153,14 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
         uint32_t koff[4];
         dmma_koff(lane, koff);
         double s_trp = 0.0, s_e = 0.0, s_x = 0.0, s_trn = 0.0;
-        int slab = 0, job = 0;
+        int slab = 0;
         StageRelease release;
         BatchItem w;
-        for (int64_t u = r0; u < r1;) {
-            const int64_t u_item = u;                // first unit of this item
-            batch_next(tb, u, r1, job, w);
+        BatchWalk walk;
+        int64_t tail0, u_item;
+        batch_walk_init(walk, tb->job, tb->n_jobs, tb->tiles_total, U, G, c, tail0);
+        const int64_t UT = U - tail0;
+        while (batch_walk_next(walk, tb->job, G, c, w, u_item)) {
             const BatchJob &jb = tb->job[w.job];
             const int KT = jb.KT;
             int I, J;
@@ -166,7 +204,7 @@ x2_dense_fp64_batch_kernel(const BatchTable *__restrict__ tb, Sp2Ctl *__restrict
                 // ---------- owner of a split tile: add the following CTAs' partials in ascending CTA order ----------
                 const int64_t tile_end = u_item + KT;        // kt0 == 0: the tile's units are [u_item, u_item + KT)
                 for (int c2 = c + 1; c2 < G; ++c2) {
-                    const int64_t v0 = (int64_t)c2 * U / G, v1 = (int64_t)(c2 + 1) * U / G;
+                    const int64_t v0 = tail0 + (int64_t)c2 * UT / G, v1 = tail0 + (int64_t)(c2 + 1) * UT / G;
                     if (v0 >= tile_end) break;
                     if (v1 <= v0) continue;
                     if (ctid == 0) {
@@ -278,20 +316,23 @@ int dense_batch_fill(void *h_table, int n_jobs, const int32_t *n, double *const 
     BatchTable *tb = (BatchTable *)h_table;
     memset(tb, 0, sizeof(*tb));
     tb->n_jobs = n_jobs;
-    int64_t units = 0;
+    int64_t units = 0, tiles = 0;
     for (int p = 0; p < n_jobs; ++p) {
         if (n[p] < 1 || (ld[p] % 16) != 0 || ld[p] < n[p] || ((uintptr_t)buf0[p] & 127) || ((uintptr_t)buf1[p] & 127))
             return BML_ERR_INVALID;
         BatchJob &jb = tb->job[p];
         const int T = (n[p] + 127) / 128;
         jb.buf0 = buf0[p]; jb.buf1 = buf1[p]; jb.core = core ? core[p] : nullptr; jb.ld = ld[p];
-        jb.N = n[p]; jb.KT = (n[p] + D_BK - 1) / D_BK; jb.tiles = T * (T + 1) / 2; jb.unit0 = units;
+        jb.N = n[p]; jb.KT = (n[p] + D_BK - 1) / D_BK; jb.tiles = T * (T + 1) / 2; jb.unit0 = units; jb.tile0 = (int32_t)tiles;
         units += (int64_t)jb.tiles * jb.KT;
+        tiles += jb.tiles;
+        if (tiles > 0x3fffffff) return BML_ERR_INVALID;
         int r;
         if ((r = make_dense_map128(&tb->map[0][p], buf0[p], n[p], ld[p]))) return r;
         if ((r = make_dense_map128(&tb->map[1][p], buf1[p], n[p], ld[p]))) return r;
     }
     tb->units = units;
+    tb->tiles_total = (int32_t)tiles;
     return 0;
 }
 
@@ -299,28 +340,23 @@ int dense_batch_fill(void *h_table, int n_jobs, const int32_t *n, double *const 
 int dense_batch_work_item(int n_jobs, const int32_t *n, int n_ctas, int cta, int it, int32_t out[5])
 {
     if (n_jobs < 1 || n_jobs > BATCH_MAX_JOBS || n_ctas < 1 || cta < 0 || cta >= n_ctas || it < 0) return BML_ERR_INVALID;
-    int64_t unit0[BATCH_MAX_JOBS + 1];
-    int KT[BATCH_MAX_JOBS], tiles[BATCH_MAX_JOBS];
-    unit0[0] = 0;
+    static thread_local BatchJob jobs[BATCH_MAX_JOBS];
+    int64_t units = 0;
+    int tiles = 0;
     for (int p = 0; p < n_jobs; ++p) {
         if (n[p] < 1) return BML_ERR_INVALID;
         const int T = (n[p] + 127) / 128;
-        KT[p] = (n[p] + D_BK - 1) / D_BK; tiles[p] = T * (T + 1) / 2;
-        unit0[p + 1] = unit0[p] + (int64_t)tiles[p] * KT[p];
+        jobs[p].N = n[p]; jobs[p].KT = (n[p] + D_BK - 1) / D_BK; jobs[p].tiles = T * (T + 1) / 2;
+        jobs[p].unit0 = units; jobs[p].tile0 = tiles;
+        units += (int64_t)jobs[p].tiles * jobs[p].KT;
+        tiles += jobs[p].tiles;
     }
-    const int64_t U = unit0[n_jobs];
-    int64_t u = (int64_t)cta * U / n_ctas;
-    const int64_t u1 = (int64_t)(cta + 1) * U / n_ctas;
-    int job = 0;
-    for (int q = 0; u < u1; ++q) {
-        while (u >= unit0[job + 1]) ++job;
-        const int64_t rel = u - unit0[job];
-        const int tile = (int)(rel / KT[job]), kt0 = (int)(rel - (int64_t)tile * KT[job]);
-        const int64_t left = u1 - u;
-        const int kt1 = (int64_t)(KT[job] - kt0) <= left ? KT[job] : kt0 + (int)left;
-        if (q == it) { out[0] = job; out[1] = tile; out[2] = kt0; out[3] = kt1; out[4] = KT[job]; return 0; }
-        u += kt1 - kt0;
-    }
+    BatchWalk walk;
+    BatchItem w;
+    int64_t tail0, u_item;
+    batch_walk_init(walk, jobs, n_jobs, tiles, units, n_ctas, cta, tail0);
+    for (int q = 0; batch_walk_next(walk, jobs, n_ctas, cta, w, u_item); ++q)
+        if (q == it) { out[0] = w.job; out[1] = w.tile; out[2] = w.kt0; out[3] = w.kt1; out[4] = jobs[w.job].KT; return 0; }
     return 1;
 }
 

@@ -23,34 +23,40 @@ namespace bmlsp2 {
 
 constexpr int E_SLOTS = BML_ELL_ACC_SLOTS;
 constexpr int E_MASK = E_SLOTS - 1;
-constexpr int E_BUCKETS = E_SLOTS / 32;
-constexpr int E_BUCKET_SHIFT = 32 - 7;  // log2(E_BUCKETS) = 7
-static_assert(E_BUCKETS == 128, "bucket hash is written for 4096 slots");
+#ifndef BML_ELL_BUCKET_LOG2
+#define BML_ELL_BUCKET_LOG2 5          // columns per bucket = 32
+#endif
+constexpr int E_BL = BML_ELL_BUCKET_LOG2;
+constexpr int E_BW = 1 << E_BL;                 // bucket width (consecutive columns that stay consecutive slots)
+constexpr int E_BUCKETS = E_SLOTS / E_BW;
+constexpr int E_BUCKET_LOG2 = 12 - E_BL;        // log2(E_BUCKETS) for 4096 slots
+constexpr int E_BUCKET_SHIFT = 32 - E_BUCKET_LOG2;
+static_assert(E_SLOTS == 4096, "bucket hash is written for 4096 slots");
 constexpr int E_EMPTY = -1;
 constexpr int E_GW = 4;               // warps per row group
 constexpr int E_GT = E_GW * 32;       // threads per row group
 constexpr int E_MAX_GROUPS = 4;       // row groups (= rows in flight) per CTA
 constexpr int E_MAX_GRID = 1024;
 
-// bucket and in-bucket rotation from the 32-column block id: the rotation spreads columns that sit at the same
-// position of many blocks (the centre of a stencil) over all 32 positions, while 32 consecutive columns still map
-// to 32 distinct banks
+// bucket and in-bucket rotation from the column-block id: the rotation spreads columns that sit at the same position of
+// many blocks (the centre of a stencil) over all positions, while E_BW consecutive columns still map to E_BW consecutive
+// (rotated) slots of one bucket
 __device__ __forceinline__ int e_hash(int j)
 {
-    const uint32_t h = (uint32_t)(j >> 5) * 2654435761u;
-    return (int)((h >> E_BUCKET_SHIFT) << 5) | (int)((j + (h >> (E_BUCKET_SHIFT - 5))) & 31u);
+    const uint32_t h = (uint32_t)(j >> E_BL) * 2654435761u;
+    return (int)((h >> E_BUCKET_SHIFT) << E_BL) | (int)((j + (h >> (E_BUCKET_SHIFT - E_BL))) & (uint32_t)(E_BW - 1));
 }
 // probe sequence (double hashing on the bucket): same position, `stride` buckets further (stride odd, so all buckets
 // are visited); after a full cycle over the buckets, the next position
 __device__ __forceinline__ int e_stride(int j)
 {
-    const uint32_t h = (uint32_t)(j >> 5) * 2654435761u;
-    return (int)((((h >> 8) & (E_BUCKETS - 1)) | 1u) << 5);
+    const uint32_t h = (uint32_t)(j >> E_BL) * 2654435761u;
+    return (int)((((h >> 8) & (E_BUCKETS - 1)) | 1u) << E_BL);
 }
 __device__ __forceinline__ int e_next(int slot, int tries, int stride)
 {
     slot = (slot + stride) & E_MASK;
-    if ((tries & (E_BUCKETS - 1)) == 0) slot = (slot + 1) & E_MASK;
+    if ((tries & (E_BUCKETS - 1)) == 0) slot = (slot & ~(E_BW - 1)) | ((slot + 1) & (E_BW - 1));
     return slot;
 }
 

@@ -139,25 +139,34 @@ def test_schedule_rejects_bad_k():
 @pytest.mark.parametrize("sizes,G", [([5600, 5600, 5600, 5600], 148), ([896, 896, 896], 148), ([5657, 5810, 300, 1, 129], 148),
                                      ([200], 148), ([1500, 64], 7), ([128] * 40, 148), ([3000, 2000, 1000], 1)])
 def test_batched_work_list_covers_every_unit_of_every_part_once(sizes, G):
-    """The batched symmetric-square kernel of the graph-based SP2 solver (dense_batch.cu): pure stream-K over the units
-    (part, upper-triangle tile, 16-column k-slab) of parts of UNEQUAL sizes.  Every unit exactly once; a tile cut by a
-    range boundary has one owner (the piece starting at k-slab 0) followed by contributors on the next CTAs; a CTA
-    contributes to at most one tile and that piece is the FIRST item of its range (so hand-offs cannot cycle)."""
+    """The batched symmetric-square kernel of the graph-based SP2 solver (dense_batch.cu) over parts of UNEQUAL sizes:
+    every CTA first takes W = tiles // G whole tiles dealt in waves (tile w G + c: concurrently running CTAs sit on
+    consecutive tiles and share row panels in L2), then the units (16-column k-slabs) of the remaining tiles are cut
+    into G equal contiguous ranges.  Every unit exactly once; a cut tile has one owner (the piece starting at k-slab 0)
+    followed by contributors on the next CTAs; a CTA contributes to at most one tile and that piece is the FIRST item of
+    its tail range (so hand-offs cannot cycle); only the last item of a range may be cut short."""
+    tiles_of = [((n + 127) // 128) * ((n + 127) // 128 + 1) // 2 for n in sizes]
+    W = sum(tiles_of) // G
     cover = {}
-    units = []
+    tail_units = []
     for c in range(G):
         items = api.bml_dense_batch_work_items(sizes, G, c)
-        units.append(sum(k1 - k0 for _, _, k0, k1, _ in items))
+        assert len(items) >= W
+        tail_units.append(sum(k1 - k0 for _, _, k0, k1, _ in items[W:]))
+        flat0 = None
         for pos, (job, tile, k0, k1, KT) in enumerate(items):
             T = (sizes[job] + 127) // 128
             assert 0 <= job < len(sizes) and 0 <= tile < T * (T + 1) // 2 and KT == (sizes[job] + 15) // 16
             assert 0 <= k0 < k1 <= KT
+            if pos < W:
+                assert (k0, k1) == (0, KT)
+                assert sum(tiles_of[:job]) + tile == pos * G + c, "wave w deals tile w G + c to CTA c"
             if k0 > 0:
-                assert pos == 0, "a contributed piece must come first in the CTA's range"
+                assert pos == W, "a contributed piece must come first in the CTA's tail range"
             if k1 < KT:
                 assert pos == len(items) - 1, "only the last item of a range may be cut short"
             cover.setdefault((job, tile), []).append((k0, k1, c))
-    want = {(j, t) for j, n in enumerate(sizes) for t in range(((n + 127) // 128) * ((n + 127) // 128 + 1) // 2)}
+    want = {(j, t) for j, n in enumerate(sizes) for t in range(tiles_of[j])}
     assert set(cover) == want
     for (job, tile), parts in cover.items():
         KT = (sizes[job] + 15) // 16
@@ -165,7 +174,7 @@ def test_batched_work_list_covers_every_unit_of_every_part_once(sizes, G):
         assert parts[0][0] == 0 and parts[-1][1] == KT
         for (a0, a1, ca), (b0, b1, cb) in zip(parts, parts[1:]):
             assert a1 == b0 and cb > ca
-        # contributors are consecutive CTAs, up to CTAs whose range is empty (tiny batches on many CTAs)
+        # contributors are consecutive CTAs, up to CTAs whose tail range is empty (tiny batches on many CTAs)
         ctas = [p[2] for p in parts]
-        assert all(units[c] == 0 for c in range(ctas[0], ctas[-1] + 1) if c not in ctas)
-    assert max(units) - min(units) <= 1
+        assert all(tail_units[c] == 0 for c in range(ctas[0], ctas[-1] + 1) if c not in ctas)
+    assert max(tail_units) - min(tail_units) <= 1
