@@ -107,8 +107,8 @@ template <int BS>
 __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                          const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
-                         int NB, int MB, double tau, int cand_cap, Sp2Ctl *__restrict__ ctl, double *__restrict__ tv,
-                         int32_t *__restrict__ ti, int32_t *__restrict__ tn)
+                         int NB, int MB, double tau, int cand_cap, int use_map, Sp2Ctl *__restrict__ ctl,
+                         double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn)
 {
     constexpr int MT = (BS + 7) / 8, KS = (BS + 3) / 4, BB = BS * BS;
     if (ctl->done) return;
@@ -123,16 +123,26 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     int *sI = (int *)(sA + (size_t)MB * BB);                         // [MB] their block columns
     int *cand = sI + MB;                                             // [cand_cap]
     unsigned *bitmap = (unsigned *)(cand + cand_cap);                // [NBW]
-    __shared__ int s_scan[EB_WARPS], s_keep[EB_WARPS];
+    // direct map block column -> 1 + position in row I (0 = absent), when NB is small enough to afford 2 NB bytes: one
+    // shared-memory load per entry of row J instead of a binary search in row I's list
+    unsigned short *spos = use_map ? (unsigned short *)(bitmap + NBW) : nullptr;
+    __shared__ int s_scan[EB_WARPS];
+    __shared__ int s_ticket, s_commit, s_kept;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     for (int w = tid; w < NBW; w += EB_THREADS) bitmap[w] = 0u;
+    if (use_map) for (int w = tid; w < NB; w += EB_THREADS) spos[w] = 0;
 
     for (int I = blockIdx.x; I < NB; I += gridDim.x) {
         const int nI = min(xn[I], MB);
         __syncthreads();
-        for (int p = tid; p < nI; p += EB_THREADS) sI[p] = xi[(int64_t)I * MB + p];
+        for (int p = tid; p < nI; p += EB_THREADS) {
+            const int K = xi[(int64_t)I * MB + p];
+            sI[p] = K;
+            if (use_map) spos[K] = (unsigned short)(p + 1);
+        }
+        if (tid == 0) { s_ticket = 0; s_commit = 0; s_kept = 0; }
         {
             const double2 *src = (const double2 *)(xv + (int64_t)I * MB * BB);
             double2 *dst = (double2 *)sA;
@@ -144,9 +154,15 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
         // more candidate blocks (before thresholding) than the list holds: the capacity failure -6, like the scalar
         // path's accumulator table
         if (ncand_all > cand_cap && tid == 0) atomicMin(&ctl->acc_row, I);
-        int kept_total = 0;
-        for (int c0 = 0; c0 < ncand; c0 += EB_WARPS) {
-            const int c = c0 + warp;
+        // Candidates are handed out by a ticket counter (a warp that drew a candidate with few matches takes the next one
+        // instead of waiting at a batch barrier) and COMMITTED in ticket order: after its chain a warp waits until every
+        // earlier candidate has committed, takes the next output position if its block is kept, and passes the turn on --
+        // so the kept blocks still land in ascending block-column order.
+        while (true) {
+            int c = 0;
+            if (lane == 0) c = atomicAdd(&s_ticket, 1);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c >= ncand) break;
             bool keep = false;
             double acc[MT][MT][2];
 #pragma unroll
@@ -154,7 +170,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
 #pragma unroll
                 for (int b = 0; b < MT; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
             int J = -1;
-            if (c < ncand) {
+            {
                 J = cand[c];
                 const int nJ = min(xn[J], MB);
                 const int32_t *rowJ = xi + (int64_t)J * MB;
@@ -167,7 +183,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                   for (int u = 0; u < EB_CHUNKS; ++u) {
                     const int q0 = qg + u * 32;
                     if (q0 >= nJ) break;
-                    const int pI = kq[u] >= 0 ? eb_find(sI, nI, kq[u]) : -1;
+                    const int pI = kq[u] < 0 ? -1 : (use_map ? (int)spos[kq[u]] - 1 : eb_find(sI, nI, kq[u]));
                     unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
                     // matches in ascending K (row J is in ascending order), EB_PIPE at a time: the operand blocks of row
                     // J come from L2 and their loads are issued for the whole group before the first DMMA needs them
@@ -232,11 +248,16 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 nrm2 = warp_sum(nrm2);
                 keep = sqrt(nrm2) >= tau || J == I;
             }
-            if (lane == 0) s_keep[warp] = keep ? 1 : 0;
-            __syncthreads();
-            int pos = kept_total, total = 0;
-#pragma unroll
-            for (int w2 = 0; w2 < EB_WARPS; ++w2) { const int k = s_keep[w2]; if (w2 < warp) pos += k; total += k; }
+            // in-order commit
+            int pos = 0;
+            if (lane == 0) {
+                while (*(volatile int *)&s_commit != c) { }
+                pos = *(volatile int *)&s_kept;
+                if (keep) *(volatile int *)&s_kept = pos + 1;
+                __threadfence_block();
+                *(volatile int *)&s_commit = c + 1;
+            }
+            pos = __shfl_sync(0xffffffffu, pos, 0);
             if (keep && pos < MB) {
                 double *out = tv + ((int64_t)I * MB + pos) * BB;
 #pragma unroll
@@ -249,9 +270,10 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                     }
                 if (lane == 0) ti[(int64_t)I * MB + pos] = J;
             }
-            kept_total += total;
-            __syncthreads();
         }
+        __syncthreads();
+        if (use_map) for (int p = tid; p < nI; p += EB_THREADS) spos[sI[p]] = 0;
+        const int kept_total = s_kept;
         if (tid == 0) tn[I] = kept_total;      // may exceed MB: kernel 2 reports the overflow
     }
 }
@@ -605,7 +627,8 @@ size_t ellblock_rowstats_bytes() { return (size_t)EB_MAX_GRID * 4 * sizeof(doubl
 bool ellblock_shape_ok(int64_t NB, int MB, int bs)
 {
     if (!(bs == 4 || bs == 8 || bs == 16) || NB < 1 || NB > (1 << 19) || MB < 1) return false;
-    const size_t smem1 = (size_t)MB * bs * bs * 8 + (size_t)MB * 4 + (size_t)eb_cand_cap(MB) * 4 + (size_t)((NB + 31) / 32) * 4;
+    const size_t smem1 = (size_t)MB * bs * bs * 8 + (size_t)MB * 4 + (size_t)eb_cand_cap(MB) * 4 + (size_t)((NB + 31) / 32) * 4 +
+                         (NB <= 32768 ? (size_t)NB * 2 + 16 : 0);
     return smem1 <= 227 * 1024 - 2048;
 }
 
@@ -622,7 +645,8 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     int32_t *tn = (int32_t *)p;
     const int cap = eb_cand_cap(MB);
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
-    const size_t smem1 = (size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw;
+    const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
+    const size_t smem1 = (size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
     const size_t smem2 = (size_t)MB * 4 + (size_t)cap * 4 + nbw;
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
     if (ensure_smem_attr(x2_ellblock_upper_kernel<BS>, smem1, a1, 48 * 1024)) return BML_ERR_CUDA;
@@ -631,8 +655,8 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int64_t per_sm1 = (int64_t)((227 * 1024) / (smem1 + 1024)) > 0 ? (int64_t)((227 * 1024) / (smem1 + 1024)) : 1;
     const int64_t res1 = per_sm1 * EB_THREADS > 2048 ? 2048 / EB_THREADS : per_sm1;
     if (grid1 > sms * res1) grid1 = sms * res1;
-    x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, ctl,
-                                                                          tv, ti, tn);
+    x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
+                                                                          ctl, tv, ti, tn);
     EB_CHECK();
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
