@@ -54,7 +54,7 @@ BML_API int bml_sp2_ellblock(const bml_ellblock_t *H, const bml_sp2_params_t *p,
 
 /*
  * One fused product on a caller-supplied iterate (block rows in ascending order, X symmetric as in E3), for per-kernel
- * parity tests and timing: Xnext <- branch ? thr(2X - thr(X X)) : thr(X X).  d_sums: DEVICE double[4] <-
+ * parity tests and timing: Xnext <- branch ? thr(2X - thr(X X)) : thr(X X) (slots beyond nnz[I] are left untouched).  d_sums: DEVICE double[4] <-
  * { tr thr(X X), ||thr(X X) - X||_F^2 over the union block pattern, ||X||_F^2, tr Xnext }; d_info: DEVICE int32[4] <-
  * { lowest block row with more than MB kept blocks or INT32_MAX, INT32_MAX, max kept blocks per block row, that of
  * thr(X X) }.  Asynchronous.  Return 0, -1, -4.

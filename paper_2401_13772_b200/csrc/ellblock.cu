@@ -285,7 +285,7 @@ template <int BS>
 __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__restrict__ n0,
                             double *__restrict__ v1, int32_t *__restrict__ i1, int32_t *__restrict__ n1, int NB, int MB,
-                            double tau, int cand_cap, Sp2Ctl *__restrict__ ctl, double *__restrict__ partials,
+                            double tau, int cand_cap, int use_map, Sp2Ctl *__restrict__ ctl, double *__restrict__ partials,
                             const double *__restrict__ tv, const int32_t *__restrict__ ti, const int32_t *__restrict__ tn)
 {
     constexpr int BB = BS * BS, EPL = (BB + 31) / 32;        // elements of a block per lane
@@ -304,11 +304,13 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
     int *sX = (int *)smem;                                           // [MB] block columns of row J of X
     int *cand = sX + MB;                                             // [cand_cap]
     unsigned *bitmap = (unsigned *)(cand + cand_cap);                // [NBW]
+    unsigned short *spos = use_map ? (unsigned short *)(bitmap + NBW) : nullptr;   // block column -> 1 + position in row J of X
     __shared__ int s_scan[EB_WARPS], s_keep[EB_WARPS], s_pcnt[EB_WARPS], s_last;
     __shared__ double s_part[EB_WARPS][4];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int w = tid; w < NBW; w += EB_THREADS) bitmap[w] = 0u;
+    if (use_map) for (int w = tid; w < NB; w += EB_THREADS) spos[w] = 0;
     double w_trp = 0.0, w_e = 0.0, w_x = 0.0, w_trn = 0.0;
     int w_ovf_p = INT32_MAX, w_ovf_u = INT32_MAX, w_max_p = 0, w_max_u = 0;
 
@@ -316,7 +318,11 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
         const int nX = min(xn[J], MB);
         const int nU = tn[J];                                        // own upper blocks (may read MB + 1 = overflow)
         __syncthreads();
-        for (int p = tid; p < nX; p += EB_THREADS) sX[p] = xi[(int64_t)J * MB + p];
+        for (int p = tid; p < nX; p += EB_THREADS) {
+            const int K = xi[(int64_t)J * MB + p];
+            sX[p] = K;
+            if (use_map) spos[K] = (unsigned short)(p + 1);
+        }
         __syncthreads();
         const int ncand_all = eb_candidates(xi, xn, MB, NB, sX, nX, 0, bitmap, cand, cand_cap, s_scan);
         const int ncand = min(ncand_all, cand_cap);
@@ -342,7 +348,7 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                     const int pos = eb_find_warp(ti + (int64_t)C * MB, nC, J, lane);
                     if (pos >= 0) { P = tv + ((int64_t)C * MB + pos) * BB; transposed = true; }
                 }
-                const int px = eb_find(sX, nX, C);
+                const int px = use_map ? (int)spos[C] - 1 : eb_find(sX, nX, C);
                 const double *X = px >= 0 ? xv + ((int64_t)J * MB + px) * BB : nullptr;
                 haveP = P != nullptr;
                 double r_e = 0.0, r_x = 0.0, r_trp = 0.0, r_trn = 0.0, nrm2 = 0.0;
@@ -400,14 +406,8 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                 else on[J] = kept_total;
             }
         }
-        // unused slots of the written row: (0, zero block), as the format's contract says
-        if (!ovf_p && kept_total <= MB) {
-            for (int q = kept_total + warp; q < MB; q += EB_WARPS) {
-                double *out = ov + ((int64_t)J * MB + q) * BB;
-                for (int el = lane; el < BB; el += 32) out[el] = 0.0;
-                if (lane == 0) oi[(int64_t)J * MB + q] = 0;
-            }
-        }
+        // slots beyond the count are not written here (every reader goes by nnz); the copy-out zeroes them in D
+        if (use_map) { __syncthreads(); for (int p = tid; p < nX; p += EB_THREADS) spos[sX[p]] = 0; }
     }
     // ---------------- per-CTA partials (fixed order), flags, last-CTA finaliser ----------------
     w_trp = warp_sum(w_trp); w_e = warp_sum(w_e); w_x = warp_sum(w_x); w_trn = warp_sum(w_trn);
@@ -603,8 +603,12 @@ copy_out_ellblock_kernel(const double *__restrict__ v0, const int32_t *__restric
     const int32_t *__restrict__ sn = parity ? n1 : n0;
     const int64_t nv = NB * MB * (int64_t)bb, nm = NB * (int64_t)MB;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (int64_t e = t0; e < nv; e += stride) dv[e] = sv[e];
-    for (int64_t e = t0; e < nm; e += stride) di[e] = si[e];
+    // slots beyond nnz hold stale data in the iterates: D gets (0, zero block) there, as the format's contract says
+    for (int64_t e = t0; e < nv; e += stride) {
+        const int64_t slot = e / bb;
+        dv[e] = (slot % MB) < sn[slot / MB] ? sv[e] : 0.0;
+    }
+    for (int64_t e = t0; e < nm; e += stride) di[e] = (e % MB) < sn[e / MB] ? si[e] : 0;
     for (int64_t e = t0; e < NB; e += stride) dn[e] = sn[e];
 }
 
@@ -647,7 +651,7 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
     const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
     const size_t smem1 = (size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
-    const size_t smem2 = (size_t)MB * 4 + (size_t)cap * 4 + nbw;
+    const size_t smem2 = (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
     if (ensure_smem_attr(x2_ellblock_upper_kernel<BS>, smem1, a1, 48 * 1024)) return BML_ERR_CUDA;
     if (ensure_smem_attr(x2_ellblock_assemble_kernel<BS>, smem2, a2, 48 * 1024)) return BML_ERR_CUDA;
@@ -661,8 +665,8 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
     if (grid2 > EB_MAX_GRID) grid2 = EB_MAX_GRID;
-    x2_ellblock_assemble_kernel<BS><<<(unsigned)grid2, EB_THREADS, smem2, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, ctl,
-                                                                             partials, tv, ti, tn);
+    x2_ellblock_assemble_kernel<BS><<<(unsigned)grid2, EB_THREADS, smem2, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
+                                                                             ctl, partials, tv, ti, tn);
     EB_CHECK();
     return 0;
 }
