@@ -84,7 +84,7 @@ typedef struct {
     double   idem_tol;      /* tolerance on e_m = ||X_m^2 - X_m||_F / ||X_m||_F                                 */
     double   drop_tol;      /* tau: keep |v| >= tau or the diagonal (ellpack only; 0 keeps everything)          */
     int32_t  precision;     /* dense only: 0 = FP64 DMMA products; 1, 2 = mixed precision: tcgen05 products of 16-bit
-                               planes of X with FP32 TMEM accumulation promoted to FP64 every 128 columns of K, FP64
+                               planes of X with FP32 TMEM accumulation promoted to FP64 every 512 columns of K, FP64
                                traces, norms and updates.  1 = two FP16 planes, X = Xh + 2^-11 Xl (3 cross terms);
                                2 = three BF16 planes, X = Xh + Xm + Xl (6 cross terms)                            */
     uint32_t flags;         /* BML_SP2_FLAG_* */

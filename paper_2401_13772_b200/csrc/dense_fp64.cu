@@ -249,7 +249,8 @@ sp2_dense_fp64_loop_kernel(const __grid_constant__ CUtensorMap map0, const __gri
             for (int w = 0; w < D_CONSUMER_WARPS; ++w) v += s_red[w][threadIdx.x];
             __stcg(&part[(size_t)blockIdx.x * 4 + threadIdx.x], v);
         }
-        __threadfence();
+        // no __threadfence() here: grid.sync() orders every thread's earlier global writes (X', the partial sums) before
+        // every thread's later reads; a fence per thread on top of it cost 3.9 us per product (measured, N = 256)
         grid.sync();
         // every warp adds the partials in the same fixed order: all threads of all CTAs hold identical sums
         double sm[4] = {0.0, 0.0, 0.0, 0.0};
@@ -259,7 +260,9 @@ sp2_dense_fp64_loop_kernel(const __grid_constant__ CUtensorMap map0, const __gri
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) sm[q] = warp_sum(sm[q]);
-        if (blockIdx.x == 0 && threadIdx.x == 0) sp2_finalise(ctl, sm);       // the record: same rules, same numbers
+        // the record (same rules, same numbers), written by a warp that has no role in the next product's pipeline
+        // (thread 0 is the TMA producer: the record on its path delayed CTA 0, and with it every grid barrier)
+        if (blockIdx.x == 0 && warp_all == D_PRODUCER_WARPS - 1 && lane == 0) sp2_finalise(ctl, sm);
         if (!loop_mode) { done = true; break; }
         // the decision of sp2_finalise (common.cuh), taken locally
         const double e = sqrt(sm[1]) / sqrt(sm[2]);
