@@ -43,7 +43,10 @@ EXPORTS = [
     # include/bml_ellblock.h
     "bml_gershgorin_ellblock_workspace_bytes", "bml_gershgorin_ellblock", "bml_trace_ellblock",
     "bml_sp2_ellblock_workspace_bytes", "bml_sp2_ellblock", "bml_x2_ellblock_workspace_bytes", "bml_x2_ellblock",
+    # include/bml_no_alloc.h
+    "bml_gershgorin_static", "bml_no_alloc_status_string",
 ]
+GERSHGORIN_STATIC_MAX_N = 65536
 GRAPH_MAX_PARTS = 256
 CHEB_MAX_K, CHEB_MAX_M, CHEB_MAX_TERMS, SYMM_MAX_JOBS = 32, 32, 1024, 16
 
@@ -199,6 +202,10 @@ def load(build_if_missing: bool = True):
     L.bml_gershgorin.argtypes = [MP, vp, vp, sz, vp]
     L.bml_trace.restype = ctypes.c_int
     L.bml_trace.argtypes = [MP, vp, vp]
+    L.bml_gershgorin_static.restype = ctypes.c_int
+    L.bml_gershgorin_static.argtypes = [MP, vp, vp]
+    L.bml_no_alloc_status_string.restype = ctypes.c_char_p
+    L.bml_no_alloc_status_string.argtypes = [ctypes.c_int]
     L.bml_lanczos_bounds_workspace_bytes.restype = sz
     L.bml_lanczos_bounds_workspace_bytes.argtypes = [i64]
     L.bml_lanczos_bounds.restype = ctypes.c_int
@@ -371,6 +378,20 @@ def bml_gershgorin(H, out: torch.Tensor | None = None) -> torch.Tensor:
     rc = L.bml_gershgorin(ctypes.byref(desc), out.data_ptr(), ws.data_ptr(), nbytes, _stream())
     if rc != 0:
         raise RuntimeError(f"bml_gershgorin: {bml_status_string(rc)}")
+    return out
+
+
+def bml_gershgorin_static(H, out: torch.Tensor) -> torch.Tensor:
+    """include/bml_no_alloc.h: bml_gershgorin with the library's static scratch; allocates nothing, so `out` (CUDA float64
+    [2]) is the caller's.  N <= GERSHGORIN_STATIC_MAX_N; calls that overlap on the GPU race on the scratch."""
+    L = load()
+    desc = dense_desc(H) if isinstance(H, torch.Tensor) else ellpack_desc(*H)
+    _require_cuda(out, torch.float64, "bounds")
+    if out.numel() < 2 or not out.is_contiguous():
+        raise ValueError("bounds: contiguous float64[2] expected")
+    rc = L.bml_gershgorin_static(ctypes.byref(desc), out.data_ptr(), _stream())
+    if rc != 0:
+        raise RuntimeError(f"bml_gershgorin_static: {L.bml_no_alloc_status_string(rc).decode()}")
     return out
 
 

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 LIB_PATH = os.path.join(_HERE, "libbmlsp2.so")
-SOURCES = ["api.cu", "dense_fp64.cu", "dense_mixed.cu", "ellpack.cu", "reductions.cu", "probe.cu", "symm_ab.cu",
+SOURCES = ["api.cu", "dense_fp64.cu", "dense_mixed.cu", "ellpack.cu", "reductions.cu", "gershgorin_static.cu", "probe.cu", "symm_ab.cu",
            "chebyshev.cu", "graph.cu", "bounds.cu", "dense_batch.cu", "ellblock.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
