@@ -14,7 +14,8 @@
 // 8 x 8 blocks per block row) does not fit shared memory.  Two kernels per product:
 //   kernel 1 (upper): block row I per CTA; the candidate block columns J >= I (those reachable through some K) are
 //     enumerated in ascending order from a bitmap over the block columns; a warp intersects the sorted block lists of
-//     rows I and J, chains the DMMAs, takes the block norm, and the kept blocks are written in ascending J.
+//     rows I and J, chains the DMMAs, takes the block norm, and the kept blocks are written in arrival order (kernel 2
+//     looks them up with a whole-warp scan; every iterate it writes is in ascending order again).
 //   kernel 2 (assemble): block row J per CTA; for every candidate column C (both triangles) the block of thr(X X) is
 //     read from its own upper list (C >= J) or transposed from row C's upper list (C < J); update against X on the
 //     union of the patterns, block threshold, norms, traces, ascending write-back, last-CTA finaliser.
@@ -29,7 +30,7 @@ constexpr int EB_THREADS = 512;
 constexpr int EB_WARPS = EB_THREADS / 32;
 constexpr int EB_MAX_GRID = 1024;
 constexpr int EB_CHUNKS = 8;             // 32-entry chunks of a block row's index list fetched together (kernel 1)
-constexpr int EB_PIPE = 4;               // block pairs whose operand loads are in flight together (kernel 1)
+constexpr int EB_PIPE_MAX = 8;               // block pairs whose operand loads are in flight together (kernel 1)
 
 __device__ __forceinline__ int eb_find(const int *__restrict__ list, int n, int key)
 {
@@ -107,10 +108,11 @@ template <int BS>
 __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                          const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
-                         int NB, int MB, double tau, int cand_cap, int use_map, Sp2Ctl *__restrict__ ctl,
+                         int NB, int MB, double tau, int cand_cap, int use_map, int match_off, Sp2Ctl *__restrict__ ctl,
                          double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn)
 {
     constexpr int MT = (BS + 7) / 8, KS = (BS + 3) / 4, BB = BS * BS;
+    constexpr int EB_PIPE = BS == 16 ? 4 : EB_PIPE_MAX;        // bs = 16: 16 operand registers per block pair
     if (ctl->done) return;
     const int parity = ctl->parity;
     const double *__restrict__ xv = parity ? v1 : v0;
@@ -126,8 +128,10 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     // direct map block column -> 1 + position in row I (0 = absent), when NB is small enough to afford 2 NB bytes: one
     // shared-memory load per entry of row J instead of a binary search in row I's list
     unsigned short *spos = use_map ? (unsigned short *)(bitmap + NBW) : nullptr;
+    // per warp: the matches of the candidate in hand, [MB] entries (after the map, 4-byte aligned: NB * 2 + 16 bytes)
+    unsigned *mlist = (unsigned *)(smem + match_off) + (size_t)(threadIdx.x >> 5) * MB;
     __shared__ int s_scan[EB_WARPS];
-    __shared__ int s_ticket, s_commit, s_kept;
+    __shared__ int s_ticket, s_kept;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
@@ -142,7 +146,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
             sI[p] = K;
             if (use_map) spos[K] = (unsigned short)(p + 1);
         }
-        if (tid == 0) { s_ticket = 0; s_commit = 0; s_kept = 0; }
+        if (tid == 0) { s_ticket = 0; s_kept = 0; }
         {
             const double2 *src = (const double2 *)(xv + (int64_t)I * MB * BB);
             double2 *dst = (double2 *)sA;
@@ -154,10 +158,8 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
         // more candidate blocks (before thresholding) than the list holds: the capacity failure -6, like the scalar
         // path's accumulator table
         if (ncand_all > cand_cap && tid == 0) atomicMin(&ctl->acc_row, I);
-        // Candidates are handed out by a ticket counter (a warp that drew a candidate with few matches takes the next one
-        // instead of waiting at a batch barrier) and COMMITTED in ticket order: after its chain a warp waits until every
-        // earlier candidate has committed, takes the next output position if its block is kept, and passes the turn on --
-        // so the kept blocks still land in ascending block-column order.
+        // Candidates are handed out by a ticket counter: a warp that drew a candidate with few matches takes the next
+        // one instead of waiting at a batch barrier.
         while (true) {
             int c = 0;
             if (lane == 0) c = atomicAdd(&s_ticket, 1);
@@ -175,67 +177,69 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 const int nJ = min(xn[J], MB);
                 const int32_t *rowJ = xi + (int64_t)J * MB;
                 const double *valJ = xv + (int64_t)J * MB * BB;
+                // (1) intersection of the block lists of rows I and J, written to the warp's match list in ascending K
+                // (row J is in ascending order): entry = (position in row I << 16) | position in row J
+                int nmatch = 0;
                 for (int qg = 0; qg < nJ; qg += 32 * EB_CHUNKS) {
-                  int kq[EB_CHUNKS];                       // block columns of row J, EB_CHUNKS x 32 at a time (one round trip)
+                    int kq[EB_CHUNKS];                     // block columns of row J, EB_CHUNKS x 32 at a time (one round trip)
 #pragma unroll
-                  for (int u = 0; u < EB_CHUNKS; ++u) { const int q = qg + u * 32 + lane; kq[u] = q < nJ ? __ldg(rowJ + q) : -1; }
+                    for (int u = 0; u < EB_CHUNKS; ++u) { const int q = qg + u * 32 + lane; kq[u] = q < nJ ? __ldg(rowJ + q) : -1; }
 #pragma unroll
-                  for (int u = 0; u < EB_CHUNKS; ++u) {
-                    const int q0 = qg + u * 32;
-                    if (q0 >= nJ) break;
-                    const int pI = kq[u] < 0 ? -1 : (use_map ? (int)spos[kq[u]] - 1 : eb_find(sI, nI, kq[u]));
-                    unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
-                    // matches in ascending K (row J is in ascending order), EB_PIPE at a time: the operand blocks of row
-                    // J come from L2 and their loads are issued for the whole group before the first DMMA needs them
-                    // (one match at a time left every warp waiting a full L2 round trip per block pair)
-                    while (bal) {
-                        int pA[EB_PIPE];
-                        const double *Bp[EB_PIPE];
-                        double bq[EB_PIPE][KS][MT];
-                        int nm = 0;
+                    for (int u = 0; u < EB_CHUNKS; ++u) {
+                        const int q0 = qg + u * 32;
+                        if (q0 >= nJ) break;
+                        const int pI = kq[u] < 0 ? -1 : (use_map ? (int)spos[kq[u]] - 1 : eb_find(sI, nI, kq[u]));
+                        const unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
+                        if (pI >= 0) mlist[nmatch + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)pI << 16) | (unsigned)(q0 + lane);
+                        nmatch += __popc(bal);
+                    }
+                }
+                __syncwarp();
+                // (2) the block products, EB_PIPE at a time: the operand blocks of row J come from L2 and the loads of a
+                // whole group are issued before the first DMMA needs them (one match at a time left every warp waiting
+                // a full L2 round trip per block pair; groups cut at the 32-entry chunks of the list held ~4 in flight)
+                for (int m0 = 0; m0 < nmatch; m0 += EB_PIPE) {
+                    const int nm = min(EB_PIPE, nmatch - m0);
+                    int pA[EB_PIPE];
+                    const double *Bp[EB_PIPE];
+                    double bq[EB_PIPE][KS][MT];
 #pragma unroll
-                        for (int u = 0; u < EB_PIPE; ++u) {
-                            pA[u] = -1; Bp[u] = valJ;
-                            if (bal) {
-                                const int src = __ffs(bal) - 1;
-                                bal &= bal - 1;
-                                pA[u] = __shfl_sync(0xffffffffu, pI, src);
-                                Bp[u] = valJ + (size_t)(q0 + src) * BB;
-                                nm = u + 1;
+                    for (int u = 0; u < EB_PIPE; ++u) {
+                        const unsigned e = u < nm ? mlist[m0 + u] : 0u;           // broadcast
+                        pA[u] = (int)(e >> 16);
+                        Bp[u] = valJ + (size_t)(e & 0xffffu) * BB;
+                    }
+#pragma unroll
+                    for (int u = 0; u < EB_PIPE; ++u)
+#pragma unroll
+                        for (int s = 0; s < KS; ++s)
+#pragma unroll
+                            for (int m = 0; m < MT; ++m) {
+                                const int r = m * 8 + g, col = 4 * s + t;
+                                bq[u][s][m] = (u < nm && r < BS && col < BS) ? __ldg(Bp[u] + r * BS + col) : 0.0;
                             }
-                        }
 #pragma unroll
-                        for (int u = 0; u < EB_PIPE; ++u)
+                    for (int u = 0; u < EB_PIPE; ++u) {
+                        if (u < nm) {                      // warp-uniform
+                            const double *A = sA + (size_t)pA[u] * BB;
 #pragma unroll
-                            for (int s = 0; s < KS; ++s)
+                            for (int s = 0; s < KS; ++s) {
+                                double a[MT];
+                                const int col = 4 * s + t;
 #pragma unroll
                                 for (int m = 0; m < MT; ++m) {
-                                    const int r = m * 8 + g, col = 4 * s + t;
-                                    bq[u][s][m] = (u < nm && r < BS && col < BS) ? __ldg(Bp[u] + r * BS + col) : 0.0;
+                                    const int r = m * 8 + g;
+                                    a[m] = (r < BS && col < BS) ? A[r * BS + col] : 0.0;
                                 }
 #pragma unroll
-                        for (int u = 0; u < EB_PIPE; ++u) {
-                            if (u < nm) {                  // warp-uniform
-                                const double *A = sA + (size_t)pA[u] * BB;
+                                for (int m = 0; m < MT; ++m)
 #pragma unroll
-                                for (int s = 0; s < KS; ++s) {
-                                    double a[MT];
-                                    const int col = 4 * s + t;
-#pragma unroll
-                                    for (int m = 0; m < MT; ++m) {
-                                        const int r = m * 8 + g;
-                                        a[m] = (r < BS && col < BS) ? A[r * BS + col] : 0.0;
-                                    }
-#pragma unroll
-                                    for (int m = 0; m < MT; ++m)
-#pragma unroll
-                                        for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], bq[u][s][n]);
-                                }
+                                    for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], bq[u][s][n]);
                             }
                         }
                     }
                 }
-                }
+                __syncwarp();                              // the list is rewritten for the next candidate
                 double nrm2 = 0.0;
 #pragma unroll
                 for (int m = 0; m < MT; ++m)
@@ -248,15 +252,11 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 nrm2 = warp_sum(nrm2);
                 keep = sqrt(nrm2) >= tau || J == I;
             }
-            // in-order commit
+            // a kept block takes the next free slot of the row: the upper list is in ARRIVAL order (kernel 2 finds blocks
+            // in it with a whole-warp scan, which needs no order; an in-order commit cost 23% of this kernel's warp time
+            // in waits behind longer candidates)
             int pos = 0;
-            if (lane == 0) {
-                while (*(volatile int *)&s_commit != c) { }
-                pos = *(volatile int *)&s_kept;
-                if (keep) *(volatile int *)&s_kept = pos + 1;
-                __threadfence_block();
-                *(volatile int *)&s_commit = c + 1;
-            }
+            if (keep && lane == 0) pos = atomicAdd(&s_kept, 1);
             pos = __shfl_sync(0xffffffffu, pos, 0);
             if (keep && pos < MB) {
                 double *out = tv + ((int64_t)I * MB + pos) * BB;
@@ -632,7 +632,7 @@ bool ellblock_shape_ok(int64_t NB, int MB, int bs)
 {
     if (!(bs == 4 || bs == 8 || bs == 16) || NB < 1 || NB > (1 << 19) || MB < 1) return false;
     const size_t smem1 = (size_t)MB * bs * bs * 8 + (size_t)MB * 4 + (size_t)eb_cand_cap(MB) * 4 + (size_t)((NB + 31) / 32) * 4 +
-                         (NB <= 32768 ? (size_t)NB * 2 + 16 : 0);
+                         (NB <= 32768 ? (size_t)NB * 2 + 16 : 0) + 16 + (size_t)EB_WARPS * MB * 4;
     return smem1 <= 227 * 1024 - 2048;
 }
 
@@ -650,7 +650,8 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int cap = eb_cand_cap(MB);
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
     const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
-    const size_t smem1 = (size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
+    const size_t match_off = ((size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
+    const size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4;
     const size_t smem2 = (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
     if (ensure_smem_attr(x2_ellblock_upper_kernel<BS>, smem1, a1, 48 * 1024)) return BML_ERR_CUDA;
@@ -660,7 +661,7 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int64_t res1 = per_sm1 * EB_THREADS > 2048 ? 2048 / EB_THREADS : per_sm1;
     if (grid1 > sms * res1) grid1 = sms * res1;
     x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                          ctl, tv, ti, tn);
+                                                                          (int)match_off, ctl, tv, ti, tn);
     EB_CHECK();
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
