@@ -30,6 +30,8 @@ constexpr int EB_THREADS = 512;
 constexpr int EB_WARPS = EB_THREADS / 32;
 constexpr int EB_MAX_GRID = 1024;
 constexpr int EB_CHUNKS = 8;             // 32-entry chunks of a block row's index list fetched together (kernel 1)
+constexpr int EB_REF_SHIFT = 13;         // reference to a stored block: (block row << 13) | slot; NB <= 2^19, MB < 2^13 - 1
+constexpr uint32_t EB_REF_NONE = 0xFFFFFFFFu;
 constexpr int EB_PIPE_MAX = 8;               // block pairs whose operand loads are in flight together (kernel 1)
 
 __device__ __forceinline__ int eb_find(const int *__restrict__ list, int n, int key)
@@ -109,7 +111,8 @@ __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                          const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
                          int NB, int MB, double tau, int cand_cap, int use_map, int match_off, Sp2Ctl *__restrict__ ctl,
-                         double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn)
+                         double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn,
+                         uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt)
 {
     constexpr int MT = (BS + 7) / 8, KS = (BS + 3) / 4, BB = BS * BS;
     constexpr int EB_PIPE = BS == 16 ? 4 : EB_PIPE_MAX;        // bs = 16: 16 operand registers per block pair
@@ -270,6 +273,13 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                     }
                 if (lane == 0) ti[(int64_t)I * MB + pos] = J;
             }
+            // the mirror block P_JI = P_IJ^T belongs to row J: leave a reference (row, slot) in row J's lower list, so that
+            // kernel 2 finds it without searching row I.  The counter counts ALL kept blocks (row lengths stay exact when
+            // a list runs over MB); a block that found no slot leaves an invalid reference.
+            if (keep && J != I && lane == 0) {
+                const int k = atomicAdd(&lcnt[J], 1);
+                if (k < MB) lref[(int64_t)J * MB + k] = pos < MB ? (((uint32_t)I << EB_REF_SHIFT) | (uint32_t)pos) : EB_REF_NONE;
+            }
         }
         __syncthreads();
         if (use_map) for (int p = tid; p < nI; p += EB_THREADS) spos[sI[p]] = 0;
@@ -285,8 +295,9 @@ template <int BS>
 __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, int32_t *__restrict__ n0,
                             double *__restrict__ v1, int32_t *__restrict__ i1, int32_t *__restrict__ n1, int NB, int MB,
-                            double tau, int cand_cap, int use_map, Sp2Ctl *__restrict__ ctl, double *__restrict__ partials,
-                            const double *__restrict__ tv, const int32_t *__restrict__ ti, const int32_t *__restrict__ tn)
+                            double tau, int cand_cap, int use_map, int pref_off, Sp2Ctl *__restrict__ ctl,
+                            double *__restrict__ partials, const double *__restrict__ tv, const int32_t *__restrict__ ti, const int32_t *__restrict__ tn,
+                            const uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt)
 {
     constexpr int BB = BS * BS, EPL = (BB + 31) / 32;        // elements of a block per lane
     if (ctl->done) return;
@@ -305,6 +316,7 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
     int *cand = sX + MB;                                             // [cand_cap]
     unsigned *bitmap = (unsigned *)(cand + cand_cap);                // [NBW]
     unsigned short *spos = use_map ? (unsigned short *)(bitmap + NBW) : nullptr;   // block column -> 1 + position in row J of X
+    uint32_t *pref = (uint32_t *)(smem + pref_off);                  // [cand_cap] where the block of thr(X X) of a candidate is
     __shared__ int s_scan[EB_WARPS], s_keep[EB_WARPS], s_pcnt[EB_WARPS], s_last;
     __shared__ double s_part[EB_WARPS][4];
 
@@ -316,7 +328,8 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
 
     for (int J = blockIdx.x; J < NB; J += gridDim.x) {
         const int nX = min(xn[J], MB);
-        const int nU = tn[J];                                        // own upper blocks (may read MB + 1 = overflow)
+        const int nU = tn[J];                                        // own upper blocks (may exceed MB = overflow)
+        const int nL = lcnt[J];                                      // references to the blocks of the rows above (all of them)
         __syncthreads();
         for (int p = tid; p < nX; p += EB_THREADS) {
             const int K = xi[(int64_t)J * MB + p];
@@ -327,8 +340,26 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
         const int ncand_all = eb_candidates(xi, xn, MB, NB, sX, nX, 0, bitmap, cand, cand_cap, s_scan);
         const int ncand = min(ncand_all, cand_cap);
         if (ncand_all > cand_cap && tid == 0) atomicMin(&ctl->acc_row, J);
-        bool ovf_p = nU > MB;
-        int kept_total = 0, p_total = 0;
+        // where the block of thr(X X) of every candidate is: own upper list (row J, slot q) or, transposed, a block of a
+        // row above (references left by kernel 1); the positions in the candidate list by binary search in shared memory
+        for (int q = tid; q < ncand; q += EB_THREADS) pref[q] = EB_REF_NONE;
+        if (tid == 0) lcnt[J] = 0;                                   // every thread has read it (barrier above): for the next product
+        __syncthreads();
+        for (int q = tid; q < min(nU, MB); q += EB_THREADS) {
+            const int c = eb_find(cand, ncand, ti[(int64_t)J * MB + q]);
+            if (c >= 0) pref[c] = ((uint32_t)J << EB_REF_SHIFT) | (uint32_t)q;
+        }
+        for (int q = tid; q < min(nL, MB); q += EB_THREADS) {
+            const uint32_t ref = lref[(int64_t)J * MB + q];
+            if (ref != EB_REF_NONE) {
+                const int c = eb_find(cand, ncand, (int)(ref >> EB_REF_SHIFT));
+                if (c >= 0) pref[c] = ref;
+            }
+        }
+        __syncthreads();
+        const bool ovf_p = nU + nL > MB;                             // the full row of thr(X X) has nU + nL blocks
+        int kept_total = 0;
+        const int p_total = nU + nL;
         for (int c0 = 0; c0 < ncand; c0 += EB_WARPS) {
             const int c = c0 + warp;
             bool keep = false, haveP = false;
@@ -338,16 +369,10 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
             int C = -1;
             if (c < ncand) {
                 C = cand[c];
-                const double *P = nullptr;
-                bool transposed = false;
-                if (C >= J) {
-                    const int pos = eb_find_warp(ti + (int64_t)J * MB, min(nU, MB), C, lane);
-                    if (pos >= 0) P = tv + ((int64_t)J * MB + pos) * BB;
-                } else {
-                    const int nC = min(tn[C], MB);
-                    const int pos = eb_find_warp(ti + (int64_t)C * MB, nC, J, lane);
-                    if (pos >= 0) { P = tv + ((int64_t)C * MB + pos) * BB; transposed = true; }
-                }
+                const uint32_t ref = pref[c];
+                const int prow = (int)(ref >> EB_REF_SHIFT);
+                const double *P = ref != EB_REF_NONE ? tv + ((int64_t)prow * MB + (ref & ((1u << EB_REF_SHIFT) - 1u))) * BB : nullptr;
+                const bool transposed = P && prow != J;
                 const int px = use_map ? (int)spos[C] - 1 : eb_find(sX, nX, C);
                 const double *X = px >= 0 ? xv + ((int64_t)J * MB + px) * BB : nullptr;
                 haveP = P != nullptr;
@@ -382,7 +407,6 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                 const int k = s_keep[w2];
                 if (w2 < warp) pos += k;
                 total += k;
-                p_total += s_pcnt[w2];
             }
             if (keep && pos < MB) {
                 double *out = ov + ((int64_t)J * MB + pos) * BB;
@@ -396,7 +420,6 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
             kept_total += total;
             __syncthreads();
         }
-        if (p_total > MB) ovf_p = true;
         if (tid == 0) {
             w_max_p = max(w_max_p, ovf_p ? max(p_total, MB + 1) : p_total);
             if (ovf_p) { w_ovf_p = min(w_ovf_p, J); on[J] = 0; }
@@ -624,13 +647,13 @@ static inline int eb_cand_cap(int MB) { int c = 8 * MB; return c < 256 ? 256 : (
 size_t ellblock_sym_bytes(int64_t NB, int MB, int bs)
 {
     const size_t nm = (size_t)NB * (size_t)MB;
-    return eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4);
+    return eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4) + eb_up(nm * 4) + eb_up((size_t)NB * 4);
 }
 size_t ellblock_rowstats_bytes() { return (size_t)EB_MAX_GRID * 4 * sizeof(double); }
 
 bool ellblock_shape_ok(int64_t NB, int MB, int bs)
 {
-    if (!(bs == 4 || bs == 8 || bs == 16) || NB < 1 || NB > (1 << 19) || MB < 1) return false;
+    if (!(bs == 4 || bs == 8 || bs == 16) || NB < 1 || NB > (1 << 19) || MB < 1 || MB >= (1 << EB_REF_SHIFT) - 1) return false;
     const size_t smem1 = (size_t)MB * bs * bs * 8 + (size_t)MB * 4 + (size_t)eb_cand_cap(MB) * 4 + (size_t)((NB + 31) / 32) * 4 +
                          (NB <= 32768 ? (size_t)NB * 2 + 16 : 0) + 16 + (size_t)EB_WARPS * MB * 4;
     return smem1 <= 227 * 1024 - 2048;
@@ -646,13 +669,16 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     uint8_t *p = (uint8_t *)sym;
     double *tv = (double *)p; p += eb_up(nm * (size_t)BS * BS * 8);
     int32_t *ti = (int32_t *)p; p += eb_up(nm * 4);
-    int32_t *tn = (int32_t *)p;
+    int32_t *tn = (int32_t *)p; p += eb_up((size_t)NB * 4);
+    uint32_t *lref = (uint32_t *)p; p += eb_up(nm * 4);
+    int32_t *lcnt = (int32_t *)p;
     const int cap = eb_cand_cap(MB);
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
     const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
     const size_t match_off = ((size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
     const size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4;
-    const size_t smem2 = (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0);
+    const size_t pref_off = ((size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
+    const size_t smem2 = pref_off + (size_t)cap * 4;
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
     if (ensure_smem_attr(x2_ellblock_upper_kernel<BS>, smem1, a1, 48 * 1024)) return BML_ERR_CUDA;
     if (ensure_smem_attr(x2_ellblock_assemble_kernel<BS>, smem2, a2, 48 * 1024)) return BML_ERR_CUDA;
@@ -661,15 +687,23 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int64_t res1 = per_sm1 * EB_THREADS > 2048 ? 2048 / EB_THREADS : per_sm1;
     if (grid1 > sms * res1) grid1 = sms * res1;
     x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                          (int)match_off, ctl, tv, ti, tn);
+                                                                          (int)match_off, ctl, tv, ti, tn, lref, lcnt);
     EB_CHECK();
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
     if (grid2 > EB_MAX_GRID) grid2 = EB_MAX_GRID;
     x2_ellblock_assemble_kernel<BS><<<(unsigned)grid2, EB_THREADS, smem2, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                             ctl, partials, tv, ti, tn);
+                                                                             (int)pref_off, ctl, partials, tv, ti, tn, lref, lcnt);
     EB_CHECK();
     return 0;
+}
+
+// the lower-list counters must be zero when a solve starts (kernel 2 re-zeroes them after every product)
+int launch_ellblock_sym_reset(void *sym, int64_t NB, int MB, int bs, cudaStream_t st)
+{
+    const size_t nm = (size_t)NB * (size_t)MB;
+    uint8_t *p = (uint8_t *)sym + eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4) + eb_up(nm * 4);
+    return cudaMemsetAsync(p, 0, (size_t)NB * 4, st) == cudaSuccess ? 0 : BML_ERR_CUDA;
 }
 
 int launch_x2_ellblock(double *v0, int32_t *i0, int32_t *n0, double *v1, int32_t *i1, int32_t *n1, int64_t NB, int MB, int bs,
@@ -851,6 +885,7 @@ int bml_sp2_ellblock(const bml_ellblock_t *H, const bml_sp2_params_t *p, bml_ell
     if ((r = launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                              w.scal->fail_flag, st)))
         return fail(r);
+    if ((r = launch_ellblock_sym_reset(w.sym, NB, MB, bs, st))) return fail(r);
     if ((r = enqueue_products([&]() { return launch_x2_ellblock(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, NB, MB, bs, p->drop_tol,
                                                                 w.ctl, w.rowstats, w.sym, st); },
                               w.ctl, p->max_products, st, 0, stats == nullptr)))
@@ -872,6 +907,7 @@ int bml_x2_ellblock(const bml_ellblock_t *X, bml_ellblock_t *Xnext, int32_t bran
     EbWs w = carve_ellblock(d_workspace, X->NB, X->MB, X->bs, false);
     int r = launch_init_ctl(w.ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
     if (r) return r;
+    if ((r = launch_ellblock_sym_reset(w.sym, X->NB, X->MB, X->bs, st))) return r;
     // buffer 0 = X (read only while parity == 0), buffer 1 = Xnext
     r = launch_x2_ellblock(X->value, X->index, X->nnz, Xnext->value, Xnext->index, Xnext->nnz, X->NB, X->MB, X->bs, drop_tol,
                            w.ctl, w.rowstats, w.sym, st);
