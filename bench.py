@@ -1146,7 +1146,7 @@ def run_ellblock(args):
             "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
             "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run",
             "note": "executed DMMA flops of the upper-triangle block products (2 bs^3 per block pair) / time of the two "
-                    "kernels; the operand blocks come from L2 (2 flop per byte at bs = 8), so the L2 -> SM fabric, not "
+                    "kernels; the operand blocks come from L2 (2 flop per byte at bs = 8), so L2 latency / bandwidth, not "
                     "the tensor pipe, bounds this kernel",
             "launch_ms": k_ms, "flops_per_launch": 2.0 * macs, "mean_blocks_per_block_row": blocks / NB,
             "stored_fill": None, "gathered_bytes": gathered, "gathered_gbs": gathered / (k_ms * 1e-3) / 1e9,
