@@ -744,6 +744,25 @@ def per_config_block(rk: Ranks, skip: str, only=None):
             "roofline": rec["roofline"], "clocks": rec["clocks"], "gpu_launches_per_step": rec["launches_per_step"],
             "bench_wall_s": round(time.perf_counter() - t0, 1),
         }
+    # the two widening rows of SURVEY 8(f) that have workloads of their own (not BASELINE.json configs): the graph-based
+    # construction with SP2 as the local solver (f-2) and the ELLBLOCK path (f-4), so that their numbers are in the
+    # driver-run record too
+    for wname, fn, tag in (("graph_sp2_n12800", run_graph_sp2, "SURVEY 8(f) f-2"), ("ellblock_n65536", run_ellblock, "SURVEY 8(f) f-4")):
+        if wname == skip or (only and wname not in only):
+            continue
+        t0 = time.perf_counter()
+        try:
+            sub = argparse.Namespace(workload=wname, steps=3, warmup=3, no_cpu_baseline=True)
+            rec = fn(sub, rk=rk, emit=False)
+        except Exception as e:
+            out[wname] = {"error": f"{type(e).__name__}: {e}"}
+            continue
+        rec = {k: rec[k] for k in ("config", "dtype", "value", "steps", "warmup", "step_ms_min", "step_ms_max", "status",
+                                   "n_products", "branch", "ms_per_product", "e2e", "roofline", "clocks") if k in rec}
+        rec["ms"] = rec.pop("value")
+        rec["row"] = tag
+        rec["bench_wall_s"] = round(time.perf_counter() - t0, 1)
+        out[wname] = rec
     return out
 
 
@@ -989,12 +1008,13 @@ def run_graph(args):
 # ----------------------------------------------------------------------------------------------------------
 # our arm, graph-based workloads with SP2 as the local solver: one bml_graph_sp2_ellpack call per step
 # ----------------------------------------------------------------------------------------------------------
-def run_graph_sp2(args):
+def run_graph_sp2(args, rk=None, emit=True):
+    """emit=False: return the JSON record instead of printing it (per_config of the default run; `rk` is the caller's)."""
     import torch
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    rk = Ranks()
+    rk = rk or Ranks()
     api.load()
     dev = rk.dev
     w = hm.WORKLOADS[args.workload]
@@ -1070,6 +1090,8 @@ def run_graph_sp2(args):
                              f"{min(n_enq, 100)} batched product launches of which {n_prod} do work, scatter per part",
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
+    if not emit:
+        return line
     print(json.dumps(line), flush=True)
     rk.finish()
     return 0
@@ -1095,12 +1117,13 @@ def ellblock_block_macs(index, nnz, bs: int) -> int:
     return total * bs ** 3
 
 
-def run_ellblock(args):
+def run_ellblock(args, rk=None, emit=True):
+    """emit=False: return the JSON record instead of printing it (per_config of the default run; `rk` is the caller's)."""
     import torch
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    rk = Ranks()
+    rk = rk or Ranks()
     api.load()
     dev = rk.dev
     w = hm.WORKLOADS[args.workload]
@@ -1188,6 +1211,8 @@ def run_ellblock(args):
         "gpu_launches_note": f"{launches_per_step} per step (upper bound); a product is two kernels",
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
+    if not emit:
+        return line
     print(json.dumps(line), flush=True)
     rk.finish()
     return 0
