@@ -744,10 +744,26 @@ def per_config_block(rk: Ranks, skip: str, only=None):
             "roofline": rec["roofline"], "clocks": rec["clocks"], "gpu_launches_per_step": rec["launches_per_step"],
             "bench_wall_s": round(time.perf_counter() - t0, 1),
         }
-    # the two widening rows of SURVEY 8(f) that have workloads of their own (not BASELINE.json configs): the graph-based
-    # construction with SP2 as the local solver (f-2) and the ELLBLOCK path (f-4), so that their numbers are in the
-    # driver-run record too
-    for wname, fn, tag in (("graph_sp2_n12800", run_graph_sp2, "SURVEY 8(f) f-2"), ("ellblock_n65536", run_ellblock, "SURVEY 8(f) f-4")):
+    # the widening rows of SURVEY 8(f) (not BASELINE.json configs), so that their numbers are in the driver-run record
+    # too: the Chebyshev expansion (f-1), the graph-based construction with SP2 as the local solver (f-2), SP2 from
+    # Lanczos-tightened bounds (f-3) and the ELLBLOCK path (f-4)
+    if not (only and "dense_n8192_lanczos32" not in only):
+        t0 = time.perf_counter()
+        try:
+            rec, _ = sp2_measure(rk, "dense_n8192", 3, 3, 32, e2e_steps=2)
+            res = rec["res"]
+            out["dense_n8192_lanczos32"] = {
+                "config": workload_config("dense_n8192"), "row": "SURVEY 8(f) f-3", "dtype": rec["dtype"], "ms": rec["ms"],
+                "steps": 3, "warmup": 3, "status": int(res.status), "n_products": rec["n_products"], "branch": res.branch,
+                "spectral_bounds": {"emin": res.emin, "emax": res.emax, "kind": "lanczos(32) within gershgorin"},
+                "e2e": {"value": rec["e2e_ms"], "unit": "ms", "h2d_bytes_per_step": rec["h2d"],
+                        "d2h_bytes_per_step": rec["d2h"], "steps": rec["e2e_steps"]},
+                "roofline": rec["roofline"], "clocks": rec["clocks"], "bench_wall_s": round(time.perf_counter() - t0, 1),
+            }
+        except Exception as e:
+            out["dense_n8192_lanczos32"] = {"error": f"{type(e).__name__}: {e}"}
+    for wname, fn, tag in (("cheby_n2000", run_cheby, "SURVEY 8(f) f-1"), ("graph_sp2_n12800", run_graph_sp2, "SURVEY 8(f) f-2"),
+                           ("ellblock_n65536", run_ellblock, "SURVEY 8(f) f-4")):
         if wname == skip or (only and wname not in only):
             continue
         t0 = time.perf_counter()
@@ -821,12 +837,13 @@ def run_ours(args):
 # ----------------------------------------------------------------------------------------------------------
 # our arm, Chebyshev workloads: same contract, one bml_chebyshev_dense call per step
 # ----------------------------------------------------------------------------------------------------------
-def run_cheby(args):
+def run_cheby(args, rk=None, emit=True):
+    """emit=False: return the JSON record instead of printing it (per_config of the default run; `rk` is the caller's)."""
     import torch
 
     from paper_2401_13772_b200 import api, hamiltonians as hm
 
-    rk = Ranks()
+    rk = rk or Ranks()
     api.load()
     dev = rk.dev
     w = hm.WORKLOADS[args.workload]
@@ -906,6 +923,8 @@ def run_cheby(args):
                              f"{int(res.n_launches)} grouped product launches ({n_prod} products) + partial sums + trace",
         "roofline": roof, "cpu_baseline": cpu, "clocks": clocks,
     }
+    if not emit:
+        return line
     print(json.dumps(line), flush=True)
     rk.finish()
     return 0
