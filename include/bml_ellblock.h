@@ -11,8 +11,9 @@
  *   E4. everything else -- Gershgorin bounds over stored entries, Eq. 5 with a missing diagonal block inserted, the
  *       idempotency measure over the union of the block patterns, stop rules S1-S3, D = X_{m*}, more than MB blocks
  *       in a block row = failure -3 (stats->overflow_row = the BLOCK row) -- is bml_sp2_ellpack's, per element.
- * stats->max_row_nnz counts BLOCKS per block row.  Status -6 (BML_ERR_ACC_CAPACITY): a block row of X*X reaches more
- * than 8 * MB (at most 8192) distinct block columns BEFORE thresholding, the capacity of the candidate lists.
+ * stats->max_row_nnz counts BLOCKS per block row.  Status -6 (BML_ERR_ACC_CAPACITY): the upper part (J >= I) of a block
+ * row of X*X reaches more than 8 * MB (at most 8192) distinct block columns BEFORE thresholding, the capacity of the
+ * candidate lists.
  */
 #ifndef BML_ELLBLOCK_H
 #define BML_ELLBLOCK_H

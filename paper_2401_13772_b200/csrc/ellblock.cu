@@ -57,24 +57,12 @@ __device__ __forceinline__ int eb_find_warp(const int *__restrict__ list, int n,
     return bal ? __shfl_sync(0xffffffffu, hit, __ffs(bal) - 1) : -1;
 }
 
-// Candidate block columns of block row I: every J (>= jmin) stored in some row K with K stored in row I.  Sets the bits,
-// then writes the ascending list cand[0 .. ncand) (clearing the bitmap on the way).  All threads of the CTA take part.
-__device__ __forceinline__ int eb_candidates(const int32_t *__restrict__ xi, const int32_t *__restrict__ xn, int MB, int NB,
-                                             const int *sI, int nI, int jmin, unsigned *bitmap, int *cand, int cand_cap,
-                                             int *s_scan)
+// The set bits of the bitmap as the ascending list cand[0 .. n) (clearing the bitmap on the way); returns n, which may
+// exceed cand_cap (entries beyond it are not written).  All threads of the CTA take part; the caller has synchronised
+// after setting the bits.
+__device__ __forceinline__ int eb_scan_bitmap(unsigned *bitmap, int NBW, int *cand, int cand_cap, int *s_scan)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int NBW = (NB + 31) >> 5;
-    for (int p = warp; p < nI; p += EB_WARPS) {
-        const int K = sI[p];
-        const int nK = min(xn[K], MB);
-        const int32_t *row = xi + (int64_t)K * MB;
-        for (int q = lane; q < nK; q += 32) {
-            const int J = row[q];
-            if (J >= jmin) atomicOr(&bitmap[J >> 5], 1u << (J & 31));
-        }
-    }
-    __syncthreads();
     int base = 0;
     for (int w0 = 0; w0 < NBW; w0 += EB_THREADS) {
         const int w = w0 + tid;
@@ -101,6 +89,26 @@ __device__ __forceinline__ int eb_candidates(const int32_t *__restrict__ xi, con
         __syncthreads();
     }
     return base;
+}
+
+// Candidate block columns of block row I: every J (>= jmin) stored in some row K with K stored in row I.  Sets the bits,
+// then writes the ascending list cand[0 .. ncand).  All threads of the CTA take part.
+__device__ __forceinline__ int eb_candidates(const int32_t *__restrict__ xi, const int32_t *__restrict__ xn, int MB, int NB,
+                                             const int *sI, int nI, int jmin, unsigned *bitmap, int *cand, int cand_cap,
+                                             int *s_scan)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int p = warp; p < nI; p += EB_WARPS) {
+        const int K = sI[p];
+        const int nK = min(xn[K], MB);
+        const int32_t *row = xi + (int64_t)K * MB;
+        for (int q = lane; q < nK; q += 32) {
+            const int J = row[q];
+            if (J >= jmin) atomicOr(&bitmap[J >> 5], 1u << (J & 31));
+        }
+    }
+    __syncthreads();
+    return eb_scan_bitmap(bitmap, (NB + 31) >> 5, cand, cand_cap, s_scan);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -337,11 +345,22 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
             if (use_map) spos[K] = (unsigned short)(p + 1);
         }
         __syncthreads();
-        const int ncand_all = eb_candidates(xi, xn, MB, NB, sX, nX, 0, bitmap, cand, cand_cap, s_scan);
-        const int ncand = min(ncand_all, cand_cap);
-        if (ncand_all > cand_cap && tid == 0) atomicMin(&ctl->acc_row, J);
+        // The union pattern of row J, in ascending order: the blocks of thr(X X) -- own upper list and the references to
+        // blocks of the rows above that kernel 1 left -- and the blocks of X.  (No two-hop enumeration here: a block
+        // column that is in neither contributes nothing to the update or to the norms.)  At most 3 MB <= cand_cap entries.
+        for (int q = tid; q < min(nU, MB); q += EB_THREADS) {
+            const int C = ti[(int64_t)J * MB + q];
+            atomicOr(&bitmap[C >> 5], 1u << (C & 31));
+        }
+        for (int q = tid; q < min(nL, MB); q += EB_THREADS) {
+            const uint32_t ref = lref[(int64_t)J * MB + q];
+            if (ref != EB_REF_NONE) { const int C = (int)(ref >> EB_REF_SHIFT); atomicOr(&bitmap[C >> 5], 1u << (C & 31)); }
+        }
+        for (int q = tid; q < nX; q += EB_THREADS) { const int C = sX[q]; atomicOr(&bitmap[C >> 5], 1u << (C & 31)); }
+        __syncthreads();
+        const int ncand = min(eb_scan_bitmap(bitmap, NBW, cand, cand_cap, s_scan), cand_cap);
         // where the block of thr(X X) of every candidate is: own upper list (row J, slot q) or, transposed, a block of a
-        // row above (references left by kernel 1); the positions in the candidate list by binary search in shared memory
+        // row above; the positions in the candidate list by binary search in shared memory
         for (int q = tid; q < ncand; q += EB_THREADS) pref[q] = EB_REF_NONE;
         if (tid == 0) lcnt[J] = 0;                                   // every thread has read it (barrier above): for the next product
         __syncthreads();
