@@ -120,7 +120,8 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                          const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
                          int NB, int MB, double tau, int cand_cap, int use_map, int match_off, Sp2Ctl *__restrict__ ctl,
                          double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn,
-                         uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt)
+                         uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt, const double *__restrict__ bn0,
+                         const double *__restrict__ bn1)
 {
     constexpr int MT = (BS + 7) / 8, KS = (BS + 3) / 4, BB = BS * BS;
     constexpr int EB_PIPE = BS == 16 ? 4 : EB_PIPE_MAX;        // bs = 16: 16 operand registers per block pair
@@ -129,6 +130,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     const double *__restrict__ xv = parity ? v1 : v0;
     const int32_t *__restrict__ xi = parity ? i1 : i0;
     const int32_t *__restrict__ xn = parity ? n1 : n0;
+    const double *__restrict__ bnX = parity ? bn1 : bn0;             // Frobenius norms of the blocks of X
 
     extern __shared__ __align__(16) uint8_t smem[];
     const int NBW = (NB + 31) >> 5;
@@ -141,6 +143,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     unsigned short *spos = use_map ? (unsigned short *)(bitmap + NBW) : nullptr;
     // per warp: the matches of the candidate in hand, [MB] entries (after the map, 4-byte aligned: NB * 2 + 16 bytes)
     unsigned *mlist = (unsigned *)(smem + match_off) + (size_t)(threadIdx.x >> 5) * MB;
+    double *snrm = (double *)(smem + match_off + (size_t)EB_WARPS * MB * 4);      // [MB] norms of the blocks of row I
     __shared__ int s_scan[EB_WARPS];
     __shared__ int s_ticket, s_kept;
 
@@ -155,6 +158,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
         for (int p = tid; p < nI; p += EB_THREADS) {
             const int K = xi[(int64_t)I * MB + p];
             sI[p] = K;
+            snrm[p] = bnX[(int64_t)I * MB + p];
             if (use_map) spos[K] = (unsigned short)(p + 1);
         }
         if (tid == 0) { s_ticket = 0; s_kept = 0; }
@@ -206,6 +210,19 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                     }
                 }
                 __syncwarp();
+                // Pre-screen: ||P_IJ||_F <= sum_K ||X_IK||_F ||X_JK||_F.  When that bound is below tau the block is
+                // dropped whatever its entries are, so its products -- and the 512-byte operand loads -- are skipped;
+                // the outcome is the oracle's (the 1e-9 margin covers the round-off of the norms and of the bound).
+                // Most two-hop candidates of a decaying matrix end here.
+                if (J != I && tau > 0.0) {
+                    double bound = 0.0;
+                    for (int m = lane; m < nmatch; m += 32) {
+                        const unsigned e = mlist[m];
+                        bound += snrm[e >> 16] * __ldg(bnX + (int64_t)J * MB + (e & 0xffffu));
+                    }
+                    bound = warp_sum(bound);
+                    if (bound < tau * (1.0 - 1e-9)) nmatch = 0;
+                }
                 // (2) the block products, EB_PIPE at a time: the operand blocks of row J come from L2 and the loads of a
                 // whole group are issued before the first DMMA needs them (one match at a time left every warp waiting
                 // a full L2 round trip per block pair; groups cut at the 32-entry chunks of the list held ~4 in flight)
@@ -305,7 +322,8 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                             double *__restrict__ v1, int32_t *__restrict__ i1, int32_t *__restrict__ n1, int NB, int MB,
                             double tau, int cand_cap, int use_map, int pref_off, Sp2Ctl *__restrict__ ctl,
                             double *__restrict__ partials, const double *__restrict__ tv, const int32_t *__restrict__ ti, const int32_t *__restrict__ tn,
-                            const uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt)
+                            const uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt, double *__restrict__ bn0,
+                            double *__restrict__ bn1)
 {
     constexpr int BB = BS * BS, EPL = (BB + 31) / 32;        // elements of a block per lane
     if (ctl->done) return;
@@ -317,6 +335,7 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
     double *__restrict__ ov = parity ? v0 : v1;
     int32_t *__restrict__ oi = parity ? i0 : i1;
     int32_t *__restrict__ on = parity ? n0 : n1;
+    double *__restrict__ bnO = parity ? bn0 : bn1;                   // Frobenius norms of the blocks of X'
 
     extern __shared__ __align__(16) uint8_t smem[];
     const int NBW = (NB + 31) >> 5;
@@ -382,6 +401,7 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
         for (int c0 = 0; c0 < ncand; c0 += EB_WARPS) {
             const int c = c0 + warp;
             bool keep = false, haveP = false;
+            double blk_nrm = 0.0;                                    // ||X'_JC||_F of a kept block
             double xnew[EPL];
 #pragma unroll
             for (int e = 0; e < EPL; ++e) xnew[e] = 0.0;
@@ -413,7 +433,8 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                     }
                 }
                 nrm2 = warp_sum(nrm2);
-                if (branch) keep = (P || X) && (sqrt(nrm2) >= tau || C == J);
+                blk_nrm = sqrt(nrm2);
+                if (branch) keep = (P || X) && (blk_nrm >= tau || C == J);
                 else keep = haveP;                                   // X' = thr(X X) as it stands
                 if (P || X) { w_e += r_e; w_x += r_x; w_trp += r_trp; }
                 if (keep) w_trn += r_trn;
@@ -434,7 +455,7 @@ x2_ellblock_assemble_kernel(double *__restrict__ v0, int32_t *__restrict__ i0, i
                     const int el = e * 32 + lane;
                     if (el < BB) out[el] = xnew[e];
                 }
-                if (lane == 0) oi[(int64_t)J * MB + pos] = C;
+                if (lane == 0) { oi[(int64_t)J * MB + pos] = C; bnO[(int64_t)J * MB + pos] = blk_nrm; }
             }
             kept_total += total;
             __syncthreads();
@@ -666,7 +687,8 @@ static inline int eb_cand_cap(int MB) { int c = 8 * MB; return c < 256 ? 256 : (
 size_t ellblock_sym_bytes(int64_t NB, int MB, int bs)
 {
     const size_t nm = (size_t)NB * (size_t)MB;
-    return eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4) + eb_up(nm * 4) + eb_up((size_t)NB * 4);
+    return eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4) + eb_up(nm * 4) + eb_up((size_t)NB * 4) +
+           2 * eb_up(nm * 8);
 }
 size_t ellblock_rowstats_bytes() { return (size_t)EB_MAX_GRID * 4 * sizeof(double); }
 
@@ -674,7 +696,7 @@ bool ellblock_shape_ok(int64_t NB, int MB, int bs)
 {
     if (!(bs == 4 || bs == 8 || bs == 16) || NB < 1 || NB > (1 << 19) || MB < 1 || MB >= (1 << EB_REF_SHIFT) - 1) return false;
     const size_t smem1 = (size_t)MB * bs * bs * 8 + (size_t)MB * 4 + (size_t)eb_cand_cap(MB) * 4 + (size_t)((NB + 31) / 32) * 4 +
-                         (NB <= 32768 ? (size_t)NB * 2 + 16 : 0) + 16 + (size_t)EB_WARPS * MB * 4;
+                         (NB <= 32768 ? (size_t)NB * 2 + 16 : 0) + 16 + (size_t)EB_WARPS * MB * 4 + (size_t)MB * 8;
     return smem1 <= 227 * 1024 - 2048;
 }
 
@@ -690,12 +712,14 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     int32_t *ti = (int32_t *)p; p += eb_up(nm * 4);
     int32_t *tn = (int32_t *)p; p += eb_up((size_t)NB * 4);
     uint32_t *lref = (uint32_t *)p; p += eb_up(nm * 4);
-    int32_t *lcnt = (int32_t *)p;
+    int32_t *lcnt = (int32_t *)p; p += eb_up((size_t)NB * 4);
+    double *bn0 = (double *)p; p += eb_up(nm * 8);
+    double *bn1 = (double *)p;
     const int cap = eb_cand_cap(MB);
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
     const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
     const size_t match_off = ((size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
-    const size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4;
+    const size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4 + (size_t)MB * 8;
     const size_t pref_off = ((size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
     const size_t smem2 = pref_off + (size_t)cap * 4;
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
@@ -706,23 +730,44 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int64_t res1 = per_sm1 * EB_THREADS > 2048 ? 2048 / EB_THREADS : per_sm1;
     if (grid1 > sms * res1) grid1 = sms * res1;
     x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                          (int)match_off, ctl, tv, ti, tn, lref, lcnt);
+                                                                          (int)match_off, ctl, tv, ti, tn, lref, lcnt, bn0, bn1);
     EB_CHECK();
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
     if (grid2 > EB_MAX_GRID) grid2 = EB_MAX_GRID;
     x2_ellblock_assemble_kernel<BS><<<(unsigned)grid2, EB_THREADS, smem2, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                             (int)pref_off, ctl, partials, tv, ti, tn, lref, lcnt);
+                                                                             (int)pref_off, ctl, partials, tv, ti, tn, lref, lcnt, bn0, bn1);
     EB_CHECK();
     return 0;
 }
 
-// the lower-list counters must be zero when a solve starts (kernel 2 re-zeroes them after every product)
-int launch_ellblock_sym_reset(void *sym, int64_t NB, int MB, int bs, cudaStream_t st)
+// Frobenius norms of the stored blocks of an iterate, one warp per block (the pre-screen of kernel 1 reads them; kernel
+// 2 writes those of every X' itself, so this runs once per solve, on X_0)
+__global__ void __launch_bounds__(256) ellblock_norms_kernel(const double *__restrict__ v, const int32_t *__restrict__ nnz,
+                                                             int NB, int MB, int bb, double *__restrict__ bn)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t slot = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (slot >= (int64_t)NB * MB) return;
+    if ((int)(slot % MB) >= min(nnz[slot / MB], MB)) return;
+    const double *b = v + slot * bb;
+    double s = 0.0;
+    for (int e = lane; e < bb; e += 32) s = fma(b[e], b[e], s);
+    s = warp_sum(s);
+    if (lane == 0) bn[slot] = sqrt(s);
+}
+
+// start of a solve (or of a single product on a caller's iterate in buffer 0): the lower-list counters must be zero
+// (kernel 2 re-zeroes them after every product), and the block norms of the first iterate are needed
+int launch_ellblock_sym_init(void *sym, const double *xv, const int32_t *xn, int64_t NB, int MB, int bs, cudaStream_t st)
 {
     const size_t nm = (size_t)NB * (size_t)MB;
     uint8_t *p = (uint8_t *)sym + eb_up(nm * (size_t)bs * bs * 8) + eb_up(nm * 4) + eb_up((size_t)NB * 4) + eb_up(nm * 4);
-    return cudaMemsetAsync(p, 0, (size_t)NB * 4, st) == cudaSuccess ? 0 : BML_ERR_CUDA;
+    if (cudaMemsetAsync(p, 0, (size_t)NB * 4, st) != cudaSuccess) return BML_ERR_CUDA;
+    double *bn0 = (double *)(p + eb_up((size_t)NB * 4));
+    ellblock_norms_kernel<<<(unsigned)((nm + 7) / 8), 256, 0, st>>>(xv, xn, (int)NB, MB, bs * bs, bn0);
+    EB_CHECK();
+    return 0;
 }
 
 int launch_x2_ellblock(double *v0, int32_t *i0, int32_t *n0, double *v1, int32_t *i1, int32_t *n1, int64_t NB, int MB, int bs,
@@ -904,7 +949,7 @@ int bml_sp2_ellblock(const bml_ellblock_t *H, const bml_sp2_params_t *p, bml_ell
     if ((r = launch_init_ctl(w.ctl, w.scal->bounds, &w.scal->tr0, p->n_occ, p->max_products, p->idem_tol, 1, 0,
                              w.scal->fail_flag, st)))
         return fail(r);
-    if ((r = launch_ellblock_sym_reset(w.sym, NB, MB, bs, st))) return fail(r);
+    if ((r = launch_ellblock_sym_init(w.sym, w.v0, w.n0, NB, MB, bs, st))) return fail(r);
     if ((r = enqueue_products([&]() { return launch_x2_ellblock(w.v0, w.i0, w.n0, w.v1, w.i1, w.n1, NB, MB, bs, p->drop_tol,
                                                                 w.ctl, w.rowstats, w.sym, st); },
                               w.ctl, p->max_products, st, 0, stats == nullptr)))
@@ -926,7 +971,7 @@ int bml_x2_ellblock(const bml_ellblock_t *X, bml_ellblock_t *Xnext, int32_t bran
     EbWs w = carve_ellblock(d_workspace, X->NB, X->MB, X->bs, false);
     int r = launch_init_ctl(w.ctl, nullptr, nullptr, 1, 1, 1.0, 0, branch ? 1 : 0, nullptr, st);
     if (r) return r;
-    if ((r = launch_ellblock_sym_reset(w.sym, X->NB, X->MB, X->bs, st))) return r;
+    if ((r = launch_ellblock_sym_init(w.sym, X->value, X->nnz, X->NB, X->MB, X->bs, st))) return r;
     // buffer 0 = X (read only while parity == 0), buffer 1 = Xnext
     r = launch_x2_ellblock(X->value, X->index, X->nnz, Xnext->value, Xnext->index, Xnext->nnz, X->NB, X->MB, X->bs, drop_tol,
                            w.ctl, w.rowstats, w.sym, st);
