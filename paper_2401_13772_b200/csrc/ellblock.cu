@@ -194,18 +194,30 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 const double *valJ = xv + (int64_t)J * MB * BB;
                 // (1) intersection of the block lists of rows I and J, written to the warp's match list in ascending K
                 // (row J is in ascending order): entry = (position in row I << 16) | position in row J
+                // The block norms of row J travel with its block columns (same round trip): the pre-screen below needs
+                // those of the matches, and a second, dependent load would cost the skipped candidates as much again.
                 int nmatch = 0;
+                double bound = 0.0;
+                const double *bnJ = bnX + (int64_t)J * MB;
                 for (int qg = 0; qg < nJ; qg += 32 * EB_CHUNKS) {
                     int kq[EB_CHUNKS];                     // block columns of row J, EB_CHUNKS x 32 at a time (one round trip)
+                    double nq[EB_CHUNKS];
 #pragma unroll
-                    for (int u = 0; u < EB_CHUNKS; ++u) { const int q = qg + u * 32 + lane; kq[u] = q < nJ ? __ldg(rowJ + q) : -1; }
+                    for (int u = 0; u < EB_CHUNKS; ++u) {
+                        const int q = qg + u * 32 + lane;
+                        kq[u] = q < nJ ? __ldg(rowJ + q) : -1;
+                        nq[u] = q < nJ ? __ldg(bnJ + q) : 0.0;
+                    }
 #pragma unroll
                     for (int u = 0; u < EB_CHUNKS; ++u) {
                         const int q0 = qg + u * 32;
                         if (q0 >= nJ) break;
                         const int pI = kq[u] < 0 ? -1 : (use_map ? (int)spos[kq[u]] - 1 : eb_find(sI, nI, kq[u]));
                         const unsigned bal = __ballot_sync(0xffffffffu, pI >= 0);
-                        if (pI >= 0) mlist[nmatch + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)pI << 16) | (unsigned)(q0 + lane);
+                        if (pI >= 0) {
+                            mlist[nmatch + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)pI << 16) | (unsigned)(q0 + lane);
+                            bound += snrm[pI] * nq[u];
+                        }
                         nmatch += __popc(bal);
                     }
                 }
@@ -214,15 +226,8 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 // dropped whatever its entries are, so its products -- and the 512-byte operand loads -- are skipped;
                 // the outcome is the oracle's (the 1e-9 margin covers the round-off of the norms and of the bound).
                 // Most two-hop candidates of a decaying matrix end here.
-                if (J != I && tau > 0.0) {
-                    double bound = 0.0;
-                    for (int m = lane; m < nmatch; m += 32) {
-                        const unsigned e = mlist[m];
-                        bound += snrm[e >> 16] * __ldg(bnX + (int64_t)J * MB + (e & 0xffffu));
-                    }
-                    bound = warp_sum(bound);
-                    if (bound < tau * (1.0 - 1e-9)) nmatch = 0;
-                }
+                bound = warp_sum(bound);
+                if (J != I && tau > 0.0 && bound < tau * (1.0 - 1e-9)) nmatch = 0;
                 // (2) the block products, EB_PIPE at a time: the operand blocks of row J come from L2 and the loads of a
                 // whole group are issued before the first DMMA needs them (one match at a time left every warp waiting
                 // a full L2 round trip per block pair; groups cut at the 32-entry chunks of the list held ~4 in flight)
