@@ -111,6 +111,70 @@ __device__ __forceinline__ int eb_candidates(const int32_t *__restrict__ xi, con
     return eb_scan_bitmap(bitmap, (NB + 31) >> 5, cand, cand_cap, s_scan);
 }
 
+// The same enumeration with the pre-screen folded in: while the two-hop neighbours J of row I are marked, the bound
+// sum_K ||X_IK||_F ||X_KJ||_F >= ||P_IJ||_F is accumulated per block column (FP32 atomics in shared memory; X is symmetric,
+// so ||X_KJ|| = ||X_JK||), and only the columns whose bound reaches tau (or J = I) enter the list -- the others would be
+// dropped whatever their entries are.  The 1e-4 margin covers the FP32 rounding of up to MB positive terms; which side
+// of the margin a borderline column falls on does not change any result (kernel 1 repeats the test in FP64).
+__device__ __forceinline__ int eb_candidates_bounded(const int32_t *__restrict__ xi, const int32_t *__restrict__ xn,
+                                                     const double *__restrict__ bnX, int MB, int NB, const int *sI,
+                                                     const double *snrm, int nI, int I, double tau, unsigned *bitmap,
+                                                     float *sbound, int *cand, int cand_cap, int *s_scan)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int NBW = (NB + 31) >> 5;
+    for (int p = warp; p < nI; p += EB_WARPS) {
+        const int K = sI[p];
+        const double nIK = snrm[p];
+        const int nK = min(xn[K], MB);
+        const int32_t *row = xi + (int64_t)K * MB;
+        const double *nrow = bnX + (int64_t)K * MB;
+        for (int q = lane; q < nK; q += 32) {
+            const int J = row[q];
+            if (J >= I) {
+                atomicOr(&bitmap[J >> 5], 1u << (J & 31));
+                atomicAdd(&sbound[J], (float)(nIK * nrow[q]));
+            }
+        }
+    }
+    __syncthreads();
+    const float thr = (float)(tau * (1.0 - 1e-4));
+    int base = 0;
+    for (int w0 = 0; w0 < NBW; w0 += EB_THREADS) {
+        const int w = w0 + tid;
+        unsigned b = w < NBW ? bitmap[w] : 0u;
+        if (w < NBW) bitmap[w] = 0u;
+        unsigned bits = 0u;
+        while (b) {
+            const int bit = __ffs(b) - 1;
+            b &= b - 1;
+            const int J = (w << 5) | bit;
+            const float v = sbound[J];
+            sbound[J] = 0.0f;
+            if (J == I || v >= thr) bits |= 1u << bit;
+        }
+        const int cnt = __popc(bits);
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+        if (lane == 31) s_scan[warp] = inc;
+        __syncthreads();
+        int wbase = 0, total = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < EB_WARPS; ++w2) { const int t = s_scan[w2]; if (w2 < warp) wbase += t; total += t; }
+        int pos = base + wbase + inc - cnt;
+        while (bits) {
+            const int bit = __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (pos < cand_cap) cand[pos] = (w << 5) | bit;
+            ++pos;
+        }
+        base += total;
+        __syncthreads();
+    }
+    return base;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // Kernel 1: upper blocks of thr(X X)
 // ------------------------------------------------------------------------------------------------------------
@@ -118,7 +182,8 @@ template <int BS>
 __global__ void __launch_bounds__(EB_THREADS, 1)
 x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                          const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
-                         int NB, int MB, double tau, int cand_cap, int use_map, int match_off, Sp2Ctl *__restrict__ ctl,
+                         int NB, int MB, double tau, int cand_cap, int use_map, int match_off, int bound_off,
+                         Sp2Ctl *__restrict__ ctl,
                          double *__restrict__ tv, int32_t *__restrict__ ti, int32_t *__restrict__ tn,
                          uint32_t *__restrict__ lref, int32_t *__restrict__ lcnt, const double *__restrict__ bn0,
                          const double *__restrict__ bn1)
@@ -144,6 +209,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     // per warp: the matches of the candidate in hand, [MB] entries (after the map, 4-byte aligned: NB * 2 + 16 bytes)
     unsigned *mlist = (unsigned *)(smem + match_off) + (size_t)(threadIdx.x >> 5) * MB;
     double *snrm = (double *)(smem + match_off + (size_t)EB_WARPS * MB * 4);      // [MB] norms of the blocks of row I
+    float *sbound = bound_off ? (float *)(smem + bound_off) : nullptr;            // [NB] pre-screen bound per block column
     __shared__ int s_scan[EB_WARPS];
     __shared__ int s_ticket, s_kept;
 
@@ -151,6 +217,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     const int g = lane >> 2, t = lane & 3;
     for (int w = tid; w < NBW; w += EB_THREADS) bitmap[w] = 0u;
     if (use_map) for (int w = tid; w < NB; w += EB_THREADS) spos[w] = 0;
+    if (sbound) for (int w = tid; w < NB; w += EB_THREADS) sbound[w] = 0.0f;
 
     for (int I = blockIdx.x; I < NB; I += gridDim.x) {
         const int nI = min(xn[I], MB);
@@ -168,7 +235,9 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
             for (int e = tid; e < nI * BB / 2; e += EB_THREADS) dst[e] = src[e];
         }
         __syncthreads();
-        const int ncand_all = eb_candidates(xi, xn, MB, NB, sI, nI, I, bitmap, cand, cand_cap, s_scan);
+        const int ncand_all = sbound ? eb_candidates_bounded(xi, xn, bnX, MB, NB, sI, snrm, nI, I, tau, bitmap, sbound, cand,
+                                                             cand_cap, s_scan)
+                                     : eb_candidates(xi, xn, MB, NB, sI, nI, I, bitmap, cand, cand_cap, s_scan);
         const int ncand = min(ncand_all, cand_cap);
         // more candidate blocks (before thresholding) than the list holds: the capacity failure -6, like the scalar
         // path's accumulator table
@@ -724,7 +793,10 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const size_t nbw = (size_t)((NB + 31) / 32) * 4;
     const int use_map = (NB <= 32768 && MB < 65535) ? 1 : 0;
     const size_t match_off = ((size_t)MB * BS * BS * 8 + (size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
-    const size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4 + (size_t)MB * 8;
+    size_t smem1 = match_off + (size_t)EB_WARPS * MB * 4 + (size_t)MB * 8;
+    // the per-column bound of the folded pre-screen, when 4 NB more bytes fit
+    size_t bound_off = 0;
+    if (smem1 + (size_t)NB * 4 <= 227 * 1024 - 2048) { bound_off = smem1; smem1 += (size_t)NB * 4; }
     const size_t pref_off = ((size_t)MB * 4 + (size_t)cap * 4 + nbw + (use_map ? (size_t)NB * 2 + 16 : 0) + 15) / 16 * 16;
     const size_t smem2 = pref_off + (size_t)cap * 4;
     static size_t a1[MAX_DEVICES] = {}, a2[MAX_DEVICES] = {};
@@ -735,7 +807,7 @@ static int launch_x2_ellblock_t(double *v0, int32_t *i0, int32_t *n0, double *v1
     const int64_t res1 = per_sm1 * EB_THREADS > 2048 ? 2048 / EB_THREADS : per_sm1;
     if (grid1 > sms * res1) grid1 = sms * res1;
     x2_ellblock_upper_kernel<BS><<<(unsigned)grid1, EB_THREADS, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)NB, MB, tau, cap, use_map,
-                                                                          (int)match_off, ctl, tv, ti, tn, lref, lcnt, bn0, bn1);
+                                                                          (int)match_off, (int)bound_off, ctl, tv, ti, tn, lref, lcnt, bn0, bn1);
     EB_CHECK();
     int64_t grid2 = NB;
     if (grid2 > sms * 4) grid2 = sms * 4;
