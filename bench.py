@@ -1187,9 +1187,11 @@ def run_ellblock(args, rk=None, emit=True):
             "bound": "tensor", "kernel": "x2_ellblock_upper_kernel + x2_ellblock_assemble_kernel", "achieved": achieved,
             "peak": peak_probe, "unit": "TFLOP/s", "frac": achieved / peak_probe, "traffic": ncu_traffic(args.workload)["bytes"],
             "peak_source": "FP64 DMMA issue peak measured live by bml_probe_fp64_tensor_peak in this run",
-            "note": "executed DMMA flops of the upper-triangle block products (2 bs^3 per block pair) / time of the two "
-                    "kernels; the operand blocks come from L2 (2 flop per byte at bs = 8), so L2 latency / bandwidth, not "
-                    "the tensor pipe, bounds this kernel",
+            "note": "flops of ALL upper-triangle block products (2 bs^3 per block pair with a common block column) / time "
+                    "of the two kernels; kernel 1's norm pre-screen does not execute the pairs of candidates that are "
+                    "certain to be dropped (about a third on the 5' model), so the executed DMMA rate is lower; the operand "
+                    "blocks come from L2 (2 flop per byte at bs = 8), so L2 latency and instruction issue, not the tensor "
+                    "pipe, bound this kernel",
             "launch_ms": k_ms, "flops_per_launch": 2.0 * macs, "mean_blocks_per_block_row": blocks / NB,
             "stored_fill": None, "gathered_bytes": gathered, "gathered_gbs": gathered / (k_ms * 1e-3) / 1e9,
             "compulsory_bytes": 2.0 * blocks * (w.bs * w.bs * 8 + 4),
