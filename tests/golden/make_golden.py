@@ -38,7 +38,8 @@ import oracle  # noqa: E402
 from paper_2401_13772_b200 import hamiltonians as hm  # noqa: E402  (input generators only)
 
 OUT = os.path.join(HERE, "sp2_expected.json")
-CASES = ["dense_n256", "dense_n2048", "dense_n8192", "ellpack_small_12x10x8", "ellpack_n65536", "mixed_n16384_first4"]
+CASES = ["dense_n256", "dense_n2048", "dense_n8192", "ellpack_small_12x10x8", "ellpack_n65536", "mixed_n16384_first4",
+         "ellblock_n65536"]
 PROBE_SEED = 20240126          # the paper's date; any fixed seed does
 SAMPLED_ROWS = 16
 SAMPLE = [(0, 0), (0, 1), (1, 0), (5, 17), (100, 100), (127, 128), (128, 127), (255, 255)]
@@ -125,7 +126,45 @@ def ellpack_full_case(name):
     }
 
 
+def ellblock_matvec(dv, di, dn, v):
+    """y = D v for D in ELLBLOCK form (numpy; the GPU test does the same product with torch on its own D)."""
+    NB, MB, bs, _ = dv.shape
+    live = (np.arange(MB)[None, :] < dn[:, None])[:, :, None, None]
+    y = np.zeros((NB, bs))
+    vb = v.reshape(NB, bs)
+    for I0 in range(0, NB, 512):
+        I1 = min(NB, I0 + 512)
+        y[I0:I1] = np.einsum("ipab,ipb->ia", dv[I0:I1] * live[I0:I1], vb[di[I0:I1]])
+    return y.reshape(-1)
+
+
+def ellblock_full_case(name):
+    """SURVEY 8(f) f-4 at BASELINE size: the ELLBLOCK oracle's whole solve of the 5' model in bs x bs blocks."""
+    w = hm.WORKLOADS[name]
+    H = hm.make_ellblock(name)
+    (dv, di, dn), st = oracle.sp2_ellblock(*H, w.n_occ, w.idem_tol, w.drop_tol, 100)
+    NB = dv.shape[0]
+    dv4 = dv.reshape(NB, w.MB, w.bs, w.bs)
+    live = np.arange(w.MB)[None, :] < dn[:, None]
+    write_vector(name + "_Dv.txt", ellblock_matvec(dv4, di, dn, probe_vector(w.N)))
+    rows = [int(r) for r in np.random.default_rng(PROBE_SEED).integers(0, NB, 6)] + [0, NB - 1]
+    return {
+        "kind": "ellblock", "workload": name, "N": w.N, "bs": w.bs, "MB": w.MB, "n_occ": w.n_occ, "idem_tol": w.idem_tol,
+        "drop_tol": w.drop_tol, "Dv_file": name + "_Dv.txt", "probe_seed": PROBE_SEED,
+        "emin": st["emin"], "emax": st["emax"], "status": st["status"], "m_star": st["m_star"],
+        "n_products": st["n_products"], "branch": st["branch"],
+        "trace": [float(x) for x in st["trace"]], "idem": [float(x) for x in st["idem"]],
+        "max_row_nnz": [int(x) for x in st["max_row_nnz"]],
+        "D_blocks_total": int(dn.sum()), "D_blocks_max": int(dn.max()),
+        "D_fro": float(np.sqrt((dv4[live] ** 2).sum())), "D_trace": float(oracle.trace_ellblock(dv, di, dn)),
+        "D_rows": [{"row": r, "index": [int(x) for x in di[r, : dn[r]]],
+                    "block_norm": [float(np.linalg.norm(dv4[r, q])) for q in range(dn[r])]} for r in rows],
+    }
+
+
 def run_case(name):
+    if name.startswith("ellblock_"):
+        return ellblock_full_case(name)
     if name == "ellpack_small_12x10x8":
         return ellpack_small_case()
     if name == "ellpack_n65536":
@@ -143,8 +182,9 @@ def main():
     data = json.load(open(OUT)) if os.path.exists(OUT) else {}
     for name in todo:
         t0 = time.time()
-        data = json.load(open(OUT)) if os.path.exists(OUT) else {}      # re-read: cases may be run one at a time
-        data[name] = run_case(name)
+        case = run_case(name)
+        data = json.load(open(OUT)) if os.path.exists(OUT) else {}      # re-read: cases may be run side by side
+        data[name] = case
         data[name]["oracle_seconds"] = round(time.time() - t0, 1)
         data[name]["oracle_threads"] = oracle.omp_threads()
         print(f"{name}: products={data[name]['n_products']} branch={data[name]['branch']} "

@@ -139,6 +139,47 @@ def test_gpu_matches_golden_ellpack_n65536_full_solve_bit_exact(api, gold):
 
 
 @pytest.mark.gpu
+def test_gpu_matches_golden_ellblock_n65536_full_solve(api, gold):
+    """SURVEY 8(f) f-4 at BASELINE size: the 5' model in 8 x 8 blocks (N = 65536, MB = 256, tau = 1e-6 on block norms), the
+    whole 18-product ELLBLOCK solve against the ELLBLOCK oracle's: status, branch string, traces, blocks per block row and
+    product, block count of D, sampled block rows (columns bit for bit, block norms to round-off), and D over every
+    entry through the seeded probe y = D v.  The kernels' norm pre-screen must not change any of it."""
+    import torch
+
+    if "ellblock_n65536" not in gold:
+        pytest.skip("ellblock_n65536 not in the golden file yet (run tests/golden/make_golden.py ellblock_n65536)")
+    g = gold["ellblock_n65536"]
+    w = hm.WORKLOADS["ellblock_n65536"]
+    assert (g["N"], g["bs"], g["MB"], g["n_occ"], g["idem_tol"], g["drop_tol"]) == (w.N, w.bs, w.MB, w.n_occ, w.idem_tol, w.drop_tol)
+    H = hm.make_ellblock("ellblock_n65536")
+    (dv, di, dn), res = api.bml_sp2_ellblock(*(torch.from_numpy(a).cuda() for a in H), w.n_occ, w.idem_tol, w.drop_tol)
+    assert res.status == g["status"] and res.n_products == g["n_products"] and res.m_star == g["m_star"]
+    assert res.branch == g["branch"]
+    assert (res.emin, res.emax) == (g["emin"], g["emax"])
+    assert [int(x) for x in res.max_row_nnz] == g["max_row_nnz"]
+    np.testing.assert_allclose(res.trace, g["trace"], rtol=0, atol=1e-7)
+    np.testing.assert_allclose(res.idem, g["idem"], rtol=1e-6, atol=1e-14)
+    assert int(dn.sum().item()) == g["D_blocks_total"] and int(dn.max().item()) == g["D_blocks_max"]
+    NB = dv.shape[0]
+    live = torch.arange(w.MB, device=dn.device)[None, :] < dn[:, None]
+    assert abs(torch.sqrt((dv[live] ** 2).sum()).item() - g["D_fro"]) <= TOL_D * g["D_fro"]
+    for r in g["D_rows"]:
+        n = int(dn[r["row"]].item())
+        assert di[r["row"], :n].tolist() == r["index"], r["row"]
+        norms = torch.linalg.norm(dv[r["row"], :n].reshape(n, -1), dim=1).cpu().numpy()
+        np.testing.assert_allclose(norms, r["block_norm"], rtol=0, atol=TOL_D * g["D_fro"])
+    # y = D v with the seeded Gaussian probe: ||D_gpu v - y|| estimates ||D_gpu - D_oracle||_F over every entry
+    v = torch.from_numpy(np.random.default_rng(g["probe_seed"]).standard_normal(g["N"])).cuda().reshape(NB, w.bs)
+    y = torch.zeros(NB, w.bs, dtype=torch.float64, device="cuda")
+    for I0 in range(0, NB, 512):
+        I1 = min(NB, I0 + 512)
+        blk = dv[I0:I1] * live[I0:I1, :, None, None]
+        y[I0:I1] = torch.einsum("ipab,ipb->ia", blk, v[di[I0:I1].long()])
+    y_ref = torch.from_numpy(np.loadtxt(os.path.join(os.path.dirname(GOLD), g["Dv_file"]))).cuda()
+    assert (torch.linalg.norm(y.reshape(-1) - y_ref) / g["D_fro"]).item() <= 3 * TOL_D
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("precision", [1, 2])
 def test_gpu_mixed_n16384_first_products_match_the_fp64_oracle(api, gold, precision):
     """configs[3] against the ORACLE (not against this library's FP64 path): the FP64 oracle stopped by S3 after 4
