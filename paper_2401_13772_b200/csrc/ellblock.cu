@@ -175,6 +175,56 @@ __device__ __forceinline__ int eb_candidates_bounded(const int32_t *__restrict__
     return base;
 }
 
+__device__ __forceinline__ double lds_f64(uint32_t saddr)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(saddr));
+    return v;
+}
+
+// PIPE block pairs of one candidate: acc += X_IK * X_JK^T for the matches list[0 .. nm), in order.  The operand blocks
+// of row J (global memory: L2) are all requested before the first DMMA; row I's blocks come from shared memory (32-bit
+// address sA_u32).  FULL: nm == PIPE, no predicates.
+template <int BS, int PIPE, bool FULL>
+__device__ __forceinline__ void eb_group(double (&acc)[(BS + 7) / 8][(BS + 7) / 8][2], const unsigned *list, int nm,
+                                         uint32_t sA_u32, const double *__restrict__ valJ, int g, int t)
+{
+    constexpr int MT = (BS + 7) / 8, KS = (BS + 3) / 4, BB = BS * BS;
+    uint32_t aoff[PIPE];
+    double bq[PIPE][KS][MT];
+#pragma unroll
+    for (int u = 0; u < PIPE; ++u) {
+        const unsigned e = (FULL || u < nm) ? list[u] : 0u;                       // broadcast
+        aoff[u] = sA_u32 + (e >> 16) * (uint32_t)(BB * 8);
+        const double *Bp = valJ + (size_t)(e & 0xffffu) * BB;
+#pragma unroll
+        for (int s = 0; s < KS; ++s)
+#pragma unroll
+            for (int m = 0; m < MT; ++m) {
+                const int r = m * 8 + g, col = 4 * s + t;
+                bq[u][s][m] = ((FULL || u < nm) && r < BS && col < BS) ? __ldg(Bp + r * BS + col) : 0.0;
+            }
+    }
+#pragma unroll
+    for (int u = 0; u < PIPE; ++u) {
+        if (FULL || u < nm) {                      // warp-uniform
+#pragma unroll
+            for (int s = 0; s < KS; ++s) {
+                double a[MT];
+#pragma unroll
+                for (int m = 0; m < MT; ++m) {
+                    const int r = m * 8 + g, col = 4 * s + t;
+                    a[m] = (r < BS && col < BS) ? lds_f64(aoff[u] + (uint32_t)(r * BS + col) * 8u) : 0.0;
+                }
+#pragma unroll
+                for (int m = 0; m < MT; ++m)
+#pragma unroll
+                    for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], bq[u][s][n]);
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // Kernel 1: upper blocks of thr(X X)
 // ------------------------------------------------------------------------------------------------------------
@@ -200,6 +250,7 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
     extern __shared__ __align__(16) uint8_t smem[];
     const int NBW = (NB + 31) >> 5;
     double *sA = (double *)smem;                                     // [MB][BS*BS] blocks of block row I
+    const uint32_t sA_u32 = smem_u32(sA);
     int *sI = (int *)(sA + (size_t)MB * BB);                         // [MB] their block columns
     int *cand = sI + MB;                                             // [cand_cap]
     unsigned *bitmap = (unsigned *)(cand + cand_cap);                // [NBW]
@@ -300,47 +351,13 @@ x2_ellblock_upper_kernel(const double *__restrict__ v0, const int32_t *__restric
                 // (2) the block products, EB_PIPE at a time: the operand blocks of row J come from L2 and the loads of a
                 // whole group are issued before the first DMMA needs them (one match at a time left every warp waiting
                 // a full L2 round trip per block pair; groups cut at the 32-entry chunks of the list held ~4 in flight)
-                for (int m0 = 0; m0 < nmatch; m0 += EB_PIPE) {
-                    const int nm = min(EB_PIPE, nmatch - m0);
-                    int pA[EB_PIPE];
-                    const double *Bp[EB_PIPE];
-                    double bq[EB_PIPE][KS][MT];
-#pragma unroll
-                    for (int u = 0; u < EB_PIPE; ++u) {
-                        const unsigned e = u < nm ? mlist[m0 + u] : 0u;           // broadcast
-                        pA[u] = (int)(e >> 16);
-                        Bp[u] = valJ + (size_t)(e & 0xffffu) * BB;
-                    }
-#pragma unroll
-                    for (int u = 0; u < EB_PIPE; ++u)
-#pragma unroll
-                        for (int s = 0; s < KS; ++s)
-#pragma unroll
-                            for (int m = 0; m < MT; ++m) {
-                                const int r = m * 8 + g, col = 4 * s + t;
-                                bq[u][s][m] = (u < nm && r < BS && col < BS) ? __ldg(Bp[u] + r * BS + col) : 0.0;
-                            }
-#pragma unroll
-                    for (int u = 0; u < EB_PIPE; ++u) {
-                        if (u < nm) {                      // warp-uniform
-                            const double *A = sA + (size_t)pA[u] * BB;
-#pragma unroll
-                            for (int s = 0; s < KS; ++s) {
-                                double a[MT];
-                                const int col = 4 * s + t;
-#pragma unroll
-                                for (int m = 0; m < MT; ++m) {
-                                    const int r = m * 8 + g;
-                                    a[m] = (r < BS && col < BS) ? A[r * BS + col] : 0.0;
-                                }
-#pragma unroll
-                                for (int m = 0; m < MT; ++m)
-#pragma unroll
-                                    for (int n = 0; n < MT; ++n) dmma884(acc[m][n][0], acc[m][n][1], a[m], bq[u][s][n]);
-                            }
-                        }
-                    }
-                }
+                // Full groups take a path without predicates or zero-filled operands (almost all of them: a surviving
+                // candidate has ~64 matches); row I's operands are read through a 32-bit shared-memory address (the
+                // generic pointer made the compiler rebuild the shared window base for every block pair).
+                int m0 = 0;
+                for (; m0 + EB_PIPE <= nmatch; m0 += EB_PIPE)
+                    eb_group<BS, EB_PIPE, true>(acc, mlist + m0, EB_PIPE, sA_u32, valJ, g, t);
+                if (m0 < nmatch) eb_group<BS, EB_PIPE, false>(acc, mlist + m0, nmatch - m0, sA_u32, valJ, g, t);
                 __syncwarp();                              // the list is rewritten for the next candidate
                 double nrm2 = 0.0;
 #pragma unroll
