@@ -666,7 +666,8 @@ def sp2_measure(rk: Ranks, wname: str, steps: int, warmup: int, lanczos_steps: i
         gathered = 12.0 * macs
         achieved = comp_bytes / (k_ms * 1e-3) / 1e9
         roof = {
-            "bound": "hbm", "kernel": "x2_ellpack_upper_kernel + x2_ellpack_assemble_kernel", "achieved": achieved,
+            "bound": "hbm", "kernel": "ell_block_summary_kernel + x2_ellpack_upper_kernel (pre-screened small tables, then "
+                                      "large tables for the rows passed on) + x2_ellpack_assemble_kernel", "achieved": achieved,
             "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": achieved / pk["hbm_gbs"],
             "frac_uses": "compulsory bytes (read X_5 + write X_6: 12 B per stored entry + 4 B per row)",
             "traffic": traffic["bytes"], "traffic_source": traffic["source"],
@@ -700,8 +701,12 @@ def sp2_measure(rk: Ranks, wname: str, steps: int, warmup: int, lanczos_steps: i
             break
     n_enq = min(n_enq, 100)
     pre = (2 + 1 + 1 + 1 + (1 if w.precision != 0 else 0)) if dense else (2 + 2 + 1)
-    # a sparse product is two kernels; a mixed product is the FP64-diagonal kernel + the tcgen05 kernel
-    launches_per_step = pre + n_enq * (2 if (not dense or w.precision != 0) else 1) + 1
+    # a mixed product is the FP64-diagonal kernel + the tcgen05 kernel; a sparse product is the column-block summary, the
+    # pre-screened small-table kernel, the large-table kernel for the rows it passed on, and the assemble kernel (two
+    # kernels when the pre-screen does not apply: tau = 0, M > 512 or N > 131072)
+    ell_screened = (not dense) and w.drop_tol > 0 and w.M <= 512 and w.N <= 131072
+    per_product = 1 if (dense and w.precision == 0) else (2 if dense else (4 if ell_screened else 2))
+    launches_per_step = pre + n_enq * per_product + 1
     if dense and w.precision == 0 and w.N <= 1024:
         launches_per_step = pre + 1 + 1           # all products run inside ONE cooperative launch (whole-solve kernel)
     rec = {

@@ -21,49 +21,55 @@
 
 namespace bmlsp2 {
 
-constexpr int E_SLOTS = BML_ELL_ACC_SLOTS;
-constexpr int E_MASK = E_SLOTS - 1;
+constexpr int E_SLOTS = BML_ELL_ACC_SLOTS;      // the large table: the documented capacity (status -6 beyond it)
 #ifndef BML_ELL_BUCKET_LOG2
 #define BML_ELL_BUCKET_LOG2 5          // columns per bucket = 32
 #endif
 constexpr int E_BL = BML_ELL_BUCKET_LOG2;
 constexpr int E_BW = 1 << E_BL;                 // bucket width (consecutive columns that stay consecutive slots)
-constexpr int E_BUCKETS = E_SLOTS / E_BW;
-constexpr int E_BUCKET_LOG2 = 12 - E_BL;        // log2(E_BUCKETS) for 4096 slots
-constexpr int E_BUCKET_SHIFT = 32 - E_BUCKET_LOG2;
-static_assert(E_SLOTS == 4096, "bucket hash is written for 4096 slots");
+static_assert(E_SLOTS == 4096, "the large table is written for 4096 slots");
+constexpr int E_SL2_BIG = 12;                   // log2 of the large table
+constexpr int E_SL2_SMALL = 11;                 // log2 of the small table of the pre-screened kernel (2048 slots)
 constexpr int E_EMPTY = -1;
 constexpr int E_GW = 4;               // warps per row group
 constexpr int E_GT = E_GW * 32;       // threads per row group
-constexpr int E_MAX_GROUPS = 4;       // row groups (= rows in flight) per CTA
+constexpr int E_MAX_GROUPS = 4;       // row groups (= rows in flight) per CTA with the large table
+constexpr int E_MAX_GROUPS_SMALL = 7; // ... with the small table
 constexpr int E_MAX_GRID = 1024;
+constexpr int E_SCREEN_MAX_N = 32 * 2 * (1 << E_SL2_SMALL);     // one FP32 bound per 32-column block, aliased on the values
 
 // bucket and in-bucket rotation from the column-block id: the rotation spreads columns that sit at the same position of
 // many blocks (the centre of a stencil) over all positions, while E_BW consecutive columns still map to E_BW consecutive
-// (rotated) slots of one bucket
+// (rotated) slots of one bucket.  SL2 = log2 of the table size.
+template <int SL2>
 __device__ __forceinline__ int e_hash(int j)
 {
+    constexpr int SHIFT = 32 - (SL2 - E_BL);
     const uint32_t h = (uint32_t)(j >> E_BL) * 2654435761u;
-    return (int)((h >> E_BUCKET_SHIFT) << E_BL) | (int)((j + (h >> (E_BUCKET_SHIFT - E_BL))) & (uint32_t)(E_BW - 1));
+    return (int)((h >> SHIFT) << E_BL) | (int)((j + (h >> (SHIFT - E_BL))) & (uint32_t)(E_BW - 1));
 }
 // probe sequence (double hashing on the bucket): same position, `stride` buckets further (stride odd, so all buckets
 // are visited); after a full cycle over the buckets, the next position
+template <int SL2>
 __device__ __forceinline__ int e_stride(int j)
 {
+    constexpr int BUCKETS = 1 << (SL2 - E_BL);
     const uint32_t h = (uint32_t)(j >> E_BL) * 2654435761u;
-    return (int)((((h >> 8) & (E_BUCKETS - 1)) | 1u) << E_BL);
+    return (int)((((h >> 8) & (BUCKETS - 1)) | 1u) << E_BL);
 }
+template <int SL2>
 __device__ __forceinline__ int e_next(int slot, int tries, int stride)
 {
-    slot = (slot + stride) & E_MASK;
-    if ((tries & (E_BUCKETS - 1)) == 0) slot = (slot & ~(E_BW - 1)) | ((slot + 1) & (E_BW - 1));
+    constexpr int BUCKETS = 1 << (SL2 - E_BL);
+    slot = (slot + stride) & ((1 << SL2) - 1);
+    if ((tries & (BUCKETS - 1)) == 0) slot = (slot & ~(E_BW - 1)) | ((slot + 1) & (E_BW - 1));
     return slot;
 }
 
 static inline int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 // row stage sa[M] f64, sk[M] int, sn[M] int; later aliased by the (column, slot) sort buffer of >= 32 entries
 static inline size_t e_scratch_bytes(int M) { return M >= 16 ? (size_t)16 * (size_t)M : 256; }
-static inline size_t e_group_bytes(int M) { return (size_t)E_SLOTS * 12 + e_scratch_bytes(M); }
+static inline size_t e_group_bytes(int M, int slots = E_SLOTS) { return (size_t)slots * 12 + e_scratch_bytes(M); }
 
 size_t ellpack_rowstats_bytes(int64_t) { return (size_t)E_MAX_GRID * 4 * sizeof(double); }
 
@@ -138,9 +144,10 @@ struct Gather {
 
 // slow path of the accumulator lookup: the home slot of column j holds another key or is empty.  Walks the probe
 // sequence, inserting j (value 0) if it is not there yet.  Returns the slot, or -1 when the table is full.
+template <int SL2>
 __device__ __forceinline__ int e_probe_insert(int *keys, double *vals, int j, int s, int kk)
 {
-    const int stride = e_stride(j);
+    const int stride = e_stride<SL2>(j);
     int tries = 0;
     while (true) {
         if (kk == E_EMPTY) {
@@ -149,8 +156,8 @@ __device__ __forceinline__ int e_probe_insert(int *keys, double *vals, int j, in
             kk = old;
         }
         if (kk == j) return s;
-        if (++tries > E_SLOTS) return -1;
-        s = e_next(s, tries, stride);
+        if (++tries > (1 << SL2)) return -1;
+        s = e_next<SL2>(s, tries, stride);
         kk = keys[s];
     }
 }
@@ -164,45 +171,56 @@ __device__ __forceinline__ int e_probe_insert(int *keys, double *vals, int j, in
 // P = sorted(lower list) ++ upper part and runs the fused update / threshold / norms / write-back against row i of X.
 // ============================================================================================================
 
-// gather of the suffix of row k = sk[p]: sn[p] = (first slot << 16) | count
+// gather of the suffix of row k = sk[p]: sn[p] = (first slot << 16) | count.  Only the lanes that have an entry load;
+// the others keep what an earlier step left in g (the structs are zeroed once per row), and every use is guarded by the
+// lane's position against `cnt`.  Unsigned 32 x 32 -> 64-bit offset arithmetic: one IMAD.WIDE.U32.
 template <int CC>
 __device__ __forceinline__ void s_gather(Gather<CC> &g, int &cnt, int p, int n_i, const double *__restrict__ xv,
-                                         const int32_t *__restrict__ xi, int M, const int *sk, const int *sn, int tg)
+                                         const int32_t *__restrict__ xi, unsigned M, const int *sk, const int *sn, int tg)
 {
-#pragma unroll
-    for (int c = 0; c < CC; ++c) { g.j[c] = -1; g.v[c] = 0.0; }
     cnt = 0;
     if (p < n_i) {
-        const int pk = sn[p];
-        const int n_k = pk & 0xffff;
+        const unsigned pk = (unsigned)sn[p];
+        const int n_k = (int)(pk & 0xffffu);
         cnt = n_k;
-        const int64_t base = (int64_t)sk[p] * M + (pk >> 16) + tg;
-        const int32_t *pi = xi + base;
-        const double *pv = xv + base;
+        const uint64_t off = (uint64_t)(unsigned)sk[p] * M + ((pk >> 16) + (unsigned)tg);
+        const int32_t *pi = xi + off;
+        const double *pv = xv + off;
 #pragma unroll
         for (int c = 0; c < CC; ++c) {
-            if (c * E_GT < n_k) {             // group-uniform: chunks beyond the suffix issue nothing
-                if (c * E_GT + tg < n_k) { g.j[c] = __ldg(pi + c * E_GT); g.v[c] = __ldg(pv + c * E_GT); }
-            }
+            if (c * E_GT + tg < n_k) { g.j[c] = __ldg(pi + c * E_GT); g.v[c] = __ldg(pv + c * E_GT); }
         }
     }
 }
 
-// hash update of the first NC chunks of a gathered suffix (straight-line: the NC lookups are independent)
-template <int NC, int CC>
-__device__ __forceinline__ bool s_accumulate(const Gather<CC> &g, double a, int *keys, double *vals)
+// column j passed the pre-screen of this row (one bit per 32-column block)
+__device__ __forceinline__ bool e_allowed(const unsigned *allow, int j)
+{
+    return (allow[(unsigned)j >> 10] >> (((unsigned)j >> 5) & 31u)) & 1u;
+}
+
+// hash update of the first NC chunks of a gathered suffix (straight-line: the NC lookups are independent).
+// SCREEN: entries whose 32-column block failed the row's pre-screen are skipped (they would be dropped anyway).
+// Returns true when the table is full.
+template <int SL2, bool SCREEN, int NC, int CC>
+__device__ __forceinline__ bool s_accumulate(const Gather<CC> &g, int cnt, int tg, double a, int *keys, double *vals,
+                                             const unsigned *allow)
 {
     static_assert(NC <= CC, "chunk count");
     int slot[NC], key[NC];
+    bool ok[NC];
     bool full = false;
 #pragma unroll
-    for (int c = 0; c < NC; ++c) slot[c] = e_hash(g.j[c]);
+    for (int c = 0; c < NC; ++c) {
+        ok[c] = c * E_GT + tg < cnt && (!SCREEN || e_allowed(allow, g.j[c]));      // g.j is a valid column on every lane
+        slot[c] = e_hash<SL2>(g.j[c]);
+    }
 #pragma unroll
     for (int c = 0; c < NC; ++c) key[c] = keys[slot[c]];
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
-        if (g.j[c] >= 0 && key[c] != g.j[c]) {
-            slot[c] = e_probe_insert(keys, vals, g.j[c], slot[c], key[c]);
+        if (ok[c] && key[c] != g.j[c]) {
+            slot[c] = e_probe_insert<SL2>(keys, vals, g.j[c], slot[c], key[c]);
             if (slot[c] < 0) { full = true; slot[c] = 0; }
         }
     }
@@ -211,49 +229,129 @@ __device__ __forceinline__ bool s_accumulate(const Gather<CC> &g, double a, int 
     for (int c = 0; c < NC; ++c) acc[c] = vals[slot[c]];
 #pragma unroll
     for (int c = 0; c < NC; ++c)
-        if (g.j[c] >= 0 && !full) vals[slot[c]] = fma(a, g.v[c], acc[c]);
+        if (ok[c] && !full) vals[slot[c]] = fma(a, g.v[c], acc[c]);
     return full;
 }
 
-// one p-step: dispatch on the number of E_GT-entry chunks the suffix really has (group-uniform), then the group
-// barrier that orders step p before step p + 1; an empty suffix costs nothing
-template <int CC>
-__device__ __forceinline__ bool s_step(const Gather<CC> &g, int cnt, double a, int *keys, double *vals, int grp, bool full)
+// one p-step: a warp dispatches on the number of E_GT-entry chunks in which IT has lanes (warp-uniform; a warp beyond
+// the end of a short suffix goes straight to the barrier), then the group barrier that orders step p before step
+// p + 1; an empty suffix costs nothing.  REDUCE: the barrier also ORs the table-full flag over the group into `stop`
+// (every third step: the flag only has to stop a failing row early).  Returns the thread's own flag.
+template <int SL2, bool SCREEN, int CC>
+__device__ __forceinline__ bool s_step(const Gather<CC> &g, int cnt, double a, int *keys, double *vals, const unsigned *allow,
+                                       int grp, int tg, bool full, bool &stop, const bool REDUCE)
 {
-    if (cnt <= 0) return full;
-    const int nc = (cnt + E_GT - 1) / E_GT;
-    if (nc == 1) full |= s_accumulate<1, CC>(g, a, keys, vals);
-    else if (CC >= 2 && nc == 2) full |= s_accumulate<(CC >= 2 ? 2 : CC), CC>(g, a, keys, vals);
-    else if (CC >= 3 && nc == 3) full |= s_accumulate<(CC >= 3 ? 3 : CC), CC>(g, a, keys, vals);
-    else if (CC >= 4 && nc == 4) full |= s_accumulate<(CC >= 4 ? 4 : CC), CC>(g, a, keys, vals);
-    else full |= s_accumulate<CC, CC>(g, a, keys, vals);
-    return group_bar_or(grp, full);
+    if (cnt <= 0) return full;          // group-uniform; `stop` is only ever set group-uniformly
+    const int mine = cnt - (tg & ~31);  // entries at or beyond this warp's first lane, chunk 0
+    if (mine > 0) {
+        const int nc = (mine + E_GT - 1) / E_GT;
+        if (nc == 1) full |= s_accumulate<SL2, SCREEN, 1, CC>(g, cnt, tg, a, keys, vals, allow);
+        else if (CC >= 2 && nc == 2) full |= s_accumulate<SL2, SCREEN, (CC >= 2 ? 2 : CC), CC>(g, cnt, tg, a, keys, vals, allow);
+        else if (CC >= 3 && nc == 3) full |= s_accumulate<SL2, SCREEN, (CC >= 3 ? 3 : CC), CC>(g, cnt, tg, a, keys, vals, allow);
+        else if (CC >= 4 && nc == 4) full |= s_accumulate<SL2, SCREEN, (CC >= 4 ? 4 : CC), CC>(g, cnt, tg, a, keys, vals, allow);
+        else full |= s_accumulate<SL2, SCREEN, CC, CC>(g, cnt, tg, a, keys, vals, allow);
+    }
+    if (REDUCE) { stop = group_bar_or(grp, full); return full; }
+    group_bar(grp);
+    return full;
 }
 
-template <int CC>
+// returns true (group-uniform) when the accumulator ran out of slots
+template <int SL2, bool SCREEN, int CC>
 __device__ __forceinline__ bool s_accumulate_row(const double *__restrict__ xv, const int32_t *__restrict__ xi, int M,
                                                  int n_i, const double *sa, const int *sk, const int *sn, int *keys,
-                                                 double *vals, int tg, int grp)
+                                                 double *vals, const unsigned *allow, int row, int tg, int grp)
 {
-    bool full = false;
+    bool full = false, stop = false;
     Gather<CC> gA, gB, gC;
+#pragma unroll
+    for (int c = 0; c < CC; ++c) { gA.j[c] = gB.j[c] = gC.j[c] = row; gA.v[c] = gB.v[c] = gC.v[c] = 0.0; }
     int nA, nB, nC;
-    s_gather<CC>(gA, nA, 0, n_i, xv, xi, M, sk, sn, tg);
-    s_gather<CC>(gB, nB, 1, n_i, xv, xi, M, sk, sn, tg);
+    s_gather<CC>(gA, nA, 0, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+    s_gather<CC>(gB, nB, 1, n_i, xv, xi, (unsigned)M, sk, sn, tg);
     for (int p = 0; p < n_i; p += 3) {
-        s_gather<CC>(gC, nC, p + 2, n_i, xv, xi, M, sk, sn, tg);
-        full = s_step<CC>(gA, nA, sa[p], keys, vals, grp, full);
+        s_gather<CC>(gC, nC, p + 2, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+        full = s_step<SL2, SCREEN, CC>(gA, nA, sa[p], keys, vals, allow, grp, tg, full, stop, false);
         if (p + 1 < n_i) {
-            s_gather<CC>(gA, nA, p + 3, n_i, xv, xi, M, sk, sn, tg);
-            full = s_step<CC>(gB, nB, sa[p + 1], keys, vals, grp, full);
+            s_gather<CC>(gA, nA, p + 3, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+            full = s_step<SL2, SCREEN, CC>(gB, nB, sa[p + 1], keys, vals, allow, grp, tg, full, stop, false);
         }
         if (p + 2 < n_i) {
-            s_gather<CC>(gB, nB, p + 4, n_i, xv, xi, M, sk, sn, tg);
-            full = s_step<CC>(gC, nC, sa[p + 2], keys, vals, grp, full);
+            s_gather<CC>(gB, nB, p + 4, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+            full = s_step<SL2, SCREEN, CC>(gC, nC, sa[p + 2], keys, vals, allow, grp, tg, full, stop, true);
+            if (stop) break;               // group-uniform: the OR came with the barrier
         }
-        if (full) break;
     }
-    return full;
+    return group_bar_or(grp, full);        // flags raised in steps whose barrier did not carry them
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Exact pre-screen of one output row (small-table kernel).  |P_ij| <= sum_k |x_ik| |x_kj| <= sum_k |x_ik| max_{j' in
+// block(j)} |x_kj'| =: bound(block(j)), with block = 32 consecutive columns.  The per-row block maxima of X come from
+// ell_block_summary_kernel (one (block id, max) list per row).  A block whose bound is below tau holds only entries the
+// threshold drops, so the numeric pass neither inserts nor accumulates them: the accumulator shrinks from the two-hop
+// candidate set (up to ~2300 columns of the upper half on the 5' model) to about the kept set (<= ~1000), which is
+// what lets a 2048-slot table -- and seven rows in flight per SM instead of four -- do.  The bounds are summed in FP32
+// with shared-memory atomics (order-free: no barrier per k); |x| is rounded up, and the 1e-3 margin on tau covers the
+// rounding of the sum, so every skipped entry is one the oracle drops as well.  The bound array aliases the values of
+// the (not yet initialised) table.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int E_PS_U = 8;      // rows k whose block lists are in flight per warp
+__device__ __forceinline__ void s_prescreen(int row, int n_i, int N, int SB, const double *sa, const int *sk,
+                                            const int32_t *__restrict__ sb_id, const float *__restrict__ sb_mx,
+                                            const int32_t *__restrict__ sb_n, float *bnd, unsigned *allow, double tau,
+                                            int tg, int grp)
+{
+    const int lane = tg & 31, wg = tg >> 5;
+    const int NBK = (N + 31) >> 5, rb = row >> 5;
+    for (int b = tg; b < NBK; b += E_GT) bnd[b] = 0.0f;
+    group_bar(grp);
+    for (int p0 = wg * 32; p0 < n_i; p0 += E_GW * 32) {
+        const int pl = p0 + lane;
+        int kl = 0, cl = 0;
+        float al = 0.0f;
+        if (pl < n_i) { kl = sk[pl]; cl = __ldg(sb_n + kl); al = __double2float_ru(fabs(sa[pl])); }
+        const int nu = min(32, n_i - p0);
+        for (int u0 = 0; u0 < nu; u0 += E_PS_U) {
+            int id[E_PS_U][2];
+            float mx[E_PS_U][2], au[E_PS_U];
+#pragma unroll
+            for (int u = 0; u < E_PS_U; ++u) {
+                const int src = min(u0 + u, 31);
+                const int k = __shfl_sync(0xffffffffu, kl, src);
+                const int c = (u0 + u < nu) ? __shfl_sync(0xffffffffu, cl, src) : 0;
+                au[u] = __shfl_sync(0xffffffffu, al, src);
+                const int64_t base = (int64_t)k * SB;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int e = h * 32 + lane;
+                    id[u][h] = e < c ? __ldg(sb_id + base + e) : -1;
+                    mx[u][h] = e < c ? __ldg(sb_mx + base + e) : 0.0f;
+                }
+                for (int e = 64 + lane; e < c; e += 32) {          // a row with more than 64 column blocks: rare
+                    const int b = __ldg(sb_id + base + e);
+                    if (b >= rb) atomicAdd(&bnd[b], au[u] * __ldg(sb_mx + base + e));
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < E_PS_U; ++u)
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (id[u][h] >= rb) atomicAdd(&bnd[id[u][h]], au[u] * mx[u][h]);
+        }
+    }
+    group_bar(grp);
+    const float thr = (float)(tau * (1.0 - 1e-3));
+    for (int w = tg; w < ((NBK + 31) >> 5); w += E_GT) {
+        unsigned bits = 0u;
+        for (int b = 0; b < 32; ++b) {
+            const int bb = (w << 5) + b;
+            if (bb < NBK && bnd[bb] >= thr) bits |= 1u << b;
+        }
+        if (w == (rb >> 5)) bits |= 1u << (rb & 31);          // the diagonal is kept whatever its value
+        allow[w] = bits;
+    }
+    group_bar(grp);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -262,13 +360,22 @@ __device__ __forceinline__ bool s_accumulate_row(const double *__restrict__ xv, 
 //   lv/li/lcnt : per row j, the entries (i, P_ji = P_ij) with i < j, in arrival order; lcnt[j] counts ALL arrivals
 //                (slots beyond M are not written: the row has overflowed then anyway)
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(E_MAX_GROUPS * E_GT, 1)
+// Two instances.  <E_SL2_SMALL, true, 7>: 2048-slot tables behind the exact pre-screen (s_prescreen), seven rows in
+// flight per SM; a row whose screened fill still does not fit (or whose gathered rows need more than four chunks) goes
+// to fail_list.  <E_SL2_BIG, false, 4>: the 4096-slot tables without a screen, over all rows (tau = 0, large N or M) or
+// over row_list[0 .. *row_count) -- the rows the first instance passed on; a table that overflows here is status -6.
+template <int SL2, bool SCREEN, int MAXG>
+__global__ void __launch_bounds__(MAXG * E_GT, 1)
 x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                         const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
                         int N, int M, double tau, int sort_cap, Sp2Ctl *__restrict__ ctl, double *__restrict__ tv,
                         int32_t *__restrict__ ti, int32_t *__restrict__ tn, double *__restrict__ lv,
-                        int32_t *__restrict__ li, int32_t *__restrict__ lcnt)
+                        int32_t *__restrict__ li, int32_t *__restrict__ lcnt, const int32_t *__restrict__ sb_id,
+                        const float *__restrict__ sb_mx, const int32_t *__restrict__ sb_n, int32_t *__restrict__ fail_list,
+                        int32_t *__restrict__ fail_count, const int32_t *__restrict__ row_list,
+                        const int32_t *__restrict__ row_count, int allow_off)
 {
+    constexpr int SLOTS = 1 << SL2;
     if (ctl->done) return;
     const int parity = ctl->parity;
     const double *__restrict__ xv = parity ? v1 : v0;
@@ -278,28 +385,31 @@ x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict
     extern __shared__ __align__(16) uint8_t smem[];
     const int ngroups = blockDim.x / E_GT;
     const int grp = threadIdx.x / E_GT, tg = threadIdx.x % E_GT, lane = threadIdx.x & 31;
-    uint8_t *gbase = smem + (size_t)grp * ((size_t)E_SLOTS * 12 + (size_t)sort_cap * 8);
+    uint8_t *gbase = smem + (size_t)grp * ((size_t)SLOTS * 12 + (size_t)sort_cap * 8);
     double *vals = (double *)gbase;
-    int *keys = (int *)(gbase + (size_t)E_SLOTS * 8);
-    uint8_t *scratch = gbase + (size_t)E_SLOTS * 12;
+    int *keys = (int *)(gbase + (size_t)SLOTS * 8);
+    uint8_t *scratch = gbase + (size_t)SLOTS * 12;
     double *sa = (double *)scratch;
     int *sk = (int *)(scratch + (size_t)8 * M);
     int *sn = sk + M;
     unsigned long long *sortbuf = (unsigned long long *)scratch;     // aliases sa/sk/sn after the accumulation
-    __shared__ int s_kept[E_MAX_GROUPS], s_nkmax[E_MAX_GROUPS][2];
+    // [(N / 32 + 31) / 32] words per group: the 32-column blocks of the row in hand that passed the pre-screen
+    unsigned *allow = SCREEN ? (unsigned *)(smem + allow_off) + (size_t)grp * ((((N + 31) >> 5) + 31) >> 5) : nullptr;
+    __shared__ int s_kept[MAXG], s_nkmax[MAXG][2];
 
     int w_acc = INT32_MAX;
     if (tg == 0) { s_nkmax[grp][0] = 0; s_nkmax[grp][1] = 0; }
     group_bar(grp);
     int it = 0;
-    for (int64_t row64 = (int64_t)blockIdx.x * ngroups + grp; row64 < N; row64 += (int64_t)gridDim.x * ngroups) {
-        const int row = (int)row64;
+    const int nrows = row_list ? *row_count : N;
+    for (int64_t row64 = (int64_t)blockIdx.x * ngroups + grp; row64 < nrows; row64 += (int64_t)gridDim.x * ngroups) {
+        const int row = row_list ? row_list[row64] : (int)row64;
         const int64_t rbase = (int64_t)row * M;
         const int n_i = min(xn[row], M);
         {
             int4 *k4 = (int4 *)keys;
             const int4 e4 = make_int4(E_EMPTY, E_EMPTY, E_EMPTY, E_EMPTY);
-            for (int s = tg; s < E_SLOTS / 4; s += E_GT) k4[s] = e4;
+            for (int s = tg; s < SLOTS / 4; s += E_GT) k4[s] = e4;
         }
         int nk_max = 0;
         // Four entries of row i per thread at a time (one pass for n_i <= 4 E_GT): their binary searches -- about
@@ -351,26 +461,33 @@ x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict
         const int chunks = (s_nkmax[grp][it & 1] + E_GT - 1) / E_GT;
         ++it;
 
-        bool full;
-#define S_ACC(CC) full = s_accumulate_row<CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, tg, grp)
+        if (SCREEN) s_prescreen(row, n_i, N, M, sa, sk, sb_id, sb_mx, sb_n, (float *)vals, allow, tau, tg, grp);
+
+        bool full = false;
+#define S_ACC(CC) full = s_accumulate_row<SL2, SCREEN, CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, allow, row, tg, grp)
         if (chunks <= 1) S_ACC(1);
         else if (chunks == 2) S_ACC(2);
         else if (chunks == 3) S_ACC(3);
         else if (chunks == 4) S_ACC(4);
+        else if (SCREEN) full = true;     // longer gathered rows need more registers than seven groups leave: large table
         else if (chunks <= 6) S_ACC(6);
         else S_ACC(8);
 #undef S_ACC
-        if (full) {                       // accumulator capacity exceeded: status -6
-            w_acc = min(w_acc, row);
-            if (tg == 0) tn[row] = 0;
+        if (full) {
+            if (SCREEN) {                 // passed on to the large-table instance
+                if (tg == 0) fail_list[atomicAdd(fail_count, 1)] = row;
+            } else {                      // accumulator capacity exceeded: status -6
+                w_acc = min(w_acc, row);
+                if (tg == 0) tn[row] = 0;
+            }
             group_bar(grp);
             continue;
         }
 
         // threshold (keep |p| >= tau or the diagonal) and compact (column, slot) into the sort buffer
-        for (int s0 = 0; s0 < E_SLOTS; s0 += E_GT) {
+        for (int s0 = 0; s0 < SLOTS; s0 += E_GT) {
             const int s = s0 + tg;
-            const int key = s < E_SLOTS ? keys[s] : E_EMPTY;
+            const int key = s < SLOTS ? keys[s] : E_EMPTY;
             const bool keep = key != E_EMPTY && (fabs(vals[s]) >= tau || key == row);
             if (keep && key != row) {         // mirror: P_ji = P_ij, appended to row j = key (j > row); counts are exact
                 const int pos = atomicAdd(&lcnt[key], 1);
@@ -740,6 +857,58 @@ __global__ void x2_ellpack_info_kernel(const Sp2Ctl *__restrict__ ctl, int32_t *
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Per-row column-block summary of the iterate X (input of s_prescreen): for every row, the 32-column blocks it has
+// entries in (ascending, rows are sorted) and the largest |x| in each, rounded up to FP32.  One warp per row; the
+// entries of one block are contiguous, so a block is a run of equal (column >> 5).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int E_SUM_WARPS = 8;
+__global__ void __launch_bounds__(E_SUM_WARPS * 32)
+ell_block_summary_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
+                         const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
+                         int N, int M, const Sp2Ctl *__restrict__ ctl, int32_t *__restrict__ sb_id,
+                         float *__restrict__ sb_mx, int32_t *__restrict__ sb_n)
+{
+    if (ctl->done) return;
+    const int parity = ctl->parity;
+    const double *__restrict__ xv = parity ? v1 : v0;
+    const int32_t *__restrict__ xi = parity ? i1 : i0;
+    const int32_t *__restrict__ xn = parity ? n1 : n0;
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int *s_id = (int *)smem + (size_t)warp * 2 * M;
+    unsigned *s_mx = (unsigned *)(s_id + M);
+    for (int row = blockIdx.x * E_SUM_WARPS + warp; row < N; row += gridDim.x * E_SUM_WARPS) {
+        const int n = min(xn[row], M);
+        const int64_t rbase = (int64_t)row * M;
+        for (int q = lane; q < n; q += 32) s_mx[q] = 0u;
+        __syncwarp();
+        int nseg = 0, last_b = -1;
+        for (int c0 = 0; c0 < n; c0 += 32) {
+            const int e = c0 + lane;
+            const bool valid = e < n;
+            const int b = valid ? (xi[rbase + e] >> E_BL) : -2;
+            int pb = __shfl_up_sync(0xffffffffu, b, 1);
+            if (lane == 0) pb = last_b;
+            const bool head = valid && b != pb;
+            const unsigned hb = __ballot_sync(0xffffffffu, head);
+            const int seg = nseg + __popc(hb & (0xffffffffu >> (31 - lane))) - 1;       // heads at or before this lane
+            if (head) s_id[seg] = b;
+            // non-negative floats order like their bit patterns
+            if (valid) atomicMax(&s_mx[seg], __float_as_uint(__double2float_ru(fabs(xv[rbase + e]))));
+            nseg += __popc(hb);
+            last_b = __shfl_sync(0xffffffffu, b, min(31, n - 1 - c0));
+        }
+        __syncwarp();
+        for (int q = lane; q < nseg; q += 32) {
+            sb_id[rbase + q] = s_id[q];
+            sb_mx[rbase + q] = __uint_as_float(s_mx[q]);
+        }
+        if (lane == 0) sb_n[row] = nseg;
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------------------------
 #define BML_CHECK_LAUNCH() do { if (cudaGetLastError() != cudaSuccess) return BML_ERR_CUDA; } while (0)
@@ -751,7 +920,9 @@ size_t ellpack_sym_bytes(int64_t N, int M)
 {
     const size_t nm = (size_t)N * (size_t)M;
     auto up = [](size_t x) { return (x + 1023) / 1024 * 1024; };
-    return 2 * up(nm * 8) + 2 * up(nm * 4) + 2 * up((size_t)N * 4);
+    // + the column-block summaries of the iterate (ids, maxima, counts), the list of rows passed on to the large
+    //   tables and its counter
+    return 2 * up(nm * 8) + 2 * up(nm * 4) + 2 * up((size_t)N * 4) + 2 * up(nm * 4) + 2 * up((size_t)N * 4) + 1024;
 }
 
 // the lower-list counters must be zero when a solve starts (kernel 2 re-zeroes them after every product)
@@ -777,21 +948,62 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
     int32_t *ti = (int32_t *)p; p += up(nm * 4);
     int32_t *li = (int32_t *)p; p += up(nm * 4);
     int32_t *tn = (int32_t *)p; p += up((size_t)N * 4);
-    int32_t *lcnt = (int32_t *)p;
+    int32_t *lcnt = (int32_t *)p; p += up((size_t)N * 4);
+    int32_t *sb_id = (int32_t *)p; p += up(nm * 4);
+    float *sb_mx = (float *)p; p += up(nm * 4);
+    int32_t *sb_n = (int32_t *)p; p += up((size_t)N * 4);
+    int32_t *fail_list = (int32_t *)p; p += up((size_t)N * 4);
+    int32_t *fail_count = (int32_t *)p;
 
     // ---- kernel 1
     const size_t smem_cap = 227 * 1024 - 1024;
-    int ngroups = (int)(smem_cap / e_group_bytes(M));
-    if (ngroups > E_MAX_GROUPS) ngroups = E_MAX_GROUPS;
-    if (ngroups < 1 || M > 8 * E_GT) return BML_ERR_INVALID;
-    const size_t smem1 = (size_t)ngroups * e_group_bytes(M);
-    static size_t attr1[MAX_DEVICES] = {};
-    if (ensure_smem_attr(x2_ellpack_upper_kernel, smem1, attr1)) return BML_ERR_CUDA;
-    int64_t grid1 = (N + ngroups - 1) / ngroups;
-    if (grid1 > sms) grid1 = sms;
-    x2_ellpack_upper_kernel<<<(unsigned)grid1, ngroups * E_GT, smem1, st>>>(
-        v0, i0, n0, v1, i1, n1, (int)N, M, tau, (int)(e_scratch_bytes(M) / 8), ctl, tv, ti, tn, lv, li, lcnt);
-    BML_CHECK_LAUNCH();
+    const int sort_cap = (int)(e_scratch_bytes(M) / 8);
+    if (M > 8 * E_GT) return BML_ERR_INVALID;
+    // (a) small tables behind the pre-screen, when it applies: tau > 0, rows gathered in <= 4 chunks, one FP32 bound per
+    //     32-column block fits the values of a small table
+    const size_t allow_bytes = (size_t)((((N + 31) / 32) + 31) / 32) * 4;
+    int ng_small = (int)(smem_cap / (e_group_bytes(M, 1 << E_SL2_SMALL) + allow_bytes));
+    if (ng_small > E_MAX_GROUPS_SMALL) ng_small = E_MAX_GROUPS_SMALL;
+    const bool screened = tau > 0.0 && M <= 4 * E_GT && N <= E_SCREEN_MAX_N && ng_small > E_MAX_GROUPS;
+    if (screened) {
+        if (cudaMemsetAsync(fail_count, 0, sizeof(int32_t), st) != cudaSuccess) return BML_ERR_CUDA;
+        const size_t sum_smem = (size_t)E_SUM_WARPS * 2 * M * 4;
+        static size_t attr_s[MAX_DEVICES] = {};
+        if (ensure_smem_attr(ell_block_summary_kernel, sum_smem, attr_s, 48 * 1024)) return BML_ERR_CUDA;
+        int64_t grid_s = (N + E_SUM_WARPS - 1) / E_SUM_WARPS;
+        if (grid_s > (int64_t)sms * 8) grid_s = (int64_t)sms * 8;
+        ell_block_summary_kernel<<<(unsigned)grid_s, E_SUM_WARPS * 32, sum_smem, st>>>(v0, i0, n0, v1, i1, n1, (int)N, M, ctl,
+                                                                                       sb_id, sb_mx, sb_n);
+        BML_CHECK_LAUNCH();
+        const size_t gb = e_group_bytes(M, 1 << E_SL2_SMALL);
+        const size_t allow_off = (size_t)ng_small * gb;
+        const size_t smem_a = allow_off + (size_t)ng_small * allow_bytes;
+        auto ka = x2_ellpack_upper_kernel<E_SL2_SMALL, true, E_MAX_GROUPS_SMALL>;
+        static size_t attr_a[MAX_DEVICES] = {};
+        if (ensure_smem_attr(ka, smem_a, attr_a)) return BML_ERR_CUDA;
+        int64_t grid_a = (N + ng_small - 1) / ng_small;
+        if (grid_a > sms) grid_a = sms;
+        ka<<<(unsigned)grid_a, ng_small * E_GT, smem_a, st>>>(v0, i0, n0, v1, i1, n1, (int)N, M, tau, sort_cap, ctl, tv, ti, tn,
+                                                             lv, li, lcnt, sb_id, sb_mx, sb_n, fail_list, fail_count, nullptr,
+                                                             nullptr, (int)allow_off);
+        BML_CHECK_LAUNCH();
+    }
+    // (b) the large tables: every row, or the rows (a) passed on
+    {
+        int ngroups = (int)(smem_cap / e_group_bytes(M));
+        if (ngroups > E_MAX_GROUPS) ngroups = E_MAX_GROUPS;
+        if (ngroups < 1) return BML_ERR_INVALID;
+        const size_t smem1 = (size_t)ngroups * e_group_bytes(M);
+        auto kb = x2_ellpack_upper_kernel<E_SL2_BIG, false, E_MAX_GROUPS>;
+        static size_t attr1[MAX_DEVICES] = {};
+        if (ensure_smem_attr(kb, smem1, attr1)) return BML_ERR_CUDA;
+        int64_t grid1 = (N + ngroups - 1) / ngroups;
+        if (grid1 > sms) grid1 = sms;
+        kb<<<(unsigned)grid1, ngroups * E_GT, smem1, st>>>(v0, i0, n0, v1, i1, n1, (int)N, M, tau, sort_cap, ctl, tv, ti, tn, lv,
+                                                          li, lcnt, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                                          screened ? fail_list : nullptr, screened ? fail_count : nullptr, 0);
+        BML_CHECK_LAUNCH();
+    }
 
     // ---- kernel 2
     const size_t wbytes = a_warp_bytes(M);
