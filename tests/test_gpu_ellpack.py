@@ -75,6 +75,43 @@ def test_x2_ellpack_one_product_bit_exact(api, oracle_mod, L, M, tau, branch):
     assert np.allclose(sums.cpu().numpy(), ref, rtol=1e-12, atol=1e-15)
 
 
+def test_x2_ellpack_rows_that_outgrow_the_small_table_go_to_the_large_one(api, oracle_mod):
+    """Kernel 1 runs 2048-slot tables behind an exact pre-screen (bound per 32-column block from the block maxima of
+    X) and hands rows that still do not fit to the 4096-slot instance.  Here every 32-column block a row touches holds
+    one entry of magnitude 0.05 - 0.1 and a few of 1e-5 (random signs), tau = 1e-6: the block bounds all pass, so the
+    screen removes nothing; the first rows reach ~2100 distinct columns j >= i (more than the small table holds, fewer
+    than the large one), the last rows a handful -- both instances run -- and only the large x large products survive
+    the threshold, so the rows fit M.  Bit-exact against the oracle, both branches."""
+    rng = np.random.default_rng(11)
+    N, M, tau = 8192, 512, 1e-6
+    A = np.zeros((N, N))
+    nb = N // 32
+    for i in range(N):
+        for b in rng.choice(nb, 7, replace=False):
+            cols = b * 32 + rng.choice(32, 8, replace=False)
+            A[i, cols[0]] = rng.choice([-1.0, 1.0]) * rng.uniform(0.05, 0.1)
+            A[i, cols[1:]] = rng.choice([-1.0, 1.0], 7) * 1e-5
+    A = np.triu(A, 1)
+    A = A + A.T + np.diag(rng.uniform(0.3, 0.7, N))
+    X = hm.ellpack_from_dense(A, M)
+    assert X[2].max() <= M
+    pv, pi, pn, bad, mx = oracle_mod.x2_ellpack(*X, tau)
+    assert bad < 0
+    # the construction does what the docstring says: the upper part of row 0 outgrows 2048 slots before thresholding
+    touched = np.unique(np.concatenate([X[1][k, : X[2][k]] for k in X[1][0, : X[2][0]]]))
+    assert 2048 < touched.size < 4096
+    for branch in (0, 1):
+        if branch:
+            ev, ei, en, bad_u, _ = oracle_mod.update_ellpack(X, (pv, pi, pn), tau)
+            assert bad_u < 0
+        else:
+            ev, ei, en = pv, pi, pn
+        out, sums, info = api.bml_x2_ellpack(to_gpu(X), branch, tau)
+        assert_ell_equal(to_cpu(out), (ev, ei, en))
+        info = info.cpu().numpy()
+        assert info[0] == np.iinfo(np.int32).max and info[1] == np.iinfo(np.int32).max
+
+
 def test_x2_ellpack_second_iterate_wider_rows(api, oracle_mod):
     """Rows after one product are several times wider (pre-threshold fill in the thousands at full size): run a
     second product on the oracle's X_1."""
