@@ -1,12 +1,16 @@
 // ellpack.cu -- the sparse path of DESIGN.md on ELLPACK-R (Listing 1): S1 rescale, S3 thresholded row-wise
 // SpGEMM X*X, S4 fused update / norms / canonical (ascending-column) write-back, S5 finaliser.
 //
-// Gustavson row merge ("sparse-sparse matrix multiply") in two kernels per product:
+// Gustavson row merge ("sparse-sparse matrix multiply"), per product:
+//   ell_block_summary_kernel   per row of X: its 32-column blocks and the largest |x| in each (input of the pre-screen)
 //   x2_ellpack_upper_kernel    row i of thr(X X) for the columns j >= i only (X is bitwise symmetric, so P_ij and P_ji
-//                              are the same chain of fma's); every kept entry is also appended to the list of row j
+//                              are the same chain of fma's); every kept entry is also appended to the list of row j.
+//                              Instance <small table, pre-screen, 7 groups> over all rows, then instance <large table,
+//                              no screen, 4 groups> over the rows the first one passed on (or over all rows when the
+//                              pre-screen does not apply: tau = 0, M > 512, N > 131072)
 //   x2_ellpack_assemble_kernel full row = sorted(appended entries) ++ upper part; update, threshold, norms, write-back
-// Kernel 1: a GROUP of E_GW warps owns one output row at a time; E_MAX_GROUPS groups share a CTA (one CTA per SM),
-// each with its own open-addressing hash accumulator in shared memory (BML_ELL_ACC_SLOTS keys + FP64 values).  For
+// Kernel 1: a GROUP of E_GW warps owns one output row at a time; several groups share a CTA (one CTA per SM), each
+// with its own open-addressing hash accumulator in shared memory (2048 or BML_ELL_ACC_SLOTS keys + FP64 values).  For
 // every stored entry p of row i (ascending p) the group's 128 threads take the entries of row k = index[i][p] with
 // column >= i (a suffix found by binary search while row i is staged) and do acc[j] = fma(x_ik, x_kj, acc[j]); a
 // group barrier separates step p from step p+1.  Contributions to one output entry are therefore added in order of
