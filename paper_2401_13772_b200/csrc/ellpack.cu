@@ -39,6 +39,8 @@ constexpr int E_GW = 4;               // warps per row group
 constexpr int E_GT = E_GW * 32;       // threads per row group
 constexpr int E_MAX_GROUPS = 4;       // row groups (= rows in flight) per CTA with the large table
 constexpr int E_MAX_GROUPS_SMALL = 7; // ... with the small table
+constexpr int E_NBUF_SMALL = 2;       // rotating gather buffers of the small-table instance (28 warps per SM hide the
+                                      // L2 latency of a one-step look-ahead; a third buffer spills at 72 registers)
 constexpr int E_MAX_GRID = 1024;
 constexpr int E_SCREEN_MAX_N = 32 * 2 * (1 << E_SL2_SMALL);     // one FP32 bound per 32-column block, aliased on the values
 
@@ -260,11 +262,40 @@ __device__ __forceinline__ bool s_step(const Gather<CC> &g, int cnt, double a, i
     return full;
 }
 
-// returns true (group-uniform) when the accumulator ran out of slots
-template <int SL2, bool SCREEN, int CC>
+// returns true (group-uniform) when the accumulator ran out of slots.  The gathers run NB - 1 p-steps ahead of the
+// accumulation in NB rotating register buffers.
+template <int SL2, bool SCREEN, int CC, int NB>
 __device__ __forceinline__ bool s_accumulate_row(const double *__restrict__ xv, const int32_t *__restrict__ xi, int M,
                                                  int n_i, const double *sa, const int *sk, const int *sn, int *keys,
                                                  double *vals, const unsigned *allow, int row, int tg, int grp)
+{
+    bool full = false, stop = false;
+    Gather<CC> g[NB];
+    int n[NB];
+#pragma unroll
+    for (int u = 0; u < NB; ++u)
+#pragma unroll
+        for (int c = 0; c < CC; ++c) { g[u].j[c] = row; g[u].v[c] = 0.0; }
+#pragma unroll
+    for (int u = 0; u < NB - 1; ++u) s_gather<CC>(g[u], n[u], u, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+    for (int p = 0; p < n_i; p += NB) {
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            if (p + u < n_i) {             // group-uniform
+                s_gather<CC>(g[(u + NB - 1) % NB], n[(u + NB - 1) % NB], p + u + NB - 1, n_i, xv, xi, (unsigned)M, sk, sn, tg);
+                full = s_step<SL2, SCREEN, CC>(g[u], n[u], sa[p + u], keys, vals, allow, grp, tg, full, stop, u == NB - 1);
+            }
+        }
+        if (stop) break;                   // group-uniform: the OR came with the last step's barrier
+    }
+    return group_bar_or(grp, full);        // flags raised in steps whose barrier did not carry them
+}
+
+// the same with three buffers rotated by name (the large-table instance: the indexed form above costs it registers)
+template <int SL2, bool SCREEN, int CC>
+__device__ __forceinline__ bool s_accumulate_row3(const double *__restrict__ xv, const int32_t *__restrict__ xi, int M,
+                                                  int n_i, const double *sa, const int *sk, const int *sn, int *keys,
+                                                  double *vals, const unsigned *allow, int row, int tg, int grp)
 {
     bool full = false, stop = false;
     Gather<CC> gA, gB, gC;
@@ -368,7 +399,7 @@ __device__ __forceinline__ void s_prescreen(int row, int n_i, int N, int SB, con
 // flight per SM; a row whose screened fill still does not fit (or whose gathered rows need more than four chunks) goes
 // to fail_list.  <E_SL2_BIG, false, 4>: the 4096-slot tables without a screen, over all rows (tau = 0, large N or M) or
 // over row_list[0 .. *row_count) -- the rows the first instance passed on; a table that overflows here is status -6.
-template <int SL2, bool SCREEN, int MAXG>
+template <int SL2, bool SCREEN, int MAXG, int NBUF>
 __global__ void __launch_bounds__(MAXG * E_GT, 1)
 x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict__ i0, const int32_t *__restrict__ n0,
                         const double *__restrict__ v1, const int32_t *__restrict__ i1, const int32_t *__restrict__ n1,
@@ -468,7 +499,10 @@ x2_ellpack_upper_kernel(const double *__restrict__ v0, const int32_t *__restrict
         if (SCREEN) s_prescreen(row, n_i, N, M, sa, sk, sb_id, sb_mx, sb_n, (float *)vals, allow, tau, tg, grp);
 
         bool full = false;
-#define S_ACC(CC) full = s_accumulate_row<SL2, SCREEN, CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, allow, row, tg, grp)
+#define S_ACC(CC)                                                                                                      \
+    full = (NBUF == 3) ? s_accumulate_row3<SL2, SCREEN, CC>(xv, xi, M, n_i, sa, sk, sn, keys, vals, allow, row, tg, grp)   \
+                       : s_accumulate_row<SL2, SCREEN, CC, (NBUF == 3 ? 2 : NBUF)>(xv, xi, M, n_i, sa, sk, sn, keys, vals, \
+                                                                                  allow, row, tg, grp)
         if (chunks <= 1) S_ACC(1);
         else if (chunks == 2) S_ACC(2);
         else if (chunks == 3) S_ACC(3);
@@ -982,7 +1016,7 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
         const size_t gb = e_group_bytes(M, 1 << E_SL2_SMALL);
         const size_t allow_off = (size_t)ng_small * gb;
         const size_t smem_a = allow_off + (size_t)ng_small * allow_bytes;
-        auto ka = x2_ellpack_upper_kernel<E_SL2_SMALL, true, E_MAX_GROUPS_SMALL>;
+        auto ka = x2_ellpack_upper_kernel<E_SL2_SMALL, true, E_MAX_GROUPS_SMALL, E_NBUF_SMALL>;
         static size_t attr_a[MAX_DEVICES] = {};
         if (ensure_smem_attr(ka, smem_a, attr_a)) return BML_ERR_CUDA;
         int64_t grid_a = (N + ng_small - 1) / ng_small;
@@ -998,7 +1032,7 @@ int launch_x2_ellpack(const double *v0, const int32_t *i0, const int32_t *n0, do
         if (ngroups > E_MAX_GROUPS) ngroups = E_MAX_GROUPS;
         if (ngroups < 1) return BML_ERR_INVALID;
         const size_t smem1 = (size_t)ngroups * e_group_bytes(M);
-        auto kb = x2_ellpack_upper_kernel<E_SL2_BIG, false, E_MAX_GROUPS>;
+        auto kb = x2_ellpack_upper_kernel<E_SL2_BIG, false, E_MAX_GROUPS, 3>;
         static size_t attr1[MAX_DEVICES] = {};
         if (ensure_smem_attr(kb, smem1, attr1)) return BML_ERR_CUDA;
         int64_t grid1 = (N + ngroups - 1) / ngroups;
